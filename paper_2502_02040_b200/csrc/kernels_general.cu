@@ -1,0 +1,675 @@
+// kernels_general.cu — per-operation sm_100a kernels of the M2R2 path.
+//
+// These kernels serve every shape the ABI accepts (fp32 and bf16 storage, any number of
+// activation rows: dual-stream decode, k-token verify, batched decode, chunked prefill, MoE).
+// The batch-1 bf16 dense decode step has a faster persistent implementation in
+// kernels_fused.cu; both compute the same operations.
+//
+// Row convention: activations are [rows][*] fp32.  Rows [0, slow_rows) belong to the slow
+// stream h, rows [slow_rows, rows) to the accelerated stream p (Eq. 1 / Eq. 2).
+#include "m2r2_internal.cuh"
+
+// =====================================================================================
+// a1  embed + stream init:  h_0 = Emb[token],  p_0 <- h_0
+// =====================================================================================
+template <typename WT>
+__global__ void embed_kernel(const WT* __restrict__ emb, const int* __restrict__ tok, int d,
+                             float* out, float* out2, float* trace, float* trace2) {
+  int r = blockIdx.x;
+  const WT* src = emb + (size_t)tok[r] * d;
+  for (int j = threadIdx.x; j < d; j += blockDim.x) {
+    float v = to_f32(src[j]);
+    out[(size_t)r * d + j] = v;
+    if (out2) out2[(size_t)r * d + j] = v;
+    if (trace) trace[(size_t)r * d + j] = v;
+    if (trace2) trace2[(size_t)r * d + j] = v;
+  }
+}
+
+void launch_embed(cudaStream_t st, int dtype, const void* emb, const int* tok, int rows, int d,
+                  float* out, float* out2, float* trace, float* trace2) {
+  if (dtype == M2R2_FP32)
+    embed_kernel<float><<<rows, 256, 0, st>>>((const float*)emb, tok, d, out, out2, trace, trace2);
+  else
+    embed_kernel<__nv_bfloat16><<<rows, 256, 0, st>>>((const __nv_bfloat16*)emb, tok, d, out, out2, trace, trace2);
+}
+
+// =====================================================================================
+// RMSNorm (+ adapter down-projection u = A x^ for accelerated rows)
+//   rms(x; g) = x * g / sqrt(mean(x^2) + eps)                       (Q1)
+//   u[row][a*r + j] = A_a[j, :] . x^       a < nA packed adapters   (Q3)
+// =====================================================================================
+template <typename WT>
+__global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict__ X, int d,
+                                                        const WT* __restrict__ g, float eps,
+                                                        float* __restrict__ xn, const WT* __restrict__ A,
+                                                        int nA, int r, int lora_row0,
+                                                        float* __restrict__ U, int ldu) {
+  extern __shared__ float sx[];
+  __shared__ float red[8];
+  int row = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const float* x = X + (size_t)row * d;
+  float ss = 0.f;
+  for (int j = tid; j < d; j += 256) {
+    float v = x[j];
+    sx[j] = v;
+    ss += v * v;
+  }
+  ss = warp_sum(ss);
+  if (lane == 0) red[warp] = ss;
+  __syncthreads();
+  float tot = 0.f;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) tot += red[w];
+  float inv = rsqrtf(tot / (float)d + eps);
+  for (int j = tid; j < d; j += 256) {
+    float v = sx[j] * inv * to_f32(g[j]);
+    sx[j] = v;
+    xn[(size_t)row * d + j] = v;
+  }
+  if (A == nullptr || row < lora_row0) return;
+  __syncthreads();
+  for (int t = warp; t < nA * r; t += 8) {
+    const WT* a = A + (size_t)t * d;
+    float acc = 0.f;
+    for (int k = lane * 8; k < d; k += 256) {
+      float w[8];
+      load8(a + k, w);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) acc += w[e] * sx[k + e];
+    }
+    acc = warp_sum(acc);
+    if (lane == 0) U[(size_t)row * ldu + t] = acc;
+  }
+}
+
+void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int d, const void* g,
+                      float eps, float* xn, const void* A, int nA, int r, int lora_row0, float* U,
+                      int ldu) {
+  size_t sh = (size_t)d * sizeof(float);
+  if (dtype == M2R2_FP32)
+    norm_lora_kernel<float><<<rows, 256, sh, st>>>(X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
+  else
+    norm_lora_kernel<__nv_bfloat16><<<rows, 256, sh, st>>>(X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
+}
+
+// u[row][j] = A[j, :] . x[row][xmap(:)]   (no norm; A_o on the compact o^, A_d on the activations)
+template <typename WT>
+__global__ void __launch_bounds__(256) lora_down_kernel(const float* __restrict__ X, int ldx, int row0, int K,
+                                                        const int* __restrict__ xmap,
+                                                        const WT* __restrict__ A, int r,
+                                                        float* __restrict__ U, int ldu) {
+  int row = row0 + blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const float* x = X + (size_t)row * ldx;
+  for (int j = warp; j < r; j += 8) {
+    const WT* a = A + (size_t)j * K;
+    float acc = 0.f;
+    for (int k = lane * 8; k < K; k += 256) {
+      float w[8];
+      load8(a + k, w);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) acc += w[e] * x[xmap ? xmap[k + e] : (k + e)];
+    }
+    acc = warp_sum(acc);
+    if (lane == 0) U[(size_t)row * ldu + j] = acc;
+  }
+}
+
+void launch_lora_down(cudaStream_t st, int dtype, const float* X, int ldx, int row0, int rows, int K,
+                      const int* xmap, const void* A, int r, float* U, int ldu) {
+  if (rows <= 0) return;
+  if (dtype == M2R2_FP32)
+    lora_down_kernel<float><<<rows, 256, 0, st>>>(X, ldx, row0, K, xmap, (const float*)A, r, U, ldu);
+  else
+    lora_down_kernel<__nv_bfloat16><<<rows, 256, 0, st>>>(X, ldx, row0, K, xmap, (const __nv_bfloat16*)A, r, U, ldu);
+}
+
+// =====================================================================================
+// a2/a5/a6/a7/a8/a9/a16  weight-streaming GEMV / skinny GEMM on CUDA cores.
+//   out[row][n] = resid + (addin + scale * (W[n,:] . x[row]))  (+ B[bmap(n),:] . u[row])
+// One warp owns NW output rows for RT activation rows; lanes stride K with 128-bit loads;
+// the RT activation rows live in shared memory in K-chunks of KC.
+// swiglu variant: act[row][n] = silu(Wg[n].x + lora_g) * (Wu[n].x + lora_u)    (a6)
+// =====================================================================================
+constexpr int GEMV_KC = 1024;
+constexpr int GEMV_NW = 2;
+
+template <typename WT, int RT, bool SWIGLU>
+__global__ void __launch_bounds__(256) gemv_kernel(GemvArgs a) {
+  __shared__ __align__(16) float xs[RT][GEMV_KC];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int row0 = blockIdx.y * RT;
+  const int n0 = (blockIdx.x * 8 + warp) * GEMV_NW;
+  constexpr int NM = SWIGLU ? 2 : 1;   // matrices per output
+  float acc[NM][GEMV_NW][RT];
+#pragma unroll
+  for (int m = 0; m < NM; ++m)
+#pragma unroll
+    for (int j = 0; j < GEMV_NW; ++j)
+#pragma unroll
+      for (int r = 0; r < RT; ++r) acc[m][j][r] = 0.f;
+
+  const WT* W = (const WT*)a.W;
+  const WT* W2 = (const WT*)a.W2;
+  for (int kc0 = 0; kc0 < a.K; kc0 += GEMV_KC) {
+    const int kl = min(GEMV_KC, a.K - kc0);
+    __syncthreads();
+    for (int i = tid; i < RT * (GEMV_KC / 4); i += 256) {
+      int r = i / (GEMV_KC / 4), k4 = (i % (GEMV_KC / 4)) * 4;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (row0 + r < a.n_rows && k4 < kl) v = *(const float4*)(a.X + (size_t)(row0 + r) * a.ldx + kc0 + k4);
+      *(float4*)&xs[r][k4] = v;
+    }
+    __syncthreads();
+    for (int k = lane * 8; k < kl; k += 256) {
+      float xv[RT][8];
+#pragma unroll
+      for (int r = 0; r < RT; ++r) {
+        float4 x0 = *(const float4*)&xs[r][k], x1 = *(const float4*)&xs[r][k + 4];
+        xv[r][0] = x0.x; xv[r][1] = x0.y; xv[r][2] = x0.z; xv[r][3] = x0.w;
+        xv[r][4] = x1.x; xv[r][5] = x1.y; xv[r][6] = x1.z; xv[r][7] = x1.w;
+      }
+#pragma unroll
+      for (int j = 0; j < GEMV_NW; ++j) {
+        if (n0 + j < a.n_out) {
+          float w[8];
+          load8(W + (size_t)(n0 + j) * a.K + kc0 + k, w);
+#pragma unroll
+          for (int r = 0; r < RT; ++r)
+#pragma unroll
+            for (int e = 0; e < 8; ++e) acc[0][j][r] += w[e] * xv[r][e];
+          if (SWIGLU) {
+            load8(W2 + (size_t)(n0 + j) * a.K + kc0 + k, w);
+#pragma unroll
+            for (int r = 0; r < RT; ++r)
+#pragma unroll
+              for (int e = 0; e < 8; ++e) acc[NM - 1][j][r] += w[e] * xv[r][e];
+          }
+        }
+      }
+    }
+  }
+  // reduce over lanes; lane (j*RT + r) finishes output (n0+j, row0+r)
+#pragma unroll
+  for (int m = 0; m < NM; ++m)
+#pragma unroll
+    for (int j = 0; j < GEMV_NW; ++j)
+#pragma unroll
+      for (int r = 0; r < RT; ++r) acc[m][j][r] = warp_sum(acc[m][j][r]);
+  float v0 = 0.f, v1 = 0.f;
+#pragma unroll
+  for (int j = 0; j < GEMV_NW; ++j)
+#pragma unroll
+    for (int r = 0; r < RT; ++r)
+      if (lane == j * RT + r) {
+        v0 = acc[0][j][r];
+        v1 = acc[NM - 1][j][r];
+      }
+  if (lane >= GEMV_NW * RT) return;
+  const int n = n0 + lane / RT, row = row0 + lane % RT;
+  if (n >= a.n_out || row >= a.n_rows) return;
+  // parallel adapter term for accelerated rows
+  if (a.Bm != nullptr && row >= a.lora_row0) {
+    int bn = a.bmap ? a.bmap[n] : n;
+    if (bn >= 0) {
+      int usel = a.usel_div ? n / a.usel_div : 0;
+      const float* u = a.U + (size_t)row * a.ldu + usel * a.r;
+      const WT* b = (const WT*)a.Bm + (size_t)bn * a.r;
+      float s = 0.f;
+      for (int q = 0; q < a.r; ++q) s += to_f32(b[q]) * u[q];
+      v0 += s;
+      if (SWIGLU) {
+        const float* u2 = a.U + (size_t)row * a.ldu + a.r;
+        const WT* b2 = (const WT*)a.Bm2 + (size_t)bn * a.r;
+        float s2 = 0.f;
+        for (int q = 0; q < a.r; ++q) s2 += to_f32(b2[q]) * u2[q];
+        v1 += s2;
+      }
+    }
+  }
+  float res;
+  if (SWIGLU) {
+    res = (v0 / (1.f + __expf(-v0))) * v1;
+  } else {
+    res = v0;
+    if (a.scale) res *= a.scale[(size_t)row * a.scale_ld];
+    if (a.addin) res += a.addin[(size_t)row * a.ldo + n];
+    if (a.resid) res += a.resid[(size_t)row * a.ldo + n];
+  }
+  a.out[(size_t)row * a.ldo + n] = res;
+  if (a.trace) a.trace[(size_t)row * a.ldo + n] = res;
+}
+
+template <typename WT, bool SWIGLU>
+static void launch_gemv_t(cudaStream_t st, const GemvArgs& a) {
+  int rt = a.n_rows <= 1 ? 1 : a.n_rows <= 2 ? 2 : a.n_rows <= 4 ? 4 : 8;
+  dim3 grid((a.n_out + 8 * GEMV_NW - 1) / (8 * GEMV_NW), (a.n_rows + rt - 1) / rt);
+  switch (rt) {
+    case 1: gemv_kernel<WT, 1, SWIGLU><<<grid, 256, 0, st>>>(a); break;
+    case 2: gemv_kernel<WT, 2, SWIGLU><<<grid, 256, 0, st>>>(a); break;
+    case 4: gemv_kernel<WT, 4, SWIGLU><<<grid, 256, 0, st>>>(a); break;
+    default: gemv_kernel<WT, 8, SWIGLU><<<grid, 256, 0, st>>>(a); break;
+  }
+}
+
+void launch_gemv(cudaStream_t st, int dtype, const GemvArgs& a, bool swiglu) {
+  if (a.n_rows <= 0 || a.n_out <= 0) return;
+  if (dtype == M2R2_FP32) {
+    if (swiglu) launch_gemv_t<float, true>(st, a); else launch_gemv_t<float, false>(st, a);
+  } else {
+    if (swiglu) launch_gemv_t<__nv_bfloat16, true>(st, a); else launch_gemv_t<__nv_bfloat16, false>(st, a);
+  }
+}
+
+// =====================================================================================
+// a3  RoPE + KV append.  rope(v, t): pairs (j, j + dh/2), angle t * theta^(-2j/dh) from a host
+// double-precision table.  Slow rows store K/V (rounded to the cache dtype) at
+// [seq][head][pos][dh]; accelerated rows keep k^, v^ in scratch (never cached).
+// =====================================================================================
+template <typename KT>
+__global__ void rope_append_kernel(float* __restrict__ qkv, int slow_rows, const int* __restrict__ row_seq,
+                                   const int* __restrict__ row_pos, const float2* __restrict__ rope_tab,
+                                   KT* __restrict__ Kc, KT* __restrict__ Vc, int n_heads, int dh,
+                                   int max_seq) {
+  int row = blockIdx.x, head = blockIdx.y, half = dh / 2, d = n_heads * dh;
+  int pos = row_pos[row], seq = row_seq[row];
+  float* q = qkv + (size_t)row * 3 * d + head * dh;
+  float* k = q + d;
+  float* v = k + d;
+  size_t cbase = (((size_t)seq * n_heads + head) * max_seq + pos) * dh;
+  for (int j = threadIdx.x; j < half; j += blockDim.x) {
+    float2 cs = rope_tab[(size_t)pos * half + j];
+    float a = q[j], b = q[j + half];
+    q[j] = a * cs.x - b * cs.y;
+    q[j + half] = b * cs.x + a * cs.y;
+    a = k[j]; b = k[j + half];
+    float k0 = a * cs.x - b * cs.y, k1 = b * cs.x + a * cs.y;
+    if (row < slow_rows) {
+      Kc[cbase + j] = from_f32<KT>(k0);
+      Kc[cbase + j + half] = from_f32<KT>(k1);
+      Vc[cbase + j] = from_f32<KT>(v[j]);
+      Vc[cbase + j + half] = from_f32<KT>(v[j + half]);
+    } else {
+      k[j] = k0;
+      k[j + half] = k1;
+    }
+  }
+}
+
+void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int slow_rows, const int* row_seq,
+                        const int* row_pos, const float2* rope_tab, void* Kc, void* Vc, int n_heads,
+                        int dh, int max_seq) {
+  dim3 grid(rows, n_heads);
+  if (dtype == M2R2_FP32)
+    rope_append_kernel<float><<<grid, 64, 0, st>>>(qkv, slow_rows, row_seq, row_pos, rope_tab, (float*)Kc, (float*)Vc, n_heads, dh, max_seq);
+  else
+    rope_append_kernel<__nv_bfloat16><<<grid, 64, 0, st>>>(qkv, slow_rows, row_seq, row_pos, rope_tab, (__nv_bfloat16*)Kc, (__nv_bfloat16*)Vc, n_heads, dh, max_seq);
+}
+
+// =====================================================================================
+// a4 / a11  split-K flash-decode attention, up to M2R2_MAXQ query rows of one sequence sharing
+// every K/V tile (slow + accelerated row of a decode step, or the k+1 rows of a verify pass).
+// Query row q sees cache positions [0, limit_q).  Online softmax per lane segment, merged
+// through shared memory; one (m, l, o) partial per (row, head, split).
+// Lane layout: a position's K row (dh elements) is covered by LPP lanes with 16-byte loads;
+// SEG = next power of two >= LPP lanes form a segment; a warp handles 32/SEG positions at once.
+// =====================================================================================
+template <typename KT> struct KVec;
+template <> struct KVec<__nv_bfloat16> { static constexpr int EPL = 8; };
+template <> struct KVec<float> { static constexpr int EPL = 4; };
+
+template <typename KT>
+__device__ __forceinline__ void load_kv(const KT* p, float out[8]);
+template <>
+__device__ __forceinline__ void load_kv<__nv_bfloat16>(const __nv_bfloat16* p, float out[8]) {
+  uint4 u = *(const uint4*)p;
+  bf16x2_to_f32(u.x, out[0], out[1]);
+  bf16x2_to_f32(u.y, out[2], out[3]);
+  bf16x2_to_f32(u.z, out[4], out[5]);
+  bf16x2_to_f32(u.w, out[6], out[7]);
+}
+template <>
+__device__ __forceinline__ void load_kv<float>(const float* p, float out[8]) {
+  float4 u = *(const float4*)p;
+  out[0] = u.x; out[1] = u.y; out[2] = u.z; out[3] = u.w;
+  out[4] = out[5] = out[6] = out[7] = 0.f;
+}
+
+template <typename KT, int SEG>
+__global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
+  constexpr int EPL = KVec<KT>::EPL;
+  constexpr int NSEG = 4 * (32 / SEG);           // segments per CTA
+  extern __shared__ float sm[];
+  const int head = blockIdx.x, grp = blockIdx.y, split = blockIdx.z;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int dh = a.dh, lpp = dh / EPL;
+  float* qs = sm;                                // [MAXQ][dh], pre-scaled
+  float* red = sm + M2R2_MAXQ * dh;              // [NSEG][MAXQ][dh + 2]
+  __shared__ int s_row[M2R2_MAXQ], s_lim[M2R2_MAXQ];
+  __shared__ int s_seq, s_maxlim;
+  const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
+  if (tid < M2R2_MAXQ) {
+    int r = a.grp_rows[grp * M2R2_MAXQ + tid];
+    if (r >= a.slow_rows && !accel_head) r = -1;  // accelerated rows only use heads in S
+    s_row[tid] = r;
+    s_lim[tid] = r >= 0 ? a.row_limit[r] : 0;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int mx = 0, sq = 0;
+    for (int q = 0; q < M2R2_MAXQ; ++q)
+      if (s_row[q] >= 0) { mx = max(mx, s_lim[q]); sq = a.row_seq[s_row[q]]; }
+    s_maxlim = mx;
+    s_seq = sq;
+  }
+  for (int i = tid; i < M2R2_MAXQ * dh; i += 128) {
+    int q = i / dh, j = i % dh, r = s_row[q];
+    qs[i] = r >= 0 ? a.qkv[(size_t)r * 3 * a.d + head * dh + j] * a.scale : 0.f;
+  }
+  __syncthreads();
+  const int maxlim = s_maxlim;
+  const int chunk = (maxlim + a.n_splits - 1) / a.n_splits;
+  const int u0 = split * chunk, u1 = min(maxlim, u0 + chunk);
+  const KT* Kb = (const KT*)a.Kc + ((size_t)s_seq * a.n_heads + head) * a.max_seq * dh;
+  const KT* Vb = (const KT*)a.Vc + ((size_t)s_seq * a.n_heads + head) * a.max_seq * dh;
+
+  const int seg = lane / SEG, sl = lane % SEG;   // segment in warp, lane in segment
+  const bool active = sl < lpp;
+  float m[M2R2_MAXQ], l[M2R2_MAXQ], o[M2R2_MAXQ][EPL];
+  int lim[M2R2_MAXQ];
+#pragma unroll
+  for (int q = 0; q < M2R2_MAXQ; ++q) {
+    m[q] = -INFINITY; l[q] = 0.f; lim[q] = s_lim[q];
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) o[q][e] = 0.f;
+  }
+  constexpr int PPW = 32 / SEG;
+  for (int ub = u0 + warp * PPW; ub < u1; ub += 4 * PPW) {
+    const int u = ub + seg;
+    const bool valid = u < u1;
+    float kv[8], vv[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) { kv[e] = 0.f; vv[e] = 0.f; }
+    if (valid && active) {
+      load_kv<KT>(Kb + (size_t)u * dh + sl * EPL, kv);
+      load_kv<KT>(Vb + (size_t)u * dh + sl * EPL, vv);
+    }
+#pragma unroll
+    for (int q = 0; q < M2R2_MAXQ; ++q) {
+      float s = 0.f;
+      if (active) {
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) s += qs[q * dh + sl * EPL + e] * kv[e];
+      }
+#pragma unroll
+      for (int off = SEG / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+      if (valid && u < lim[q]) {
+        float mn = fmaxf(m[q], s);
+        float corr = __expf(m[q] - mn), p = __expf(s - mn);
+        l[q] = l[q] * corr + p;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) o[q][e] = o[q][e] * corr + p * vv[e];
+        m[q] = mn;
+      }
+    }
+  }
+  // merge the NSEG running states through shared memory
+  const int gseg = warp * PPW + seg;
+#pragma unroll
+  for (int q = 0; q < M2R2_MAXQ; ++q) {
+    float* dst = red + ((size_t)gseg * M2R2_MAXQ + q) * (dh + 2);
+    if (active) {
+#pragma unroll
+      for (int e = 0; e < EPL; ++e) dst[sl * EPL + e] = o[q][e];
+    }
+    if (sl == 0) { dst[dh] = m[q]; dst[dh + 1] = l[q]; }
+  }
+  __syncthreads();
+  for (int i = tid; i < M2R2_MAXQ * dh; i += 128) {
+    int q = i / dh, j = i % dh, r = s_row[q];
+    if (r < 0) continue;
+    float M = -INFINITY;
+    for (int s = 0; s < NSEG; ++s) M = fmaxf(M, red[((size_t)s * M2R2_MAXQ + q) * (dh + 2) + dh]);
+    float L = 0.f, O = 0.f;
+    for (int s = 0; s < NSEG; ++s) {
+      const float* src = red + ((size_t)s * M2R2_MAXQ + q) * (dh + 2);
+      float ls = src[dh + 1];
+      if (ls > 0.f) {
+        float w = __expf(src[dh] - M);
+        L += ls * w;
+        O += src[j] * w;
+      }
+    }
+    size_t pidx = ((size_t)r * a.n_heads + head) * a.n_splits + split;
+    a.part_o[pidx * dh + j] = O;
+    if (j == 0) { a.part_ml[pidx * 2] = M; a.part_ml[pidx * 2 + 1] = L; }
+  }
+}
+
+void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups) {
+  dim3 grid(a.n_heads, n_groups, a.n_splits);
+  int epl = dtype == M2R2_FP32 ? 4 : 8;
+  int lpp = a.dh / epl;
+  int seg = lpp <= 4 ? 4 : lpp <= 8 ? 8 : lpp <= 16 ? 16 : 32;
+  int nseg = 4 * (32 / seg);
+  size_t sh = ((size_t)M2R2_MAXQ * a.dh + (size_t)nseg * M2R2_MAXQ * (a.dh + 2)) * sizeof(float);
+#define ATTN_CASE(KT, S)                                                                       \
+  {                                                                                            \
+    static bool attr_set = false;                                                              \
+    if (!attr_set) {                                                                           \
+      cudaFuncSetAttribute(attn_kernel<KT, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024); \
+      attr_set = true;                                                                         \
+    }                                                                                          \
+    attn_kernel<KT, S><<<grid, 128, sh, st>>>(a);                                              \
+  }
+  if (dtype == M2R2_FP32) {
+    if (seg == 4) ATTN_CASE(float, 4) else if (seg == 8) ATTN_CASE(float, 8)
+    else if (seg == 16) ATTN_CASE(float, 16) else ATTN_CASE(float, 32)
+  } else {
+    if (seg == 4) ATTN_CASE(__nv_bfloat16, 4) else if (seg == 8) ATTN_CASE(__nv_bfloat16, 8)
+    else if (seg == 16) ATTN_CASE(__nv_bfloat16, 16) else ATTN_CASE(__nv_bfloat16, 32)
+  }
+#undef ATTN_CASE
+}
+
+// merge of the split partials; accelerated rows add their own (k^_t, v^_t) as one more key:
+//   MHA(p_t, h_<t (+) p_t, h_<t (+) p_t)
+__global__ void merge_kernel(MergeArgs a) {
+  const int row = blockIdx.x, head = blockIdx.y, j = threadIdx.x, dh = a.dh;
+  const bool is_accel = row >= a.slow_rows;
+  const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
+  float* out = a.out + (size_t)row * a.d + head * dh;
+  if (is_accel && !accel_head) {
+    if (j < dh) out[j] = 0.f;
+    return;
+  }
+  __shared__ float red[4];
+  float M = -INFINITY;
+  size_t pbase = ((size_t)row * a.n_heads + head) * a.n_splits;
+  for (int s = 0; s < a.n_splits; ++s)
+    if (a.part_ml[(pbase + s) * 2 + 1] > 0.f) M = fmaxf(M, a.part_ml[(pbase + s) * 2]);
+  float s_own = 0.f;
+  if (is_accel) {
+    const float* q = a.qkv + (size_t)row * 3 * a.d + head * dh;
+    float part = j < dh ? q[j] * q[a.d + j] : 0.f;
+    part = warp_sum(part);
+    if ((j & 31) == 0) red[j >> 5] = part;
+    __syncthreads();
+    float tot = 0.f;
+    for (int w = 0; w < (dh + 31) / 32; ++w) tot += red[w];
+    s_own = tot * a.scale;
+    M = fmaxf(M, s_own);
+  }
+  if (j >= dh) return;
+  float L = 0.f, O = 0.f;
+  for (int s = 0; s < a.n_splits; ++s) {
+    float ls = a.part_ml[(pbase + s) * 2 + 1];
+    if (ls > 0.f) {
+      float w = __expf(a.part_ml[(pbase + s) * 2] - M);
+      L += ls * w;
+      O += a.part_o[(pbase + s) * dh + j] * w;
+    }
+  }
+  if (is_accel) {
+    float w = __expf(s_own - M);
+    L += w;
+    O += w * a.qkv[(size_t)row * 3 * a.d + 2 * a.d + head * dh + j];
+  }
+  out[j] = O / L;
+}
+
+void launch_merge(cudaStream_t st, const MergeArgs& a, int rows) {
+  dim3 grid(rows, a.n_heads);
+  merge_kernel<<<grid, 128, 0, st>>>(a);
+}
+
+// =====================================================================================
+// a8/a9  greedy argmax with the logit-script bias hook; lowest index wins ties.
+// =====================================================================================
+__global__ void __launch_bounds__(1024) argmax_kernel(const float* __restrict__ logits, int ldl, int V,
+                                                      const int* __restrict__ row_seq,
+                                                      const int* __restrict__ row_pos,
+                                                      const int* __restrict__ script, int script_first,
+                                                      int script_n, float beta, int* __restrict__ out,
+                                                      int out_stride) {
+  int row = blockIdx.x;
+  const float* lg = logits + (size_t)row * ldl;
+  int bidx = -1;
+  if (script) {
+    int s = row_pos[row] + 1 - script_first;   // logits of the token at pos predict pos+1
+    if (s >= 0 && s < script_n) bidx = script[(size_t)row_seq[row] * script_n + s];
+  }
+  float bv = -INFINITY;
+  int bi = 0x7fffffff;
+  for (int i = threadIdx.x; i < V; i += 1024) {
+    float v = lg[i] + (i == bidx ? beta : 0.f);
+    if (v > bv || (v == bv && i < bi)) { bv = v; bi = i; }
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    float ov = __shfl_xor_sync(0xffffffffu, bv, off);
+    int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+    if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+  }
+  __shared__ float sv[32];
+  __shared__ int si[32];
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { sv[warp] = bv; si[warp] = bi; }
+  __syncthreads();
+  if (warp == 0) {
+    bv = sv[lane]; bi = si[lane];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      float ov = __shfl_xor_sync(0xffffffffu, bv, off);
+      int oi = __shfl_xor_sync(0xffffffffu, bi, off);
+      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if (lane == 0) out[(size_t)row * out_stride] = bi;
+  }
+}
+
+void launch_argmax(cudaStream_t st, const float* logits, int ldl, int rows, int V, const int* row_seq,
+                   const int* row_pos, const int* script, int script_first, int script_n, float beta,
+                   int* out, int out_stride) {
+  if (rows <= 0) return;
+  argmax_kernel<<<rows, 1024, 0, st>>>(logits, ldl, V, row_seq, row_pos, script, script_first, script_n, beta, out, out_stride);
+}
+
+__global__ void copy_rows_kernel(const float* __restrict__ src, float* __restrict__ dst, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = src[i];
+}
+void launch_copy_rows(cudaStream_t st, const float* src, float* dst, int rows, int d) {
+  size_t n = (size_t)rows * d;
+  if (n == 0) return;
+  copy_rows_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(src, dst, n);
+}
+
+// =====================================================================================
+// a13/a14  router / expert predictor: logits = W_r . rms(x; g) (+ script), softmax over all
+// experts, top-k (lower index wins ties), renormalise over the selected (Q19).
+// One block per row.
+// =====================================================================================
+template <typename WT>
+__global__ void __launch_bounds__(256) route_kernel(const float* __restrict__ X, int ldx, int d,
+                                                    const WT* __restrict__ g, float eps, int do_norm,
+                                                    const WT* __restrict__ Wr, int n_experts, int top_k,
+                                                    int renorm, const int* __restrict__ row_pos,
+                                                    const int* __restrict__ script, int script_first,
+                                                    int script_n, int n_layers, int layer, float beta,
+                                                    int* __restrict__ idx_out, float* __restrict__ w_out) {
+  extern __shared__ float sx[];
+  __shared__ float red[8];
+  __shared__ float lg[M2R2_MAX_EXPERTS];
+  int row = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const float* x = X + (size_t)row * ldx;
+  float ss = 0.f;
+  for (int j = tid; j < d; j += 256) { float v = x[j]; sx[j] = v; ss += v * v; }
+  ss = warp_sum(ss);
+  if (lane == 0) red[warp] = ss;
+  __syncthreads();
+  if (do_norm) {
+    float tot = 0.f;
+    for (int w = 0; w < 8; ++w) tot += red[w];
+    float inv = rsqrtf(tot / (float)d + eps);
+    for (int j = tid; j < d; j += 256) sx[j] = sx[j] * inv * to_f32(g[j]);
+    __syncthreads();
+  }
+  for (int e = warp; e < n_experts; e += 8) {
+    const WT* w = Wr + (size_t)e * d;
+    float acc = 0.f;
+    for (int k = lane * 8; k < d; k += 256) {
+      float wv[8];
+      load8(w + k, wv);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) acc += wv[q] * sx[k + q];
+    }
+    acc = warp_sum(acc);
+    if (lane == 0) lg[e] = acc;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    if (script) {
+      int s = row_pos[row] - script_first;
+      if (s >= 0 && s < script_n) {
+        const int* pr = script + ((size_t)s * n_layers + layer) * 2;
+        lg[pr[0]] += beta;
+        lg[pr[1]] += beta - 8.0f;
+      }
+    }
+    float mx = lg[0];
+    for (int e = 1; e < n_experts; ++e) mx = fmaxf(mx, lg[e]);
+    float sum = 0.f;
+    for (int e = 0; e < n_experts; ++e) sum += expf(lg[e] - mx);
+    int sel[M2R2_MAX_TOPK];
+    float wsum = 0.f;
+    for (int k = 0; k < top_k; ++k) {
+      int best = -1;
+      for (int e = 0; e < n_experts; ++e) {
+        bool taken = false;
+        for (int q = 0; q < k; ++q) taken |= (sel[q] == e);
+        if (taken) continue;
+        if (best < 0 || lg[e] > lg[best]) best = e;
+      }
+      sel[k] = best;
+      wsum += expf(lg[best] - mx) / sum;
+    }
+    for (int k = 0; k < top_k; ++k) {
+      float p = expf(lg[sel[k]] - mx) / sum;
+      idx_out[(size_t)row * top_k + k] = sel[k];
+      w_out[(size_t)row * top_k + k] = renorm ? p / wsum : p;
+    }
+  }
+}
+
+void launch_route(cudaStream_t st, int dtype, const float* X, int ldx, int rows, int d, const void* g,
+                  float eps, int do_norm, const void* Wr, int n_experts, int top_k, int renorm,
+                  const int* row_pos, const int* script, int script_first, int script_n, int n_layers,
+                  int layer, float beta, int* idx_out, float* w_out) {
+  if (rows <= 0) return;
+  size_t sh = (size_t)d * sizeof(float);
+  if (dtype == M2R2_FP32)
+    route_kernel<float><<<rows, 256, sh, st>>>(X, ldx, d, (const float*)g, eps, do_norm, (const float*)Wr, n_experts, top_k, renorm, row_pos, script, script_first, script_n, n_layers, layer, beta, idx_out, w_out);
+  else
+    route_kernel<__nv_bfloat16><<<rows, 256, sh, st>>>(X, ldx, d, (const __nv_bfloat16*)g, eps, do_norm, (const __nv_bfloat16*)Wr, n_experts, top_k, renorm, row_pos, script, script_first, script_n, n_layers, layer, beta, idx_out, w_out);
+}

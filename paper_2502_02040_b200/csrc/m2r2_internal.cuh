@@ -1,0 +1,146 @@
+// m2r2_internal.cuh — shared declarations of the CUDA path (host orchestration + kernels).
+// Product code: nothing here is shared with oracle/.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/m2r2.h"
+
+#define M2R2_MAXQ 8        // query rows of one sequence that share K/V tiles in attention
+#define M2R2_MAX_SPLITS 32
+
+// ------------------------------------------------------------------ storage helpers
+__device__ __forceinline__ float to_f32(float v) { return v; }
+__device__ __forceinline__ float to_f32(__nv_bfloat16 v) { return __bfloat162float(v); }
+
+template <typename T> __device__ __forceinline__ T from_f32(float v);
+template <> __device__ __forceinline__ float from_f32<float>(float v) { return v; }
+template <> __device__ __forceinline__ __nv_bfloat16 from_f32<__nv_bfloat16>(float v) {
+  return __float2bfloat16_rn(v);
+}
+
+// streaming 16-byte load (weights are read once per step: do not pollute L1)
+__device__ __forceinline__ uint4 ldg_stream(const void* p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+__device__ __forceinline__ void bf16x2_to_f32(uint32_t u, float& lo, float& hi) {
+  lo = __uint_as_float(u << 16);
+  hi = __uint_as_float(u & 0xFFFF0000u);
+}
+
+// 8 consecutive elements starting at p (16-byte aligned for bf16, 32-byte for fp32) -> fp32
+__device__ __forceinline__ void load8(const __nv_bfloat16* p, float w[8]) {
+  uint4 u = ldg_stream(p);
+  bf16x2_to_f32(u.x, w[0], w[1]);
+  bf16x2_to_f32(u.y, w[2], w[3]);
+  bf16x2_to_f32(u.z, w[4], w[5]);
+  bf16x2_to_f32(u.w, w[6], w[7]);
+}
+__device__ __forceinline__ void load8(const float* p, float w[8]) {
+  uint4 a = ldg_stream(p), b = ldg_stream(p + 4);
+  w[0] = __uint_as_float(a.x); w[1] = __uint_as_float(a.y);
+  w[2] = __uint_as_float(a.z); w[3] = __uint_as_float(a.w);
+  w[4] = __uint_as_float(b.x); w[5] = __uint_as_float(b.y);
+  w[6] = __uint_as_float(b.z); w[7] = __uint_as_float(b.w);
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// ------------------------------------------------------------------ HBM layout helpers
+struct DevLayer {   // device pointers into the resident-weights buffer (storage dtype)
+  const void *g1, *g2, *wqkv, *wo, *wgate, *wup, *wdown;
+  const void *Aqkv, *Bqkv, *Ao, *Bo, *Agu, *Bg, *Bu, *Ad, *Bd;
+  const void *router, *Ug, *Uu, *Ud;
+};
+
+struct Carver {   // bump allocator over a caller buffer; base == nullptr -> size query only
+  char* base;
+  size_t off = 0;
+  explicit Carver(void* b) : base((char*)b) {}
+  template <typename T> T* take(size_t n) {
+    off = (off + 255) & ~(size_t)255;
+    T* p = base ? (T*)(base + off) : nullptr;
+    off += n * sizeof(T);
+    return p;
+  }
+  size_t size() const { return (off + 255) & ~(size_t)255; }
+};
+
+// ------------------------------------------------------------------ launch argument blocks
+struct GemvArgs {
+  const void* W;        // [n_out, K] row-major (storage dtype)
+  const void* W2;       // swiglu: up matrix [n_out, K]
+  const float* X;       // [n_rows, ldx] fp32 activations
+  int ldx, n_rows, K, n_out;
+  float* out;           // [n_rows, ldo]
+  int ldo;
+  const float* resid;   // nullable, [n_rows, ldo]: out = resid + ...
+  const float* addin;   // nullable, [n_rows, ldo]: out = resid + (addin + scale*acc)
+  const float* scale;   // nullable, per-row scale, stride scale_ld
+  int scale_ld;
+  float* trace;         // nullable, [n_rows? no: n_trace_rows][ldo] second copy of `out`
+  // parallel low-rank adapters: rows >= lora_row0 get  + B[bmap(n)] . U[row][usel*r ..]
+  const void* Bm;       // nullable; [*, r] storage dtype
+  const void* Bm2;      // swiglu: B of the up projection
+  const int* bmap;      // nullable -> identity; -1 = no adapter row for this output
+  const float* U;       // [n_rows, ldu]
+  int ldu, r, lora_row0, usel_div;   // usel = usel_div ? n / usel_div : 0; (swiglu: up uses usel 1)
+};
+
+struct AttnArgs {
+  const float* qkv;     // [rows][3d] : q | k | v (q,k already rotated)
+  const void* Kc;       // this layer's K cache [B][n_heads][max_seq][dh]
+  const void* Vc;
+  const int* row_seq;   // [rows]
+  const int* row_limit; // [rows] number of visible cache positions
+  const int* grp_rows;  // [n_groups][M2R2_MAXQ] row ids, -1 padded
+  float* part_o;        // [rows][n_heads][splits][dh]
+  float* part_ml;       // [rows][n_heads][splits][2]
+  int n_heads, dh, d, max_seq, n_splits, slow_rows;  // rows >= slow_rows are accelerated rows
+  uint32_t accel_head_mask[4];
+  float scale;
+};
+
+struct MergeArgs {
+  const float* qkv;
+  const float* part_o;
+  const float* part_ml;
+  const int* row_limit;
+  float* out;           // [rows][d]
+  int n_heads, dh, d, n_splits, slow_rows;
+  uint32_t accel_head_mask[4];
+  float scale;
+};
+
+// ------------------------------------------------------------------ kernel launchers (kernels_general.cu)
+void launch_embed(cudaStream_t st, int dtype, const void* emb, const int* tok, int rows, int d,
+                  float* out, float* out2, float* trace, float* trace2);
+void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int d, const void* g,
+                      float eps, float* xn, const void* A, int nA, int r, int lora_row0, float* U,
+                      int ldu);
+void launch_lora_down(cudaStream_t st, int dtype, const float* X, int ldx, int row0, int rows, int K,
+                      const int* xmap, const void* A, int r, float* U, int ldu);
+void launch_gemv(cudaStream_t st, int dtype, const GemvArgs& a, bool swiglu);
+void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int slow_rows, const int* row_seq,
+                        const int* row_pos, const float2* rope_tab, void* Kc, void* Vc, int n_heads,
+                        int dh, int max_seq);
+void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups);
+void launch_merge(cudaStream_t st, const MergeArgs& a, int rows);
+void launch_argmax(cudaStream_t st, const float* logits, int ldl, int rows, int V, const int* row_seq,
+                   const int* row_pos, const int* script, int script_first, int script_n, float beta,
+                   int* out, int out_stride);
+void launch_copy_rows(cudaStream_t st, const float* src, float* dst, int rows, int d);
+void launch_route(cudaStream_t st, int dtype, const float* X, int ldx, int rows, int d, const void* g,
+                  float eps, int do_norm, const void* Wr, int n_experts, int top_k, int renorm,
+                  const int* row_pos, const int* script, int script_first, int script_n, int n_layers,
+                  int layer, float beta, int* idx_out, float* w_out);
