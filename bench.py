@@ -1,0 +1,362 @@
+#!/usr/bin/env python
+"""bench.py — M2R2 decode throughput on B200 (contract: see DESIGN.md §Measurement).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+Workload (BASELINE.json configs[1], "C2"): 3.8B-class bf16 decoder (32 layers, d 3072, 32x96 heads,
+FFN 8192, vocab 32064), batch 1, 512-token random prompt, then K dual-stream M2R2 decode steps (slow
+and accelerated residual streams both carried through all 32 layers).  A "step" = one
+m2r2_decode_step = one generated token.  Synthetic seeded weights N(0, 0.02) and uniform-random
+prompt (m2r2_synth).  N > 1 = N independent replicas (no collective).
+
+Prints ONE JSON line (rank 0).  `value` is device-timed (CUDA events on the library's compute
+stream, inputs resident in HBM, tokens stay on the device); `e2e` is the same metric through the C
+ABI with host buffers (the forced input token goes host->device, the produced token device->host,
+every step, inside the timed region).  `roofline` is for the dominant kernel class measured live by
+the library's event profile; `cpu_baseline` is the oracle timed on this box's host cores.
+`--impl reference` times the oracle (CPU) on the same config and metric.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "decode tokens/s at batch 1 (M2R2 dual-stream decode, 3.8B-class bf16)"
+PROMPT = 512
+HBM_NOMINAL_GBS = 8000.0      # BASELINE.json: "achieved HBM GB/s vs 8 TB/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------------
+# byte model (DESIGN.md §Byte model): algorithmic bytes one decode step must move
+# ---------------------------------------------------------------------------------------------
+def step_bytes(cfg, T, exit_heads):
+    """T = positions already cached (kv_len before the step)."""
+    e, d, F, r = cfg.elt_bytes, cfg.d_model, cfg.d_ff, cfg.adapter_rank
+    da = cfg.n_accel_heads * cfg.head_dim
+    w_layer = (4 * d * d + 3 * d * F) * e
+    ad_layer = (3 * (r * d + da * r) + r * da + d * r + 2 * (r * d + F * r) + r * F + d * r) * e
+    n_acc = cfg.accel_end_layer if cfg.accel_enabled else 0
+    by = {"qkv": cfg.n_layers * 3 * d * d * e + n_acc * 3 * (r * d + da * r) * e,
+          "o_proj": cfg.n_layers * d * d * e + n_acc * (r * da + d * r) * e,
+          "gate_up": cfg.n_layers * 2 * d * F * e + n_acc * 2 * (r * d + F * r) * e,
+          "down": cfg.n_layers * d * F * e + n_acc * (r * F + d * r) * e,
+          "attention": cfg.n_layers * 2 * d * (T + 1) * e,
+          "rope_append": cfg.n_layers * 2 * d * e,
+          "heads": (1 + (len(cfg.gates) if exit_heads else 0)) * cfg.vocab * d * e,
+          "other": d * e}
+    total = sum(by.values())
+    assert total == cfg.n_layers * w_layer + n_acc * ad_layer + by["attention"] + by["rope_append"] + by["heads"] + by["other"]
+    return total, by
+
+
+# ---------------------------------------------------------------------------------------------
+# clocks (B200_PROFILING.md): nvidia-smi sampled DURING the timed region
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1]))
+                mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline leg and --impl reference): oracle/ as it stands, host cores
+# ---------------------------------------------------------------------------------------------
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def time_oracle(cfg, W, n_steps, warmup, prefill_tokens=8, budget_s=None):
+    """Oracle decode steps on the C2 model after a short prefill.  A 3.8B decode step streams the
+    same 7.6 GB of weights whatever the context length (KV is 2.6% of the bytes at T=512), so a
+    short context is a fair bounded sample of the workload.  -> (tokens/s, steps timed, description)"""
+    import m2r2_synth as S
+    from oracle import Oracle
+    orc = Oracle(cfg, W)
+    orc.prefill(S.gen_prompt(cfg, prefill_tokens))
+    t_first = None
+    for _ in range(max(1, warmup)):
+        t0 = time.perf_counter()
+        orc.decode_step()
+        t_first = time.perf_counter() - t0
+    if budget_s is not None and t_first * n_steps > budget_s:
+        n_steps = max(2, int(budget_s / t_first))
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        orc.decode_step()
+    dt = time.perf_counter() - t0
+    orc.close()
+    desc = ("%d oracle decode steps of the C2 model (all 32 layers, both streams) at context %d..%d after a "
+            "%d-token prefill and %d warm-up steps" % (n_steps, prefill_tokens + max(1, warmup),
+                                                      prefill_tokens + max(1, warmup) + n_steps,
+                                                      prefill_tokens, max(1, warmup)))
+    return n_steps / dt, n_steps, dt, desc
+
+
+def bench_config():
+    import m2r2_synth as S
+    return S.config_c2()
+
+
+def config_json(cfg, extra=None):
+    c = {"workload": "C2 (BASELINE.json configs[1]): 3.8B-class bf16 dense decoder, batch 1, prompt %d, "
+                     "plain M2R2 dual-stream decode steps (slow + accelerated stream in all %d layers, "
+                     "accel heads %d of %d, adapter rank %d, gates %s re-initialise p from h)"
+                     % (PROMPT, cfg.n_layers, cfg.n_accel_heads, cfg.n_heads, cfg.adapter_rank, list(cfg.gates)),
+         "n_layers": cfg.n_layers, "d_model": cfg.d_model, "n_heads": cfg.n_heads, "head_dim": cfg.head_dim,
+         "d_ff": cfg.d_ff, "vocab": cfg.vocab, "batch": 1, "prompt_len": PROMPT,
+         "l2_policy": "inputs larger than L2: every step streams >= 7.6 GB of weights + KV (L2 is 126 MB)",
+         "parallelism": "replicas"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+def run_reference(args, rk):
+    """--impl reference: the oracle on host cores, same config / metric / unit (tier framing ④)."""
+    from paper_2502_02040_b200 import replicas
+    if rk.rank != 0:
+        return 0
+    import m2r2_synth as S
+    cfg = bench_config()
+    W = S.gen_weights(cfg)
+    tps, n, dt, desc = time_oracle(cfg, W, args.steps, args.warmup, budget_s=150.0)
+    line = {"impl": "reference", "metric": METRIC, "value": tps, "unit": "tokens/s", "n_gpus": args.gpus,
+            "steps": n, "steps_requested": args.steps, "warmup": max(1, args.warmup),
+            "ms_per_step": 1e3 * dt / n, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 arithmetic with f64 accumulation (bf16 weights + KV)", "data": "synthetic",
+            "config": config_json(cfg),
+            "cpu_baseline": {"value": tps, "unit": "tokens/s", "cores": host_cores(), "kind": "oracle", "sample": desc},
+            "e2e": {"value": tps, "unit": "tokens/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args, rk):
+    import torch
+    import m2r2_synth as S
+    import paper_2502_02040_b200 as M
+    from paper_2502_02040_b200 import replicas
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    dev = "cuda:%d" % rk.local_rank
+    torch.cuda.set_device(dev)
+    cfg = bench_config()
+    K, Wm = args.steps, max(3, args.warmup)
+    if PROMPT + 2 * (Wm + K) + 8 > cfg.max_seq:
+        from dataclasses import replace
+        cfg = replace(cfg, max_seq=PROMPT + 2 * (Wm + K) + 8)
+    exit_heads = bool(args.exit_heads)
+    W = S.gen_weights(cfg)
+    eng = M.Engine(cfg, W, exit_heads=exit_heads, device=dev)
+    if args.no_fused:
+        eng.set_fused(False)
+    prompt = S.gen_prompt(cfg, PROMPT, seed=replicas.replica_seed(1000 + 2, rk))
+    stream = eng.compute_stream
+    peak, peak_src = measured_peaks()
+
+    def timed_device(n):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(n):
+            eng.decode_step(want_tokens=False)      # token stays on the device
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1)
+
+    # ---- device-timed region: K steps, inputs resident in HBM
+    eng.prefill(prompt)
+    for _ in range(Wm):
+        eng.decode_step(want_tokens=False)
+    eng.sync()
+    launches0 = eng.get_stats()["kernel_launches"]
+    kv0 = eng.get_stats()["kv_len"][0]
+    replicas.barrier(rk)
+    torch.cuda.synchronize()
+    clocks = ClockSampler(rk.local_rank) if rk.rank == 0 else None
+    ms = timed_device(K)
+    torch.cuda.synchronize()
+    replicas.barrier(rk)
+    clk = clocks.stop() if clocks else None
+    launches = eng.get_stats()["kernel_launches"] - launches0
+    ms_max, units = replicas.aggregate(rk, ms, K)
+    value = units / (ms_max * 1e-3)
+
+    # ---- algorithmic bytes of the timed steps (T grows kv0 .. kv0+K-1)
+    tot_bytes = sum(step_bytes(cfg, kv0 + s, exit_heads)[0] for s in range(K))
+    step_gbs = tot_bytes / (ms * 1e-3) / 1e9
+    lib_bytes = eng.get_stats()["algorithmic_bytes_last"]
+    model_last = step_bytes(cfg, kv0 + K - 1, exit_heads)[0]
+    assert abs(lib_bytes - model_last) <= 1e-6 * model_last, (lib_bytes, model_last)
+
+    # ---- per-class profile pass (same steps, events between kernel groups) -> dominant kernel roofline
+    eng.prefill(prompt)
+    for _ in range(Wm):
+        eng.decode_step(want_tokens=False)
+    eng.set_profile(True)
+    n_prof = min(K, 32)
+    for _ in range(n_prof):
+        eng.decode_step(want_tokens=False)
+    prof = eng.get_profile()
+    eng.set_profile(False)
+    _, by_cls = step_bytes(cfg, kv0 + n_prof // 2, exit_heads)
+    per_class = {}
+    for c, t_ms in prof["ms"].items():
+        b = tot_bytes / K if c == "fused_step" else by_cls.get(c, 0)
+        per_class[c] = {"ms_per_step": t_ms, "launch_groups_per_step": prof["segments"][c],
+                        "algorithmic_bytes_per_step": b, "GB/s": b / (t_ms * 1e-3) / 1e9 if t_ms > 0 else None}
+    dom = max(prof["ms"], key=lambda c: prof["ms"][c])
+    dom_groups = prof["segments"][dom]
+    dom_bytes = per_class[dom]["algorithmic_bytes_per_step"] / dom_groups
+    dom_ms = prof["ms"][dom] / dom_groups
+    achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
+    kernel_names = {"gate_up": "gemv_kernel<bf16, 2 rows, SWIGLU> (+ norm_lora_kernel)", "qkv": "gemv_kernel<bf16, 2 rows> (+ norm_lora_kernel)",
+                    "down": "gemv_kernel<bf16, 2 rows>", "o_proj": "gemv_kernel<bf16, 2 rows>", "heads": "gemv_kernel<bf16> LM head",
+                    "attention": "attn_kernel + merge_kernel", "fused_step": "m2r2_fused_decode_kernel (persistent, whole step)"}
+    roofline = {"bound": "hbm", "kernel": kernel_names.get(dom, dom), "class": dom,
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
+                "traffic": args.traffic, "step": {"achieved": step_gbs, "frac": step_gbs / peak,
+                                                  "frac_of_nominal_8TBs": step_gbs / HBM_NOMINAL_GBS,
+                                                  "algorithmic_bytes_per_step": tot_bytes / K},
+                "per_class": per_class}
+
+    # ---- e2e: same metric through the C ABI with HOST buffers, one H2D + one D2H per step
+    first = eng.prefill(prompt)
+    tok = np.array([int(first[0])], dtype=np.int32)
+    for _ in range(Wm):
+        tok = eng.decode_step(force_tokens=tok)
+    replicas.barrier(rk)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(K):
+        tok = eng.decode_step(force_tokens=tok)      # host token in (H2D), host token out (D2H + sync)
+    e1.record(stream)
+    e1.synchronize()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    e2e_ms = max(e0.elapsed_time(e1), wall_ms)
+    e2e_max, e2e_units = replicas.aggregate(rk, e2e_ms, K)
+    e2e = {"value": e2e_units / (e2e_max * 1e-3), "unit": "tokens/s", "h2d_bytes_per_step": 4, "d2h_bytes_per_step": 4,
+           "ms_per_step": e2e_max / K}
+
+    line = {"metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": rk.world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32 arithmetic (bf16 weights + KV cache)", "data": "synthetic",
+            "config": config_json(cfg, {"exit_heads_at_gates": exit_heads, "kv_len_start": kv0,
+                                        "implementation": "per-operation kernels" if args.no_fused else "default"}),
+            "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
+
+    # ---- cpu_baseline: oracle on this box's host cores (rank 0, N = 1 only)
+    eng.close()
+    del eng
+    torch.cuda.empty_cache()
+    if rk.rank == 0 and rk.world == 1 and not args.no_cpu_baseline:
+        tps, n, dt, desc = time_oracle(cfg, W, 12, 1, budget_s=25.0)
+        line["cpu_baseline"] = {"value": tps, "unit": "tokens/s", "cores": host_cores(), "kind": "oracle", "sample": desc}
+    if rk.rank == 0:
+        print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=256)
+    ap.add_argument("--warmup", type=int, default=8)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--exit-heads", type=int, default=0, help="evaluate the exit argmax at every gate (SURVEY Q15 second row)")
+    ap.add_argument("--no-fused", action="store_true", help="force the per-operation kernels")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")
+    args = ap.parse_args()
+    from paper_2502_02040_b200 import replicas
+    rk = replicas.init_from_env(backend="gloo" if args.impl == "reference" else None)
+    if args.gpus != rk.world and rk.world > 1:
+        raise SystemExit("--gpus %d but WORLD_SIZE %d" % (args.gpus, rk.world))
+    try:
+        rc = run_reference(args, rk) if args.impl == "reference" else run_ours(args, rk)
+    finally:
+        replicas.shutdown(rk)
+    sys.exit(rc)
+
+
+if __name__ == "__main__":
+    main()

@@ -131,6 +131,23 @@ typedef struct m2r2_stats {
   int64_t kernel_launches;           /* kernels launched by this library so far */
 } m2r2_stats;
 
+/* Per-operation device timing (CUDA events on the compute stream, recorded between the kernel
+ * groups of a step).  Classes follow SURVEY §8(a): a2 QKV (with its RMSNorm), a3 RoPE+append,
+ * a4 attention (+ split merge), a5 O-proj, a6 gate/up+SwiGLU (with its RMSNorm), a7 down +
+ * residual, a8/a9 heads (norm + LM head + argmax), everything else (embed, row set-up, gate
+ * copies, router), and the persistent fused step when that implementation runs. */
+#define M2R2_PROF_CLASSES 10
+enum {
+  M2R2_PROF_QKV = 0, M2R2_PROF_ROPE = 1, M2R2_PROF_ATTN = 2, M2R2_PROF_OPROJ = 3,
+  M2R2_PROF_GATEUP = 4, M2R2_PROF_DOWN = 5, M2R2_PROF_HEAD = 6, M2R2_PROF_OTHER = 7,
+  M2R2_PROF_FUSED_STEP = 8
+};
+typedef struct m2r2_profile {
+  double ms[M2R2_PROF_CLASSES];        /* accumulated device time per class */
+  int64_t segments[M2R2_PROF_CLASSES]; /* number of timed segments per class */
+  int64_t steps;                       /* decode/spec steps accumulated */
+} m2r2_profile;
+
 typedef struct m2r2_ctx m2r2_ctx;
 
 /* Bytes the caller must allocate for `cfg`.  host in / host out. */
@@ -211,6 +228,12 @@ int m2r2_reset(m2r2_ctx* ctx);
  * (bf16 dense, batch 1), 0 = per-operation kernels.  Both are CUDA; results agree to fp32
  * rounding.  Exposed so tests can cross-check the two. */
 int m2r2_set_fused(m2r2_ctx* ctx, int32_t enabled);
+
+/* Profiling mode: enabled != 0 clears the accumulators and makes every following decode_step /
+ * spec_step record events between its kernel groups and synchronise at its end (so it is NOT
+ * the mode to measure whole-step throughput in).  m2r2_get_profile copies the accumulators. */
+int m2r2_set_profile(m2r2_ctx* ctx, int32_t enabled);
+int m2r2_get_profile(m2r2_ctx* ctx, m2r2_profile* out);
 
 const char* m2r2_last_error(const m2r2_ctx* ctx);
 const char* m2r2_version(void);

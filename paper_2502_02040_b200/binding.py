@@ -69,10 +69,18 @@ class Stats(ctypes.Structure):
                                    "h2d_bytes", "algorithmic_bytes_last", "kernel_launches")]
 
 
+PROF_CLASSES = ["qkv", "rope_append", "attention", "o_proj", "gate_up", "down", "heads", "other", "fused_step", "_"]
+
+
+class Profile(ctypes.Structure):
+    _fields_ = [("ms", ctypes.c_double * 10), ("segments", i64 * 10), ("steps", i64)]
+
+
 EXPORTS = ["m2r2_query_sizes", "m2r2_create", "m2r2_destroy", "m2r2_load_weights", "m2r2_prefill",
            "m2r2_decode_step", "m2r2_spec_step", "m2r2_moe_prefetch", "m2r2_set_policy",
            "m2r2_set_logit_script", "m2r2_set_router_script", "m2r2_get_stats", "m2r2_debug_read",
-           "m2r2_reset", "m2r2_set_fused", "m2r2_last_error", "m2r2_version"]
+           "m2r2_reset", "m2r2_set_fused", "m2r2_set_profile", "m2r2_get_profile", "m2r2_last_error",
+           "m2r2_version"]
 
 _lib = None
 
@@ -98,6 +106,8 @@ def lib():
         L.m2r2_debug_read.argtypes = [vp, i32, i32, i32, vp, ctypes.c_size_t]
         L.m2r2_reset.argtypes = [vp]
         L.m2r2_set_fused.argtypes = [vp, i32]
+        L.m2r2_set_profile.argtypes = [vp, i32]
+        L.m2r2_get_profile.argtypes = [vp, ctypes.POINTER(Profile)]
         L.m2r2_last_error.argtypes = [vp]
         L.m2r2_last_error.restype = ctypes.c_char_p
         L.m2r2_version.restype = ctypes.c_char_p
@@ -315,6 +325,18 @@ class Engine:
 
     def set_fused(self, on: bool):
         self._chk(self.L.m2r2_set_fused(self.h, int(on)), "set_fused")
+
+    def set_profile(self, on: bool):
+        self._chk(self.L.m2r2_set_profile(self.h, int(on)), "set_profile")
+
+    def get_profile(self) -> dict:
+        """-> {"steps": n, "ms": {class: ms per step}, "segments": {class: segments per step}}"""
+        p = Profile()
+        self._chk(self.L.m2r2_get_profile(self.h, ctypes.byref(p)), "get_profile")
+        n = max(1, p.steps)
+        return {"steps": p.steps,
+                "ms": {c: p.ms[i] / n for i, c in enumerate(PROF_CLASSES) if p.segments[i]},
+                "segments": {c: p.segments[i] / n for i, c in enumerate(PROF_CLASSES) if p.segments[i]}}
 
     def sync(self):
         self.compute_stream.synchronize()

@@ -115,8 +115,43 @@ struct m2r2_ctx {
   FusedState fs;
   uint32_t accel_mask[4];
   m2r2_stats st;
+  // profiling: segment i = [pev[i], pev[i+1]) belongs to class pcls[i]
+  bool prof = false;
+  std::vector<cudaEvent_t> pev;
+  std::vector<int> pcls;
+  int pn = 0;
+  m2r2_profile pr;
   char err[512];
 };
+
+static void prof_mark(m2r2_ctx* x, int cls) {
+  if (!x->prof) return;
+  if (x->pn > 0 && x->pcls[x->pn - 1] == cls) return;   // same class continues
+  if (x->pn == (int)x->pev.size()) {
+    cudaEvent_t e;
+    if (cudaEventCreate(&e) != cudaSuccess) return;
+    x->pev.push_back(e);
+    x->pcls.push_back(-1);
+  }
+  cudaEventRecord(x->pev[x->pn], x->cs);
+  x->pcls[x->pn] = cls;
+  x->pn++;
+}
+static void prof_resolve(m2r2_ctx* x) {
+  if (!x->prof || x->pn == 0) return;
+  prof_mark(x, -1);
+  cudaStreamSynchronize(x->cs);
+  for (int i = 0; i + 1 < x->pn; ++i) {
+    int c = x->pcls[i];
+    float ms = 0.f;
+    if (c >= 0 && c < M2R2_PROF_CLASSES && cudaEventElapsedTime(&ms, x->pev[i], x->pev[i + 1]) == cudaSuccess) {
+      x->pr.ms[c] += ms;
+      x->pr.segments[c]++;
+    }
+  }
+  x->pr.steps++;
+  x->pn = 0;
+}
 
 static int fail(m2r2_ctx* ctx, int code, const char* fmt, ...) {
   if (ctx) {
@@ -290,6 +325,7 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
   x->cps = (cudaStream_t)copy_stream;
   x->err[0] = 0;
   memset(&x->st, 0, sizeof(x->st));
+  memset(&x->pr, 0, sizeof(x->pr));
   memset(x->kv_h, 0, sizeof(x->kv_h));
   const m2r2_config& c = x->c;
   x->esz = c.dtype == M2R2_FP32 ? 4 : 2;
@@ -373,6 +409,7 @@ extern "C" int m2r2_destroy(m2r2_ctx* x) {
   if (x->ev_tmp) cudaEventDestroy(x->ev_tmp);
   if (x->ev_stage_free) cudaEventDestroy(x->ev_stage_free);
   if (x->h_pinned) cudaFreeHost(x->h_pinned);
+  for (auto e : x->pev) cudaEventDestroy(e);
   fused_destroy(&x->fs);
   delete x;
   return M2R2_OK;
@@ -571,6 +608,7 @@ static int exit_head(m2r2_ctx* x, int B, int ns, float* logits_out, int* tok_out
   const m2r2_config& c = x->c;
   const int d = c.d_model, V = c.vocab, r = c.adapter_rank;
   bool ad = x->lm_A != nullptr;
+  prof_mark(x, M2R2_PROF_HEAD);
   // norm only the accelerated rows [ns, ns+B)
   launch_norm_lora(x->cs, c.dtype, x->resid + (size_t)ns * d, B, d, x->gf, c.rms_eps, x->xn + (size_t)ns * d,
                    ad ? x->lm_A : nullptr, 1, r, 0, x->U + (size_t)ns * 64, 64);
@@ -595,6 +633,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   const int da = c.n_accel_heads * dh;
   const bool dual = p.mode == MODE_DUAL;
   const int ns = dual ? B : B * p.m;
+  prof_mark(x, M2R2_PROF_OTHER);
   setup_rows_kernel<<<B, 32, 0, x->cs>>>(p.mode, B, p.m, p.joff, p.c0, c.max_seq, x->d_kv_len, x->d_pending,
                                          x->d_drafts, p.use_force ? x->d_force : nullptr, x->d_prompt,
                                          x->d_row_tok, x->d_row_seq, x->d_row_pos, x->d_row_limit, x->d_grp_rows);
@@ -616,6 +655,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     char* Kc = (char*)x->b.kv + (size_t)i * c.max_batch * nh * c.max_seq * dh * x->esz;
     char* Vc = Kc + (size_t)c.n_layers * c.max_batch * nh * c.max_seq * dh * x->esz;
     // a2: RMSNorm + QKV (slow: all heads; accelerated: heads in S + adapters)
+    prof_mark(x, M2R2_PROF_QKV);
     launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g1, c.rms_eps, x->xn, acc_on ? L.Aqkv : nullptr, 3, r, ns, x->U, 64);
     GemvArgs g;
     memset(&g, 0, sizeof(g));
@@ -623,8 +663,10 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
     launch_gemv(x->cs, c.dtype, g, false);
     // a3: RoPE + KV append
+    prof_mark(x, M2R2_PROF_ROPE);
     launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
     // a4: split-K attention + merge
+    prof_mark(x, M2R2_PROF_ATTN);
     AttnArgs a;
     memset(&a, 0, sizeof(a));
     a.qkv = x->qkv; a.Kc = Kc; a.Vc = Vc; a.row_seq = x->d_row_seq; a.row_limit = x->d_row_limit;
@@ -647,6 +689,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     launch_merge(x->cs, mg, rows);
     count(x, 5);
     // a5: O-proj + residual
+    prof_mark(x, M2R2_PROF_OPROJ);
     if (acc_on) { launch_lora_down(x->cs, c.dtype, x->attn_o, d, ns, na, da, x->d_accel_cols, L.Ao, r, x->U, 64); count(x); }
     memset(&g, 0, sizeof(g));
     g.W = L.wo; g.X = x->attn_o; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
@@ -656,11 +699,13 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     float* trl = p.trace ? x->trace + (size_t)(i + 1) * 2 * B * d : nullptr;
     if (!c.n_experts) {
       // a6: RMSNorm + gate/up + SwiGLU;  a7: down + residual (accelerated-residual update)
+      prof_mark(x, M2R2_PROF_GATEUP);
       launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, acc_on ? L.Agu : nullptr, 2, r, ns, x->U, 64);
       memset(&g, 0, sizeof(g));
       g.W = L.wgate; g.W2 = L.wup; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = c.d_ff; g.out = x->act; g.ldo = c.d_ff;
       if (acc_on) { g.Bm = L.Bg; g.Bm2 = L.Bu; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
       launch_gemv(x->cs, c.dtype, g, true);
+      prof_mark(x, M2R2_PROF_DOWN);
       if (acc_on) { launch_lora_down(x->cs, c.dtype, x->act, c.d_ff, ns, na, c.d_ff, nullptr, L.Ad, r, x->U, 64); count(x); }
       memset(&g, 0, sizeof(g));
       g.W = L.wdown; g.X = x->act; g.ldx = c.d_ff; g.n_rows = rows; g.K = c.d_ff; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
@@ -673,6 +718,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       if (rc) return rc;
       if (trl) { launch_copy_rows(x->cs, x->resid, trl, rows, d); count(x); }
     }
+    prof_mark(x, M2R2_PROF_OTHER);
     if (trl && dual && !acc_on) { launch_copy_rows(x->cs, x->resid, trl + (size_t)B * d, B, d); count(x); }
     // gate: exit prediction on p (Eq. 4) then p <- h (L82, L101)
     if (acc_on) {
@@ -695,6 +741,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
 static int final_head(m2r2_ctx* x, int ns, int* tok_out, int tok_stride) {
   const m2r2_config& c = x->c;
   const int d = c.d_model, V = c.vocab;
+  prof_mark(x, M2R2_PROF_HEAD);
   launch_norm_lora(x->cs, c.dtype, x->resid, ns, d, x->gf, c.rms_eps, x->xn, nullptr, 0, 0, 0, x->U, 64);
   GemvArgs g;
   memset(&g, 0, sizeof(g));
@@ -716,7 +763,9 @@ static int expert_ffn(m2r2_ctx* x, const void* blob, int row, int n_rows, const 
   memset(&g, 0, sizeof(g));
   g.W = p; g.W2 = p + x->eg_bytes; g.X = x->xn + (size_t)row * d; g.ldx = d; g.n_rows = n_rows; g.K = d; g.n_out = F;
   g.out = x->act + (size_t)row * fmax_act(c); g.ldo = fmax_act(c);
+  prof_mark(x, M2R2_PROF_GATEUP);
   launch_gemv(x->cs, c.dtype, g, true);
+  prof_mark(x, M2R2_PROF_DOWN);
   memset(&g, 0, sizeof(g));
   g.W = p + 2 * x->eg_bytes; g.X = x->act + (size_t)row * fmax_act(c); g.ldx = fmax_act(c); g.n_rows = n_rows; g.K = F; g.n_out = d;
   g.ldo = d; g.scale = scale; g.scale_ld = scale_ld;
@@ -734,6 +783,7 @@ static int moe_mlp(m2r2_ctx* x, const Pass& p, int i, int ns, int na) {
   const DevLayer& L = x->L[i];
   const int d = c.d_model, tk = c.top_k, rows = ns + na;
   if (ns != 1) return fail(x, M2R2_UNSUPPORTED, "MoE layers run one slow row per pass (prefill streams experts separately)");
+  prof_mark(x, M2R2_PROF_OTHER);
   launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, nullptr, 0, 0, 0, x->U, 64);
   count(x);
   // accelerated rows: fixed adapter MLP  m^ = U_d (silu(U_g y^) * (U_u y^))   (L137, Q7)
@@ -904,6 +954,7 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
   x->st.algorithmic_bytes_last = bytes;
 
   if (x->fused && fused_supported(c, &x->fs) && B == 1) {
+    prof_mark(x, M2R2_PROF_FUSED_STEP);
     rc = fused_decode_step(c, &x->fs, x->cs, x->d_kv_len, x->d_pending, force_tokens ? x->d_force : nullptr,
                            x->kv_h[0], x->b.kv, x->trace, x->logits, x->exit_logits, x->d_out_tok, x->d_exit_tok,
                            x->ls_on ? x->d_ls_full : nullptr, x->ls_on ? x->d_ls_draft : nullptr, x->ls_first, x->ls_n,
@@ -917,6 +968,7 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
     advance_kernel<<<1, 32, 0, x->cs>>>(B, x->d_kv_len, x->d_pending, x->d_out_tok);
     count(x);
   }
+  prof_resolve(x);
   for (int b = 0; b < B; ++b) x->kv_h[b] += 1;
   x->st.steps++;
   x->st.emitted += B;
@@ -970,8 +1022,10 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
   }
   x->st.algorithmic_bytes_last = bytes;
   // a12: accept + rollback on the device
+  prof_mark(x, M2R2_PROF_OTHER);
   accept_kernel<<<1, 32, 0, x->cs>>>(B, k, x->d_drafts, x->d_vtok, x->d_accepted, x->d_nacc, x->d_kv_len, x->d_pending);
   count(x);
+  prof_resolve(x);
   CU(x, cudaMemcpyAsync(x->h_pinned, x->d_accepted, sizeof(int) * B * 8, cudaMemcpyDeviceToHost, x->cs));
   CU(x, cudaMemcpyAsync(x->h_pinned + 64, x->d_nacc, sizeof(int) * B, cudaMemcpyDeviceToHost, x->cs));
   CU(x, cudaStreamSynchronize(x->cs));
@@ -1240,6 +1294,19 @@ extern "C" int m2r2_debug_read(m2r2_ctx* x, int32_t what, int32_t layer, int32_t
 extern "C" int m2r2_set_fused(m2r2_ctx* x, int32_t enabled) {
   if (!x) return M2R2_INVALID_ARG;
   x->fused = enabled != 0;
+  return M2R2_OK;
+}
+
+extern "C" int m2r2_set_profile(m2r2_ctx* x, int32_t enabled) {
+  if (!x) return M2R2_INVALID_ARG;
+  x->prof = enabled != 0;
+  x->pn = 0;
+  if (x->prof) memset(&x->pr, 0, sizeof(x->pr));
+  return M2R2_OK;
+}
+extern "C" int m2r2_get_profile(m2r2_ctx* x, m2r2_profile* out) {
+  if (!x || !out) return M2R2_INVALID_ARG;
+  *out = x->pr;
   return M2R2_OK;
 }
 

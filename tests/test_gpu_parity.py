@@ -1,0 +1,410 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, element by element on the same
+seeded inputs.  Tolerances are BASELINE.json's: integer work bit-exact (except where the ORACLE's
+top-2 margin < 1e-3), fp32 tiny config rel-L2 <= 1e-4, bf16 hidden rel-L2 <= 1e-2 and logits
+max-abs <= 5e-2.  Every test here needs a B200 and fails loudly without one."""
+import numpy as np
+import pytest
+
+import m2r2_synth as S
+import paper_2502_02040_b200 as M
+from oracle import Oracle
+from tests.parity import MARGIN, check_logits, compare_decode_step, tolerances
+from tests.refs import rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _require_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests selected without a CUDA device: refusing to skip silently"
+    cap = torch.cuda.get_device_capability(0)
+    assert cap[0] == 10, "libm2r2.so holds sm_100a code only; found sm_%d%d" % cap
+
+
+def _pair(cfg, W=None, exit_heads=True):
+    W = W if W is not None else S.gen_weights(cfg)
+    return M.Engine(cfg, W, exit_heads=exit_heads), Oracle(cfg, W), W
+
+
+def _decode_parity(cfg, P, n_steps, W=None, check_kv=True):
+    eng, orc, W = _pair(cfg, W)
+    prompt = S.gen_prompt(cfg, P)
+    fo = orc.prefill(prompt)
+    fe = int(eng.prefill(prompt)[0])
+    check_logits(cfg, eng.debug_read(M.DBG_LOGITS, (P - 1) % 8), orc.logits(), "prefill logits")
+    assert fe == fo or orc.margin() < MARGIN
+    worst = 0.0
+    for s in range(n_steps):
+        tok_in = orc.pending
+        to, exo = orc.decode_step()
+        te, exe = eng.decode_step(force_tokens=[tok_in], want_exit=True)   # teacher forcing (Q23)
+        worst = max(worst, compare_decode_step(cfg, eng, orc, M))
+        assert int(te[0]) == to or orc.margin() < MARGIN, (s, te, to, orc.margin())
+        for j in range(len(cfg.gates)):
+            if cfg.gates[j] <= cfg.accel_end_layer:
+                check_logits(cfg, eng.debug_read(M.DBG_EXIT_LOGITS, j), orc.exit_logits(j), "exit logits %d" % j)
+                top2 = np.sort(orc.exit_logits(j))[-2:]
+                assert int(exe[0][j]) == int(exo[j]) or top2[1] - top2[0] < MARGIN
+        assert eng.get_stats()["kv_len"][0] == orc.kv_len
+    if check_kv:
+        T = orc.kv_len
+        tol = 0 if cfg.dtype == S.FP32 else 1e-2
+        for i in range(cfg.n_layers):
+            for v in (False, True):
+                got = eng.kcache(i, T, v=v)
+                want = (orc.vcache(i) if v else orc.kcache(i))[:T]
+                assert rel_l2(got, want) <= max(tol, 1e-5), (i, v, rel_l2(got, want))
+    eng.close()
+    return worst
+
+
+def test_c1_dual_stream_decode_matches_oracle():
+    """BASELINE configs[0]: prefill 32 then 32 decode steps; h_i, p_i, logits, tokens, exit tokens, KV."""
+    worst = _decode_parity(S.config_c1(), 32, 32)
+    assert worst <= 1e-4
+
+
+def test_c1_tokens_equal_golden_greedy_stream():
+    """Free-running (no teacher forcing) greedy decode on the GPU reproduces the oracle-written
+    golden token stream (tests/golden/c1_tokens.txt) unless an oracle margin is < 1e-3."""
+    import os
+    cfg = S.config_c1()
+    gold = [int(t) for t in open(os.path.join(os.path.dirname(__file__), "golden", "c1_tokens.txt")).read().split("\n")[2].split()]
+    eng, orc, _ = _pair(cfg)
+    prompt = S.gen_prompt(cfg, 32)
+    toks = [int(eng.prefill(prompt)[0])]
+    orc.prefill(prompt)
+    ok = orc.margin() >= MARGIN
+    for _ in range(31):
+        toks.append(int(eng.decode_step()[0]))
+        orc.decode_step()
+        ok = ok and orc.margin() >= MARGIN
+        if not ok:
+            break
+    n = len(toks)
+    assert toks[:n - (0 if ok else 1)] == gold[:n - (0 if ok else 1)]
+    eng.close()
+
+
+@pytest.mark.parametrize("P", [1, 7, 37])
+def test_small_bf16_decode_matches_oracle(P):
+    """bf16 storage, head_dim 96, ragged sizes (d_ff 1000, vocab 3001), two gates; short/ragged prompts."""
+    worst = _decode_parity(S.config_small_bf16(), P, 6)
+    assert worst <= 1e-2
+
+
+def test_accel_disabled_matches_oracle_and_h_is_unchanged():
+    """I2 on the GPU: the slow stream with the accelerated stream on equals the slow stream with it off."""
+    cfg_on = S.config_small_bf16()
+    cfg_off = S.config_small_bf16(accel_enabled=False, gates=(), accel_end_layer=0)
+    W = S.gen_weights(cfg_on)
+    e_on, e_off = M.Engine(cfg_on, W), M.Engine(cfg_off, W)
+    prompt = S.gen_prompt(cfg_on, 19)
+    assert e_on.prefill(prompt)[0] == e_off.prefill(prompt)[0]
+    for _ in range(4):
+        a, b = e_on.decode_step(), e_off.decode_step()
+        assert a[0] == b[0]
+        for i in range(cfg_on.n_layers + 1):
+            assert np.array_equal(e_on.debug_read(M.DBG_H, i), e_off.debug_read(M.DBG_H, i))
+    e_on.close()
+    e_off.close()
+
+
+def test_gate_reset_and_zero_adapter_invariants_on_gpu():
+    """I3/I4 on the GPU: with zero adapters and S = all heads, p_i == h_i (to fp32 rounding)."""
+    cfg = S.config_small_bf16(accel_heads=(0, 1, 2, 3))
+    W = S.gen_weights(cfg)
+    S.zero_adapters(cfg, W)
+    eng = M.Engine(cfg, W)
+    eng.prefill(S.gen_prompt(cfg, 9))
+    eng.decode_step()
+    for i in range(cfg.n_layers + 1):
+        assert rel_l2(eng.debug_read(M.DBG_P, i), eng.debug_read(M.DBG_H, i)) <= 2e-6, i
+    eng.close()
+
+
+# ------------------------------------------------------------------ self-speculative decoding
+@pytest.mark.parametrize("gamma", [0, 1, 3, 6])
+def test_c1_selfspec_matches_oracle_and_is_lossless(gamma):
+    """a10-a12: accepted tokens, accepted lengths, kv_len bit-exact vs the oracle; emitted stream ==
+    plain greedy stream (lossless)."""
+    cfg = S.config_c1()
+    eng, orc, W = _pair(cfg)
+    plain = Oracle(cfg, W)
+    prompt = S.gen_prompt(cfg, 32)
+    first = orc.prefill(prompt)
+    assert int(eng.prefill(prompt)[0]) == first
+    stream_plain = [plain.prefill(prompt)]
+    emitted = [first]
+    tie = False
+    while len(emitted) < 33:
+        acc_o, _ = orc.spec_step(gamma)
+        tie = tie or orc.margin() < MARGIN or orc.draft_margin() < MARGIN
+        acc_e, n_e = eng.spec_step(gamma)
+        if tie:
+            break
+        assert acc_e[0][:n_e[0]].tolist() == acc_o
+        assert (acc_e[0][n_e[0]:] == -1).all()
+        assert eng.get_stats()["kv_len"][0] == orc.kv_len
+        check_logits(cfg, eng.debug_read(M.DBG_LOGITS, gamma), orc.logits(), "verify logits row gamma")
+        emitted += acc_o
+    while len(stream_plain) < len(emitted):
+        stream_plain.append(plain.decode_step()[0])
+    if not tie:
+        assert emitted == stream_plain[:len(emitted)]
+    st = eng.get_stats()
+    so = orc.stats()
+    if not tie:
+        assert (st["drafted"], st["accepted"], st["emitted"]) == (so["drafted"], so["accepted"], so["emitted"])
+    eng.close()
+
+
+@pytest.mark.parametrize("alpha", [0.5, 0.9])
+@pytest.mark.parametrize("gamma", [2, 4, 6])
+def test_bf16_selfspec_closed_form_acceptance(alpha, gamma):
+    """I10 on the GPU: under the logit script the accepted lengths are computable from the seed
+    alone: n_accepted - 1 = min(gamma, first j with g != f); kv_len is the running sum; the
+    emitted stream is exactly f.  Then KV[0..kv_len) equals the oracle's after rollback (I8)."""
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2, lm_head_adapter=True)
+    eng, orc, _ = _pair(cfg)
+    P, n_script = 21, 120
+    f, g = S.gen_logit_script(cfg, n_script, alpha)
+    prompt = S.gen_prompt(cfg, P)
+    eng.set_logit_script(f, g, P)
+    orc.set_logit_script(f, g, P)
+    assert int(eng.prefill(prompt)[0]) == f[0] == orc.prefill(prompt)
+    pos = P          # position of the pending token
+    emitted = 1
+    while emitted + gamma + 1 < 100:
+        acc_e, n_e = eng.spec_step(gamma)
+        acc_o, _ = orc.spec_step(gamma)
+        n = int(n_e[0])
+        a = 0
+        while a < gamma and g[pos + 1 + a - P] == f[pos + 1 + a - P]:
+            a += 1
+        assert n == a + 1 == len(acc_o)
+        assert acc_e[0][:n].tolist() == f[pos + 1 - P: pos + 1 - P + n].tolist() == acc_o
+        pos += n
+        emitted += n
+        assert eng.get_stats()["kv_len"][0] == pos == orc.kv_len
+    for i in range(cfg.n_layers):
+        assert rel_l2(eng.kcache(i, pos), orc.kcache(i)[:pos]) <= 1e-2
+        assert rel_l2(eng.kcache(i, pos, v=True), orc.vcache(i)[:pos]) <= 1e-2
+    # continuing with plain decode after rollback reproduces the scripted stream
+    for _ in range(3):
+        t = int(eng.decode_step()[0])
+        assert t == f[pos + 1 - P]
+        pos += 1
+    eng.close()
+
+
+def test_spec_step_zero_equals_decode_step_on_gpu():
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2)
+    W = S.gen_weights(cfg)
+    a, b = M.Engine(cfg, W), M.Engine(cfg, W)
+    prompt = S.gen_prompt(cfg, 11)
+    a.prefill(prompt)
+    b.prefill(prompt)
+    for _ in range(3):
+        ta = int(a.decode_step()[0])
+        acc, n = b.spec_step(0)
+        assert n[0] == 1 and int(acc[0][0]) == ta
+        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= 1e-5
+    a.close()
+    b.close()
+
+
+# ------------------------------------------------------------------ batch (C4 structure, reduced)
+def test_batched_selfspec_per_sequence_divergence():
+    """B=3 sequences, per-sequence scripts => per-sequence accepted lengths and kv_len diverge; each
+    sequence must equal its own single-sequence oracle."""
+    B, P, gamma = 3, 13, 4
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2, lm_head_adapter=True, max_batch=B)
+    W = S.gen_weights(cfg)
+    eng = M.Engine(cfg, W)
+    orcs = [Oracle(cfg, W) for _ in range(B)]
+    prompts = np.stack([S.gen_prompt(cfg, P, seq=b) for b in range(B)])
+    scripts = [S.gen_logit_script(cfg, 80, 0.7, seq=b) for b in range(B)]
+    eng.set_logit_script(np.stack([s[0] for s in scripts]), np.stack([s[1] for s in scripts]), P)
+    for b in range(B):
+        orcs[b].set_logit_script(scripts[b][0], scripts[b][1], P)
+    first = eng.prefill(prompts)
+    for b in range(B):
+        assert int(first[b]) == orcs[b].prefill(prompts[b])
+    for _ in range(8):
+        acc, n = eng.spec_step(gamma)
+        kv = eng.get_stats()["kv_len"]
+        for b in range(B):
+            ao, _ = orcs[b].spec_step(gamma)
+            assert acc[b][:n[b]].tolist() == ao, (b, acc[b], ao)
+            assert kv[b] == orcs[b].kv_len
+    assert len(set(eng.get_stats()["kv_len"])) > 1, "scripts should make kv_len diverge"
+    for b in range(B):
+        T = orcs[b].kv_len
+        assert rel_l2(eng.kcache(0, T, b=b), orcs[b].kcache(0)[:T]) <= 1e-2
+        assert rel_l2(eng.kcache(cfg.n_layers - 1, T, b=b, v=True), orcs[b].vcache(cfg.n_layers - 1)[:T]) <= 1e-2
+    eng.close()
+
+
+def test_batched_decode_hidden_states_per_sequence():
+    B, P = 4, 10
+    cfg = S.config_small_bf16(max_batch=B)
+    W = S.gen_weights(cfg)
+    eng = M.Engine(cfg, W)
+    orcs = [Oracle(cfg, W) for _ in range(B)]
+    prompts = np.stack([S.gen_prompt(cfg, P, seq=b) for b in range(B)])
+    eng.prefill(prompts)
+    for b in range(B):
+        orcs[b].prefill(prompts[b])
+    for _ in range(3):
+        forced = [orcs[b].pending for b in range(B)]
+        for b in range(B):
+            orcs[b].decode_step()
+        eng.decode_step(force_tokens=forced)
+        for b in range(B):
+            compare_decode_step(cfg, eng, orcs[b], M, b=b)
+    eng.close()
+
+
+# ------------------------------------------------------------------ MoE + ahead-of-time expert loading
+def _moe_pair(cfg):
+    eng = M.Engine(cfg)
+    W = S.gen_weights(cfg, expert_alloc=eng.pinned_expert_alloc())
+    eng.load_weights(W)
+    return eng, Oracle(cfg, W), W
+
+
+@pytest.mark.parametrize("policy", [M.POLICY_FIXED, M.POLICY_LRU, M.POLICY_LRU_AOT])
+def test_small_moe_decode_matches_oracle(policy):
+    """a13-a17: hidden states, routed / predicted expert indices, router weights and the cache counters
+    (hits, misses, prefetched, on-demand) equal the oracle's logical LRU model (I15), natural routing."""
+    cfg = S.config_small_moe()
+    eng, orc, _ = _moe_pair(cfg)
+    eng.set_policy(policy)
+    orc.set_policy(policy)
+    prompt = S.gen_prompt(cfg, 12)
+    assert int(eng.prefill(prompt)[0]) == orc.prefill(prompt) or orc.margin() < MARGIN
+    for s in range(10):
+        tok_in = orc.pending
+        orc.decode_step()
+        eng.decode_step(force_tokens=[tok_in])
+        compare_decode_step(cfg, eng, orc, M)
+        ri = eng.debug_read(M.DBG_ROUTE_IDX).reshape(cfg.n_layers, cfg.top_k).astype(np.int32)
+        assert np.array_equal(ri, orc.route_idx()), (s, ri, orc.route_idx())
+        assert np.allclose(eng.debug_read(M.DBG_ROUTE_W).reshape(cfg.n_layers, cfg.top_k), orc.route_w(), atol=2e-3)
+        if policy == M.POLICY_LRU_AOT:
+            pi = eng.debug_read(M.DBG_PRED_IDX).reshape(cfg.n_layers, cfg.top_k).astype(np.int32)
+            po = orc.pred_idx()
+            mask = po >= 0
+            assert np.array_equal(pi[mask], po[mask]), (s, pi, po)
+        st, so = eng.get_stats(), orc.stats()
+        assert (st["expert_hits"], st["expert_misses"], st["expert_prefetched"], st["expert_on_demand"]) == \
+               (so["expert_hits"], so["expert_misses"], so["prefetched"], so["on_demand"]), (s, st, so)
+    one = 3 * cfg.d_ff_expert * cfg.d_model * 2
+    st = eng.get_stats()
+    assert st["h2d_bytes"] == (st["expert_prefetched"] + st["expert_on_demand"]) * one
+    eng.close()
+
+
+@pytest.mark.parametrize("rho,pi", [(0.25, 0.9), (0.0, 1.0)])
+def test_small_moe_router_script_counters(rho, pi):
+    """Scripted routing (seeded 'random logits', BASELINE configs[4]): with pi = 1 every targeted layer
+    has zero misses; counters equal the oracle's; output h does not depend on the policy (I14)."""
+    cfg = S.config_small_moe()
+    eng, orc, _ = _moe_pair(cfg)
+    P, n = 8, 24
+    act, pred = S.gen_router_script(cfg, n + P + 1, rho, pi)
+    eng.set_policy(M.POLICY_LRU_AOT)
+    orc.set_policy(2)
+    eng.set_router_script(act, pred, 0)
+    orc.set_router_script(act, pred, 0)
+    prompt = S.gen_prompt(cfg, P)
+    eng.prefill(prompt)
+    orc.prefill(prompt)
+    for s in range(n):
+        tok_in = orc.pending
+        orc.decode_step()
+        eng.decode_step(force_tokens=[tok_in])
+        ri = eng.debug_read(M.DBG_ROUTE_IDX).reshape(cfg.n_layers, cfg.top_k).astype(np.int32)
+        assert np.array_equal(ri, act[P + s]), (s, ri, act[P + s])
+    compare_decode_step(cfg, eng, orc, M)
+    st, so = eng.get_stats(), orc.stats()
+    assert (st["expert_hits"], st["expert_misses"], st["expert_prefetched"], st["expert_on_demand"]) == \
+           (so["expert_hits"], so["expert_misses"], so["prefetched"], so["on_demand"])
+    assert st["expert_hits"] + st["expert_misses"] == cfg.top_k * cfg.n_layers * n
+    eng.close()
+
+
+def test_moe_explicit_prefetch_pairs_then_hits():
+    """m2r2_moe_prefetch(pairs): prefetching exactly the experts the script will route makes them hits."""
+    cfg = S.config_small_moe()
+    eng, _, _ = _moe_pair(cfg)
+    P = 5
+    act, _ = S.gen_router_script(cfg, P + 4, 0.0, 1.0)
+    eng.set_policy(M.POLICY_LRU)
+    eng.set_router_script(act, act, 0)
+    eng.prefill(S.gen_prompt(cfg, P))
+    pairs = [(L, int(e)) for L in range(cfg.n_layers) for e in act[P][L]]
+    n = eng.moe_prefetch(pairs=pairs)
+    assert 0 <= n <= len(pairs)
+    eng.decode_step()
+    st = eng.get_stats()
+    assert st["expert_misses"] == 0 and st["expert_hits"] == cfg.top_k * cfg.n_layers
+    assert st["expert_prefetched"] == n
+    eng.close()
+
+
+# ------------------------------------------------------------------ error behaviour on a live context
+def test_error_codes_on_live_context():
+    cfg = S.config_c1()
+    eng = M.Engine(cfg, S.gen_weights(cfg))
+    with pytest.raises(M.M2R2Error) as e:
+        eng.B = 1
+        eng.decode_step()
+    assert e.value.code == M.BAD_STATE
+    with pytest.raises(M.M2R2Error) as e:
+        eng.prefill(np.full(4, cfg.vocab, dtype=np.int32))
+    assert e.value.code == M.INVALID_ARG
+    with pytest.raises(M.M2R2Error) as e:
+        eng.prefill(np.zeros(cfg.max_seq + 1, dtype=np.int32))
+    assert e.value.code == M.INVALID_ARG
+    eng.prefill(S.gen_prompt(cfg, cfg.max_seq - 2))
+    with pytest.raises(M.M2R2Error) as e:
+        eng.spec_step(3)
+    assert e.value.code == M.CAPACITY
+    kv = eng.get_stats()["kv_len"][0]
+    eng.decode_step()
+    eng.decode_step()
+    assert eng.get_stats()["kv_len"][0] == kv + 2 == cfg.max_seq
+    with pytest.raises(M.M2R2Error) as e:
+        eng.decode_step()
+    assert e.value.code == M.CAPACITY
+    with pytest.raises(M.M2R2Error) as e:
+        eng.spec_step(8)
+    assert e.value.code == M.INVALID_ARG
+    with pytest.raises(M.M2R2Error) as e:
+        eng.moe_prefetch(0)
+    assert e.value.code == M.UNSUPPORTED
+    eng.close()
+
+
+def test_dead_positions_do_not_leak_after_rollback():
+    """I8 on the GPU: K/V at positions >= kv_len are dead: running a spec step that rejects drafts and
+    then decoding gives the same tokens as an engine that never drafted."""
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2)
+    W = S.gen_weights(cfg)
+    a, b = M.Engine(cfg, W), M.Engine(cfg, W)
+    P = 17
+    f, g = S.gen_logit_script(cfg, 60, 0.0)      # alpha = 0: every draft is rejected
+    for e in (a, b):
+        e.set_logit_script(f, g, P)
+        e.prefill(S.gen_prompt(cfg, P))
+    for s in range(5):
+        acc, n = a.spec_step(5)
+        assert n[0] == 1
+        t = b.decode_step()
+        assert int(acc[0][0]) == int(t[0]) == f[s + 1]
+        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= 1e-5
+    a.close()
+    b.close()
