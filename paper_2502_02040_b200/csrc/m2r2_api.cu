@@ -949,7 +949,7 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
   }
   int64_t bytes = 0;
   for (int i = 0; i < c.n_layers; ++i)
-    for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + 1) * x->esz;
+    for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + 1 + 1) * x->esz;   // read T+1, append 1
   bytes += (int64_t)c.vocab * c.d_model * x->esz * (1 + (c.exit_heads_enabled ? c.n_gates : 0)) + (int64_t)c.d_model * x->esz * B;
   x->st.algorithmic_bytes_last = bytes;
 
@@ -1004,7 +1004,7 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
     rc = run_pass(x, p);
     if (rc) return rc;
     for (int i = 0; i < E; ++i)
-      for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + j + 1) * x->esz;
+      for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + j + 1 + 1) * x->esz;
     bytes += (int64_t)c.vocab * c.d_model * x->esz;
   }
   // a11: k+1-token verify pass, slow stream, all layers
@@ -1017,7 +1017,7 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
     for (int b = 0; b < B; ++b)
       CU(x, cudaMemcpyAsync(x->d_vtok + b * 8, x->d_accepted + b * (k + 1), sizeof(int) * (k + 1), cudaMemcpyDeviceToDevice, x->cs));
     for (int i = 0; i < c.n_layers; ++i)
-      for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, false, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + k + 1) * x->esz;
+      for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, false, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + k + 1 + k + 1) * x->esz;
     bytes += (int64_t)c.vocab * c.d_model * x->esz;
   }
   x->st.algorithmic_bytes_last = bytes;

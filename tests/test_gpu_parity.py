@@ -112,15 +112,18 @@ def test_accel_disabled_matches_oracle_and_h_is_unchanged():
 
 
 def test_gate_reset_and_zero_adapter_invariants_on_gpu():
-    """I3/I4 on the GPU: with zero adapters and S = all heads, p_i == h_i (to fp32 rounding)."""
-    cfg = S.config_small_bf16(accel_heads=(0, 1, 2, 3))
+    """I3/I4 on the GPU: with zero adapters and S = all heads, p_i == h_i (to fp32 rounding).
+    Run with fp32 storage: with a bf16 cache the slow stream reads its own K[t], V[t] back
+    ROUNDED while p keeps k^_t, v^_t in fp32 (Q20), so the identity only holds to
+    bf16 rounding there."""
+    cfg = S.config_small_bf16(accel_heads=(0, 1, 2, 3), dtype=S.FP32)
     W = S.gen_weights(cfg)
     S.zero_adapters(cfg, W)
     eng = M.Engine(cfg, W)
     eng.prefill(S.gen_prompt(cfg, 9))
     eng.decode_step()
     for i in range(cfg.n_layers + 1):
-        assert rel_l2(eng.debug_read(M.DBG_P, i), eng.debug_read(M.DBG_H, i)) <= 2e-6, i
+        assert rel_l2(eng.debug_read(M.DBG_P, i), eng.debug_read(M.DBG_H, i)) <= 1e-5, i
     eng.close()
 
 
