@@ -88,6 +88,7 @@ struct m2r2_ctx {
   size_t esz = 0;              // bytes per element
   // resident weights
   const void *embed = nullptr, *gf = nullptr, *lm_head = nullptr, *lm_A = nullptr, *lm_B = nullptr;
+  void* packed = nullptr;      // tile-major copy of the big matrices for the fused kernel
   std::vector<DevLayer> L;
   // MoE
   std::vector<std::vector<const void*>> eg, eu, ed;   // pinned host blobs [layer][expert]
@@ -254,6 +255,11 @@ static void walk_weights(const m2r2_config& c, WeightWalk& w, m2r2_ctx* ctx) {
     }
     if (ctx) ctx->L.push_back(L);
   }
+  size_t fb = fused_weights_bytes(c);
+  if (fb) {
+    void* pk = w.cv.take<char>(fb);
+    if (ctx) ctx->packed = pk;
+  }
 }
 
 static void carve_scratch(const m2r2_config& c, Carver& cv, m2r2_ctx* x) {
@@ -332,6 +338,8 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
   x->R = c.max_batch * 8;
   WeightWalk w(bufs->weights, x->esz);
   walk_weights(c, w, x);
+  rc = fused_create(c, &x->fs);   // before the carve: the fused scratch pointers land in fs.impl
+  if (rc) { delete x; return rc; }
   Carver cv(bufs->scratch);
   carve_scratch(c, cv, x);
   memset(x->accel_mask, 0, sizeof(x->accel_mask));
@@ -342,6 +350,7 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
     cudaError_t e_ = (call);                                                          \
     if (e_ != cudaSuccess) {                                                          \
       fprintf(stderr, "m2r2_create: %s: %s\n", #call, cudaGetErrorString(e_));        \
+      fused_destroy(&x->fs);                                                          \
       delete x;                                                                       \
       return M2R2_CUDA;                                                               \
     }                                                                                 \
@@ -392,8 +401,6 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
       CUX(cudaEventCreateWithFlags(&x->ev_copy_done[i], cudaEventDisableTiming));
     }
   }
-  rc = fused_create(c, &x->fs);
-  if (rc) { delete x; return rc; }
 #undef CUX
   *out = x;
   return M2R2_OK;
@@ -508,8 +515,9 @@ extern "C" int m2r2_load_weights(m2r2_ctx* x, const m2r2_weight_table* t) {
   x->weights_loaded = true;
   rc = reset_expert_cache(x);
   if (rc) return rc;
-  rc = fused_bind(x->c, &x->fs, x->embed, x->gf, x->lm_head, x->L.data(), sizeof(DevLayer));
-  if (rc) return fail(x, rc, "fused_bind failed");
+  rc = fused_bind(x->c, &x->fs, x->cs, x->packed, x->embed, x->gf, x->lm_head, x->lm_A, x->lm_B, x->L.data(), x->b.kv,
+                  x->rope_tab);
+  if (rc) return fail(x, rc, "fused_bind failed: %s", cudaGetErrorString(cudaGetLastError()));
   return m2r2_reset(x);
 }
 
@@ -953,13 +961,14 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
   bytes += (int64_t)c.vocab * c.d_model * x->esz * (1 + (c.exit_heads_enabled ? c.n_gates : 0)) + (int64_t)c.d_model * x->esz * B;
   x->st.algorithmic_bytes_last = bytes;
 
-  if (x->fused && fused_supported(c, &x->fs) && B == 1) {
+  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1;
+  if (use_fused) {
     prof_mark(x, M2R2_PROF_FUSED_STEP);
-    rc = fused_decode_step(c, &x->fs, x->cs, x->d_kv_len, x->d_pending, force_tokens ? x->d_force : nullptr,
-                           x->kv_h[0], x->b.kv, x->trace, x->logits, x->exit_logits, x->d_out_tok, x->d_exit_tok,
-                           x->ls_on ? x->d_ls_full : nullptr, x->ls_on ? x->d_ls_draft : nullptr, x->ls_first, x->ls_n,
-                           x->ls_beta, &x->st.kernel_launches);
-    if (rc) return fail(x, rc, "fused decode step failed: %s", cudaGetErrorString(cudaGetLastError()));
+    FusedRun fr = {c.n_layers, 0, force_tokens ? x->d_force : x->d_pending, 0, x->d_out_tok, 1, c.exit_heads_enabled, 1};
+    rc = fused_run(c, &x->fs, x->cs, fr, x->d_kv_len, x->d_pending, x->kv_h[0], x->trace, x->logits, x->exit_logits,
+                   x->d_exit_tok, x->ls_on ? x->d_ls_full : nullptr, x->ls_on ? x->d_ls_draft : nullptr, x->ls_first,
+                   x->ls_n, x->ls_beta, &x->st.kernel_launches);
+    if (rc) return fail(x, rc, "fused decode launch failed: %s", cudaGetErrorString(cudaGetLastError()));
   } else {
     Pass p = {MODE_DUAL, 1, 0, 0, c.n_layers, true, true, force_tokens != nullptr, true, false};
     rc = run_pass(x, p);
@@ -979,6 +988,7 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
       CU(x, cudaMemcpyAsync(x->h_pinned + 64, x->d_exit_tok, sizeof(int) * B * c.n_gates, cudaMemcpyDeviceToHost, x->cs));
     CU(x, cudaStreamSynchronize(x->cs));
     CU(x, cudaGetLastError());
+    if (use_fused && (rc = fused_check(&x->fs, x->cs, x->err, sizeof(x->err)))) return rc;
     if (tokens_out) memcpy(tokens_out, x->h_pinned, sizeof(int) * B);
     if (exit_tokens_out && c.n_gates) memcpy(exit_tokens_out, x->h_pinned + 64, sizeof(int) * B * c.n_gates);
   }
@@ -999,10 +1009,20 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
     if (x->kv_h[b] + k + 1 > c.max_seq) return fail(x, M2R2_CAPACITY, "kv cache full");
   int64_t bytes = 0;
   // a10: draft loop — k dependent passes of layers 0..E-1 (both streams) + draft head
+  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1;
   for (int j = 0; j < k; ++j) {
-    Pass p = {MODE_DUAL, 1, j, 0, E, true, false, false, true, true};
-    rc = run_pass(x, p);
-    if (rc) return rc;
+    if (use_fused) {
+      prof_mark(x, M2R2_PROF_FUSED_STEP);
+      FusedRun fr = {E, j, j == 0 ? x->d_pending : x->d_drafts + (j - 1), 1, x->d_drafts + j, 0, 0, 0};
+      rc = fused_run(c, &x->fs, x->cs, fr, x->d_kv_len, x->d_pending, x->kv_h[0], x->trace, x->logits, x->exit_logits,
+                     x->d_exit_tok, x->ls_on ? x->d_ls_full : nullptr, x->ls_on ? x->d_ls_draft : nullptr, x->ls_first,
+                     x->ls_n, x->ls_beta, &x->st.kernel_launches);
+      if (rc) return fail(x, rc, "fused draft launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+    } else {
+      Pass p = {MODE_DUAL, 1, j, 0, E, true, false, false, true, true};
+      rc = run_pass(x, p);
+      if (rc) return rc;
+    }
     for (int i = 0; i < E; ++i)
       for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + j + 1 + 1) * x->esz;
     bytes += (int64_t)c.vocab * c.d_model * x->esz;
@@ -1030,6 +1050,7 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
   CU(x, cudaMemcpyAsync(x->h_pinned + 64, x->d_nacc, sizeof(int) * B, cudaMemcpyDeviceToHost, x->cs));
   CU(x, cudaStreamSynchronize(x->cs));
   CU(x, cudaGetLastError());
+  if (use_fused && k > 0 && (rc = fused_check(&x->fs, x->cs, x->err, sizeof(x->err)))) return rc;
   for (int b = 0; b < B; ++b) {
     int n = x->h_pinned[64 + b];
     n_accepted[b] = n;

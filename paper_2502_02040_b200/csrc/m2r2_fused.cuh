@@ -1,19 +1,45 @@
 // m2r2_fused.cuh — interface of the persistent fused decode kernel (kernels_fused.cu).
+//
+// One cooperative launch per decode step (or per draft pass): one CTA per SM, a producer
+// thread streaming tile-major bf16 weight stages through a shared-memory ring with bulk
+// async copies (cp.async.bulk + mbarrier), eight consumer warps doing the dual-row
+// (slow h / accelerated p) dot products, grid barriers between the phases of a layer.
+// DESIGN.md §"Fused decode kernel" has the layout and the phase list.
 #pragma once
 #include "m2r2_internal.cuh"
 
+struct FusedImpl;
 struct FusedState {
   bool supported = false;
-  void* impl = nullptr;
+  FusedImpl* impl = nullptr;
 };
 
+// what one launch runs
+struct FusedRun {
+  int n_layers;            // layers [0, n_layers)
+  int joff;                // position = kv_len + joff (draft loop); 0 for decode_step
+  const int* tok_in;       // device: token consumed by this pass
+  int head_stream;         // 0: final head on h_N (decode_step); 1: draft head on p at the gate == n_layers
+  int* tok_out;            // device: greedy token of the head
+  int advance;             // kv_len += 1, pending = token (decode_step)
+  int exit_heads;          // evaluate the exit argmax at every gate <= n_layers (decode_step)
+  int trace;               // write h_i / p_i traces
+};
+
+// bytes of the tile-major weight region the fused path needs inside the weights buffer (0 if unsupported)
+size_t fused_weights_bytes(const m2r2_config& c);
+bool fused_config_ok(const m2r2_config& c);
 void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs);
 int fused_create(const m2r2_config& c, FusedState* fs);
 void fused_destroy(FusedState* fs);
-int fused_bind(const m2r2_config& c, FusedState* fs, const void* embed, const void* gf, const void* lm_head,
-               const DevLayer* layers, size_t layer_stride);
+// repack the row-major resident weights (already in HBM) into the tile-major stage stream at `packed`
+int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* packed, const void* embed,
+               const void* gf, const void* lm_head, const void* lm_A, const void* lm_B,
+               const DevLayer* layers, void* kv, const float2* rope_tab);
 bool fused_supported(const m2r2_config& c, const FusedState* fs);
-int fused_decode_step(const m2r2_config& c, FusedState* fs, cudaStream_t st, int* d_kv_len, int* d_pending,
-                      const int* d_force, int kv_len_host, void* kv, float* trace, float* logits,
-                      float* exit_logits, int* d_out_tok, int* d_exit_tok, const int* ls_full,
-                      const int* ls_draft, int ls_first, int ls_n, float ls_beta, int64_t* launches);
+int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const FusedRun& run, int* d_kv_len,
+              int* d_pending, int kv_len_host, float* trace, float* logits, float* exit_logits,
+              int* d_exit_tok, const int* ls_full, const int* ls_draft, int ls_first, int ls_n,
+              float ls_beta, int64_t* launches);
+// 0 if the last launches completed normally; otherwise a description (device-side timeout)
+int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n);
