@@ -18,6 +18,7 @@
 // row-block): partial sums go to a fixed slot, the LAST contributor (atomic ticket) adds the slots
 // in slot order and runs the phase epilogue, so results are deterministic.
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -90,6 +91,7 @@ struct FParams {
   int ls_first, ls_n;
   float ls_beta;
   int ns;   // attention splits
+  u64* tl;  // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
 };
 
 // ------------------------------------------------------------------ PTX helpers
@@ -155,6 +157,14 @@ __device__ __forceinline__ u64 amax_key(float v, int n) {
 __device__ __forceinline__ int range_lo(int S, int v, int G) { return (int)(((long long)S * v) / G); }
 __device__ __forceinline__ int stage_owner(int S, int s, int G) { return (int)((((long long)(s + 1)) * G + S - 1) / S) - 1; }
 __device__ __forceinline__ int phase_rot(int layer, int ph, int G) { return (int)(((unsigned)(layer * 5 + ph) * 29u) % (unsigned)G); }
+
+#ifdef M2R2_FUSED_DEBUG
+constexpr int TL_MAX = 1024;
+__device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TL(ev) do { if (P.tl && threadIdx.x == 0 && tl_n < TL_MAX) { P.tl[(size_t)blockIdx.x * TL_MAX + tl_n] = (gtime() << 8) | (u64)(ev); ++tl_n; } } while (0)
+#else
+#define TL(ev) do { } while (0)
+#endif
 
 struct Smem {
   unsigned char* ring;
@@ -451,8 +461,8 @@ struct GemvDesc {
   int kpad8;          // kpad / 8
 };
 
-__device__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd, const PhaseCtx& pc0, int G,
-                           unsigned int& stage_ctr, float* part, int* cnt) {
+__device__ __noinline__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd, const PhaseCtx& pc0, int G,
+                                        unsigned int& stage_ctr, float* part, int* cnt, int& tl_n) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int S = gd.n_rb * gd.n_kc;
   const int rot = phase_rot(pc0.layer, pc0.ph, G);
@@ -488,6 +498,7 @@ __device__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd,
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.empty[slot]);   // stage consumed by this warp
+    TL(40);
     if (kc == gd.n_kc - 1 || s == s1 - 1) {
       // ---- end of this CTA's segment of row-block rb: reduce over lanes (16 values, butterfly)
       float v16[16];
@@ -528,9 +539,6 @@ __device__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd,
       const int myslot = S >= G ? v - vf : kc;
       PhaseCtx pc = pc0;
       pc.rb = rb;
-#ifdef M2R2_FUSED_DEBUG
-      if (tid == 0 && pc0.layer == 0) printf("cta %d ph %d rb %d s %d [%d,%d) v %d vf %d vl %d t0 %f\n", (int)blockIdx.x, pc0.ph, rb, s, s0, s1, v, vf, vl, sm.tile_out[0]);
-#endif
       if (ncontrib == 1) {
         finalize_block(P, sm, pc);
       } else {
@@ -552,9 +560,6 @@ __device__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd,
             sm.tile_out[tid] = sum;
           }
           bar_consumers();
-#ifdef M2R2_FUSED_DEBUG
-          if (tid == 0 && pc0.layer == 0) printf("  finalize cta %d ph %d rb %d sum0 %f\n", (int)blockIdx.x, pc0.ph, rb, sm.tile_out[0]);
-#endif
           finalize_block(P, sm, pc);
         }
       }
@@ -786,6 +791,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
 
   // ================= consumers
   unsigned int nbar = 0, stage_ctr = 0, attn_uses = 0;
+  int tl_n = 0;
+  (void)tl_n;
   const int d = P.d;
   const int pos = *(volatile int*)P.kv_len + P.joff;
   const int tok = *(volatile const int*)P.tok_in;
@@ -796,7 +803,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
     P.resid[d + k] = v;
     if (P.do_trace) { P.trace[k] = v; P.trace[d + k] = v; }
   }
+  TL(1);
   grid_sync(P, nbar, G);
+  TL(2);
 
   for (int i = 0; i < P.n_layers_run; ++i) {
     const FLayer* L = P.layers + i;
@@ -807,30 +816,44 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
     // ---- a2 (+a3): RMSNorm + QKV, RoPE + KV append
     xload_norm(P, sm, P.resid, P.resid + d, L->g1, d, P.d_pad, accel);
     if (accel) compute_u(sm, L->Aqkv, 3 * P.r, d, nullptr, P.d_pad / 8);
+    TL(10);
     pc.ph = PH_QKV; gd.n_rb = P.rb_qkv; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt);
+    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    TL(11);
     grid_sync(P, nbar, G);
+    TL(12);
     // ---- a4: attention
     attn_phase(P, sm, L, pos, accel, G, attn_uses);
+    TL(13);
     grid_sync(P, nbar, G);
+    TL(14);
     // ---- a5: O-proj + residual
     xload_plain(sm, P.attn_o, P.attn_o + d, d, P.d_pad, accel);
     if (accel) compute_u(sm, L->Ao, P.r, P.da, P.accel_cols, P.d_pad / 8);
+    TL(15);
     pc.ph = PH_OPROJ; gd.n_rb = P.rb_o;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt);
+    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    TL(16);
     grid_sync(P, nbar, G);
+    TL(17);
     // ---- a6: RMSNorm + gate/up + SwiGLU
     xload_norm(P, sm, P.resid, P.resid + d, L->g2, d, P.d_pad, accel);
     if (accel) compute_u(sm, L->Agu, 2 * P.r, d, nullptr, P.d_pad / 8);
+    TL(18);
     pc.ph = PH_GATEUP; gd.n_rb = P.rb_gu;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt);
+    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    TL(19);
     grid_sync(P, nbar, G);
+    TL(20);
     // ---- a7: down + residual, gate
     xload_plain(sm, P.act, P.act + P.F_pad, P.F, P.F_pad, accel);
     if (accel) compute_u(sm, L->Ad, P.r, P.F, nullptr, P.F_pad / 8);
+    TL(21);
     pc.ph = PH_DOWN; gd.n_rb = P.rb_d; gd.n_kc = n_kc_f; gd.kpad8 = P.F_pad / 8;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt);
+    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    TL(22);
     grid_sync(P, nbar, G);
+    TL(23);
     // ---- a8: exit head at a gate (Eq. 4), when asked
     if (L->gate && accel && P.exit_heads && !(P.head_stream == 1 && i + 1 == head_layers)) {
       const float* pe = P.pexit + (size_t)(L->gate - 1) * d;
@@ -839,7 +862,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
       PhaseCtx pe_c = pc;
       pe_c.ph = PH_EXIT; pe_c.layer = L->gate - 1;
       gd.n_rb = P.rb_v; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
-      gemv_phase(P, sm, gd, pe_c, G, stage_ctr, P.part, P.cnt);
+      gemv_phase(P, sm, gd, pe_c, G, stage_ctr, P.part, P.cnt, tl_n);
       grid_sync(P, nbar, G);
     }
   }
@@ -852,8 +875,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
     if (P.head_stream == 1 && P.lmA) compute_u(sm, P.lmA, P.r, d, nullptr, P.d_pad / 8);
     GemvDesc gd;
     gd.n_rb = P.rb_v; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt);
+    TL(30);
+    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    TL(31);
     grid_sync(P, nbar, G);
+    TL(32);
   }
   if (blockIdx.x == 0 && tid == 0) {
     u64 key = *(volatile u64*)&P.ctl->amax[0];
@@ -915,6 +941,7 @@ struct FusedImpl {
   unsigned int bar_base = 0;
   Ctl* h_ctl = nullptr;       // pinned
   bool bound = false;
+  u64* d_tl = nullptr;        // debug timeline (M2R2_FUSED_DEBUG builds)
   // scratch carve
   float *resid, *attn_o, *act, *qbuf, *khat, *vhat, *pexit, *part, *apart;
   int *cnt, *acnt, *accel_cols;
@@ -1092,6 +1119,11 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   p.resid = im->resid; p.attn_o = im->attn_o; p.act = im->act; p.qbuf = im->qbuf; p.khat = im->khat; p.vhat = im->vhat;
   p.pexit = im->pexit; p.part = im->part; p.cnt = im->cnt; p.apart = im->apart; p.acnt = im->acnt;
   p.ctl = im->d_ctl;
+  p.tl = nullptr;
+#ifdef M2R2_FUSED_DEBUG
+  if (getenv("M2R2_TL_OUT") && !im->d_tl) cudaMalloc((void**)&im->d_tl, sizeof(u64) * TL_MAX * im->G);
+  p.tl = im->d_tl;
+#endif
   im->bound = true;
   return 0;
 }
@@ -1146,6 +1178,14 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
   FusedImpl* im = fs->impl;
   if (cudaMemcpyAsync(im->h_ctl, im->d_ctl, sizeof(Ctl), cudaMemcpyDeviceToHost, st) != cudaSuccess) return M2R2_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;
+#ifdef M2R2_FUSED_DEBUG
+  if (im->d_tl && getenv("M2R2_TL_OUT")) {   // dump the timeline of the last launch
+    std::vector<u64> h((size_t)TL_MAX * im->G);
+    cudaMemcpy(h.data(), im->d_tl, h.size() * sizeof(u64), cudaMemcpyDeviceToHost);
+    FILE* f = fopen(getenv("M2R2_TL_OUT"), "wb");
+    if (f) { int hdr[2] = {im->G, TL_MAX}; fwrite(hdr, sizeof(int), 2, f); fwrite(h.data(), sizeof(u64), h.size(), f); fclose(f); }
+  }
+#endif
   if (im->h_ctl->abort_flag) {
     snprintf(msg, n, "fused kernel wait timed out (site 0x%x)", im->h_ctl->abort_where);
     // re-arm: barrier counter and flags back to a clean state
