@@ -1,22 +1,34 @@
-// kernels_fused.cu — persistent fused dual-stream decode pass (bf16 storage, dense FFN, batch 1).
+// kernels_fused.cu — persistent fused dual-stream decode pass, v2 (bf16 storage, dense FFN, batch 1).
 //
 // One cooperative launch runs a whole pass (a1-a9 of SURVEY §8(a)): embed, then per layer
 //   QKV   fused RMSNorm + QKV GEMV for h and p (+ adapters) with RoPE + KV append in the epilogue
-//   ATTN  split-K flash-decode attention, slow query and accelerated query on the same K/V tiles
-//   OPROJ O-projection + residual                        GATEUP RMSNorm + gate/up GEMV + SwiGLU
-//   DOWN  down GEMV + residual = accelerated-residual update, gate reset p <- h
+//   ATTN  split-K flash-decode attention, slow query and accelerated query on the same K/V loads
+//   OPROJ O-projection (split-K, partial sums to fixed slots)
+//   GATEUP residual + RMSNorm + gate/up GEMV + SwiGLU
+//   DOWN  down GEMV (split-K slots); the accelerated-residual update and the gate reset p <- h
+//          happen where the next phase loads the residual
 // and the LM head + greedy argmax (final head on h_N, or exit/draft head on p at a gate).
 //
-// Design (DESIGN.md §"Fused decode kernel"): one CTA per SM.  The big matrices are stored
-// TILE-MAJOR: a stage = 64 output rows x 256 inputs of bf16 = 32 KB contiguous, stages ordered
-// (row-block, k-chunk).  Weights never depend on activations, so ONE producer thread per CTA
-// streams the CTA's statically known stage sequence of the WHOLE pass through a shared-memory
-// ring with cp.async.bulk (UBLKCP) + mbarrier, running ahead across phase and grid barriers: HBM
-// stays busy while the consumers wait for activations.  Eight consumer warps take 8 rows each of
-// a stage, lanes stride K with 128-bit LDS, both activation rows (h, p) in registers per k-chunk.
-// The stages of a phase are split evenly over the CTAs (a CTA's range may start/end inside a
-// row-block): partial sums go to a fixed slot, the LAST contributor (atomic ticket) adds the slots
-// in slot order and runs the phase epilogue, so results are deterministic.
+// Design (DESIGN.md §"Fused decode kernel"): one CTA per SM, 16 consumer warps + 1 producer warp.
+//  * Weights are stored FRAGMENT-MAJOR: a tile = 16 output rows x 16 inputs laid out so that lane
+//    L's 16 bytes are its A fragment of mma.sync.m16n8k16; a stage = one row-tile x 1024 inputs =
+//    64 tiles = 32 KB contiguous; stages ordered (row-tile, k-stage).
+//  * Weights never depend on activations, so ONE producer thread per CTA streams the CTA's
+//    statically known stage sequence of the WHOLE pass through a 4-stage shared-memory ring with
+//    cp.async.bulk (UBLKCP) + mbarrier, and keeps an L2 prefetch window (cp.async.bulk.prefetch.L2)
+//    running further ahead, across phase boundaries and grid barriers: HBM stays busy while the
+//    consumers wait for activations.  The KV ranges a CTA will attend to are prefetched the same way.
+//  * Consumers: one LDS.128 per lane = one A fragment; the B operand is the activation vector split
+//    into bf16 hi + lo parts (columns h_hi, h_lo, p_hi, p_lo of the n=8 tile), so the product is
+//    exact to ~2^-17 and accumulates in fp32 on the tensor pipe (HMMA) at ~2 instructions per 256
+//    weights.  It is a GEMV, not a contraction: the tensor pipe is used as a wide FMA, the bound is HBM.
+//  * Row-owned phases (QKV, GATEUP, heads): a CTA owns whole row-tiles, epilogue is local.
+//    Split-K phases (OPROJ, DOWN): a CTA owns a contiguous stage range; partial sums of a row-tile go
+//    to slot (contributor index); the NEXT phase's loader adds residual + slots in slot order
+//    (deterministic, no tickets, no atomics on data).
+//  * Adapter down-projections u = A x^ are computed distributed (each CTA one row
+//    chunk) right after the loader, published with a release counter, and picked up at the first
+//    epilogue of the phase.
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -31,24 +43,32 @@ namespace {
 typedef __nv_bfloat16 bf16;
 typedef unsigned long long u64;
 
-constexpr int TILE_ROWS = 64;
-constexpr int TILE_K = 256;
-constexpr int STAGE_BYTES = TILE_ROWS * TILE_K * 2;   // 32 KB
+constexpr int STAGE_K = 1024;                  // inputs per stage
+constexpr int STAGE_TILES = STAGE_K / 16;      // 64 m16k16 tiles
+constexpr int STAGE_BYTES = STAGE_TILES * 512; // 32 KB
 constexpr int NSTAGE = 4;
-constexpr int NCW = 8;                 // consumer warps
+constexpr int NCW = 16;                // consumer warps
 constexpr int NCT = NCW * 32;          // consumer threads
 constexpr int NTHREADS = NCT + 32;     // + producer warp
-constexpr int AREA_BYTES = 96 * 1024;  // activation rows (x) / attention K,V staging
-constexpr int ATT_RED_FLOATS = 16 * 2 * (128 + 2);
-constexpr int MISC_BYTES = 2560;
-constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + AREA_BYTES + MISC_BYTES;
+constexpr int TPW = STAGE_TILES / NCW; // tiles per warp per stage (4)
+constexpr int KMAX = 8192;             // largest padded inner dimension
+constexpr int XCOL = KMAX + 8;         // bf16 elements per activation column (+8: LDS.128 bank spread)
+constexpr int X_BYTES = 4 * XCOL * 2;  // h_hi, h_lo, p_hi, p_lo
+constexpr int RED_FLOATS = 2 * NCW * 32;
+constexpr int MISC_BYTES = RED_FLOATS * 4 + 4096;
+constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + X_BYTES + MISC_BYTES;
 constexpr int MAX_R = 16;              // adapter rank limit
+constexpr int MAX_NJ = 3 * MAX_R;
+constexpr int UPART_Q = 64;            // max k-chunks per adapter row
+constexpr int MAX_SLOTS = KMAX / STAGE_K;
+constexpr int NORM_CH = 4;             // float4 chunks per thread in a norm loader (d <= 8192)
+constexpr int PF_DEFAULT = 10;         // L2 prefetch window, stages ahead of the ring
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
 
 enum { PH_QKV = 0, PH_OPROJ = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4, PH_EXIT = 5, N_PH = 6 };
 
 struct FLayer {
-  const uint4 *Wqkv, *Wo, *Wgu, *Wd;   // tile-major
+  const uint4 *Wqkv, *Wo, *Wgu, *Wd;   // fragment-major
   const bf16 *g1, *g2;
   const bf16 *Aqkv, *Bqkv, *Ao, *Bo, *Agu, *Bg, *Bu, *Ad, *Bd;
   bf16 *Kc, *Vc;                        // this layer's cache, sequence 0: [head][max_seq][dh]
@@ -60,14 +80,14 @@ struct Ctl {
   unsigned int bar;        // grid-barrier arrivals (monotonic across launches)
   unsigned int abort_flag; // a wait timed out
   unsigned int abort_where;
-  unsigned int pad;
+  unsigned int ucnt;       // adapter-partial publications of this launch (reset at its end)
   u64 amax[1 + M2R2_MAX_GATES];   // argmax keys: [0] head of the pass, [1+j] exit head of gate j
 };
 
 struct FParams {
   int n_layers_run, d, n_heads, dh, F, V, r, da, max_seq;
   int d_pad, F_pad;
-  int rb_qkv, rb_o, rb_gu, rb_d, rb_v;
+  int rt_qkv, rt_o, rt_gu, rt_d, rt_v;    // row-tiles per matrix
   float eps, scale;
   const FLayer* layers;
   const bf16 *embed, *gf, *lmA, *lmB;
@@ -79,19 +99,21 @@ struct FParams {
   int* tok_out;
   int* exit_tok;
   int n_gates, exit_heads, advance, head_stream, joff, do_trace, head_gate;
-  float *resid, *attn_o, *act, *qbuf, *khat, *vhat, *pexit;
-  float *part;
-  int *cnt;
-  float* apart;
-  int* acnt;
+  float *RA, *RB;            // residual pair [2][d]: RA = (h', p') after attention; RB = (h_i, p_i) entering a layer
+  float *oslots, *dslots;    // [MAX_SLOTS][2][d] split-K partial sums of OPROJ / DOWN
+  float *act, *qbuf, *khat, *vhat, *pexit;
+  float *apart;              // [head][split][2][dh+4]
+  float *upart;              // [2][MAX_NJ][UPART_Q]
   float *trace, *logits, *exit_logits;
   Ctl* ctl;
   unsigned int bar_base;
   const int *ls_full, *ls_draft;
   int ls_first, ls_n;
   float ls_beta;
-  int ns;   // attention splits
-  u64* tl;  // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
+  int ns;        // attention splits
+  int pos_host;  // kv_len + joff as the host knows it (producer-side KV prefetch only)
+  int pf_ahead;  // L2 prefetch window in stages
+  u64* tl;       // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
 };
 
 // ------------------------------------------------------------------ PTX helpers
@@ -122,17 +144,14 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ u64 policy_evict_first() {
   u64 p;
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
-__device__ __forceinline__ u64 policy_evict_last() {
-  u64 p;
-  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-  return p;
-}
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory"); }
 __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
   unsigned int v;
@@ -141,11 +160,15 @@ __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
 }
 __device__ __forceinline__ float ldcg(const float* p) { return __ldcg(p); }
 __device__ __forceinline__ float4 ldcg4(const float* p) { return __ldcg((const float4*)p); }
+__device__ __forceinline__ uint4 ldcg16(const void* p) { return __ldcg((const uint4*)p); }
 __device__ __forceinline__ float bf(const bf16* p) { return __bfloat162float(*p); }
-__device__ __forceinline__ float ldcg_bf16(const bf16* p) {   // written earlier in this launch by another SM: L2 only
-  return __uint_as_float((unsigned int)__ldcg((const unsigned short*)p) << 16);
-}
 __device__ __forceinline__ float silu(float z) { return z / (1.f + __expf(-z)); }
+__device__ __forceinline__ void mma_bf16(float c[4], const uint4& a, uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b0), "r"(b1));
+}
 
 __device__ __forceinline__ u64 amax_key(float v, int n) {
   unsigned int b = __float_as_uint(v);
@@ -153,9 +176,11 @@ __device__ __forceinline__ u64 amax_key(float v, int n) {
   return ((u64)b << 32) | (u64)(0xFFFFFFFFu - (unsigned int)n);   // ties: lowest index wins
 }
 
-// stage range of virtual CTA v among G for a phase of S stages, and the owner of a stage
-__device__ __forceinline__ int range_lo(int S, int v, int G) { return (int)(((long long)S * v) / G); }
-__device__ __forceinline__ int stage_owner(int S, int s, int G) { return (int)((((long long)(s + 1)) * G + S - 1) / S) - 1; }
+// ------------------------------------------------------------------ static work split
+// A phase has S stages (row-tile-major).  Virtual CTA v of G owns units [U*v/G, U*(v+1)/G) where a
+// unit is `gran` consecutive stages (gran = stages per row-tile for row-owned phases, 1 for split-K).
+__device__ __forceinline__ int range_lo(int U, int v, int G) { return (int)(((long long)U * v) / G); }
+__device__ __forceinline__ int unit_owner(int U, int u, int G) { return (int)((((long long)(u + 1)) * G + U - 1) / U) - 1; }
 __device__ __forceinline__ int phase_rot(int layer, int ph, int G) { return (int)(((unsigned)(layer * 5 + ph) * 29u) % (unsigned)G); }
 
 #ifdef M2R2_FUSED_DEBUG
@@ -168,28 +193,27 @@ __device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%glob
 
 struct Smem {
   unsigned char* ring;
-  float* area;
-  float* tile_out;    // [64][2]
-  float* u;           // [64] adapter down-projections of the current phase
-  float* red;         // [64]
+  bf16* x;            // 4 columns of XCOL
+  float* red;         // [2][NCW][32] cross-warp reduction of a row-tile
+  float* tile_out;    // [16][2]
+  float* u;           // [MAX_NJ] adapter down-projections of the current phase
+  float* sred;        // [64] block reductions
   u64* full;          // [NSTAGE]
   u64* empty;         // [NSTAGE]
-  u64* abar;          // attention staging
-  int* flag;          // [4]
 };
 
 __device__ __forceinline__ Smem carve_smem(unsigned char* base) {
   Smem s;
   s.ring = base;
-  s.area = (float*)(base + NSTAGE * STAGE_BYTES);
-  unsigned char* m = base + NSTAGE * STAGE_BYTES + AREA_BYTES;
-  s.tile_out = (float*)m;            // 512 B
-  s.u = (float*)(m + 512);           // 256 B
-  s.red = (float*)(m + 768);         // 256 B
+  s.x = (bf16*)(base + NSTAGE * STAGE_BYTES);
+  unsigned char* m = base + NSTAGE * STAGE_BYTES + X_BYTES;
+  s.red = (float*)m;
+  m += RED_FLOATS * 4;
+  s.tile_out = (float*)m;            // 128 B
+  s.u = (float*)(m + 256);           // 256 B
+  s.sred = (float*)(m + 512);        // 256 B
   s.full = (u64*)(m + 1024);
   s.empty = s.full + NSTAGE;
-  s.abar = s.empty + NSTAGE;
-  s.flag = (int*)(m + 1024 + 8 * (2 * NSTAGE + 1) + 8);
   return s;
 }
 
@@ -233,91 +257,243 @@ __device__ __forceinline__ void grid_sync(const FParams& P, unsigned int& nbar, 
   bar_consumers();
 }
 
-// ------------------------------------------------------------------ activation rows in shared memory
-// x[stream][k] is stored as float4 planes so that a lane's 8 consecutive k are two conflict-free
-// LDS.128: plane(half, stream)[g] = x[stream][8g + 4*half .. +4]
-__device__ __forceinline__ float4* xplane(const Smem& sm, int half, int stream, int kpad8) {
-  return (float4*)sm.area + (size_t)(half * 2 + stream) * kpad8;
+// ------------------------------------------------------------------ activation vectors in shared memory
+// Four bf16 columns (h_hi, h_lo, p_hi, p_lo) of XCOL elements.  Within every group of 64 inputs the
+// order is [t][tile i][half][2] so that lane (g, t) of a warp reads the B fragments (b0, b1) of its
+// four m16n8k16 tiles with two LDS.128:  pos(k) = 64*(k/64) + 16*t + 4*i + 2*half + (k&1),
+// i = (k/16)%4, t = ((k%16)%8)/2, half = (k%16)/8.
+__device__ __forceinline__ int xpos(int k) {
+  const int o = k & 15;
+  return (k & ~63) + (((o & 7) >> 1) << 4) + (((k >> 4) & 3) << 2) + ((o >> 3) << 1) + (o & 1);
+}
+__device__ __forceinline__ uint32_t pack_bf16(bf16 a, bf16 b) {
+  return (uint32_t)__bfloat16_as_ushort(a) | ((uint32_t)__bfloat16_as_ushort(b) << 16);
+}
+// store x[k..k+3] (k % 4 == 0) as hi + lo parts into the column pair (hi, lo)
+__device__ __forceinline__ void xstore4(bf16* hi, bf16* lo, int k, float4 v) {
+  const int p = xpos(k);
+  const bf16 h0 = __float2bfloat16_rn(v.x), h1 = __float2bfloat16_rn(v.y), h2 = __float2bfloat16_rn(v.z), h3 = __float2bfloat16_rn(v.w);
+  const bf16 l0 = __float2bfloat16_rn(v.x - __bfloat162float(h0)), l1 = __float2bfloat16_rn(v.y - __bfloat162float(h1));
+  const bf16 l2 = __float2bfloat16_rn(v.z - __bfloat162float(h2)), l3 = __float2bfloat16_rn(v.w - __bfloat162float(h3));
+  *(uint32_t*)(hi + p) = pack_bf16(h0, h1);
+  *(uint32_t*)(hi + p + 16) = pack_bf16(h2, h3);
+  *(uint32_t*)(lo + p) = pack_bf16(l0, l1);
+  *(uint32_t*)(lo + p + 16) = pack_bf16(l2, l3);
+}
+__device__ __forceinline__ float xval(const bf16* hi, const bf16* lo, int k) {
+  const int p = xpos(k);
+  return __bfloat162float(hi[p]) + __bfloat162float(lo[p]);
+}
+__device__ __forceinline__ float4 f4add(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
+__device__ __forceinline__ float f4ss(float4 a) { return a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w; }
+__device__ __forceinline__ void st4(float* p, float4 v) { __stcg((float4*)p, v); }
+
+// contributors of row-tile rt in a split-K phase of n_rt x nks stages
+__device__ __forceinline__ int n_contrib(int n_rt, int nks, int rt, int G) {
+  const int S = n_rt * nks;
+  if (S < G) return nks;
+  return unit_owner(S, rt * nks + nks - 1, G) - unit_owner(S, rt * nks, G) + 1;
 }
 
-// x <- rms(src; g) for both streams (stream 1 zero when the layer does not carry p)
-__device__ void xload_norm(const FParams& P, const Smem& sm, const float* src0, const float* src1,
-                           const bf16* g, int K, int kpad, bool have1) {
-  const int tid = threadIdx.x, kpad8 = kpad / 8;
-  float ss0 = 0.f, ss1 = 0.f;
-  for (int i = tid; i < kpad / 4; i += NCT) {
-    int k = i * 4;
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-    if (k < K) {
-      a = ldcg4(src0 + k);
-      if (have1) b = ldcg4(src1 + k);
-    }
-    ss0 += a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w;
-    ss1 += b.x * b.x + b.y * b.y + b.z * b.z + b.w * b.w;
-    xplane(sm, i & 1, 0, kpad8)[i >> 1] = a;
-    xplane(sm, i & 1, 1, kpad8)[i >> 1] = b;
-  }
-  ss0 = warp_sum(ss0);
-  ss1 = warp_sum(ss1);
-  if ((tid & 31) == 0) { sm.red[tid >> 5] = ss0; sm.red[8 + (tid >> 5)] = ss1; }
-  bar_consumers();
-  float t0 = 0.f, t1 = 0.f;
+enum { LN_QKV = 0, LN_GU = 1, LN_HEAD_H = 2, LN_HEAD_P = 3 };
+
+// Residual loader of the norm phases.  Every CTA rebuilds the full residual pair
+//   (h, p) = base + sum over split-K slots of the producing phase      (Eq. 1 / Eq. 2 residual adds)
+// applies the gate  p <- h when the producing layer ends at a gate, writes its
+// share of the pair back (wb), and leaves x = rms(.; g) of both streams in shared memory.
+struct LoadSrc {
+  const float* base;     // [2][d] or nullptr (then emb)
+  const bf16* emb;       // embedding row
+  const float* slots;    // or nullptr
+  int n_rt, nks;         // geometry of the producing split-K phase
+  bool p_live;           // the producing layer carried p
+  int gate;              // 1 + gate index: emit pexit, then p <- h
+};
+__device__ void loader_norm(const FParams& P, const Smem& sm, int mode, const LoadSrc& src, float* wb, float* trace_dst,
+                            const bf16* g, int G) {
+  const int tid = threadIdx.x, d = P.d;
+  bar_consumers();   // x of the previous phase is dead in every warp
+  float4 xh[NORM_CH], xp[NORM_CH];
+  float ssh = 0.f, ssp = 0.f;
 #pragma unroll
-  for (int w = 0; w < NCW; ++w) { t0 += sm.red[w]; t1 += sm.red[8 + w]; }
-  const float inv0 = rsqrtf(t0 / (float)K + P.eps), inv1 = rsqrtf(t1 / (float)K + P.eps);
-  for (int i = tid; i < K / 4; i += NCT) {
-    int k = i * 4;
-    float g0 = bf(g + k), g1 = bf(g + k + 1), g2 = bf(g + k + 2), g3 = bf(g + k + 3);
-    float4* pa = &xplane(sm, i & 1, 0, kpad8)[i >> 1];
-    float4* pb = &xplane(sm, i & 1, 1, kpad8)[i >> 1];
-    float4 a = *pa, b = *pb;
-    a.x = a.x * inv0 * g0; a.y = a.y * inv0 * g1; a.z = a.z * inv0 * g2; a.w = a.w * inv0 * g3;
-    b.x = b.x * inv1 * g0; b.y = b.y * inv1 * g1; b.z = b.z * inv1 * g2; b.w = b.w * inv1 * g3;
-    *pa = a;
-    *pb = b;
-  }
-  bar_consumers();
-}
-
-// x <- src (no norm)
-__device__ void xload_plain(const Smem& sm, const float* src0, const float* src1, int K, int kpad, bool have1) {
-  const int tid = threadIdx.x, kpad8 = kpad / 8;
-  for (int i = tid; i < kpad / 4; i += NCT) {
-    int k = i * 4;
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-    if (k < K) {
-      a = ldcg4(src0 + k);
-      if (have1) b = ldcg4(src1 + k);
+  for (int j = 0; j < NORM_CH; ++j) {
+    const int ci = tid + j * NCT, k = ci * 4;
+    xh[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+    xp[j] = xh[j];
+    if (k < d) {
+      float4 hv, pv;
+      if (src.base) {
+        hv = ldcg4(src.base + k);
+        pv = src.p_live ? ldcg4(src.base + d + k) : hv;
+      } else {
+        const uint2 e = *(const uint2*)(src.emb + k);
+        bf16x2_to_f32(e.x, hv.x, hv.y);
+        bf16x2_to_f32(e.y, hv.z, hv.w);
+        pv = hv;
+      }
+      if (src.slots) {
+        const int nc = n_contrib(src.n_rt, src.nks, k >> 4, G);
+        for (int sl = 0; sl < nc; ++sl) {
+          hv = f4add(hv, ldcg4(src.slots + (size_t)(sl * 2) * d + k));
+          if (src.p_live) pv = f4add(pv, ldcg4(src.slots + (size_t)(sl * 2 + 1) * d + k));
+        }
+      }
+      if (!src.p_live) pv = hv;
+      const bool owner = (ci % G) == (int)blockIdx.x;
+      const float4 pbefore = pv;
+      if (src.gate) {
+        if (owner) st4(P.pexit + (size_t)(src.gate - 1) * d + k, pv);
+        pv = hv;
+      }
+      if (owner && trace_dst) { st4(trace_dst + k, hv); st4(trace_dst + d + k, pbefore); }
+      if (owner && wb) { st4(wb + k, hv); st4(wb + d + k, pv); }
+      if (mode == LN_HEAD_P) { xh[j] = pbefore; xp[j] = pbefore; }
+      else if (mode == LN_HEAD_H) { xh[j] = hv; xp[j] = hv; }
+      else { xh[j] = hv; xp[j] = pv; }
+      ssh += f4ss(xh[j]);
+      ssp += f4ss(xp[j]);
     }
-    xplane(sm, i & 1, 0, kpad8)[i >> 1] = a;
-    xplane(sm, i & 1, 1, kpad8)[i >> 1] = b;
+  }
+  ssh = warp_sum(ssh);
+  ssp = warp_sum(ssp);
+  if ((tid & 31) == 0) { sm.sred[tid >> 5] = ssh; sm.sred[NCW + (tid >> 5)] = ssp; }
+  bar_consumers();
+  float th = 0.f, tp = 0.f;
+#pragma unroll
+  for (int w = 0; w < NCW; ++w) { th += sm.sred[w]; tp += sm.sred[NCW + w]; }
+  const float ih = rsqrtf(th / (float)d + P.eps), ip = rsqrtf(tp / (float)d + P.eps);
+  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+#pragma unroll
+  for (int j = 0; j < NORM_CH; ++j) {
+    const int ci = tid + j * NCT, k = ci * 4;
+    if (k < P.d_pad) {
+      float4 a = xh[j], b = xp[j];
+      if (k < d) {
+        const uint2 ge = *(const uint2*)(g + k);
+        float g0, g1, g2, g3;
+        bf16x2_to_f32(ge.x, g0, g1);
+        bf16x2_to_f32(ge.y, g2, g3);
+        a.x = a.x * ih * g0; a.y = a.y * ih * g1; a.z = a.z * ih * g2; a.w = a.w * ih * g3;
+        b.x = b.x * ip * g0; b.y = b.y * ip * g1; b.z = b.z * ip * g2; b.w = b.w * ip * g3;
+      }
+      xstore4(c0, c1, k, a);
+      xstore4(c2, c3, k, b);
+    }
   }
   bar_consumers();
 }
 
-// u[j] = A[j, :] . x^   (adapter down-projection of the accelerated row), rows j < n_rows.
-// A is [n_rows][Kc] row-major; compact column c of A maps to x granule gmap[c/8 ...] when cols != nullptr.
-__device__ void compute_u(const Smem& sm, const bf16* A, int n_rows, int Kc, const int* cols, int kpad8) {
+// x <- attention output of both queries: merge of the split partials (m, l, o) in split order (a4)
+__device__ void loader_attn(const FParams& P, const Smem& sm, bool accel) {
+  const int tid = threadIdx.x, d = P.d, dh = P.dh, NS = P.ns, dq = d >> 2;
+  bar_consumers();
+  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+  for (int idx = tid; idx < 2 * (P.d_pad >> 2); idx += NCT) {
+    const int q = idx >= (P.d_pad >> 2), k = (idx - q * (P.d_pad >> 2)) * 4;
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (k < d) {
+      const int head = k / dh, j = k - head * dh;
+      if (q == 0 || (accel && P.sidx[head] >= 0)) {
+        const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
+        float M = -INFINITY;
+        for (int s = 0; s < NS; ++s) {
+          const float* ps = pp + (size_t)s * 2 * (dh + 4);
+          if (ldcg(ps + dh + 1) > 0.f) M = fmaxf(M, ldcg(ps + dh));
+        }
+        float Lsum = 0.f;
+        for (int s = 0; s < NS; ++s) {
+          const float* ps = pp + (size_t)s * 2 * (dh + 4);
+          const float ls = ldcg(ps + dh + 1);
+          if (ls > 0.f) {
+            const float wgt = __expf(ldcg(ps + dh) - M);
+            const float4 v = ldcg4(ps + j);
+            Lsum += ls * wgt;
+            o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
+          }
+        }
+        const float inv = 1.f / Lsum;
+        o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+      }
+    }
+    (void)dq;
+    if (q == 0) xstore4(c0, c1, k, o); else xstore4(c2, c3, k, o);
+  }
+  bar_consumers();
+}
+
+// x <- SwiGLU activations of both streams (a7 input)
+__device__ void loader_act(const FParams& P, const Smem& sm, bool accel) {
+  const int tid = threadIdx.x;
+  bar_consumers();
+  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+  for (int idx = tid; idx < (P.F_pad >> 2); idx += NCT) {
+    const int k = idx * 4;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+    if (k < P.F) {
+      a = ldcg4(P.act + k);
+      if (accel) b = ldcg4(P.act + P.F_pad + k);
+    }
+    xstore4(c0, c1, k, a);
+    xstore4(c2, c3, k, b);
+  }
+  bar_consumers();
+}
+
+// Adapter down-projection u = A x^ of the accelerated row, distributed: CTA c computes
+// row j = c / q over k-chunk c % q and publishes it; fetch_u() sums the q chunks of every row in order.
+struct UState {
+  unsigned int target;   // publications expected so far in this launch
+  int buf;               // upart buffer of the current phase
+  int nj, q;             // geometry of the current phase
+  bool ready;            // warp 0: sm.u holds the current phase's u
+};
+__device__ void publish_u(const FParams& P, const Smem& sm, UState& us, const bf16* A, int nj, int Kc, const int* cols, int G) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const float4* x0 = xplane(sm, 0, 1, kpad8);
-  const float4* x1 = xplane(sm, 1, 1, kpad8);
-  for (int j = warp; j < n_rows; j += NCW) {
+  const int q = min(G / nj, UPART_Q);
+  us.buf ^= 1;
+  us.nj = nj;
+  us.q = q;
+  us.target += (unsigned int)(nj * q);
+  us.ready = false;
+  const int c = blockIdx.x;
+  if (warp == 1 && c < nj * q) {
+    const int j = c / q, ch = c - j * q;
+    const int chunk = (((Kc + q - 1) / q) + 7) & ~7;
+    const int k0 = ch * chunk, k1 = min(Kc, k0 + chunk);
     const bf16* a = A + (size_t)j * Kc;
     float acc = 0.f;
-    for (int c = lane * 8; c < Kc; c += 256) {
-      uint4 w = __ldg((const uint4*)(a + c));
-      int g = (cols ? cols[c] : c) >> 3;
-      float4 lo = x0[g], hi = x1[g];
-      float f0, f1;
-      bf16x2_to_f32(w.x, f0, f1); acc += f0 * lo.x + f1 * lo.y;
-      bf16x2_to_f32(w.y, f0, f1); acc += f0 * lo.z + f1 * lo.w;
-      bf16x2_to_f32(w.z, f0, f1); acc += f0 * hi.x + f1 * hi.y;
-      bf16x2_to_f32(w.w, f0, f1); acc += f0 * hi.z + f1 * hi.w;
-    }
+    for (int k = k0 + lane; k < k1; k += 32) acc += bf(a + k) * xval(sm.x + 2 * XCOL, sm.x + 3 * XCOL, cols ? cols[k] : k);
     acc = warp_sum(acc);
-    if (lane == 0) sm.u[j] = acc;
+    if (lane == 0) {
+      __stcg(P.upart + ((size_t)us.buf * MAX_NJ + j) * UPART_Q + ch, acc);
+      __threadfence();
+      atomicAdd(&P.ctl->ucnt, 1u);
+    }
   }
-  bar_consumers();
+}
+// warp 0 only
+__device__ void fetch_u(const FParams& P, const Smem& sm, UState& us) {
+  const int lane = threadIdx.x & 31;
+  if (lane == 0) {
+    long long t0 = clock64();
+    unsigned int n = 0;
+    while ((int)(ld_acquire(&P.ctl->ucnt) - us.target) < 0) {
+      if ((++n & 255u) == 0u) {
+        if (aborted(P.ctl)) break;
+        if (clock64() - t0 > SPIN_LIMIT) { set_abort(P.ctl, 0x500u); break; }
+      }
+    }
+    __threadfence();
+  }
+  __syncwarp();
+  for (int j = lane; j < us.nj; j += 32) {
+    const float* up = P.upart + ((size_t)us.buf * MAX_NJ + j) * UPART_Q;
+    float s = 0.f;
+    for (int ch = 0; ch < us.q; ++ch) s += ldcg(up + ch);
+    sm.u[j] = s;
+  }
+  __syncwarp();
+  us.ready = true;
 }
 
 __device__ __forceinline__ float lora_dot(const bf16* Brow, const float* u, int r) {
@@ -326,23 +502,23 @@ __device__ __forceinline__ float lora_dot(const bf16* Brow, const float* u, int 
   return s;
 }
 
-// ------------------------------------------------------------------ phase epilogues (one 64-row block, sums in sm.tile_out[row][stream])
+// ------------------------------------------------------------------ phase epilogues (warp 0; one 16-row tile, sums in sm.tile_out[row][stream])
 struct PhaseCtx {
-  int ph, layer, rb;
+  int ph, layer;
   const FLayer* L;
   int pos;          // position of the token of this pass
   bool accel;       // stream 1 live
 };
 
-__device__ void finalize_block(const FParams& P, const Smem& sm, const PhaseCtx& c) {
-  const int tid = threadIdx.x;
+__device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& c, int rt, int slot) {
+  const int lane = threadIdx.x & 31;
   const float* T = sm.tile_out;
   const int d = P.d, dh = P.dh, half = dh >> 1, r = P.r;
   if (c.ph == PH_QKV) {
     // a3 fused: RoPE (pairs are adjacent packed rows) + KV append (slow) / k^,v^ kept in scratch (accel)
-    if (tid < 64) {
-      const int m = tid >> 1, s = tid & 1;
-      const int r0 = c.rb * 64 + 2 * m;
+    if (lane < 16) {
+      const int m = lane >> 1, s = lane & 1;
+      const int r0 = rt * 16 + 2 * m;
       if (r0 < 3 * d && (s == 0 || c.accel)) {
         const int which = r0 / d, w = r0 % d, head = w / dh, i = w % dh;
         float v0 = T[(2 * m) * 2 + s], v1 = T[(2 * m + 1) * 2 + s];
@@ -366,224 +542,140 @@ __device__ void finalize_block(const FParams& P, const Smem& sm, const PhaseCtx&
           }
           const int o0 = head * dh + e0, o1 = head * dh + e1;
           if (which == 0) {
-            P.qbuf[s * d + o0] = v0; P.qbuf[s * d + o1] = v1;
+            __stcg(P.qbuf + s * d + o0, v0); __stcg(P.qbuf + s * d + o1, v1);
           } else if (s == 0) {
             bf16* C = (which == 1 ? c.L->Kc : c.L->Vc) + ((size_t)head * P.max_seq + c.pos) * dh;
             C[e0] = __float2bfloat16_rn(v0);
             C[e1] = __float2bfloat16_rn(v1);
           } else {
             float* C = which == 1 ? P.khat : P.vhat;
-            C[o0] = v0; C[o1] = v1;
+            __stcg(C + o0, v0); __stcg(C + o1, v1);
           }
         }
       }
     }
-  } else if (c.ph == PH_OPROJ) {
-    if (tid < 128) {
-      const int row = tid >> 1, s = tid & 1, n = c.rb * 64 + row;
-      if (n < d && (s == 0 || c.accel)) {
-        float v = T[row * 2 + s];
-        if (s == 1) v += lora_dot(c.L->Bo + (size_t)n * r, sm.u, r);
-        float* R = P.resid + s * d + n;
-        *R = ldcg(R) + v;
-      }
+  } else if (c.ph == PH_OPROJ || c.ph == PH_DOWN) {
+    // split-K partial of a row-tile -> slot; the contributor of slot 0 adds the adapter term once
+    const int row = lane >> 1, s = lane & 1, n = rt * 16 + row;
+    if (n < d && (s == 0 || c.accel)) {
+      float v = T[lane];
+      if (s == 1 && slot == 0) v += lora_dot((c.ph == PH_OPROJ ? c.L->Bo : c.L->Bd) + (size_t)n * r, sm.u, r);
+      float* S = c.ph == PH_OPROJ ? P.oslots : P.dslots;
+      __stcg(S + (size_t)(slot * 2 + s) * d + n, v);
     }
   } else if (c.ph == PH_GATEUP) {
-    // packed rows: warp-group of 8 = gate rows n..n+3 then up rows n..n+3
-    if (tid < 64) {
-      const int nl = tid >> 1, s = tid & 1, n = c.rb * 32 + nl;
+    // packed tile: gate rows n..n+7 then up rows n..n+7
+    if (lane < 16) {
+      const int nl = lane >> 1, s = lane & 1, n = rt * 8 + nl;
       if (n < P.F && (s == 0 || c.accel)) {
-        const int grow = (nl >> 2) * 8 + (nl & 3), urow = grow + 4;
-        float g = T[grow * 2 + s], up = T[urow * 2 + s];
+        float g = T[nl * 2 + s], up = T[(8 + nl) * 2 + s];
         if (s == 1) {
           g += lora_dot(c.L->Bg + (size_t)n * r, sm.u, r);
           up += lora_dot(c.L->Bu + (size_t)n * r, sm.u + r, r);
         }
-        P.act[s * P.F_pad + n] = silu(g) * up;
-      }
-    }
-  } else if (c.ph == PH_DOWN) {
-    // accelerated-residual update (Eq. 2) and gate: p <- h (L82, L101)
-    if (tid < 64) {
-      const int n = c.rb * 64 + tid;
-      if (n < d) {
-        float h = ldcg(P.resid + n) + T[tid * 2];
-        P.resid[n] = h;
-        float p = h;
-        if (c.accel) p = ldcg(P.resid + d + n) + T[tid * 2 + 1] + lora_dot(c.L->Bd + (size_t)n * r, sm.u, r);
-        if (P.do_trace) {
-          float* tr = P.trace + (size_t)(c.layer + 1) * 2 * d;
-          tr[n] = h;
-          tr[d + n] = p;
-        }
-        if (c.accel) {
-          if (c.L->gate) {
-            P.pexit[(size_t)(c.L->gate - 1) * d + n] = p;
-            p = h;
-          }
-          P.resid[d + n] = p;
-        }
+        __stcg(P.act + s * P.F_pad + n, silu(g) * up);
       }
     }
   } else {
-    // PH_HEAD (stream 0: final head on h_N) / PH_EXIT (stream 1: exit or draft head on p at a gate)
-    const int s = c.ph == PH_HEAD ? P.head_stream : 1;
+    // PH_HEAD (final head on h_N, or draft head on p) / PH_EXIT (exit head on p at a gate); the loader
+    // put the head's input into both columns
+    const bool on_p = (c.ph == PH_EXIT) || P.head_stream == 1;
     const int gate = c.ph == PH_HEAD ? P.head_gate : c.layer;   // for PH_EXIT `layer` carries the gate index
     const bool is_final = (c.ph == PH_HEAD && P.head_stream == 0);
-    if (tid < 64) {
-      const int n = c.rb * 64 + tid;
-      u64 key = 0ull;
-      if (n < P.V) {
-        float v = T[tid * 2 + s];
-        if (s == 1 && P.lmB) v += lora_dot(P.lmB + (size_t)n * r, sm.u, r);
-        float* lg = is_final ? P.logits : P.exit_logits + (size_t)gate * P.V;
-        lg[n] = v;
-        const int* script = is_final ? P.ls_full : P.ls_draft;
-        if (script) {
-          int q = c.pos + 1 - P.ls_first;   // logits of the token at pos predict pos+1
-          if (q >= 0 && q < P.ls_n && script[q] == n) v += P.ls_beta;
-        }
-        key = amax_key(v, n);
+    u64 key = 0ull;
+    const int n = rt * 16 + lane;
+    if (lane < 16 && n < P.V) {
+      float v = T[lane * 2];
+      if (on_p && P.lmB) v += lora_dot(P.lmB + (size_t)n * r, sm.u, r);
+      float* lg = is_final ? P.logits : P.exit_logits + (size_t)gate * P.V;
+      lg[n] = v;
+      const int* script = is_final ? P.ls_full : P.ls_draft;
+      if (script) {
+        int q = c.pos + 1 - P.ls_first;   // logits of the token at pos predict pos+1
+        if (q >= 0 && q < P.ls_n && script[q] == n) v += P.ls_beta;
       }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        u64 other = __shfl_xor_sync(0xffffffffu, key, o);
-        key = other > key ? other : key;
-      }
-      if ((tid & 31) == 0 && key) atomicMax(&P.ctl->amax[c.ph == PH_HEAD ? 0 : 1 + gate], key);
+      key = amax_key(v, n);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      u64 other = __shfl_xor_sync(0xffffffffu, key, o);
+      key = other > key ? other : key;
+    }
+    if (lane == 0 && key) atomicMax(&P.ctl->amax[c.ph == PH_HEAD ? 0 : 1 + gate], key);
   }
 }
 
 // ------------------------------------------------------------------ one GEMV phase (consumer side)
-struct GemvDesc {
-  int n_rb, n_kc;     // row-blocks, k-chunks (stages = n_rb * n_kc)
-  int kpad8;          // kpad / 8
-};
-
-__device__ __noinline__ void gemv_phase(const FParams& P, const Smem& sm, const GemvDesc& gd, const PhaseCtx& pc0, int G,
-                                        unsigned int& stage_ctr, float* part, int* cnt, int& tl_n) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int S = gd.n_rb * gd.n_kc;
-  const int rot = phase_rot(pc0.layer, pc0.ph, G);
-  const int v = ((int)blockIdx.x + rot) % G;
-  const int s0 = range_lo(S, v, G), s1 = range_lo(S, v + 1, G);
-  float acc[8][2];
-#pragma unroll
-  for (int i = 0; i < 8; ++i) acc[i][0] = acc[i][1] = 0.f;
-  const float4* xa0p = xplane(sm, 0, 0, gd.kpad8);
-  const float4* xa1p = xplane(sm, 1, 0, gd.kpad8);
-  const float4* xb0p = xplane(sm, 0, 1, gd.kpad8);
-  const float4* xb1p = xplane(sm, 1, 1, gd.kpad8);
+// Stage (rt, ks): 64 tiles of row-tile rt, inputs [1024 ks, 1024 ks + 1024).  Warp w multiplies tiles
+// 4w..4w+3 (inputs 64 (16 ks + w) .. +64): 4 LDS.128 (A fragments) + 2 LDS.128 (B fragments) + 4 HMMA.
+__device__ __noinline__ void gemv_phase(const FParams& P, const Smem& sm, const PhaseCtx& pc, int n_rt, int nks, bool split,
+                                        bool need_u, int G, unsigned int& stage_ctr, unsigned int& flushes, UState& us,
+                                        int& tl_n) {
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int S = n_rt * nks, gran = split ? 1 : nks, U = S / gran;
+  const int v = ((int)blockIdx.x + phase_rot(pc.layer, pc.ph, G)) % G;
+  const int s0 = range_lo(U, v, G) * gran, s1 = range_lo(U, v + 1, G) * gran;
+  float ca[4] = {0.f, 0.f, 0.f, 0.f}, cb[4] = {0.f, 0.f, 0.f, 0.f};
+  const bf16* xcol = sm.x + (size_t)(g & 3) * XCOL + t * 16;
   for (int s = s0; s < s1; ++s) {
-    const int rb = s / gd.n_kc, kc = s - rb * gd.n_kc;
+    const int rt = s / nks, ks = s - rt * nks;
     const unsigned int slot = stage_ctr % NSTAGE, use = stage_ctr / NSTAGE;
     ++stage_ctr;
-    const int g = kc * 32 + lane;
-    const float4 xa0 = xa0p[g], xa1 = xa1p[g], xb0 = xb0p[g], xb1 = xb1p[g];
-    mbar_wait(&sm.full[slot], use & 1u, P.ctl, 0x200u + pc0.ph);
-    const uint4* st = (const uint4*)(sm.ring + (size_t)slot * STAGE_BYTES) + (warp * 8) * 32 + lane;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const uint4 w = st[i * 32];
-      float f0, f1;
-      bf16x2_to_f32(w.x, f0, f1);
-      acc[i][0] += f0 * xa0.x; acc[i][1] += f0 * xb0.x; acc[i][0] += f1 * xa0.y; acc[i][1] += f1 * xb0.y;
-      bf16x2_to_f32(w.y, f0, f1);
-      acc[i][0] += f0 * xa0.z; acc[i][1] += f0 * xb0.z; acc[i][0] += f1 * xa0.w; acc[i][1] += f1 * xb0.w;
-      bf16x2_to_f32(w.z, f0, f1);
-      acc[i][0] += f0 * xa1.x; acc[i][1] += f0 * xb1.x; acc[i][0] += f1 * xa1.y; acc[i][1] += f1 * xb1.y;
-      bf16x2_to_f32(w.w, f0, f1);
-      acc[i][0] += f0 * xa1.z; acc[i][1] += f0 * xb1.z; acc[i][0] += f1 * xa1.w; acc[i][1] += f1 * xb1.w;
+    uint4 b01 = make_uint4(0u, 0u, 0u, 0u), b23 = b01;
+    if (g < 4) {
+      const uint4* xb = (const uint4*)(xcol + (size_t)(ks * 16 + warp) * 64);
+      b01 = xb[0];
+      b23 = xb[1];
     }
+    mbar_wait(&sm.full[slot], use & 1u, P.ctl, 0x200u + pc.ph);
+    const uint4* st = (const uint4*)(sm.ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
+    const uint4 a0 = st[0], a1 = st[32], a2 = st[64], a3 = st[96];
+    mma_bf16(ca, a0, b01.x, b01.y);
+    mma_bf16(cb, a1, b01.z, b01.w);
+    mma_bf16(ca, a2, b23.x, b23.y);
+    mma_bf16(cb, a3, b23.z, b23.w);
     __syncwarp();
     if (lane == 0) mbar_arrive(&sm.empty[slot]);   // stage consumed by this warp
-    TL(40);
-    if (kc == gd.n_kc - 1 || s == s1 - 1) {
-      // ---- end of this CTA's segment of row-block rb: reduce over lanes (16 values, butterfly)
-      float v16[16];
-#pragma unroll
-      for (int i = 0; i < 8; ++i) { v16[2 * i] = acc[i][0]; v16[2 * i + 1] = acc[i][1]; acc[i][0] = acc[i][1] = 0.f; }
-#pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        bool up = lane & 16;
-        float send = up ? v16[i] : v16[i + 8], keep = up ? v16[i + 8] : v16[i];
-        v16[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    if (ks == nks - 1 || s == s1 - 1) {
+      // ---- end of this CTA's segment of row-tile rt: columns 0,1 = h (hi, lo parts), 2,3 = p
+      float* red = sm.red + (size_t)(flushes & 1u) * NCW * 32 + warp * 32;
+      if (t < 2) {
+        red[g * 2 + t] = (ca[0] + ca[1]) + (cb[0] + cb[1]);
+        red[(g + 8) * 2 + t] = (ca[2] + ca[3]) + (cb[2] + cb[3]);
       }
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        bool up = lane & 8;
-        float send = up ? v16[i] : v16[i + 4], keep = up ? v16[i + 4] : v16[i];
-        v16[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
-      }
-#pragma unroll
-      for (int i = 0; i < 2; ++i) {
-        bool up = lane & 4;
-        float send = up ? v16[i] : v16[i + 2], keep = up ? v16[i + 2] : v16[i];
-        v16[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
-      }
-      {
-        bool up = lane & 2;
-        float send = up ? v16[0] : v16[1], keep = up ? v16[1] : v16[0];
-        v16[0] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-      }
-      v16[0] += __shfl_xor_sync(0xffffffffu, v16[0], 1);
-      const int idx = (lane >> 1) & 15;   // = row_in_warp*2 + stream
-      if ((lane & 1) == 0) sm.tile_out[(warp * 8 + (idx >> 1)) * 2 + (idx & 1)] = v16[0];
+      for (int i = 0; i < 4; ++i) ca[i] = cb[i] = 0.f;
       bar_consumers();
-      // ---- contributors of this row-block
-      // (S >= G: every CTA owns >= 1 stage, so the owners of a row-block are consecutive CTAs;
-      //  S < G: every stage has its own CTA, so there is one contributor per k-chunk)
-      const int vf = stage_owner(S, rb * gd.n_kc, G), vl = stage_owner(S, rb * gd.n_kc + gd.n_kc - 1, G);
-      const int ncontrib = S >= G ? vl - vf + 1 : gd.n_kc;
-      const int myslot = S >= G ? v - vf : kc;
-      PhaseCtx pc = pc0;
-      pc.rb = rb;
-      if (ncontrib == 1) {
-        finalize_block(P, sm, pc);
-      } else {
-        if (tid < 128) __stcg(part + ((size_t)(rb * gd.n_kc + myslot) * 128 + tid), sm.tile_out[tid]);
-        __threadfence();
-        bar_consumers();
-        if (tid == 0) {
-          int old = atomicAdd(&cnt[rb], 1);
-          int last = old == ncontrib - 1;
-          if (last) cnt[rb] = 0;
-          sm.flag[0] = last;
-        }
-        bar_consumers();
-        if (sm.flag[0]) {
-          __threadfence();
-          if (tid < 128) {
-            float sum = 0.f;
-            for (int sl = 0; sl < ncontrib; ++sl) sum += ldcg(part + ((size_t)(rb * gd.n_kc + sl) * 128 + tid));
-            sm.tile_out[tid] = sum;
-          }
-          bar_consumers();
-          finalize_block(P, sm, pc);
-        }
+      if (warp == 0) {
+        const float* rb = sm.red + (size_t)(flushes & 1u) * NCW * 32 + lane;
+        float sum = 0.f;
+#pragma unroll
+        for (int w = 0; w < NCW; ++w) sum += rb[w * 32];
+        sm.tile_out[lane] = sum;
+        __syncwarp();
+        if (need_u && !us.ready) fetch_u(P, sm, us);
+        int sl = 0;
+        if (split) sl = S >= G ? v - unit_owner(S, rt * nks, G) : ks;
+        epilogue_tile(P, sm, pc, rt, sl);
+        __syncwarp();
       }
-      bar_consumers();   // tile_out / flag reuse
+      ++flushes;
+      TL(40);
     }
   }
 }
 
 // ------------------------------------------------------------------ attention phase (a4): split-K flash-decode, dual query
-// Work item = (head, split).  K/V of positions [0, pos) come from the cache through a bulk copy into
-// the activation area; the token's own key/value (slow: K[pos], V[pos] as stored = rounded; accel:
-// k^, v^ from scratch) is added by the head's last contributor, which also merges
-// the split partials in split order.
-__device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, int pos, bool accel, int G,
-                           unsigned int& attn_uses) {
+// Work item = (head, split), one per CTA.  Keys/values of positions [p0, p1) < pos come from the cache
+// (prefetched into L2 by the producer); both queries share every load.  The last split also takes the
+// token's own key/value: slow = K[pos], V[pos] as stored (rounded), accelerated = k^, v^ from scratch
+// (p_t attends h_<t (+) p_t).  Partials (m, l, o) go to P.apart; the O-proj loader merges.
+__device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, int pos, bool accel, int G) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int dh = P.dh, d = P.d, lpp = dh >> 3, NS = P.ns;
   const int seg = lane >> 4, sl = lane & 15;
   const bool active = sl < lpp;
-  const int CH = (AREA_BYTES - ATT_RED_FLOATS * 4) / (4 * dh);   // positions per staging round
-  bf16* Ks = (bf16*)sm.area;
-  bf16* Vs = Ks + (size_t)CH * dh;
-  float* red = sm.area + (size_t)CH * dh;   // after K and V staging (2*CH*dh bf16 = CH*dh floats)
-  const u64 pol = policy_evict_last();
+  float* red = (float*)sm.x;   // [32 segments][2 queries][dh + 2]
   const int items = P.n_heads * NS;
   for (int w = blockIdx.x; w < items; w += G) {
     const int head = w / NS, sp = w - head * NS;
@@ -594,40 +686,42 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
 #pragma unroll
     for (int e = 0; e < 8; ++e) { qa[e] = 0.f; qb[e] = 0.f; }
     if (active) {
-#pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        qa[e] = ldcg(P.qbuf + head * dh + sl * 8 + e) * P.scale;
-        if (q1) qb[e] = ldcg(P.qbuf + d + head * dh + sl * 8 + e) * P.scale;
+      const float4 a0 = ldcg4(P.qbuf + head * dh + sl * 8), a1 = ldcg4(P.qbuf + head * dh + sl * 8 + 4);
+      qa[0] = a0.x * P.scale; qa[1] = a0.y * P.scale; qa[2] = a0.z * P.scale; qa[3] = a0.w * P.scale;
+      qa[4] = a1.x * P.scale; qa[5] = a1.y * P.scale; qa[6] = a1.z * P.scale; qa[7] = a1.w * P.scale;
+      if (q1) {
+        const float4 b0 = ldcg4(P.qbuf + d + head * dh + sl * 8), b1 = ldcg4(P.qbuf + d + head * dh + sl * 8 + 4);
+        qb[0] = b0.x * P.scale; qb[1] = b0.y * P.scale; qb[2] = b0.z * P.scale; qb[3] = b0.w * P.scale;
+        qb[4] = b1.x * P.scale; qb[5] = b1.y * P.scale; qb[6] = b1.z * P.scale; qb[7] = b1.w * P.scale;
       }
     }
     float m0 = -INFINITY, l0 = 0.f, m1 = -INFINITY, l1 = 0.f, o0[8], o1[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) { o0[e] = 0.f; o1[e] = 0.f; }
-    for (int c0 = p0; c0 < p1; c0 += CH) {
-      const int cn = min(CH, p1 - c0);
-      if (tid == 0) {
-        fence_proxy_async();
-        const uint32_t bytes = (uint32_t)cn * dh * 2;
-        mbar_expect_tx(sm.abar, 2 * bytes);
-        bulk_g2s(Ks, L->Kc + ((size_t)head * P.max_seq + c0) * dh, bytes, sm.abar, pol);
-        bulk_g2s(Vs, L->Vc + ((size_t)head * P.max_seq + c0) * dh, bytes, sm.abar, pol);
-      }
-      mbar_wait(sm.abar, attn_uses & 1u, P.ctl, 0x300u);
-      ++attn_uses;
-      for (int ub = warp * 2; ub < cn; ub += NCW * 2) {
-        const int u = ub + seg;
-        const bool valid = u < cn;
-        float kf[8], vf[8];
+    const bf16* Kb = L->Kc + (size_t)head * P.max_seq * dh + sl * 8;
+    const bf16* Vb = L->Vc + (size_t)head * P.max_seq * dh + sl * 8;
+    // positions of this warp: p0 + 2*warp + seg + 32*i; two iterations in flight
+    for (int ub = p0 + warp * 2; ub < p1; ub += 2 * NCW * 2) {
+      uint4 kk[2], vv[2];
+      bool valid[2];
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { kf[e] = 0.f; vf[e] = 0.f; }
-        if (valid && active) {
-          uint4 kk = *(const uint4*)(Ks + (size_t)u * dh + sl * 8);
-          uint4 vv = *(const uint4*)(Vs + (size_t)u * dh + sl * 8);
-          bf16x2_to_f32(kk.x, kf[0], kf[1]); bf16x2_to_f32(kk.y, kf[2], kf[3]);
-          bf16x2_to_f32(kk.z, kf[4], kf[5]); bf16x2_to_f32(kk.w, kf[6], kf[7]);
-          bf16x2_to_f32(vv.x, vf[0], vf[1]); bf16x2_to_f32(vv.y, vf[2], vf[3]);
-          bf16x2_to_f32(vv.z, vf[4], vf[5]); bf16x2_to_f32(vv.w, vf[6], vf[7]);
+      for (int it = 0; it < 2; ++it) {
+        const int u = ub + it * NCW * 2 + seg;
+        valid[it] = u < p1;
+        kk[it] = make_uint4(0u, 0u, 0u, 0u);
+        vv[it] = kk[it];
+        if (valid[it] && active) {
+          kk[it] = ldcg16(Kb + (size_t)u * dh);
+          vv[it] = ldcg16(Vb + (size_t)u * dh);
         }
+      }
+#pragma unroll
+      for (int it = 0; it < 2; ++it) {
+        float kf[8], vf[8];
+        bf16x2_to_f32(kk[it].x, kf[0], kf[1]); bf16x2_to_f32(kk[it].y, kf[2], kf[3]);
+        bf16x2_to_f32(kk[it].z, kf[4], kf[5]); bf16x2_to_f32(kk[it].w, kf[6], kf[7]);
+        bf16x2_to_f32(vv[it].x, vf[0], vf[1]); bf16x2_to_f32(vv[it].y, vf[2], vf[3]);
+        bf16x2_to_f32(vv[it].z, vf[4], vf[5]); bf16x2_to_f32(vv[it].w, vf[6], vf[7]);
         float sa = 0.f, sb = 0.f;
 #pragma unroll
         for (int e = 0; e < 8; ++e) { sa += qa[e] * kf[e]; sb += qb[e] * kf[e]; }
@@ -636,7 +730,7 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
           sa += __shfl_xor_sync(0xffffffffu, sa, o);
           sb += __shfl_xor_sync(0xffffffffu, sb, o);
         }
-        if (valid) {
+        if (valid[it]) {
           float mn = fmaxf(m0, sa), corr = __expf(m0 - mn), p = __expf(sa - mn);
           l0 = l0 * corr + p;
 #pragma unroll
@@ -651,9 +745,49 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
           }
         }
       }
-      bar_consumers();   // staging buffers free for the next round / phase
     }
-    // ---- merge the 16 lane segments of the CTA -> one partial per query
+    // ---- the token's own key/value (last split, warp 0, segment 0)
+    if (sp == NS - 1 && warp == 0) {
+      float kf[8], vf[8], k2[8], v2[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { kf[e] = vf[e] = k2[e] = v2[e] = 0.f; }
+      if (seg == 0 && active) {
+        const uint4 kk = ldcg16(Kb + (size_t)pos * dh), vv = ldcg16(Vb + (size_t)pos * dh);
+        bf16x2_to_f32(kk.x, kf[0], kf[1]); bf16x2_to_f32(kk.y, kf[2], kf[3]);
+        bf16x2_to_f32(kk.z, kf[4], kf[5]); bf16x2_to_f32(kk.w, kf[6], kf[7]);
+        bf16x2_to_f32(vv.x, vf[0], vf[1]); bf16x2_to_f32(vv.y, vf[2], vf[3]);
+        bf16x2_to_f32(vv.z, vf[4], vf[5]); bf16x2_to_f32(vv.w, vf[6], vf[7]);
+        if (q1) {
+          const float4 ka = ldcg4(P.khat + head * dh + sl * 8), kb = ldcg4(P.khat + head * dh + sl * 8 + 4);
+          const float4 va = ldcg4(P.vhat + head * dh + sl * 8), vb = ldcg4(P.vhat + head * dh + sl * 8 + 4);
+          k2[0] = ka.x; k2[1] = ka.y; k2[2] = ka.z; k2[3] = ka.w; k2[4] = kb.x; k2[5] = kb.y; k2[6] = kb.z; k2[7] = kb.w;
+          v2[0] = va.x; v2[1] = va.y; v2[2] = va.z; v2[3] = va.w; v2[4] = vb.x; v2[5] = vb.y; v2[6] = vb.z; v2[7] = vb.w;
+        }
+      }
+      float sa = 0.f, sb = 0.f;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { sa += qa[e] * kf[e]; sb += qb[e] * k2[e]; }
+#pragma unroll
+      for (int o = 8; o > 0; o >>= 1) {
+        sa += __shfl_xor_sync(0xffffffffu, sa, o);
+        sb += __shfl_xor_sync(0xffffffffu, sb, o);
+      }
+      if (seg == 0) {
+        float mn = fmaxf(m0, sa), corr = __expf(m0 - mn), p = __expf(sa - mn);
+        l0 = l0 * corr + p;
+#pragma unroll
+        for (int e = 0; e < 8; ++e) o0[e] = o0[e] * corr + p * vf[e];
+        m0 = mn;
+        if (q1) {
+          mn = fmaxf(m1, sb); corr = __expf(m1 - mn); p = __expf(sb - mn);
+          l1 = l1 * corr + p;
+#pragma unroll
+          for (int e = 0; e < 8; ++e) o1[e] = o1[e] * corr + p * v2[e];
+          m1 = mn;
+        }
+      }
+    }
+    // ---- merge the 32 lane segments of the CTA -> one partial per query
     {
       const int gseg = warp * 2 + seg;
       float* dst0 = red + ((size_t)gseg * 2 + 0) * (dh + 2);
@@ -668,12 +802,12 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
     for (int i = tid; i < 2 * dh; i += NCT) {
       const int q = i / dh, j = i - q * dh;
       float M = -INFINITY;
-      for (int s = 0; s < 16; ++s) {
+      for (int s = 0; s < 2 * NCW; ++s) {
         const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
         if (src[dh + 1] > 0.f) M = fmaxf(M, src[dh]);
       }
       float Lsum = 0.f, O = 0.f;
-      for (int s = 0; s < 16; ++s) {
+      for (int s = 0; s < 2 * NCW; ++s) {
         const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
         float ls = src[dh + 1];
         if (ls > 0.f) {
@@ -682,78 +816,84 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
           O += src[j] * wgt;
         }
       }
-      float* pp = P.apart + ((size_t)(head * NS + sp) * 2 + q) * (dh + 2);
+      float* pp = P.apart + ((size_t)(head * NS + sp) * 2 + q) * (dh + 4);
       __stcg(pp + j, O);
       if (j == 0) { __stcg(pp + dh, M); __stcg(pp + dh + 1, Lsum); }
-    }
-    __threadfence();
-    bar_consumers();
-    if (tid == 0) {
-      int old = atomicAdd(&P.acnt[head], 1);
-      int last = old == NS - 1;
-      if (last) P.acnt[head] = 0;
-      sm.flag[1] = last;
-    }
-    bar_consumers();
-    if (sm.flag[1]) {
-      __threadfence();
-      // own-token scores: warp 0 -> slow query vs K[pos] (as stored), warp 1 -> accel query vs k^
-      if (warp < 2) {
-        float part = 0.f;
-        if (warp == 0 || q1) {
-          for (int j = lane; j < dh; j += 32) {
-            float qv = ldcg(P.qbuf + warp * d + head * dh + j);
-            float kv = warp == 0 ? ldcg_bf16(L->Kc + ((size_t)head * P.max_seq + pos) * dh + j) : ldcg(P.khat + head * dh + j);
-            part += qv * kv;
-          }
-        }
-        part = warp_sum(part);
-        if (lane == 0) sm.red[16 + warp] = part * P.scale;
-      }
-      bar_consumers();
-      for (int i = tid; i < 2 * dh; i += NCT) {
-        const int q = i / dh, j = i - q * dh;
-        if (q == 1 && !q1) continue;
-        const float s_own = sm.red[16 + q];
-        float M = s_own;
-        for (int s = 0; s < NS; ++s) {
-          const float* pp = P.apart + ((size_t)(head * NS + s) * 2 + q) * (dh + 2);
-          if (ldcg(pp + dh + 1) > 0.f) M = fmaxf(M, ldcg(pp + dh));
-        }
-        float Lsum = 0.f, O = 0.f;
-        for (int s = 0; s < NS; ++s) {
-          const float* pp = P.apart + ((size_t)(head * NS + s) * 2 + q) * (dh + 2);
-          float ls = ldcg(pp + dh + 1);
-          if (ls > 0.f) {
-            float wgt = __expf(ldcg(pp + dh) - M);
-            Lsum += ls * wgt;
-            O += ldcg(pp + j) * wgt;
-          }
-        }
-        float wgt = __expf(s_own - M);
-        float vown = q == 0 ? ldcg_bf16(L->Vc + ((size_t)head * P.max_seq + pos) * dh + j) : ldcg(P.vhat + head * dh + j);
-        Lsum += wgt;
-        O += wgt * vown;
-        P.attn_o[q * d + head * dh + j] = O / Lsum;
-      }
     }
     bar_consumers();
   }
 }
 
 // ------------------------------------------------------------------ producer: the CTA's weight-stage stream of the whole pass
-__device__ __forceinline__ void produce_phase(const FParams& P, const Smem& sm, const uint4* W, int n_rb, int n_kc,
-                                              int layer, int ph, int G, unsigned int& ctr, u64 pol) {
-  const int S = n_rb * n_kc;
-  const int v = ((int)blockIdx.x + phase_rot(layer, ph, G)) % G;
-  const int s0 = range_lo(S, v, G), s1 = range_lo(S, v + 1, G);
-  for (int s = s0; s < s1; ++s) {
-    const unsigned int slot = ctr % NSTAGE, use = ctr / NSTAGE;
-    ++ctr;
-    mbar_wait(&sm.empty[slot], (use & 1u) ^ 1u, P.ctl, 0x400u + ph);
-    mbar_expect_tx(&sm.full[slot], STAGE_BYTES);
-    bulk_g2s(sm.ring + (size_t)slot * STAGE_BYTES, (const unsigned char*)W + (size_t)s * STAGE_BYTES, STAGE_BYTES,
-             &sm.full[slot], pol);
+__device__ __forceinline__ bool exit_phase_after(const FParams& P, int layer) {
+  const FLayer* L = P.layers + layer;
+  return L->gate && L->accel && P.exit_heads && !(P.head_stream == 1 && layer + 1 == P.n_layers_run);
+}
+
+// Walks the CTA's stages of the pass in consumption order (must mirror the consumer loop).
+struct Cursor {
+  int layer, ph;     // ph = -1 before the first phase
+  int s, s1;
+  const unsigned char* W;
+  bool new_layer;    // set when the walk enters a layer's QKV phase
+};
+__device__ bool cursor_advance(const FParams& P, Cursor& c, int G) {
+  const int n = P.n_layers_run;
+  if (c.ph == PH_HEAD) return false;
+  bool next_layer = false;
+  if (c.ph < 0) { c.layer = -1; next_layer = true; }
+  else if (c.ph == PH_QKV) c.ph = PH_OPROJ;
+  else if (c.ph == PH_OPROJ) c.ph = PH_GATEUP;
+  else if (c.ph == PH_GATEUP) c.ph = PH_DOWN;
+  else if (c.ph == PH_DOWN) { if (exit_phase_after(P, c.layer)) c.ph = PH_EXIT; else next_layer = true; }
+  else next_layer = true;   // PH_EXIT
+  if (next_layer) {
+    ++c.layer;
+    c.ph = c.layer < n ? PH_QKV : PH_HEAD;
+    c.new_layer = c.ph == PH_QKV;
+  }
+  const int nks_d = P.d_pad / STAGE_K, nks_f = P.F_pad / STAGE_K;
+  int n_rt, nks, gran, rot_layer = c.layer;
+  const FLayer* L = P.layers + (c.layer < n ? c.layer : 0);
+  switch (c.ph) {
+    case PH_QKV:    c.W = (const unsigned char*)L->Wqkv; n_rt = P.rt_qkv; nks = nks_d; gran = nks; break;
+    case PH_OPROJ:  c.W = (const unsigned char*)L->Wo;   n_rt = P.rt_o;   nks = nks_d; gran = 1;   break;
+    case PH_GATEUP: c.W = (const unsigned char*)L->Wgu;  n_rt = P.rt_gu;  nks = nks_d; gran = nks; break;
+    case PH_DOWN:   c.W = (const unsigned char*)L->Wd;   n_rt = P.rt_d;   nks = nks_f; gran = 1;   break;
+    case PH_EXIT:   c.W = (const unsigned char*)P.Wlm;   n_rt = P.rt_v;   nks = nks_d; gran = nks; rot_layer = L->gate - 1; break;
+    default:        c.W = (const unsigned char*)P.Wlm;   n_rt = P.rt_v;   nks = nks_d; gran = nks; rot_layer = n; break;
+  }
+  const int U = n_rt * nks / gran;
+  const int v = ((int)blockIdx.x + phase_rot(rot_layer, c.ph, G)) % G;
+  c.s = range_lo(U, v, G) * gran;
+  c.s1 = range_lo(U, v + 1, G) * gran;
+  return true;
+}
+__device__ __forceinline__ bool cursor_get(const FParams& P, Cursor& c, int G, const unsigned char*& addr) {
+  while (c.s >= c.s1) {
+    if (!cursor_advance(P, c, G)) return false;
+  }
+  addr = c.W + (size_t)c.s * STAGE_BYTES;
+  ++c.s;
+  return true;
+}
+
+// L2 prefetch of the K/V positions this CTA will attend to in `layer`
+__device__ void prefetch_kv(const FParams& P, int layer, int G) {
+  const int NS = P.ns, pos = P.pos_host, dh = P.dh;
+  const FLayer* L = P.layers + layer;
+  for (int w = blockIdx.x; w < P.n_heads * NS; w += G) {
+    const int head = w / NS, sp = w - head * NS;
+    const int chunk = (pos + NS - 1) / NS;
+    const int p0 = min(pos, sp * chunk), p1 = min(pos, p0 + chunk);
+    size_t bytes = (size_t)(p1 - p0) * dh * 2;
+    const unsigned char* kp = (const unsigned char*)(L->Kc + ((size_t)head * P.max_seq + p0) * dh);
+    const unsigned char* vp = (const unsigned char*)(L->Vc + ((size_t)head * P.max_seq + p0) * dh);
+    for (size_t o = 0; o < bytes; o += 16384) {
+      const uint32_t n = (uint32_t)min((size_t)16384, bytes - o);
+      bulk_prefetch_l2(kp + o, n);
+      bulk_prefetch_l2(vp + o, n);
+    }
   }
 }
 
@@ -763,120 +903,144 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
   const int tid = threadIdx.x, G = gridDim.x;
   if (tid == 0) {
     for (int i = 0; i < NSTAGE; ++i) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], NCW); }
-    mbar_init(sm.abar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  const int n_kc_d = P.d_pad / TILE_K, n_kc_f = P.F_pad / TILE_K;
-  const int head_layers = P.n_layers_run;
+  const int nks_d = P.d_pad / STAGE_K, nks_f = P.F_pad / STAGE_K;
+  const int n_run = P.n_layers_run;
 
   if (tid >= NCT) {
     // ================= producer warp: one thread streams every weight stage of the pass
     if (tid == NCT) {
       const u64 pol = policy_evict_first();
-      unsigned int ctr = 0;
-      for (int i = 0; i < P.n_layers_run; ++i) {
-        const FLayer* L = P.layers + i;
-        produce_phase(P, sm, L->Wqkv, P.rb_qkv, n_kc_d, i, PH_QKV, G, ctr, pol);
-        produce_phase(P, sm, L->Wo, P.rb_o, n_kc_d, i, PH_OPROJ, G, ctr, pol);
-        produce_phase(P, sm, L->Wgu, P.rb_gu, n_kc_d, i, PH_GATEUP, G, ctr, pol);
-        produce_phase(P, sm, L->Wd, P.rb_d, n_kc_f, i, PH_DOWN, G, ctr, pol);
-        if (L->gate && L->accel && P.exit_heads && !(P.head_stream == 1 && i + 1 == head_layers))
-          produce_phase(P, sm, P.Wlm, P.rb_v, n_kc_d, L->gate - 1, PH_EXIT, G, ctr, pol);
+      Cursor ld, pf;
+      ld.layer = 0; ld.ph = -1; ld.s = ld.s1 = 0; ld.W = nullptr; ld.new_layer = false;
+      pf = ld;
+      bool pf_live = P.pf_ahead > 0;
+      const unsigned char* a;
+      for (int i = 0; i < P.pf_ahead && pf_live; ++i) {
+        pf_live = cursor_get(P, pf, G, a);
+        if (pf_live) bulk_prefetch_l2(a, STAGE_BYTES);
+        if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); }
       }
-      produce_phase(P, sm, P.Wlm, P.rb_v, n_kc_d, head_layers, PH_HEAD, G, ctr, pol);
+      unsigned int ctr = 0;
+      while (cursor_get(P, ld, G, a)) {
+        if (pf_live) {
+          const unsigned char* b;
+          pf_live = cursor_get(P, pf, G, b);
+          if (pf_live) bulk_prefetch_l2(b, STAGE_BYTES);
+          if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); }
+        } else if (P.pf_ahead <= 0 && ld.new_layer) {
+          ld.new_layer = false;
+          prefetch_kv(P, ld.layer, G);
+        }
+        const unsigned int slot = ctr % NSTAGE, use = ctr / NSTAGE;
+        ++ctr;
+        mbar_wait(&sm.empty[slot], (use & 1u) ^ 1u, P.ctl, 0x400u + ld.ph);
+        mbar_expect_tx(&sm.full[slot], STAGE_BYTES);
+        bulk_g2s(sm.ring + (size_t)slot * STAGE_BYTES, a, STAGE_BYTES, &sm.full[slot], pol);
+      }
     }
     return;
   }
 
   // ================= consumers
-  unsigned int nbar = 0, stage_ctr = 0, attn_uses = 0;
+  unsigned int nbar = 0, stage_ctr = 0, flushes = 0;
   int tl_n = 0;
   (void)tl_n;
+  UState us;
+  us.target = 0; us.buf = 0; us.nj = 0; us.q = 1; us.ready = false;
   const int d = P.d;
   const int pos = *(volatile int*)P.kv_len + P.joff;
   const int tok = *(volatile const int*)P.tok_in;
-  // a1: embed + stream init, p_0 <- h_0 (L82)
-  for (int k = blockIdx.x * NCT + tid; k < d; k += G * NCT) {
-    float v = bf(P.embed + (size_t)tok * d + k);
-    P.resid[k] = v;
-    P.resid[d + k] = v;
-    if (P.do_trace) { P.trace[k] = v; P.trace[d + k] = v; }
-  }
   TL(1);
-  grid_sync(P, nbar, G);
-  TL(2);
 
-  for (int i = 0; i < P.n_layers_run; ++i) {
+  for (int i = 0; i < n_run; ++i) {
     const FLayer* L = P.layers + i;
     const bool accel = L->accel != 0;
     PhaseCtx pc;
-    pc.layer = i; pc.L = L; pc.pos = pos; pc.accel = accel; pc.rb = 0;
-    GemvDesc gd;
-    // ---- a2 (+a3): RMSNorm + QKV, RoPE + KV append
-    xload_norm(P, sm, P.resid, P.resid + d, L->g1, d, P.d_pad, accel);
-    if (accel) compute_u(sm, L->Aqkv, 3 * P.r, d, nullptr, P.d_pad / 8);
+    pc.layer = i; pc.L = L; pc.pos = pos; pc.accel = accel;
+    LoadSrc src;
+    // ---- a1 / a7-tail: residual entering the layer (embedding, or previous MLP's split-K sums + gate), a2 (+a3)
+    if (i == 0) {
+      src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1;
+      src.p_live = false; src.gate = 0;
+    } else {
+      const FLayer* Lp = L - 1;
+      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
+      src.p_live = Lp->accel != 0; src.gate = Lp->accel ? Lp->gate : 0;
+    }
+    loader_norm(P, sm, LN_QKV, src, P.RB, P.do_trace ? P.trace + (size_t)i * 2 * d : nullptr, L->g1, G);
+    if (accel) publish_u(P, sm, us, L->Aqkv, 3 * P.r, d, nullptr, G);
     TL(10);
-    pc.ph = PH_QKV; gd.n_rb = P.rb_qkv; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    pc.ph = PH_QKV;
+    gemv_phase(P, sm, pc, P.rt_qkv, nks_d, false, accel, G, stage_ctr, flushes, us, tl_n);
     TL(11);
     grid_sync(P, nbar, G);
     TL(12);
     // ---- a4: attention
-    attn_phase(P, sm, L, pos, accel, G, attn_uses);
+    attn_phase(P, sm, L, pos, accel, G);
     TL(13);
     grid_sync(P, nbar, G);
     TL(14);
-    // ---- a5: O-proj + residual
-    xload_plain(sm, P.attn_o, P.attn_o + d, d, P.d_pad, accel);
-    if (accel) compute_u(sm, L->Ao, P.r, P.da, P.accel_cols, P.d_pad / 8);
+    // ---- a5: O-proj (split-K slots)
+    loader_attn(P, sm, accel);
+    if (accel) publish_u(P, sm, us, L->Ao, P.r, P.da, P.accel_cols, G);
     TL(15);
-    pc.ph = PH_OPROJ; gd.n_rb = P.rb_o;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    pc.ph = PH_OPROJ;
+    gemv_phase(P, sm, pc, P.rt_o, nks_d, true, accel, G, stage_ctr, flushes, us, tl_n);
     TL(16);
     grid_sync(P, nbar, G);
     TL(17);
-    // ---- a6: RMSNorm + gate/up + SwiGLU
-    xload_norm(P, sm, P.resid, P.resid + d, L->g2, d, P.d_pad, accel);
-    if (accel) compute_u(sm, L->Agu, 2 * P.r, d, nullptr, P.d_pad / 8);
+    // ---- a5-tail + a6: h' = h + O-proj sums; RMSNorm + gate/up + SwiGLU
+    src.base = P.RB; src.emb = nullptr; src.slots = P.oslots; src.n_rt = P.rt_o; src.nks = nks_d;
+    src.p_live = accel; src.gate = 0;
+    loader_norm(P, sm, LN_GU, src, P.RA, nullptr, L->g2, G);
+    if (accel) publish_u(P, sm, us, L->Agu, 2 * P.r, d, nullptr, G);
     TL(18);
-    pc.ph = PH_GATEUP; gd.n_rb = P.rb_gu;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    pc.ph = PH_GATEUP;
+    gemv_phase(P, sm, pc, P.rt_gu, nks_d, false, accel, G, stage_ctr, flushes, us, tl_n);
     TL(19);
     grid_sync(P, nbar, G);
     TL(20);
-    // ---- a7: down + residual, gate
-    xload_plain(sm, P.act, P.act + P.F_pad, P.F, P.F_pad, accel);
-    if (accel) compute_u(sm, L->Ad, P.r, P.F, nullptr, P.F_pad / 8);
+    // ---- a7: down (split-K slots); the residual add + gate happen in the next loader
+    loader_act(P, sm, accel);
+    if (accel) publish_u(P, sm, us, L->Ad, P.r, P.F, nullptr, G);
     TL(21);
-    pc.ph = PH_DOWN; gd.n_rb = P.rb_d; gd.n_kc = n_kc_f; gd.kpad8 = P.F_pad / 8;
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    pc.ph = PH_DOWN;
+    gemv_phase(P, sm, pc, P.rt_d, nks_f, true, accel, G, stage_ctr, flushes, us, tl_n);
     TL(22);
     grid_sync(P, nbar, G);
     TL(23);
-    // ---- a8: exit head at a gate (Eq. 4), when asked
-    if (L->gate && accel && P.exit_heads && !(P.head_stream == 1 && i + 1 == head_layers)) {
-      const float* pe = P.pexit + (size_t)(L->gate - 1) * d;
-      xload_norm(P, sm, pe, pe, P.gf, d, P.d_pad, true);
-      if (P.lmA) compute_u(sm, P.lmA, P.r, d, nullptr, P.d_pad / 8);
-      PhaseCtx pe_c = pc;
-      pe_c.ph = PH_EXIT; pe_c.layer = L->gate - 1;
-      gd.n_rb = P.rb_v; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
-      gemv_phase(P, sm, gd, pe_c, G, stage_ctr, P.part, P.cnt, tl_n);
-      grid_sync(P, nbar, G);
+    // ---- a8: exit head at a gate (Eq. 4), when asked; no grid barrier needed after it
+    if (exit_phase_after(P, i)) {
+      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
+      src.p_live = true; src.gate = 0;
+      loader_norm(P, sm, LN_HEAD_P, src, nullptr, nullptr, P.gf, G);
+      if (P.lmA) publish_u(P, sm, us, P.lmA, P.r, d, nullptr, G);
+      PhaseCtx pe = pc;
+      pe.ph = PH_EXIT; pe.layer = L->gate - 1;
+      gemv_phase(P, sm, pe, P.rt_v, nks_d, false, P.lmA != nullptr, G, stage_ctr, flushes, us, tl_n);
     }
   }
   // ---- a9 / a8: head of the pass
   {
     PhaseCtx pc;
-    pc.layer = head_layers; pc.L = nullptr; pc.pos = pos; pc.accel = true; pc.rb = 0; pc.ph = PH_HEAD;
-    const float* src = P.head_stream == 0 ? P.resid : P.pexit + (size_t)P.head_gate * d;
-    xload_norm(P, sm, src, src, P.gf, d, P.d_pad, true);
-    if (P.head_stream == 1 && P.lmA) compute_u(sm, P.lmA, P.r, d, nullptr, P.d_pad / 8);
-    GemvDesc gd;
-    gd.n_rb = P.rb_v; gd.n_kc = n_kc_d; gd.kpad8 = P.d_pad / 8;
+    pc.layer = n_run; pc.L = nullptr; pc.pos = pos; pc.accel = true; pc.ph = PH_HEAD;
+    LoadSrc src;
+    if (n_run == 0) {
+      src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1;
+      src.p_live = false; src.gate = 0;
+    } else {
+      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
+      src.p_live = P.layers[n_run - 1].accel != 0; src.gate = 0;
+    }
+    loader_norm(P, sm, P.head_stream == 0 ? LN_HEAD_H : LN_HEAD_P, src, nullptr,
+                P.do_trace ? P.trace + (size_t)n_run * 2 * d : nullptr, P.gf, G);
+    const bool hu = P.head_stream == 1 && P.lmA != nullptr;
+    if (hu) publish_u(P, sm, us, P.lmA, P.r, d, nullptr, G);
     TL(30);
-    gemv_phase(P, sm, gd, pc, G, stage_ctr, P.part, P.cnt, tl_n);
+    gemv_phase(P, sm, pc, P.rt_v, nks_d, false, hu, G, stage_ctr, flushes, us, tl_n);
     TL(31);
     grid_sync(P, nbar, G);
     TL(32);
@@ -891,40 +1055,45 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
       if (kj) P.exit_tok[j] = (int)(0xFFFFFFFFu - (unsigned int)(kj & 0xFFFFFFFFull));
       P.ctl->amax[1 + j] = 0ull;
     }
+    P.ctl->ucnt = 0u;
     if (P.advance) { *P.kv_len = pos + 1; *P.pending = t; }
   }
 }
 
-// ------------------------------------------------------------------ repack: row-major [n_out, K] -> tile-major stages
+// ------------------------------------------------------------------ repack: row-major [n_out, K] -> fragment-major stages
 // map 0: natural rows; 1: QKV (RoPE pairs (j, j+dh/2) of q and k made adjacent); 2: gate/up interleaved
-// (8-row groups = gate n..n+3, up n..n+3).  Rows / columns beyond the matrix are zero.
+// (16-row tile = gate n..n+7, up n..n+7).  Rows / columns beyond the matrix are zero.
+__device__ __forceinline__ const bf16* pack_src_row(const bf16* src, const bf16* src2, int map, int r, int n_out, int K, int d, int dh) {
+  if (map == 0) return r < n_out ? src + (size_t)r * K : nullptr;
+  if (map == 1) {
+    if (r >= n_out) return nullptr;
+    int which = r / d, w = r % d, sr = r;
+    if (which < 2) {
+      int head = w / dh, e = w % dh;
+      sr = which * d + head * dh + (e >> 1) + (e & 1) * (dh >> 1);
+    }
+    return src + (size_t)sr * K;
+  }
+  const int n = (r >> 4) * 8 + (r & 7);
+  if (n >= n_out) return nullptr;
+  return ((r & 15) < 8 ? src : src2) + (size_t)n * K;
+}
 __global__ void pack_kernel(uint4* __restrict__ dst, const bf16* __restrict__ src, const bf16* __restrict__ src2,
-                            int map, int n_out, int K, int n_rb, int n_kc, int d, int dh) {
-  const size_t total = (size_t)n_rb * n_kc * (STAGE_BYTES / 16);
+                            int map, int n_out, int K, int n_rt, int nks, int d, int dh) {
+  const size_t total = (size_t)n_rt * nks * (STAGE_BYTES / 16);
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     const size_t stage = i / (STAGE_BYTES / 16);
     const int within = (int)(i % (STAGE_BYTES / 16));
-    const int row = within / 32, c8 = within % 32;
-    const int rb = (int)(stage / n_kc), kc = (int)(stage % n_kc);
-    const int r = rb * 64 + row, k = kc * TILE_K + c8 * 8;
-    const bf16* base = nullptr;
-    if (map == 0) {
-      if (r < n_out) base = src + (size_t)r * K;
-    } else if (map == 1) {
-      if (r < n_out) {
-        int which = r / d, w = r % d, sr = r;
-        if (which < 2) {
-          int head = w / dh, e = w % dh;
-          sr = which * d + head * dh + (e >> 1) + (e & 1) * (dh >> 1);
-        }
-        base = src + (size_t)sr * K;
-      }
-    } else {
-      int n = (r >> 3) * 4 + (r & 3);
-      if (n < n_out) base = ((r & 7) < 4 ? src : src2) + (size_t)n * K;
-    }
-    uint4 v = make_uint4(0u, 0u, 0u, 0u);
-    if (base && k < K) v = *(const uint4*)(base + k);   // K % 8 == 0
+    const int tile = within >> 5, lane = within & 31, g = lane >> 2, t = lane & 3;
+    const int rt = (int)(stage / nks), ks = (int)(stage % nks);
+    const int k = ks * STAGE_K + tile * 16 + 2 * t;
+    const bf16* r0 = pack_src_row(src, src2, map, rt * 16 + g, n_out, K, d, dh);
+    const bf16* r1 = pack_src_row(src, src2, map, rt * 16 + g + 8, n_out, K, d, dh);
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);   // K % 8 == 0: a pair never straddles the end
+    if (r0 && k < K) v.x = *(const uint32_t*)(r0 + k);
+    if (r1 && k < K) v.y = *(const uint32_t*)(r1 + k);
+    if (r0 && k + 8 < K) v.z = *(const uint32_t*)(r0 + k + 8);
+    if (r1 && k + 8 < K) v.w = *(const uint32_t*)(r1 + k + 8);
     dst[i] = v;
   }
 }
@@ -943,41 +1112,40 @@ struct FusedImpl {
   bool bound = false;
   u64* d_tl = nullptr;        // debug timeline (M2R2_FUSED_DEBUG builds)
   // scratch carve
-  float *resid, *attn_o, *act, *qbuf, *khat, *vhat, *pexit, *part, *apart;
-  int *cnt, *acnt, *accel_cols;
+  float *RA, *RB, *oslots, *dslots, *act, *qbuf, *khat, *vhat, *pexit, *apart, *upart;
+  int* accel_cols;
 };
 
 static int pad_to(int v, int m) { return (v + m - 1) / m * m; }
 
 bool fused_config_ok(const m2r2_config& c) {
   if (c.dtype != M2R2_BF16 || c.n_experts != 0) return false;
-  if (c.head_dim % 8 || c.head_dim > 128 || (c.head_dim & 1)) return false;
-  if (c.d_model % 8 || c.d_ff % 8) return false;
-  if (c.accel_enabled && c.adapter_rank > MAX_R) return false;
-  int kmax = std::max(pad_to(c.d_model, TILE_K), pad_to(c.d_ff, TILE_K));
-  if ((size_t)kmax * 2 * sizeof(float) > AREA_BYTES) return false;
-  if ((AREA_BYTES - ATT_RED_FLOATS * 4) / (4 * c.head_dim) < 16) return false;
+  if (c.head_dim % 8 || c.head_dim > 128) return false;
+  if (c.d_model % 16 || c.d_ff % 8) return false;
+  if (c.accel_enabled && (c.adapter_rank > MAX_R || c.adapter_rank < 1)) return false;
+  if (pad_to(c.d_model, STAGE_K) > KMAX || pad_to(c.d_ff, STAGE_K) > KMAX) return false;
+  if ((size_t)2 * NCW * 2 * (c.head_dim + 2) * sizeof(float) > (size_t)X_BYTES) return false;
   return true;
 }
 
 struct PackedDims {
-  int d_pad, F_pad, rb_qkv, rb_o, rb_gu, rb_d, rb_v;
+  int d_pad, F_pad, rt_qkv, rt_o, rt_gu, rt_d, rt_v;
   size_t st_qkv, st_o, st_gu, st_d, st_v;   // stages
 };
 static PackedDims packed_dims(const m2r2_config& c) {
   PackedDims q;
-  q.d_pad = pad_to(c.d_model, TILE_K);
-  q.F_pad = pad_to(c.d_ff, TILE_K);
-  q.rb_qkv = pad_to(3 * c.d_model, TILE_ROWS) / TILE_ROWS;
-  q.rb_o = pad_to(c.d_model, TILE_ROWS) / TILE_ROWS;
-  q.rb_gu = pad_to(2 * pad_to(c.d_ff, 4), TILE_ROWS) / TILE_ROWS;
-  q.rb_d = q.rb_o;
-  q.rb_v = pad_to(c.vocab, TILE_ROWS) / TILE_ROWS;
-  q.st_qkv = (size_t)q.rb_qkv * (q.d_pad / TILE_K);
-  q.st_o = (size_t)q.rb_o * (q.d_pad / TILE_K);
-  q.st_gu = (size_t)q.rb_gu * (q.d_pad / TILE_K);
-  q.st_d = (size_t)q.rb_d * (q.F_pad / TILE_K);
-  q.st_v = (size_t)q.rb_v * (q.d_pad / TILE_K);
+  q.d_pad = pad_to(c.d_model, STAGE_K);
+  q.F_pad = pad_to(c.d_ff, STAGE_K);
+  q.rt_qkv = pad_to(3 * c.d_model, 16) / 16;
+  q.rt_o = pad_to(c.d_model, 16) / 16;
+  q.rt_gu = pad_to(c.d_ff, 8) / 8;
+  q.rt_d = q.rt_o;
+  q.rt_v = pad_to(c.vocab, 16) / 16;
+  q.st_qkv = (size_t)q.rt_qkv * (q.d_pad / STAGE_K);
+  q.st_o = (size_t)q.rt_o * (q.d_pad / STAGE_K);
+  q.st_gu = (size_t)q.rt_gu * (q.d_pad / STAGE_K);
+  q.st_d = (size_t)q.rt_d * (q.F_pad / STAGE_K);
+  q.st_v = (size_t)q.rt_v * (q.d_pad / STAGE_K);
   return q;
 }
 
@@ -990,21 +1158,19 @@ size_t fused_weights_bytes(const m2r2_config& c) {
 void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs) {
   if (!fused_config_ok(c)) return;
   PackedDims q = packed_dims(c);
-  const size_t d = c.d_model, G = std::max(1, c.n_gates);
-  int max_rb = std::max(std::max(q.rb_qkv, q.rb_gu), std::max(q.rb_v, q.rb_o));
-  int max_kc = std::max(q.d_pad, q.F_pad) / TILE_K;
+  const size_t d = c.d_model, NG = std::max(1, c.n_gates);
   FusedImpl* im = fs ? fs->impl : nullptr;
 #define FTAKE(field, T, n) { T* p_ = cv.take<T>(n); if (im) im->field = p_; }
   FTAKE(d_layers, FLayer, c.n_layers)
   FTAKE(d_ctl, Ctl, 1)
   FTAKE(d_sidx, int, c.n_heads)
   FTAKE(accel_cols, int, std::max(8, c.n_accel_heads * c.head_dim))
-  FTAKE(resid, float, 2 * d) FTAKE(attn_o, float, 2 * d) FTAKE(act, float, 2 * (size_t)q.F_pad)
-  FTAKE(qbuf, float, 2 * d) FTAKE(khat, float, d) FTAKE(vhat, float, d) FTAKE(pexit, float, G * d)
-  FTAKE(part, float, (size_t)max_rb * max_kc * 128)
-  FTAKE(cnt, int, max_rb)
-  FTAKE(apart, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * 2 * (c.head_dim + 2))
-  FTAKE(acnt, int, c.n_heads)
+  FTAKE(RA, float, 2 * d) FTAKE(RB, float, 2 * d)
+  FTAKE(oslots, float, (size_t)MAX_SLOTS * 2 * d) FTAKE(dslots, float, (size_t)MAX_SLOTS * 2 * d)
+  FTAKE(act, float, 2 * (size_t)q.F_pad)
+  FTAKE(qbuf, float, 2 * d) FTAKE(khat, float, d) FTAKE(vhat, float, d) FTAKE(pexit, float, NG * d)
+  FTAKE(apart, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * 2 * (c.head_dim + 4))
+  FTAKE(upart, float, (size_t)2 * MAX_NJ * UPART_Q)
 #undef FTAKE
 }
 
@@ -1017,7 +1183,7 @@ int fused_create(const m2r2_config& c, FusedState* fs) {
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (!coop || max_smem < SMEM_BYTES || sms < 1) return 0;   // per-operation kernels serve this device
+  if (!coop || max_smem < SMEM_BYTES || sms < 2 * MAX_NJ) return 0;   // per-operation kernels serve this device
   if (cudaFuncSetAttribute(m2r2_fused_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return 0;
@@ -1046,9 +1212,9 @@ void fused_destroy(FusedState* fs) {
 
 bool fused_supported(const m2r2_config&, const FusedState* fs) { return fs->supported && fs->impl && fs->impl->bound; }
 
-static int pack(cudaStream_t st, void* dst, const void* src, const void* src2, int map, int n_out, int K, int n_rb,
-                int n_kc, int d, int dh) {
-  pack_kernel<<<1184, 256, 0, st>>>((uint4*)dst, (const bf16*)src, (const bf16*)src2, map, n_out, K, n_rb, n_kc, d, dh);
+static int pack(cudaStream_t st, void* dst, const void* src, const void* src2, int map, int n_out, int K, int n_rt,
+                int nks, int d, int dh) {
+  pack_kernel<<<1184, 256, 0, st>>>((uint4*)dst, (const bf16*)src, (const bf16*)src2, map, n_out, K, n_rt, nks, d, dh);
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }
 
@@ -1059,7 +1225,7 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
   const int d = c.d_model, dh = c.head_dim, F = c.d_ff;
-  const int kc_d = q.d_pad / TILE_K, kc_f = q.F_pad / TILE_K;
+  const int ks_d = q.d_pad / STAGE_K, ks_f = q.F_pad / STAGE_K;
   char* wp = (char*)packed;
   wp = (char*)(((uintptr_t)wp + 1023) & ~(uintptr_t)1023);
   std::vector<FLayer> hl(c.n_layers);
@@ -1072,10 +1238,10 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     f.Wo = (const uint4*)wp; wp += q.st_o * STAGE_BYTES;
     f.Wgu = (const uint4*)wp; wp += q.st_gu * STAGE_BYTES;
     f.Wd = (const uint4*)wp; wp += q.st_d * STAGE_BYTES;
-    if (pack(st, (void*)f.Wqkv, L.wqkv, nullptr, 1, 3 * d, d, q.rb_qkv, kc_d, d, dh)) return M2R2_CUDA;
-    if (pack(st, (void*)f.Wo, L.wo, nullptr, 0, d, d, q.rb_o, kc_d, d, dh)) return M2R2_CUDA;
-    if (pack(st, (void*)f.Wgu, L.wgate, L.wup, 2, F, d, q.rb_gu, kc_d, d, dh)) return M2R2_CUDA;
-    if (pack(st, (void*)f.Wd, L.wdown, nullptr, 0, d, F, q.rb_d, kc_f, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wqkv, L.wqkv, nullptr, 1, 3 * d, d, q.rt_qkv, ks_d, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wo, L.wo, nullptr, 0, d, d, q.rt_o, ks_d, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wgu, L.wgate, L.wup, 2, F, d, q.rt_gu, ks_d, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wd, L.wdown, nullptr, 0, d, F, q.rt_d, ks_f, d, dh)) return M2R2_CUDA;
     f.g1 = (const bf16*)L.g1; f.g2 = (const bf16*)L.g2;
     f.Aqkv = (const bf16*)L.Aqkv; f.Bqkv = (const bf16*)L.Bqkv; f.Ao = (const bf16*)L.Ao; f.Bo = (const bf16*)L.Bo;
     f.Agu = (const bf16*)L.Agu; f.Bg = (const bf16*)L.Bg; f.Bu = (const bf16*)L.Bu; f.Ad = (const bf16*)L.Ad; f.Bd = (const bf16*)L.Bd;
@@ -1086,7 +1252,7 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     for (int j = 0; j < c.n_gates; ++j) if (c.gates[j] == i + 1) f.gate = j + 1;
   }
   const uint4* Wlm = (const uint4*)wp;
-  if (pack(st, (void*)Wlm, lm_head, nullptr, 0, c.vocab, d, q.rb_v, kc_d, d, dh)) return M2R2_CUDA;
+  if (pack(st, (void*)Wlm, lm_head, nullptr, 0, c.vocab, d, q.rt_v, ks_d, d, dh)) return M2R2_CUDA;
   if (cudaMemcpyAsync(im->d_layers, hl.data(), sizeof(FLayer) * c.n_layers, cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   std::vector<int> sidx(c.n_heads, -1), cols(std::max(8, c.n_accel_heads * dh), 0);
   if (c.accel_enabled)
@@ -1097,10 +1263,7 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   if (cudaMemcpyAsync(im->d_sidx, sidx.data(), sizeof(int) * c.n_heads, cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   if (cudaMemcpyAsync(im->accel_cols, cols.data(), sizeof(int) * cols.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
-  cudaMemsetAsync(im->attn_o, 0, sizeof(float) * 2 * d, st);
   cudaMemsetAsync(im->act, 0, sizeof(float) * 2 * q.F_pad, st);
-  cudaMemsetAsync(im->cnt, 0, sizeof(int) * std::max(std::max(q.rb_qkv, q.rb_gu), std::max(q.rb_v, q.rb_o)), st);
-  cudaMemsetAsync(im->acnt, 0, sizeof(int) * c.n_heads, st);
   cudaMemsetAsync(im->pexit, 0, sizeof(float) * std::max(1, c.n_gates) * d, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;   // hl / sidx / cols are stack-owned
   im->bar_base = 0;
@@ -1109,16 +1272,18 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   p.d = d; p.n_heads = c.n_heads; p.dh = dh; p.F = F; p.V = c.vocab; p.r = c.accel_enabled ? c.adapter_rank : 0;
   p.da = c.n_accel_heads * dh; p.max_seq = c.max_seq;
   p.d_pad = q.d_pad; p.F_pad = q.F_pad;
-  p.rb_qkv = q.rb_qkv; p.rb_o = q.rb_o; p.rb_gu = q.rb_gu; p.rb_d = q.rb_d; p.rb_v = q.rb_v;
+  p.rt_qkv = q.rt_qkv; p.rt_o = q.rt_o; p.rt_gu = q.rt_gu; p.rt_d = q.rt_d; p.rt_v = q.rt_v;
   p.eps = c.rms_eps; p.scale = 1.0f / sqrtf((float)dh);
   p.layers = im->d_layers;
   p.embed = (const bf16*)embed; p.gf = (const bf16*)gf; p.lmA = (const bf16*)lm_A; p.lmB = (const bf16*)lm_B;
   p.Wlm = Wlm;
   p.sidx = im->d_sidx; p.accel_cols = im->accel_cols; p.rope_tab = rope_tab;
   p.n_gates = c.n_gates;
-  p.resid = im->resid; p.attn_o = im->attn_o; p.act = im->act; p.qbuf = im->qbuf; p.khat = im->khat; p.vhat = im->vhat;
-  p.pexit = im->pexit; p.part = im->part; p.cnt = im->cnt; p.apart = im->apart; p.acnt = im->acnt;
+  p.RA = im->RA; p.RB = im->RB; p.oslots = im->oslots; p.dslots = im->dslots;
+  p.act = im->act; p.qbuf = im->qbuf; p.khat = im->khat; p.vhat = im->vhat;
+  p.pexit = im->pexit; p.apart = im->apart; p.upart = im->upart;
   p.ctl = im->d_ctl;
+  p.pf_ahead = getenv("M2R2_PF") ? atoi(getenv("M2R2_PF")) : PF_DEFAULT;
   p.tl = nullptr;
 #ifdef M2R2_FUSED_DEBUG
   if (getenv("M2R2_TL_OUT") && !im->d_tl) cudaMalloc((void**)&im->d_tl, sizeof(u64) * TL_MAX * im->G);
@@ -1153,16 +1318,9 @@ int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const Fused
   ns = std::min(ns, std::max(1, (pos + 31) / 32));
   ns = std::min(ns, (int)M2R2_MAX_SPLITS);
   p.ns = ns;
-  // grid barriers of this launch (must match the kernel's sequence)
-  unsigned int nbar = 1;
-  for (int i = 0; i < run.n_layers; ++i) {
-    nbar += 5;
-    bool accel = c.accel_enabled && i < c.accel_end_layer;
-    bool gate = false;
-    for (int j = 0; j < c.n_gates; ++j) gate |= (c.gates[j] == i + 1);
-    if (gate && accel && run.exit_heads && !(run.head_stream == 1 && i + 1 == run.n_layers)) nbar += 1;
-  }
-  nbar += 1;
+  p.pos_host = pos;
+  // grid barriers of this launch (must match the kernel's sequence): 5 per layer + the final one
+  const unsigned int nbar = 5u * (unsigned int)run.n_layers + 1u;
   p.bar_base = im->bar_base;
   im->bar_base += nbar * (unsigned int)G;
   void* args[] = {(void*)&p};

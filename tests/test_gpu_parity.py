@@ -11,6 +11,13 @@ from oracle import Oracle
 from tests.parity import MARGIN, check_logits, compare_decode_step, tolerances
 from tests.refs import rel_l2
 
+# Two CUDA implementations of the same step (persistent fused kernel vs per-operation kernels) are
+# cross-checked on bf16 models.  The fused kernel feeds activations to the tensor pipe as bf16
+# hi + lo pairs (relative error <= 2^-17 per element), the
+# per-operation kernels use fp32 activations, so they agree to a few 1e-5, not to fp32 rounding.
+# (Oracle parity keeps BASELINE.json's tolerances; this constant is not used there.)
+XIMPL_TOL = 1e-4
+
 pytestmark = pytest.mark.gpu
 
 
@@ -213,7 +220,7 @@ def test_spec_step_zero_equals_decode_step_on_gpu():
         ta = int(a.decode_step()[0])
         acc, n = b.spec_step(0)
         assert n[0] == 1 and int(acc[0][0]) == ta
-        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= 1e-5
+        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= XIMPL_TOL
     a.close()
     b.close()
 
@@ -408,6 +415,6 @@ def test_dead_positions_do_not_leak_after_rollback():
         assert n[0] == 1
         t = b.decode_step()
         assert int(acc[0][0]) == int(t[0]) == f[s + 1]
-        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= 1e-5
+        assert rel_l2(a.debug_read(M.DBG_LOGITS, 0), b.debug_read(M.DBG_LOGITS, 0)) <= XIMPL_TOL
     a.close()
     b.close()
