@@ -9,7 +9,7 @@
 //          happen where the next phase loads the residual
 // and the LM head + greedy argmax (final head on h_N, or exit/draft head on p at a gate).
 //
-// Design (DESIGN.md §"Fused decode kernel"): one CTA per SM, 16 consumer warps + 1 producer warp.
+// Design (DESIGN.md §"Fused decode kernel"): one CTA per SM, 8 consumer warps + 1 producer warp.
 //  * Weights are stored FRAGMENT-MAJOR: a tile = 16 output rows x 16 inputs laid out so that lane
 //    L's 16 bytes are its A fragment of mma.sync.m16n8k16; a stage = one row-tile x 1024 inputs =
 //    64 tiles = 32 KB contiguous; stages ordered (row-tile, k-stage).
@@ -47,10 +47,10 @@ constexpr int STAGE_K = 1024;                  // inputs per stage
 constexpr int STAGE_TILES = STAGE_K / 16;      // 64 m16k16 tiles
 constexpr int STAGE_BYTES = STAGE_TILES * 512; // 32 KB
 constexpr int NSTAGE = 4;
-constexpr int NCW = 16;                // consumer warps
+constexpr int NCW = 8;                 // consumer warps
 constexpr int NCT = NCW * 32;          // consumer threads
 constexpr int NTHREADS = NCT + 32;     // + producer warp
-constexpr int TPW = STAGE_TILES / NCW; // tiles per warp per stage (4)
+constexpr int TPW = STAGE_TILES / NCW; // tiles per warp per stage (8)
 constexpr int KMAX = 8192;             // largest padded inner dimension
 constexpr int XCOL = KMAX + 8;         // bf16 elements per activation column (+8: LDS.128 bank spread)
 constexpr int X_BYTES = 4 * XCOL * 2;  // h_hi, h_lo, p_hi, p_lo
@@ -61,7 +61,7 @@ constexpr int MAX_R = 16;              // adapter rank limit
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
 constexpr int MAX_SLOTS = KMAX / STAGE_K;
-constexpr int NORM_CH = 4;             // float4 chunks per thread in a norm loader (d <= 8192)
+constexpr int NORM_CH = 4;             // float4 chunks per thread in a norm loader (d <= 4096)
 constexpr int PF_DEFAULT = 10;         // L2 prefetch window, stages ahead of the ring
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
 
@@ -74,6 +74,8 @@ struct FLayer {
   bf16 *Kc, *Vc;                        // this layer's cache, sequence 0: [head][max_seq][dh]
   int accel;                            // layer carries p
   int gate;                             // 1 + gate index if layer+1 is a gate E_j, else 0
+  const unsigned char* ad_lo;           // the layer's adapter tensors are one contiguous HBM range
+  unsigned int ad_bytes;
 };
 
 struct Ctl {
@@ -191,31 +193,15 @@ __device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%glob
 #define TL(ev) do { } while (0)
 #endif
 
-struct Smem {
-  unsigned char* ring;
-  bf16* x;            // 4 columns of XCOL
-  float* red;         // [2][NCW][32] cross-warp reduction of a row-tile
-  float* tile_out;    // [16][2]
-  float* u;           // [MAX_NJ] adapter down-projections of the current phase
-  float* sred;        // [64] block reductions
-  u64* full;          // [NSTAGE]
-  u64* empty;         // [NSTAGE]
-};
-
-__device__ __forceinline__ Smem carve_smem(unsigned char* base) {
-  Smem s;
-  s.ring = base;
-  s.x = (bf16*)(base + NSTAGE * STAGE_BYTES);
-  unsigned char* m = base + NSTAGE * STAGE_BYTES + X_BYTES;
-  s.red = (float*)m;
-  m += RED_FLOATS * 4;
-  s.tile_out = (float*)m;            // 128 B
-  s.u = (float*)(m + 256);           // 256 B
-  s.sred = (float*)(m + 512);        // 256 B
-  s.full = (u64*)(m + 1024);
-  s.empty = s.full + NSTAGE;
-  return s;
-}
+// ------------------------------------------------------------------ shared memory map (fixed offsets: every access stays in the shared window)
+constexpr int OFF_X = NSTAGE * STAGE_BYTES;
+constexpr int OFF_RED = OFF_X + X_BYTES;              // [2][NCW][32] floats
+constexpr int OFF_TILE = OFF_RED + RED_FLOATS * 4;    // [16][2] floats
+constexpr int OFF_U = OFF_TILE + 256;                 // [MAX_NJ] floats
+constexpr int OFF_SRED = OFF_U + 256;                 // [64] floats
+constexpr int OFF_BAR = OFF_SRED + 256;               // full[NSTAGE], empty[NSTAGE]
+constexpr int OFF_UTMP = OFF_BAR + 256;               // [256] floats
+static_assert(OFF_UTMP + 1024 <= SMEM_BYTES, "shared memory map");
 
 __device__ __forceinline__ void set_abort(Ctl* ctl, unsigned int where) {
   if (atomicExch(&ctl->abort_flag, 1u) == 0u) ctl->abort_where = where;
@@ -235,32 +221,30 @@ __device__ __forceinline__ void mbar_wait(u64* b, uint32_t parity, Ctl* ctl, uns
 }
 
 // ------------------------------------------------------------------ grid barrier (all CTAs co-resident: cooperative launch)
-__device__ __forceinline__ void grid_sync(const FParams& P, unsigned int& nbar, int G) {
+__device__ __forceinline__ void grid_sync(Ctl* ctl, unsigned int bar_base, unsigned int& nbar, int G) {
   bar_consumers();
+  ++nbar;
   if (threadIdx.x == 0) {
     __threadfence();
-    atomicAdd(&P.ctl->bar, 1u);
-    ++nbar;
-    unsigned int target = P.bar_base + nbar * (unsigned int)G;
+    atomicAdd(&ctl->bar, 1u);
+    const unsigned int target = bar_base + nbar * (unsigned int)G;
     long long t0 = clock64();
     unsigned int n = 0;
-    while ((int)(ld_acquire(&P.ctl->bar) - target) < 0) {
+    while ((int)(ld_acquire(&ctl->bar) - target) < 0) {
       if ((++n & 255u) == 0u) {
-        if (aborted(P.ctl)) break;
-        if (clock64() - t0 > SPIN_LIMIT) { set_abort(P.ctl, 0x100u + nbar); break; }
+        if (aborted(ctl)) break;
+        if (clock64() - t0 > SPIN_LIMIT) { set_abort(ctl, 0x100u + nbar); break; }
       }
     }
     __threadfence();
-  } else {
-    ++nbar;
   }
   bar_consumers();
 }
 
 // ------------------------------------------------------------------ activation vectors in shared memory
 // Four bf16 columns (h_hi, h_lo, p_hi, p_lo) of XCOL elements.  Within every group of 64 inputs the
-// order is [t][tile i][half][2] so that lane (g, t) of a warp reads the B fragments (b0, b1) of its
-// four m16n8k16 tiles with two LDS.128:  pos(k) = 64*(k/64) + 16*t + 4*i + 2*half + (k&1),
+// order is [t][tile i][half][2] so that lane (g, t) of a warp reads the B fragments (b0, b1) of four
+// consecutive m16n8k16 tiles with two LDS.128:  pos(k) = 64*(k/64) + 16*t + 4*i + 2*half + (k&1),
 // i = (k/16)%4, t = ((k%16)%8)/2, half = (k%16)/8.
 __device__ __forceinline__ int xpos(int k) {
   const int o = k & 15;
@@ -309,31 +293,49 @@ struct LoadSrc {
   bool p_live;           // the producing layer carried p
   int gate;              // 1 + gate index: emit pexit, then p <- h
 };
-__device__ void loader_norm(const FParams& P, const Smem& sm, int mode, const LoadSrc& src, float* wb, float* trace_dst,
-                            const bf16* g, int G) {
+__device__ __forceinline__ void loader_norm(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src, float* wb,
+                                            float* trace_dst, const bf16* g, int G) {
   const int tid = threadIdx.x, d = P.d;
   bar_consumers();   // x of the previous phase is dead in every warp
   float4 xh[NORM_CH], xp[NORM_CH];
+  uint2 ge[NORM_CH];
   float ssh = 0.f, ssp = 0.f;
 #pragma unroll
   for (int j = 0; j < NORM_CH; ++j) {
     const int ci = tid + j * NCT, k = ci * 4;
     xh[j] = make_float4(0.f, 0.f, 0.f, 0.f);
     xp[j] = xh[j];
+    ge[j] = make_uint2(0u, 0u);
     if (k < d) {
+      // every load of this chunk is independent of the others: one L2 round trip
+      ge[j] = __ldg((const uint2*)(g + k));
       float4 hv, pv;
       if (src.base) {
         hv = ldcg4(src.base + k);
         pv = src.p_live ? ldcg4(src.base + d + k) : hv;
       } else {
-        const uint2 e = *(const uint2*)(src.emb + k);
+        const uint2 e = __ldg((const uint2*)(src.emb + k));
         bf16x2_to_f32(e.x, hv.x, hv.y);
         bf16x2_to_f32(e.y, hv.z, hv.w);
         pv = hv;
       }
       if (src.slots) {
         const int nc = n_contrib(src.n_rt, src.nks, k >> 4, G);
-        for (int sl = 0; sl < nc; ++sl) {
+        float4 sh[3], sp[3];
+#pragma unroll
+        for (int sl = 0; sl < 3; ++sl) {
+          sh[sl] = make_float4(0.f, 0.f, 0.f, 0.f);
+          sp[sl] = sh[sl];
+          if (sl < nc) {
+            sh[sl] = ldcg4(src.slots + (size_t)(sl * 2) * d + k);
+            if (src.p_live) sp[sl] = ldcg4(src.slots + (size_t)(sl * 2 + 1) * d + k);
+          }
+        }
+#pragma unroll
+        for (int sl = 0; sl < 3; ++sl) {
+          if (sl < nc) { hv = f4add(hv, sh[sl]); pv = f4add(pv, sp[sl]); }
+        }
+        for (int sl = 3; sl < nc; ++sl) {
           hv = f4add(hv, ldcg4(src.slots + (size_t)(sl * 2) * d + k));
           if (src.p_live) pv = f4add(pv, ldcg4(src.slots + (size_t)(sl * 2 + 1) * d + k));
         }
@@ -356,23 +358,22 @@ __device__ void loader_norm(const FParams& P, const Smem& sm, int mode, const Lo
   }
   ssh = warp_sum(ssh);
   ssp = warp_sum(ssp);
-  if ((tid & 31) == 0) { sm.sred[tid >> 5] = ssh; sm.sred[NCW + (tid >> 5)] = ssp; }
+  if ((tid & 31) == 0) { sred[tid >> 5] = ssh; sred[NCW + (tid >> 5)] = ssp; }
   bar_consumers();
   float th = 0.f, tp = 0.f;
 #pragma unroll
-  for (int w = 0; w < NCW; ++w) { th += sm.sred[w]; tp += sm.sred[NCW + w]; }
+  for (int w = 0; w < NCW; ++w) { th += sred[w]; tp += sred[NCW + w]; }
   const float ih = rsqrtf(th / (float)d + P.eps), ip = rsqrtf(tp / (float)d + P.eps);
-  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+  bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
 #pragma unroll
   for (int j = 0; j < NORM_CH; ++j) {
     const int ci = tid + j * NCT, k = ci * 4;
     if (k < P.d_pad) {
       float4 a = xh[j], b = xp[j];
       if (k < d) {
-        const uint2 ge = *(const uint2*)(g + k);
         float g0, g1, g2, g3;
-        bf16x2_to_f32(ge.x, g0, g1);
-        bf16x2_to_f32(ge.y, g2, g3);
+        bf16x2_to_f32(ge[j].x, g0, g1);
+        bf16x2_to_f32(ge[j].y, g2, g3);
         a.x = a.x * ih * g0; a.y = a.y * ih * g1; a.z = a.z * ih * g2; a.w = a.w * ih * g3;
         b.x = b.x * ip * g0; b.y = b.y * ip * g1; b.z = b.z * ip * g2; b.w = b.w * ip * g3;
       }
@@ -384,10 +385,10 @@ __device__ void loader_norm(const FParams& P, const Smem& sm, int mode, const Lo
 }
 
 // x <- attention output of both queries: merge of the split partials (m, l, o) in split order (a4)
-__device__ void loader_attn(const FParams& P, const Smem& sm, bool accel) {
-  const int tid = threadIdx.x, d = P.d, dh = P.dh, NS = P.ns, dq = d >> 2;
+__device__ __forceinline__ void loader_attn(const FParams& P, bf16* x, bool accel) {
+  const int tid = threadIdx.x, d = P.d, dh = P.dh, NS = P.ns;
   bar_consumers();
-  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+  bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
   for (int idx = tid; idx < 2 * (P.d_pad >> 2); idx += NCT) {
     const int q = idx >= (P.d_pad >> 2), k = (idx - q * (P.d_pad >> 2)) * 4;
     float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -415,17 +416,16 @@ __device__ void loader_attn(const FParams& P, const Smem& sm, bool accel) {
         o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
       }
     }
-    (void)dq;
     if (q == 0) xstore4(c0, c1, k, o); else xstore4(c2, c3, k, o);
   }
   bar_consumers();
 }
 
 // x <- SwiGLU activations of both streams (a7 input)
-__device__ void loader_act(const FParams& P, const Smem& sm, bool accel) {
+__device__ __forceinline__ void loader_act(const FParams& P, bf16* x, bool accel) {
   const int tid = threadIdx.x;
   bar_consumers();
-  bf16 *c0 = sm.x, *c1 = sm.x + XCOL, *c2 = sm.x + 2 * XCOL, *c3 = sm.x + 3 * XCOL;
+  bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
   for (int idx = tid; idx < (P.F_pad >> 2); idx += NCT) {
     const int k = idx * 4;
     float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
@@ -445,11 +445,12 @@ struct UState {
   unsigned int target;   // publications expected so far in this launch
   int buf;               // upart buffer of the current phase
   int nj, q;             // geometry of the current phase
-  bool ready;            // warp 0: sm.u holds the current phase's u
+  bool ready;            // warp 0: smem u holds the current phase's u
 };
-__device__ void publish_u(const FParams& P, const Smem& sm, UState& us, const bf16* A, int nj, int Kc, const int* cols, int G) {
+__device__ __forceinline__ void publish_u(const FParams& P, const bf16* x, UState& us, const bf16* A, int nj, int Kc,
+                                          const int* cols, int G) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = min(G / nj, UPART_Q);
+  const int q = min(min(G / nj, UPART_Q), 256 / nj);
   us.buf ^= 1;
   us.nj = nj;
   us.q = q;
@@ -461,8 +462,16 @@ __device__ void publish_u(const FParams& P, const Smem& sm, UState& us, const bf
     const int chunk = (((Kc + q - 1) / q) + 7) & ~7;
     const int k0 = ch * chunk, k1 = min(Kc, k0 + chunk);
     const bf16* a = A + (size_t)j * Kc;
+    const bf16 *xh = x + 2 * XCOL, *xl = x + 3 * XCOL;
     float acc = 0.f;
-    for (int k = k0 + lane; k < k1; k += 32) acc += bf(a + k) * xval(sm.x + 2 * XCOL, sm.x + 3 * XCOL, cols ? cols[k] : k);
+    for (int k = k0 + lane * 8; k < k1; k += 256) {   // chunk and Kc are multiples of 8
+      const uint4 w = __ldg((const uint4*)(a + k));
+      float f[8];
+      bf16x2_to_f32(w.x, f[0], f[1]); bf16x2_to_f32(w.y, f[2], f[3]);
+      bf16x2_to_f32(w.z, f[4], f[5]); bf16x2_to_f32(w.w, f[6], f[7]);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) acc += f[e] * xval(xh, xl, cols ? cols[k + e] : k + e);
+    }
     acc = warp_sum(acc);
     if (lane == 0) {
       __stcg(P.upart + ((size_t)us.buf * MAX_NJ + j) * UPART_Q + ch, acc);
@@ -472,7 +481,7 @@ __device__ void publish_u(const FParams& P, const Smem& sm, UState& us, const bf
   }
 }
 // warp 0 only
-__device__ void fetch_u(const FParams& P, const Smem& sm, UState& us) {
+__device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp, UState& us) {
   const int lane = threadIdx.x & 31;
   if (lane == 0) {
     long long t0 = clock64();
@@ -486,11 +495,24 @@ __device__ void fetch_u(const FParams& P, const Smem& sm, UState& us) {
     __threadfence();
   }
   __syncwarp();
+  const int total = us.nj * us.q;   // <= 256
+  float v[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int idx = lane + 32 * i;
+    v[i] = 0.f;
+    if (idx < total) v[i] = ldcg(P.upart + ((size_t)us.buf * MAX_NJ + idx / us.q) * UPART_Q + idx % us.q);
+  }
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const int idx = lane + 32 * i;
+    if (idx < total) utmp[idx] = v[i];
+  }
+  __syncwarp();
   for (int j = lane; j < us.nj; j += 32) {
-    const float* up = P.upart + ((size_t)us.buf * MAX_NJ + j) * UPART_Q;
     float s = 0.f;
-    for (int ch = 0; ch < us.q; ++ch) s += ldcg(up + ch);
-    sm.u[j] = s;
+    for (int ch = 0; ch < us.q; ++ch) s += utmp[j * us.q + ch];
+    u[j] = s;
   }
   __syncwarp();
   us.ready = true;
@@ -498,11 +520,22 @@ __device__ void fetch_u(const FParams& P, const Smem& sm, UState& us) {
 
 __device__ __forceinline__ float lora_dot(const bf16* Brow, const float* u, int r) {
   float s = 0.f;
-  for (int q = 0; q < r; ++q) s += bf(Brow + q) * u[q];
+  if ((r & 7) == 0) {
+    for (int q = 0; q < r; q += 8) {
+      const uint4 w = __ldg((const uint4*)(Brow + q));
+      float f[8];
+      bf16x2_to_f32(w.x, f[0], f[1]); bf16x2_to_f32(w.y, f[2], f[3]);
+      bf16x2_to_f32(w.z, f[4], f[5]); bf16x2_to_f32(w.w, f[6], f[7]);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) s += f[e] * u[q + e];
+    }
+  } else {
+    for (int q = 0; q < r; ++q) s += bf(Brow + q) * u[q];
+  }
   return s;
 }
 
-// ------------------------------------------------------------------ phase epilogues (warp 0; one 16-row tile, sums in sm.tile_out[row][stream])
+// ------------------------------------------------------------------ phase epilogues (warp 0; one 16-row tile, sums in T[row][stream])
 struct PhaseCtx {
   int ph, layer;
   const FLayer* L;
@@ -510,9 +543,8 @@ struct PhaseCtx {
   bool accel;       // stream 1 live
 };
 
-__device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& c, int rt, int slot) {
+__device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, const float* u, const PhaseCtx& c, int rt, int slot) {
   const int lane = threadIdx.x & 31;
-  const float* T = sm.tile_out;
   const int d = P.d, dh = P.dh, half = dh >> 1, r = P.r;
   if (c.ph == PH_QKV) {
     // a3 fused: RoPE (pairs are adjacent packed rows) + KV append (slow) / k^,v^ kept in scratch (accel)
@@ -530,8 +562,8 @@ __device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& 
           live = si >= 0;
           if (live) {   // parallel adapters: + B (A x^)   (Q3)
             const bf16* B = c.L->Bqkv + ((size_t)which * P.da + (size_t)si * dh) * r;
-            v0 += lora_dot(B + (size_t)e0 * r, sm.u + which * r, r);
-            v1 += lora_dot(B + (size_t)e1 * r, sm.u + which * r, r);
+            v0 += lora_dot(B + (size_t)e0 * r, u + which * r, r);
+            v1 += lora_dot(B + (size_t)e1 * r, u + which * r, r);
           }
         }
         if (live) {
@@ -559,7 +591,7 @@ __device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& 
     const int row = lane >> 1, s = lane & 1, n = rt * 16 + row;
     if (n < d && (s == 0 || c.accel)) {
       float v = T[lane];
-      if (s == 1 && slot == 0) v += lora_dot((c.ph == PH_OPROJ ? c.L->Bo : c.L->Bd) + (size_t)n * r, sm.u, r);
+      if (s == 1 && slot == 0) v += lora_dot((c.ph == PH_OPROJ ? c.L->Bo : c.L->Bd) + (size_t)n * r, u, r);
       float* S = c.ph == PH_OPROJ ? P.oslots : P.dslots;
       __stcg(S + (size_t)(slot * 2 + s) * d + n, v);
     }
@@ -570,8 +602,8 @@ __device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& 
       if (n < P.F && (s == 0 || c.accel)) {
         float g = T[nl * 2 + s], up = T[(8 + nl) * 2 + s];
         if (s == 1) {
-          g += lora_dot(c.L->Bg + (size_t)n * r, sm.u, r);
-          up += lora_dot(c.L->Bu + (size_t)n * r, sm.u + r, r);
+          g += lora_dot(c.L->Bg + (size_t)n * r, u, r);
+          up += lora_dot(c.L->Bu + (size_t)n * r, u + r, r);
         }
         __stcg(P.act + s * P.F_pad + n, silu(g) * up);
       }
@@ -586,7 +618,7 @@ __device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& 
     const int n = rt * 16 + lane;
     if (lane < 16 && n < P.V) {
       float v = T[lane * 2];
-      if (on_p && P.lmB) v += lora_dot(P.lmB + (size_t)n * r, sm.u, r);
+      if (on_p && P.lmB) v += lora_dot(P.lmB + (size_t)n * r, u, r);
       float* lg = is_final ? P.logits : P.exit_logits + (size_t)gate * P.V;
       lg[n] = v;
       const int* script = is_final ? P.ls_full : P.ls_draft;
@@ -605,78 +637,17 @@ __device__ void epilogue_tile(const FParams& P, const Smem& sm, const PhaseCtx& 
   }
 }
 
-// ------------------------------------------------------------------ one GEMV phase (consumer side)
-// Stage (rt, ks): 64 tiles of row-tile rt, inputs [1024 ks, 1024 ks + 1024).  Warp w multiplies tiles
-// 4w..4w+3 (inputs 64 (16 ks + w) .. +64): 4 LDS.128 (A fragments) + 2 LDS.128 (B fragments) + 4 HMMA.
-__device__ __noinline__ void gemv_phase(const FParams& P, const Smem& sm, const PhaseCtx& pc, int n_rt, int nks, bool split,
-                                        bool need_u, int G, unsigned int& stage_ctr, unsigned int& flushes, UState& us,
-                                        int& tl_n) {
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  const int S = n_rt * nks, gran = split ? 1 : nks, U = S / gran;
-  const int v = ((int)blockIdx.x + phase_rot(pc.layer, pc.ph, G)) % G;
-  const int s0 = range_lo(U, v, G) * gran, s1 = range_lo(U, v + 1, G) * gran;
-  float ca[4] = {0.f, 0.f, 0.f, 0.f}, cb[4] = {0.f, 0.f, 0.f, 0.f};
-  const bf16* xcol = sm.x + (size_t)(g & 3) * XCOL + t * 16;
-  for (int s = s0; s < s1; ++s) {
-    const int rt = s / nks, ks = s - rt * nks;
-    const unsigned int slot = stage_ctr % NSTAGE, use = stage_ctr / NSTAGE;
-    ++stage_ctr;
-    uint4 b01 = make_uint4(0u, 0u, 0u, 0u), b23 = b01;
-    if (g < 4) {
-      const uint4* xb = (const uint4*)(xcol + (size_t)(ks * 16 + warp) * 64);
-      b01 = xb[0];
-      b23 = xb[1];
-    }
-    mbar_wait(&sm.full[slot], use & 1u, P.ctl, 0x200u + pc.ph);
-    const uint4* st = (const uint4*)(sm.ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
-    const uint4 a0 = st[0], a1 = st[32], a2 = st[64], a3 = st[96];
-    mma_bf16(ca, a0, b01.x, b01.y);
-    mma_bf16(cb, a1, b01.z, b01.w);
-    mma_bf16(ca, a2, b23.x, b23.y);
-    mma_bf16(cb, a3, b23.z, b23.w);
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&sm.empty[slot]);   // stage consumed by this warp
-    if (ks == nks - 1 || s == s1 - 1) {
-      // ---- end of this CTA's segment of row-tile rt: columns 0,1 = h (hi, lo parts), 2,3 = p
-      float* red = sm.red + (size_t)(flushes & 1u) * NCW * 32 + warp * 32;
-      if (t < 2) {
-        red[g * 2 + t] = (ca[0] + ca[1]) + (cb[0] + cb[1]);
-        red[(g + 8) * 2 + t] = (ca[2] + ca[3]) + (cb[2] + cb[3]);
-      }
-#pragma unroll
-      for (int i = 0; i < 4; ++i) ca[i] = cb[i] = 0.f;
-      bar_consumers();
-      if (warp == 0) {
-        const float* rb = sm.red + (size_t)(flushes & 1u) * NCW * 32 + lane;
-        float sum = 0.f;
-#pragma unroll
-        for (int w = 0; w < NCW; ++w) sum += rb[w * 32];
-        sm.tile_out[lane] = sum;
-        __syncwarp();
-        if (need_u && !us.ready) fetch_u(P, sm, us);
-        int sl = 0;
-        if (split) sl = S >= G ? v - unit_owner(S, rt * nks, G) : ks;
-        epilogue_tile(P, sm, pc, rt, sl);
-        __syncwarp();
-      }
-      ++flushes;
-      TL(40);
-    }
-  }
-}
-
 // ------------------------------------------------------------------ attention phase (a4): split-K flash-decode, dual query
 // Work item = (head, split), one per CTA.  Keys/values of positions [p0, p1) < pos come from the cache
 // (prefetched into L2 by the producer); both queries share every load.  The last split also takes the
 // token's own key/value: slow = K[pos], V[pos] as stored (rounded), accelerated = k^, v^ from scratch
 // (p_t attends h_<t (+) p_t).  Partials (m, l, o) go to P.apart; the O-proj loader merges.
-__device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, int pos, bool accel, int G) {
+__device__ __forceinline__ void attn_phase(const FParams& P, float* red, const FLayer* L, int pos, bool accel, int G) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int dh = P.dh, d = P.d, lpp = dh >> 3, NS = P.ns;
   const int seg = lane >> 4, sl = lane & 15;
   const bool active = sl < lpp;
-  float* red = (float*)sm.x;   // [32 segments][2 queries][dh + 2]
-  const int items = P.n_heads * NS;
+  const int items = P.n_heads * NS;   // red: [2 NCW segments][2 queries][dh + 2]
   for (int w = blockIdx.x; w < items; w += G) {
     const int head = w / NS, sp = w - head * NS;
     const bool q1 = accel && P.sidx[head] >= 0;
@@ -700,12 +671,13 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
     for (int e = 0; e < 8; ++e) { o0[e] = 0.f; o1[e] = 0.f; }
     const bf16* Kb = L->Kc + (size_t)head * P.max_seq * dh + sl * 8;
     const bf16* Vb = L->Vc + (size_t)head * P.max_seq * dh + sl * 8;
-    // positions of this warp: p0 + 2*warp + seg + 32*i; two iterations in flight
-    for (int ub = p0 + warp * 2; ub < p1; ub += 2 * NCW * 2) {
-      uint4 kk[2], vv[2];
-      bool valid[2];
+    // positions of this warp: p0 + 2*warp + seg + 2*NCW*i; AIF iterations in flight
+    constexpr int AIF = 4;
+    for (int ub = p0 + warp * 2; ub < p1; ub += AIF * NCW * 2) {
+      uint4 kk[AIF], vv[AIF];
+      bool valid[AIF];
 #pragma unroll
-      for (int it = 0; it < 2; ++it) {
+      for (int it = 0; it < AIF; ++it) {
         const int u = ub + it * NCW * 2 + seg;
         valid[it] = u < p1;
         kk[it] = make_uint4(0u, 0u, 0u, 0u);
@@ -716,7 +688,7 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
         }
       }
 #pragma unroll
-      for (int it = 0; it < 2; ++it) {
+      for (int it = 0; it < AIF; ++it) {
         float kf[8], vf[8];
         bf16x2_to_f32(kk[it].x, kf[0], kf[1]); bf16x2_to_f32(kk[it].y, kf[2], kf[3]);
         bf16x2_to_f32(kk[it].z, kf[4], kf[5]); bf16x2_to_f32(kk[it].w, kf[6], kf[7]);
@@ -787,7 +759,7 @@ __device__ void attn_phase(const FParams& P, const Smem& sm, const FLayer* L, in
         }
       }
     }
-    // ---- merge the 32 lane segments of the CTA -> one partial per query
+    // ---- merge the lane segments of the CTA -> one partial per query
     {
       const int gseg = warp * 2 + seg;
       float* dst0 = red + ((size_t)gseg * 2 + 0) * (dh + 2);
@@ -837,7 +809,7 @@ struct Cursor {
   const unsigned char* W;
   bool new_layer;    // set when the walk enters a layer's QKV phase
 };
-__device__ bool cursor_advance(const FParams& P, Cursor& c, int G) {
+__device__ __noinline__ bool cursor_advance(const FParams& P, Cursor& c, int G) {
   const int n = P.n_layers_run;
   if (c.ph == PH_HEAD) return false;
   bool next_layer = false;
@@ -879,7 +851,7 @@ __device__ __forceinline__ bool cursor_get(const FParams& P, Cursor& c, int G, c
 }
 
 // L2 prefetch of the K/V positions this CTA will attend to in `layer`
-__device__ void prefetch_kv(const FParams& P, int layer, int G) {
+__device__ __noinline__ void prefetch_kv(const FParams& P, int layer, int G) {
   const int NS = P.ns, pos = P.pos_host, dh = P.dh;
   const FLayer* L = P.layers + layer;
   for (int w = blockIdx.x; w < P.n_heads * NS; w += G) {
@@ -897,12 +869,46 @@ __device__ void prefetch_kv(const FParams& P, int layer, int G) {
   }
 }
 
-__global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FParams P) {
+// L2 prefetch of what the consumers will read with plain loads on their critical path: the layer's
+// norm gains and adapter tensors (each CTA one slice: together the whole range), the RoPE row.
+__device__ __forceinline__ void prefetch_slice(const void* base, size_t bytes, int G) {
+  const size_t per = (((bytes + G - 1) / G) + 15) & ~(size_t)15;
+  const size_t o = (size_t)blockIdx.x * per;
+  if (o < bytes) bulk_prefetch_l2((const unsigned char*)base + o, (uint32_t)min(per, ((bytes - o) + 15) & ~(size_t)15));
+}
+__device__ __noinline__ void prefetch_params(const FParams& P, int layer, int G) {
+  const FLayer* L = P.layers + layer;
+  if ((int)blockIdx.x == layer % G) {
+    bulk_prefetch_l2(L->g1, (uint32_t)((P.d * 2 + 15) & ~15));
+    bulk_prefetch_l2(L->g2, (uint32_t)((P.d * 2 + 15) & ~15));
+    if (layer == 0) {
+      bulk_prefetch_l2(P.rope_tab + (size_t)P.pos_host * (P.dh >> 1), (uint32_t)(((P.dh >> 1) * 8 + 15) & ~15));
+      bulk_prefetch_l2(P.gf, (uint32_t)((P.d * 2 + 15) & ~15));
+    }
+  }
+  if (L->accel && L->ad_bytes) prefetch_slice(L->ad_lo, L->ad_bytes, G);
+  if (layer == 0 && P.lmA && (P.head_stream == 1 || P.exit_heads)) {
+    prefetch_slice(P.lmA, (size_t)P.r * P.d * 2, G);
+    prefetch_slice(P.lmB, (size_t)P.V * P.r * 2, G);
+  }
+}
+
+constexpr int PH_ATTN = N_PH;   // consumer-only phase (no weights)
+
+__global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __grid_constant__ FParams P) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
-  const Smem sm = carve_smem(smem_raw);
+  unsigned char* const ring = smem_raw;
+  bf16* const x = (bf16*)(smem_raw + OFF_X);
+  float* const red = (float*)(smem_raw + OFF_RED);
+  float* const tile_out = (float*)(smem_raw + OFF_TILE);
+  float* const u_s = (float*)(smem_raw + OFF_U);
+  float* const sred = (float*)(smem_raw + OFF_SRED);
+  u64* const full = (u64*)(smem_raw + OFF_BAR);
+  u64* const empty = full + NSTAGE;
+  float* const utmp = (float*)(smem_raw + OFF_UTMP);
   const int tid = threadIdx.x, G = gridDim.x;
   if (tid == 0) {
-    for (int i = 0; i < NSTAGE; ++i) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], NCW); }
+    for (int i = 0; i < NSTAGE; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NCW); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -921,7 +927,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
       for (int i = 0; i < P.pf_ahead && pf_live; ++i) {
         pf_live = cursor_get(P, pf, G, a);
         if (pf_live) bulk_prefetch_l2(a, STAGE_BYTES);
-        if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); }
+        if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); prefetch_params(P, pf.layer, G); }
       }
       unsigned int ctr = 0;
       while (cursor_get(P, ld, G, a)) {
@@ -929,22 +935,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
           const unsigned char* b;
           pf_live = cursor_get(P, pf, G, b);
           if (pf_live) bulk_prefetch_l2(b, STAGE_BYTES);
-          if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); }
+          if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); prefetch_params(P, pf.layer, G); }
         } else if (P.pf_ahead <= 0 && ld.new_layer) {
           ld.new_layer = false;
           prefetch_kv(P, ld.layer, G);
+          prefetch_params(P, ld.layer, G);
         }
         const unsigned int slot = ctr % NSTAGE, use = ctr / NSTAGE;
         ++ctr;
-        mbar_wait(&sm.empty[slot], (use & 1u) ^ 1u, P.ctl, 0x400u + ld.ph);
-        mbar_expect_tx(&sm.full[slot], STAGE_BYTES);
-        bulk_g2s(sm.ring + (size_t)slot * STAGE_BYTES, a, STAGE_BYTES, &sm.full[slot], pol);
+        mbar_wait(&empty[slot], (use & 1u) ^ 1u, P.ctl, 0x400u + ld.ph);
+        mbar_expect_tx(&full[slot], STAGE_BYTES);
+        bulk_g2s(ring + (size_t)slot * STAGE_BYTES, a, STAGE_BYTES, &full[slot], pol);
       }
     }
     return;
   }
 
-  // ================= consumers
+  // ================= consumers: one loop over the phases of the pass (every routine has one call site)
+  const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   unsigned int nbar = 0, stage_ctr = 0, flushes = 0;
   int tl_n = 0;
   (void)tl_n;
@@ -955,100 +963,155 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
   const int tok = *(volatile const int*)P.tok_in;
   TL(1);
 
-  for (int i = 0; i < n_run; ++i) {
-    const FLayer* L = P.layers + i;
-    const bool accel = L->accel != 0;
+  int layer = 0, ph = n_run > 0 ? PH_QKV : PH_HEAD;
+  for (;;) {
+    const FLayer* L = P.layers + (layer < n_run ? layer : (n_run > 0 ? n_run - 1 : 0));
+    const bool accel = ph == PH_HEAD || ph == PH_EXIT ? true : L->accel != 0;
+    if (ph == PH_ATTN) {
+      // ---- a4: attention
+      attn_phase(P, (float*)x, L, pos, accel, G);
+      TL(13);
+      grid_sync(P.ctl, P.bar_base, nbar, G);
+      TL(14);
+      ph = PH_OPROJ;
+      continue;
+    }
+    // ---- geometry of the phase
     PhaseCtx pc;
-    pc.layer = i; pc.L = L; pc.pos = pos; pc.accel = accel;
-    LoadSrc src;
-    // ---- a1 / a7-tail: residual entering the layer (embedding, or previous MLP's split-K sums + gate), a2 (+a3)
-    if (i == 0) {
-      src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1;
-      src.p_live = false; src.gate = 0;
+    pc.ph = ph; pc.layer = layer; pc.L = L; pc.pos = pos; pc.accel = accel;
+    int n_rt, nks = nks_d, nj = 0, Kc = d;
+    bool split = false, need_u = accel && P.r > 0;
+    const bf16* A = nullptr;
+    const int* cols = nullptr;
+    if (ph == PH_QKV) { n_rt = P.rt_qkv; A = L->Aqkv; nj = 3 * P.r; }
+    else if (ph == PH_OPROJ) { n_rt = P.rt_o; split = true; A = L->Ao; nj = P.r; Kc = P.da; cols = P.accel_cols; }
+    else if (ph == PH_GATEUP) { n_rt = P.rt_gu; A = L->Agu; nj = 2 * P.r; }
+    else if (ph == PH_DOWN) { n_rt = P.rt_d; nks = nks_f; split = true; A = L->Ad; nj = P.r; Kc = P.F; }
+    else {
+      n_rt = P.rt_v; A = P.lmA; nj = P.r;
+      need_u = P.lmA != nullptr && (ph == PH_EXIT || P.head_stream == 1);
+      pc.layer = ph == PH_EXIT ? L->gate - 1 : n_run;
+    }
+    // ---- loader: the phase's input vector(s) -> shared memory
+    if (ph == PH_OPROJ) {
+      loader_attn(P, x, accel);
+    } else if (ph == PH_DOWN) {
+      loader_act(P, x, accel);
     } else {
-      const FLayer* Lp = L - 1;
-      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
-      src.p_live = Lp->accel != 0; src.gate = Lp->accel ? Lp->gate : 0;
+      LoadSrc src;
+      int mode;
+      float *wb = nullptr, *tr = nullptr;
+      const bf16* gn;
+      src.emb = nullptr; src.gate = 0;
+      if (ph == PH_GATEUP) {
+        // a5-tail: h' = h + O-proj sums
+        src.base = P.RB; src.slots = P.oslots; src.n_rt = P.rt_o; src.nks = nks_d; src.p_live = accel;
+        mode = LN_GU; wb = P.RA; gn = L->g2;
+      } else if ((ph == PH_QKV && layer == 0) || (ph == PH_HEAD && n_run == 0)) {
+        // a1: embedding, p_0 <- h_0 (L82)
+        src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1; src.p_live = false;
+        mode = ph == PH_QKV ? LN_QKV : (P.head_stream == 0 ? LN_HEAD_H : LN_HEAD_P);
+        wb = ph == PH_QKV ? P.RB : nullptr;
+        gn = ph == PH_QKV ? L->g1 : P.gf;
+        tr = P.do_trace ? P.trace : nullptr;
+      } else {
+        // a7-tail: residual + down sums of the layer below (accelerated-residual update, Eq. 2), gate
+        const FLayer* Lp = ph == PH_QKV ? L - 1 : L;
+        src.base = P.RA; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f; src.p_live = Lp->accel != 0;
+        if (ph == PH_QKV) {
+          src.gate = Lp->accel ? Lp->gate : 0;
+          mode = LN_QKV; wb = P.RB; gn = L->g1;
+          tr = P.do_trace ? P.trace + (size_t)layer * 2 * d : nullptr;
+        } else if (ph == PH_EXIT) {
+          mode = LN_HEAD_P; gn = P.gf;
+        } else {
+          mode = P.head_stream == 0 ? LN_HEAD_H : LN_HEAD_P; gn = P.gf;
+          tr = P.do_trace ? P.trace + (size_t)n_run * 2 * d : nullptr;
+        }
+      }
+      loader_norm(P, x, sred, mode, src, wb, tr, gn, G);
     }
-    loader_norm(P, sm, LN_QKV, src, P.RB, P.do_trace ? P.trace + (size_t)i * 2 * d : nullptr, L->g1, G);
-    if (accel) publish_u(P, sm, us, L->Aqkv, 3 * P.r, d, nullptr, G);
-    TL(10);
-    pc.ph = PH_QKV;
-    gemv_phase(P, sm, pc, P.rt_qkv, nks_d, false, accel, G, stage_ctr, flushes, us, tl_n);
-    TL(11);
-    grid_sync(P, nbar, G);
-    TL(12);
-    // ---- a4: attention
-    attn_phase(P, sm, L, pos, accel, G);
-    TL(13);
-    grid_sync(P, nbar, G);
-    TL(14);
-    // ---- a5: O-proj (split-K slots)
-    loader_attn(P, sm, accel);
-    if (accel) publish_u(P, sm, us, L->Ao, P.r, P.da, P.accel_cols, G);
-    TL(15);
-    pc.ph = PH_OPROJ;
-    gemv_phase(P, sm, pc, P.rt_o, nks_d, true, accel, G, stage_ctr, flushes, us, tl_n);
-    TL(16);
-    grid_sync(P, nbar, G);
-    TL(17);
-    // ---- a5-tail + a6: h' = h + O-proj sums; RMSNorm + gate/up + SwiGLU
-    src.base = P.RB; src.emb = nullptr; src.slots = P.oslots; src.n_rt = P.rt_o; src.nks = nks_d;
-    src.p_live = accel; src.gate = 0;
-    loader_norm(P, sm, LN_GU, src, P.RA, nullptr, L->g2, G);
-    if (accel) publish_u(P, sm, us, L->Agu, 2 * P.r, d, nullptr, G);
-    TL(18);
-    pc.ph = PH_GATEUP;
-    gemv_phase(P, sm, pc, P.rt_gu, nks_d, false, accel, G, stage_ctr, flushes, us, tl_n);
-    TL(19);
-    grid_sync(P, nbar, G);
-    TL(20);
-    // ---- a7: down (split-K slots); the residual add + gate happen in the next loader
-    loader_act(P, sm, accel);
-    if (accel) publish_u(P, sm, us, L->Ad, P.r, P.F, nullptr, G);
-    TL(21);
-    pc.ph = PH_DOWN;
-    gemv_phase(P, sm, pc, P.rt_d, nks_f, true, accel, G, stage_ctr, flushes, us, tl_n);
-    TL(22);
-    grid_sync(P, nbar, G);
-    TL(23);
-    // ---- a8: exit head at a gate (Eq. 4), when asked; no grid barrier needed after it
-    if (exit_phase_after(P, i)) {
-      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
-      src.p_live = true; src.gate = 0;
-      loader_norm(P, sm, LN_HEAD_P, src, nullptr, nullptr, P.gf, G);
-      if (P.lmA) publish_u(P, sm, us, P.lmA, P.r, d, nullptr, G);
-      PhaseCtx pe = pc;
-      pe.ph = PH_EXIT; pe.layer = L->gate - 1;
-      gemv_phase(P, sm, pe, P.rt_v, nks_d, false, P.lmA != nullptr, G, stage_ctr, flushes, us, tl_n);
+    if (need_u) publish_u(P, x, us, A, nj, Kc, cols, G);
+    TL(10 + ph);
+    // ---- GEMV over this CTA's stages.  Stage (rt, ks): 64 tiles of row-tile rt, inputs [1024 ks, +1024).
+    // Warp w multiplies tiles 8w..8w+7: 8 LDS.128 (A fragments) + 4 LDS.128 (B fragments) + 8 HMMA.
+    {
+      const int S = n_rt * nks, gran = split ? 1 : nks, U = S / gran;
+      const int v = ((int)blockIdx.x + phase_rot(pc.layer, ph, G)) % G;
+      const int s0 = range_lo(U, v, G) * gran, s1 = range_lo(U, v + 1, G) * gran;
+      float ca[4] = {0.f, 0.f, 0.f, 0.f}, cb[4] = {0.f, 0.f, 0.f, 0.f};
+      const bf16* xcol = x + (size_t)(g & 3) * XCOL + t * 16 + warp * 128;
+      int rt = s0 / nks, ks = s0 - rt * nks;
+      for (int s = s0; s < s1; ++s) {
+        const unsigned int slot = stage_ctr % NSTAGE, use = stage_ctr / NSTAGE;
+        ++stage_ctr;
+        uint4 b0 = make_uint4(0u, 0u, 0u, 0u), b1 = b0, b2 = b0, b3 = b0;
+        if (g < 4) {
+          const uint4* xb = (const uint4*)(xcol + (size_t)ks * STAGE_K);
+          b0 = xb[0]; b1 = xb[1]; b2 = xb[8]; b3 = xb[9];
+        }
+        mbar_wait(&full[slot], use & 1u, P.ctl, 0x200u + ph);
+        const uint4* st = (const uint4*)(ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
+        const uint4 a0 = st[0], a1 = st[32], a2 = st[64], a3 = st[96];
+        const uint4 a4 = st[128], a5 = st[160], a6 = st[192], a7 = st[224];
+        mma_bf16(ca, a0, b0.x, b0.y);
+        mma_bf16(cb, a1, b0.z, b0.w);
+        mma_bf16(ca, a2, b1.x, b1.y);
+        mma_bf16(cb, a3, b1.z, b1.w);
+        mma_bf16(ca, a4, b2.x, b2.y);
+        mma_bf16(cb, a5, b2.z, b2.w);
+        mma_bf16(ca, a6, b3.x, b3.y);
+        mma_bf16(cb, a7, b3.z, b3.w);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);   // stage consumed by this warp
+        if (ks == nks - 1 || s == s1 - 1) {
+          // ---- end of this CTA's segment of row-tile rt: columns 0,1 = h (hi, lo parts), 2,3 = p
+          float* rw = red + (size_t)(flushes & 1u) * NCW * 32 + warp * 32;
+          if (t < 2) {
+            rw[g * 2 + t] = (ca[0] + ca[1]) + (cb[0] + cb[1]);
+            rw[(g + 8) * 2 + t] = (ca[2] + ca[3]) + (cb[2] + cb[3]);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) ca[i] = cb[i] = 0.f;
+          bar_consumers();
+          if (warp == 0) {
+            const float* rb = red + (size_t)(flushes & 1u) * NCW * 32 + lane;
+            float sum = 0.f;
+#pragma unroll
+            for (int w = 0; w < NCW; ++w) sum += rb[w * 32];
+            tile_out[lane] = sum;
+            __syncwarp();
+            if (need_u && !us.ready) fetch_u(P, u_s, utmp, us);
+            int sl = 0;
+            if (split) sl = S >= G ? v - unit_owner(S, rt * nks, G) : ks;
+            epilogue_tile(P, tile_out, u_s, pc, rt, sl);
+            __syncwarp();
+          }
+          ++flushes;
+          TL(40);
+        }
+        if (++ks == nks) { ks = 0; ++rt; }
+      }
     }
+    TL(20 + ph);
+    if (ph == PH_HEAD) {
+      grid_sync(P.ctl, P.bar_base, nbar, G);
+      break;
+    }
+    if (ph != PH_EXIT) grid_sync(P.ctl, P.bar_base, nbar, G);   // nothing after an exit head depends on it
+    TL(30 + ph);
+    // ---- next phase
+    if (ph == PH_QKV) ph = PH_ATTN;
+    else if (ph == PH_OPROJ) ph = PH_GATEUP;
+    else if (ph == PH_GATEUP) ph = PH_DOWN;
+    else if (ph == PH_DOWN && exit_phase_after(P, layer)) ph = PH_EXIT;
+    else { ++layer; ph = layer < n_run ? PH_QKV : PH_HEAD; }
   }
-  // ---- a9 / a8: head of the pass
-  {
-    PhaseCtx pc;
-    pc.layer = n_run; pc.L = nullptr; pc.pos = pos; pc.accel = true; pc.ph = PH_HEAD;
-    LoadSrc src;
-    if (n_run == 0) {
-      src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1;
-      src.p_live = false; src.gate = 0;
-    } else {
-      src.base = P.RA; src.emb = nullptr; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f;
-      src.p_live = P.layers[n_run - 1].accel != 0; src.gate = 0;
-    }
-    loader_norm(P, sm, P.head_stream == 0 ? LN_HEAD_H : LN_HEAD_P, src, nullptr,
-                P.do_trace ? P.trace + (size_t)n_run * 2 * d : nullptr, P.gf, G);
-    const bool hu = P.head_stream == 1 && P.lmA != nullptr;
-    if (hu) publish_u(P, sm, us, P.lmA, P.r, d, nullptr, G);
-    TL(30);
-    gemv_phase(P, sm, pc, P.rt_v, nks_d, false, hu, G, stage_ctr, flushes, us, tl_n);
-    TL(31);
-    grid_sync(P, nbar, G);
-    TL(32);
-  }
+  TL(50);
   if (blockIdx.x == 0 && tid == 0) {
     u64 key = *(volatile u64*)&P.ctl->amax[0];
-    int t = (int)(0xFFFFFFFFu - (unsigned int)(key & 0xFFFFFFFFull));
-    *P.tok_out = t;
+    int tk = (int)(0xFFFFFFFFu - (unsigned int)(key & 0xFFFFFFFFull));
+    *P.tok_out = tk;
     P.ctl->amax[0] = 0ull;
     for (int j = 0; j < P.n_gates; ++j) {
       u64 kj = *(volatile u64*)&P.ctl->amax[1 + j];
@@ -1056,7 +1119,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const FP
       P.ctl->amax[1 + j] = 0ull;
     }
     P.ctl->ucnt = 0u;
-    if (P.advance) { *P.kv_len = pos + 1; *P.pending = t; }
+    if (P.advance) { *P.kv_len = pos + 1; *P.pending = tk; }
   }
 }
 
@@ -1123,7 +1186,7 @@ bool fused_config_ok(const m2r2_config& c) {
   if (c.head_dim % 8 || c.head_dim > 128) return false;
   if (c.d_model % 16 || c.d_ff % 8) return false;
   if (c.accel_enabled && (c.adapter_rank > MAX_R || c.adapter_rank < 1)) return false;
-  if (pad_to(c.d_model, STAGE_K) > KMAX || pad_to(c.d_ff, STAGE_K) > KMAX) return false;
+  if (pad_to(c.d_model, STAGE_K) > NORM_CH * NCT * 4 || pad_to(c.d_ff, STAGE_K) > KMAX) return false;
   if ((size_t)2 * NCW * 2 * (c.head_dim + 2) * sizeof(float) > (size_t)X_BYTES) return false;
   return true;
 }
@@ -1248,6 +1311,10 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     f.Kc = (bf16*)kv + (size_t)i * per;
     f.Vc = (bf16*)kv + (size_t)c.n_layers * per + (size_t)i * per;
     f.accel = (c.accel_enabled && i < c.accel_end_layer) ? 1 : 0;
+    if (f.accel && L.Aqkv && L.Bd) {   // Aqkv .. Bd are carved back to back (m2r2_api.cu walk_weights)
+      f.ad_lo = (const unsigned char*)L.Aqkv;
+      f.ad_bytes = (unsigned int)(((const unsigned char*)L.Bd + (size_t)d * c.adapter_rank * 2) - f.ad_lo);
+    }
     f.gate = 0;
     for (int j = 0; j < c.n_gates; ++j) if (c.gates[j] == i + 1) f.gate = j + 1;
   }
