@@ -186,7 +186,7 @@ __device__ __forceinline__ int unit_owner(int U, int u, int G) { return (int)(((
 __device__ __forceinline__ int phase_rot(int layer, int ph, int G) { return (int)(((unsigned)(layer * 5 + ph) * 29u) % (unsigned)G); }
 
 #ifdef M2R2_FUSED_DEBUG
-constexpr int TL_MAX = 1024;
+constexpr int TL_MAX = 2048;
 __device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 #define TL(ev) do { if (P.tl && threadIdx.x == 0 && tl_n < TL_MAX) { P.tl[(size_t)blockIdx.x * TL_MAX + tl_n] = (gtime() << 8) | (u64)(ev); ++tl_n; } } while (0)
 #else
