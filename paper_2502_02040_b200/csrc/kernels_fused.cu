@@ -1,34 +1,38 @@
-// kernels_fused.cu — persistent fused dual-stream decode pass, v2 (bf16 storage, dense FFN, batch 1).
+// kernels_fused.cu — persistent fused dual-stream decode pass, v3 (bf16 storage, dense FFN, batch 1).
 //
 // One cooperative launch runs a whole pass (a1-a9 of SURVEY §8(a)): embed, then per layer
-//   QKV   fused RMSNorm + QKV GEMV for h and p (+ adapters) with RoPE + KV append in the epilogue
-//   ATTN  split-K flash-decode attention, slow query and accelerated query on the same K/V loads
-//   OPROJ O-projection (split-K, partial sums to fixed slots)
-//   GATEUP residual + RMSNorm + gate/up GEMV + SwiGLU
-//   DOWN  down GEMV (split-K slots); the accelerated-residual update and the gate reset p <- h
-//          happen where the next phase loads the residual
+//   QKV    fused RMSNorm + QKV GEMV for h and p (+ adapters) with RoPE + KV append in the epilogue
+//   ATTN   split-K flash-decode attention, slow query and accelerated query on the same K/V loads
+//   OPROJ  O-projection, split-K: partial sums are added into the residual pair R = (h, p)
+//   GATEUP RMSNorm + gate/up GEMV + SwiGLU
+//   DOWN   down GEMV, split-K into R: the accelerated-residual update (Eq. 2); the gate reset p <- h
+//           happens where the next phase loads the residual
 // and the LM head + greedy argmax (final head on h_N, or exit/draft head on p at a gate).
 //
-// Design (DESIGN.md §"Fused decode kernel"): one CTA per SM, 8 consumer warps + 1 producer warp.
+// Design: one CTA per SM = 8 consumer warps + 1 producer warp + 1 auxiliary warp.
 //  * Weights are stored FRAGMENT-MAJOR: a tile = 16 output rows x 16 inputs laid out so that lane
-//    L's 16 bytes are its A fragment of mma.sync.m16n8k16; a stage = one row-tile x 1024 inputs =
-//    64 tiles = 32 KB contiguous; stages ordered (row-tile, k-stage).
-//  * Weights never depend on activations, so ONE producer thread per CTA streams the CTA's
-//    statically known stage sequence of the WHOLE pass through a 4-stage shared-memory ring with
-//    cp.async.bulk (UBLKCP) + mbarrier, and keeps an L2 prefetch window (cp.async.bulk.prefetch.L2)
-//    running further ahead, across phase boundaries and grid barriers: HBM stays busy while the
-//    consumers wait for activations.  The KV ranges a CTA will attend to are prefetched the same way.
+//    L's 16 bytes are its A fragment of mma.sync.m16n8k16; a stage = 64 tiles = 32 KB contiguous.
+//      row-owned matrices (QKV, gate/up, LM head): stage = one row-tile x 1024 inputs, ordered
+//        (row-tile, k-stage); a CTA owns whole row-tiles, its 8 warps split the 1024 inputs.
+//      split-K matrices (O, down): stage = 8 row-tiles x 128 inputs, ordered (row-tile group, k-chunk);
+//        a CTA owns a contiguous stage range, warp w owns row-tile w of the stage and accumulates in
+//        registers across the k-chunks of a group, then adds its 16x2 partial sums into R with
+//        red.global.add.f32.  A CTA therefore needs only its own <= ~12 k-chunks of the input vector.
+//  * Weights never depend on activations, so ONE producer thread per CTA streams the CTA's statically
+//    known stage sequence of the WHOLE pass through a 5-stage shared-memory ring with cp.async.bulk
+//    (UBLKCP) + mbarrier: HBM stays busy while the consumers sit in a barrier or a loader.
 //  * Consumers: one LDS.128 per lane = one A fragment; the B operand is the activation vector split
-//    into bf16 hi + lo parts (columns h_hi, h_lo, p_hi, p_lo of the n=8 tile), so the product is
-//    exact to ~2^-17 and accumulates in fp32 on the tensor pipe (HMMA) at ~2 instructions per 256
-//    weights.  It is a GEMV, not a contraction: the tensor pipe is used as a wide FMA, the bound is HBM.
-//  * Row-owned phases (QKV, GATEUP, heads): a CTA owns whole row-tiles, epilogue is local.
-//    Split-K phases (OPROJ, DOWN): a CTA owns a contiguous stage range; partial sums of a row-tile go
-//    to slot (contributor index); the NEXT phase's loader adds residual + slots in slot order
-//    (deterministic, no tickets, no atomics on data).
-//  * Adapter down-projections u = A x^ are computed distributed (each CTA one row
-//    chunk) right after the loader, published with a release counter, and picked up at the first
-//    epilogue of the phase.
+//    into bf16 hi + lo parts (columns h_hi, h_lo, p_hi, p_lo of the n=8 tile), so products are exact
+//    to ~2^-17 and accumulate in fp32 on the tensor pipe.  It is a GEMV: the bound is HBM.
+//  * What every CTA must read of the other CTAs' results is kept minimal, because those replicated
+//    L2 reads (148 x the vector) share the L2->SM path with the weight stream: row-owned phases read
+//    the 24 KB residual pair, split-K phases read only their slice of the attention output / SwiGLU
+//    activations.
+//  * Epilogues of row-owned phases are deferred: partial sums of up to 8 finished row-tiles wait in
+//    shared memory and are finished by all 8 warps at once.
+//  * The auxiliary warp computes the adapter down-projections u = A x^ distributed
+//    over the CTAs (one row chunk each, published with a release counter), gathers them, and either
+//    hands u to the consumers' epilogue (QKV, GATEUP, heads) or adds B u into R.p itself (OPROJ, DOWN).
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
@@ -43,26 +47,27 @@ namespace {
 typedef __nv_bfloat16 bf16;
 typedef unsigned long long u64;
 
-constexpr int STAGE_K = 1024;                  // inputs per stage
-constexpr int STAGE_TILES = STAGE_K / 16;      // 64 m16k16 tiles
+constexpr int STAGE_K = 1024;                  // inputs per row-owned stage
+constexpr int STAGE_TILES = 64;                // m16k16 tiles per stage
 constexpr int STAGE_BYTES = STAGE_TILES * 512; // 32 KB
-constexpr int NSTAGE = 4;
+constexpr int SK_K = 128;                      // inputs per split-K stage
+constexpr int SK_RT = 8;                       // row-tiles per split-K stage
+constexpr int NSTAGE = 5;
 constexpr int NCW = 8;                 // consumer warps
 constexpr int NCT = NCW * 32;          // consumer threads
-constexpr int NTHREADS = NCT + 32;     // + producer warp
+constexpr int NTHREADS = NCT + 64;     // + producer warp + auxiliary warp
 constexpr int TPW = STAGE_TILES / NCW; // tiles per warp per stage (8)
-constexpr int KMAX = 8192;             // largest padded inner dimension
-constexpr int XCOL = KMAX + 8;         // bf16 elements per activation column (+8: LDS.128 bank spread)
+constexpr int XMAX = 4096;             // inputs held in shared memory (d_pad limit; 32 split-K chunks)
+constexpr int XSLOTS = XMAX / SK_K;
+constexpr int XCOL = XMAX + 8;         // bf16 elements per activation column (+8: LDS.128 bank spread)
 constexpr int X_BYTES = 4 * XCOL * 2;  // h_hi, h_lo, p_hi, p_lo
-constexpr int RED_FLOATS = 2 * NCW * 32;
-constexpr int MISC_BYTES = RED_FLOATS * 4 + 4096;
-constexpr int SMEM_BYTES = NSTAGE * STAGE_BYTES + X_BYTES + MISC_BYTES;
-constexpr int MAX_R = 16;              // adapter rank limit
+constexpr int KMAX = 16384;            // largest inner dimension of a split-K matrix
+constexpr int FB = 8;                  // finished row-tiles whose epilogue is deferred (one per warp)
+constexpr int RED_FLOATS = FB * NCW * 32;
+constexpr int MAX_R = 8;               // adapter rank limit (PAPER.md L399 uses 8); larger ranks take the per-operation kernels
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
-constexpr int MAX_SLOTS = KMAX / STAGE_K;
 constexpr int NORM_CH = 4;             // float4 chunks per thread in a norm loader (d <= 4096)
-constexpr int PF_DEFAULT = 10;         // L2 prefetch window, stages ahead of the ring
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
 
 enum { PH_QKV = 0, PH_OPROJ = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4, PH_EXIT = 5, N_PH = 6 };
@@ -71,6 +76,7 @@ struct FLayer {
   const uint4 *Wqkv, *Wo, *Wgu, *Wd;   // fragment-major
   const bf16 *g1, *g2;
   const bf16 *Aqkv, *Bqkv, *Ao, *Bo, *Agu, *Bg, *Bu, *Ad, *Bd;
+  const bf16 *AdT, *AoT;                // A_d transposed [F][r], A_o transposed [da][r] (fused copies)
   bf16 *Kc, *Vc;                        // this layer's cache, sequence 0: [head][max_seq][dh]
   int accel;                            // layer carries p
   int gate;                             // 1 + gate index if layer+1 is a gate E_j, else 0
@@ -82,14 +88,14 @@ struct Ctl {
   unsigned int bar;        // grid-barrier arrivals (monotonic across launches)
   unsigned int abort_flag; // a wait timed out
   unsigned int abort_where;
-  unsigned int ucnt;       // adapter-partial publications of this launch (reset at its end)
   u64 amax[1 + M2R2_MAX_GATES];   // argmax keys: [0] head of the pass, [1+j] exit head of gate j
 };
 
 struct FParams {
   int n_layers_run, d, n_heads, dh, F, V, r, da, max_seq;
-  int d_pad, F_pad;
-  int rt_qkv, rt_o, rt_gu, rt_d, rt_v;    // row-tiles per matrix
+  int d_pad, F_pad;                       // d padded to 1024 (row-owned K), F padded to 128 (split-K K)
+  int rt_qkv, rt_gu, rt_v;                // row-tiles of the row-owned matrices
+  int ng_d;                               // row-tile groups (128 rows) of the split-K matrices (n_out = d)
   float eps, scale;
   const FLayer* layers;
   const bf16 *embed, *gf, *lmA, *lmB;
@@ -101,11 +107,13 @@ struct FParams {
   int* tok_out;
   int* exit_tok;
   int n_gates, exit_heads, advance, head_stream, joff, do_trace, head_gate;
-  float *RA, *RB;            // residual pair [2][d]: RA = (h', p') after attention; RB = (h_i, p_i) entering a layer
-  float *oslots, *dslots;    // [MAX_SLOTS][2][d] split-K partial sums of OPROJ / DOWN
-  float *act, *qbuf, *khat, *vhat, *pexit;
+  float* R;                  // residual pair [2][d]: h then p; split-K phases add into it
+  float *act, *qbuf, *khat, *vhat;
   float *apart;              // [head][split][2][dh+4]
-  float *upart;              // [2][MAX_NJ][UPART_Q]
+  u64 *upart;                // [MAX_NJ][UPART_Q] (epoch << 32 | fp32 bits)
+  float *apu;                // [head][split][MAX_R]: A_o applied to the unnormalised accelerated attention partial
+  float *udpart;             // [CTA][MAX_R]: A_d applied to the CTA's own accelerated SwiGLU activations
+  int nah;                   // accelerated heads
   float *trace, *logits, *exit_logits;
   Ctl* ctl;
   unsigned int bar_base;
@@ -114,9 +122,30 @@ struct FParams {
   float ls_beta;
   int ns;        // attention splits
   int pos_host;  // kv_len + joff as the host knows it (producer-side KV prefetch only)
-  int pf_ahead;  // L2 prefetch window in stages
   u64* tl;       // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
 };
+
+// ------------------------------------------------------------------ shared memory map (fixed offsets)
+constexpr int OFF_X = NSTAGE * STAGE_BYTES;
+constexpr int OFF_RED = OFF_X + X_BYTES;              // [FB][NCW][32] floats
+constexpr int OFF_TILE = OFF_RED + RED_FLOATS * 4;    // [NCW][32] floats
+constexpr int OFF_U = OFF_TILE + NCW * 32 * 4;        // [MAX_NJ] floats (64 reserved)
+constexpr int OFF_SRED = OFF_U + 256;                 // [64] floats
+constexpr int OFF_BAR = OFF_SRED + 256;               // full[NSTAGE], empty[NSTAGE]
+constexpr int OFF_UTMP = OFF_BAR + 256;               // [256] floats
+constexpr int OFF_FRT = OFF_UTMP + 1024;              // [FB] ints: row-tile of each deferred flush
+constexpr int OFF_UD = OFF_FRT + 64;                  // [NCW][MAX_R] floats: per-warp A_d partials of the GATEUP phase
+constexpr int OFF_SIDX = OFF_UD + NCW * MAX_R * 4;    // [M2R2_MAX_HEADS] ints: head -> index in S or -1
+constexpr int MAXL_S = 64;                            // layers whose descriptors are cached in shared memory
+constexpr int OFF_LAYERS = OFF_SIDX + M2R2_MAX_HEADS * 4;   // [MAXL_S] FLayer
+constexpr int OFF_TLN = OFF_LAYERS + MAXL_S * (int)sizeof(FLayer); // debug timeline cursor
+constexpr int SMEM_BYTES = OFF_TLN + 64;
+static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
+extern __shared__ __align__(1024) unsigned char smem_raw[];
+__device__ __forceinline__ int sidx_of(int head) { return ((const int*)(smem_raw + OFF_SIDX))[head]; }
+// layer descriptors live in shared memory: every phase of every role reads them, and a global copy would
+// cost an L2 round trip after each grid barrier (its fence drops L1)
+__device__ __forceinline__ const FLayer* lay(int i) { return (const FLayer*)(smem_raw + OFF_LAYERS) + i; }
 
 // ------------------------------------------------------------------ PTX helpers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -146,6 +175,12 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
+__device__ __forceinline__ void bulk_g2s_plain(void* dst, const void* src, uint32_t bytes, u64* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+      ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
 __device__ __forceinline__ void bulk_prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
@@ -154,11 +189,18 @@ __device__ __forceinline__ u64 policy_evict_first() {
   asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
   return p;
 }
+// named barriers: 1 = the consumer warps; 2 = "phase input ready" (consumers arrive, auxiliary warp
+// waits); 3 = "auxiliary work of the phase done" (auxiliary warp arrives, consumers wait)
 __device__ __forceinline__ void bar_consumers() { asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(NCT + 32) : "memory"); }
+__device__ __forceinline__ void bar_wait(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(NCT + 32) : "memory"); }
 __device__ __forceinline__ unsigned int ld_acquire(const unsigned int* p) {
   unsigned int v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
+}
+__device__ __forceinline__ void red_add(float* p, float v) {
+  asm volatile("red.global.add.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
 }
 __device__ __forceinline__ float ldcg(const float* p) { return __ldcg(p); }
 __device__ __forceinline__ float4 ldcg4(const float* p) { return __ldcg((const float4*)p); }
@@ -179,29 +221,18 @@ __device__ __forceinline__ u64 amax_key(float v, int n) {
 }
 
 // ------------------------------------------------------------------ static work split
-// A phase has S stages (row-tile-major).  Virtual CTA v of G owns units [U*v/G, U*(v+1)/G) where a
-// unit is `gran` consecutive stages (gran = stages per row-tile for row-owned phases, 1 for split-K).
+// A phase has S stages.  Virtual CTA v of G owns units [U*v/G, U*(v+1)/G) where a unit is `gran`
+// consecutive stages (gran = stages per row-tile for row-owned phases, 1 for split-K).
 __device__ __forceinline__ int range_lo(int U, int v, int G) { return (int)(((long long)U * v) / G); }
-__device__ __forceinline__ int unit_owner(int U, int u, int G) { return (int)((((long long)(u + 1)) * G + U - 1) / U) - 1; }
 __device__ __forceinline__ int phase_rot(int layer, int ph, int G) { return (int)(((unsigned)(layer * 5 + ph) * 29u) % (unsigned)G); }
 
 #ifdef M2R2_FUSED_DEBUG
-constexpr int TL_MAX = 2048;
+constexpr int TL_MAX = 4096;
 __device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define TL(ev) do { if (P.tl && threadIdx.x == 0 && tl_n < TL_MAX) { P.tl[(size_t)blockIdx.x * TL_MAX + tl_n] = (gtime() << 8) | (u64)(ev); ++tl_n; } } while (0)
+#define TL(ev) do { int* tlp_ = (int*)(smem_raw + OFF_TLN); if (P.tl && threadIdx.x == 0 && *tlp_ < TL_MAX) { P.tl[(size_t)blockIdx.x * TL_MAX + *tlp_] = (gtime() << 8) | (u64)(ev); ++*tlp_; } } while (0)
 #else
 #define TL(ev) do { } while (0)
 #endif
-
-// ------------------------------------------------------------------ shared memory map (fixed offsets: every access stays in the shared window)
-constexpr int OFF_X = NSTAGE * STAGE_BYTES;
-constexpr int OFF_RED = OFF_X + X_BYTES;              // [2][NCW][32] floats
-constexpr int OFF_TILE = OFF_RED + RED_FLOATS * 4;    // [16][2] floats
-constexpr int OFF_U = OFF_TILE + 256;                 // [MAX_NJ] floats
-constexpr int OFF_SRED = OFF_U + 256;                 // [64] floats
-constexpr int OFF_BAR = OFF_SRED + 256;               // full[NSTAGE], empty[NSTAGE]
-constexpr int OFF_UTMP = OFF_BAR + 256;               // [256] floats
-static_assert(OFF_UTMP + 1024 <= SMEM_BYTES, "shared memory map");
 
 __device__ __forceinline__ void set_abort(Ctl* ctl, unsigned int where) {
   if (atomicExch(&ctl->abort_flag, 1u) == 0u) ctl->abort_where = where;
@@ -250,124 +281,96 @@ __device__ __forceinline__ int xpos(int k) {
   const int o = k & 15;
   return (k & ~63) + (((o & 7) >> 1) << 4) + (((k >> 4) & 3) << 2) + ((o >> 3) << 1) + (o & 1);
 }
-__device__ __forceinline__ uint32_t pack_bf16(bf16 a, bf16 b) {
-  return (uint32_t)__bfloat16_as_ushort(a) | ((uint32_t)__bfloat16_as_ushort(b) << 16);
-}
-// store x[k..k+3] (k % 4 == 0) as hi + lo parts into the column pair (hi, lo)
+__device__ __forceinline__ uint32_t bf2_u32(__nv_bfloat162 v) { return *(uint32_t*)&v; }
+// store x[k..k+3] (k % 4 == 0) as hi + lo parts into the column pair (hi, lo); packed conversions
 __device__ __forceinline__ void xstore4(bf16* hi, bf16* lo, int k, float4 v) {
   const int p = xpos(k);
-  const bf16 h0 = __float2bfloat16_rn(v.x), h1 = __float2bfloat16_rn(v.y), h2 = __float2bfloat16_rn(v.z), h3 = __float2bfloat16_rn(v.w);
-  const bf16 l0 = __float2bfloat16_rn(v.x - __bfloat162float(h0)), l1 = __float2bfloat16_rn(v.y - __bfloat162float(h1));
-  const bf16 l2 = __float2bfloat16_rn(v.z - __bfloat162float(h2)), l3 = __float2bfloat16_rn(v.w - __bfloat162float(h3));
-  *(uint32_t*)(hi + p) = pack_bf16(h0, h1);
-  *(uint32_t*)(hi + p + 16) = pack_bf16(h2, h3);
-  *(uint32_t*)(lo + p) = pack_bf16(l0, l1);
-  *(uint32_t*)(lo + p + 16) = pack_bf16(l2, l3);
+  const __nv_bfloat162 h01 = __floats2bfloat162_rn(v.x, v.y), h23 = __floats2bfloat162_rn(v.z, v.w);
+  const float2 f01 = __bfloat1622float2(h01), f23 = __bfloat1622float2(h23);
+  const __nv_bfloat162 l01 = __floats2bfloat162_rn(v.x - f01.x, v.y - f01.y), l23 = __floats2bfloat162_rn(v.z - f23.x, v.w - f23.y);
+  *(uint32_t*)(hi + p) = bf2_u32(h01);
+  *(uint32_t*)(hi + p + 16) = bf2_u32(h23);
+  *(uint32_t*)(lo + p) = bf2_u32(l01);
+  *(uint32_t*)(lo + p + 16) = bf2_u32(l23);
 }
 __device__ __forceinline__ float xval(const bf16* hi, const bf16* lo, int k) {
   const int p = xpos(k);
   return __bfloat162float(hi[p]) + __bfloat162float(lo[p]);
 }
-__device__ __forceinline__ float4 f4add(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
 __device__ __forceinline__ float f4ss(float4 a) { return a.x * a.x + a.y * a.y + a.z * a.z + a.w * a.w; }
 __device__ __forceinline__ void st4(float* p, float4 v) { __stcg((float4*)p, v); }
 
-// contributors of row-tile rt in a split-K phase of n_rt x nks stages
-__device__ __forceinline__ int n_contrib(int n_rt, int nks, int rt, int G) {
-  const int S = n_rt * nks;
-  if (S < G) return nks;
-  return unit_owner(S, rt * nks + nks - 1, G) - unit_owner(S, rt * nks, G) + 1;
-}
-
 enum { LN_QKV = 0, LN_GU = 1, LN_HEAD_H = 2, LN_HEAD_P = 3 };
 
-// Residual loader of the norm phases.  Every CTA rebuilds the full residual pair
-//   (h, p) = base + sum over split-K slots of the producing phase      (Eq. 1 / Eq. 2 residual adds)
-// applies the gate  p <- h when the producing layer ends at a gate, writes its
-// share of the pair back (wb), and leaves x = rms(.; g) of both streams in shared memory.
+// Residual loader of the row-owned phases.  Every CTA reads the residual pair (h, p) from R (or the
+// embedding row at the start of the pass: p_0 <- h_0), applies the gate p <- h
+// (L82, L101) when the producing layer ends at a gate, and leaves x = rms(.; g) of both streams in
+// shared memory.  The chunk's owner CTA writes back what changed (embedding, gate) and the trace.
 struct LoadSrc {
-  const float* base;     // [2][d] or nullptr (then emb)
-  const bf16* emb;       // embedding row
-  const float* slots;    // or nullptr
-  int n_rt, nks;         // geometry of the producing split-K phase
+  const bf16* emb;       // embedding row, or nullptr (then R)
   bool p_live;           // the producing layer carried p
-  int gate;              // 1 + gate index: emit pexit, then p <- h
+  int gate;              // 1 + gate index: p <- h
 };
-__device__ __forceinline__ void loader_norm(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src, float* wb,
-                                            float* trace_dst, const bf16* g, int G) {
+template <int NCH>
+__device__ __noinline__ void loader_norm_t(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src,
+                                           float* trace_dst, const bf16* g, int G) {
   const int tid = threadIdx.x, d = P.d;
   bar_consumers();   // x of the previous phase is dead in every warp
-  float4 xh[NORM_CH], xp[NORM_CH];
-  uint2 ge[NORM_CH];
-  float ssh = 0.f, ssp = 0.f;
+  TL(64);
+  float4 xh[NCH], xp[NCH];
+  uint2 ge[NCH];
+  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-  for (int j = 0; j < NORM_CH; ++j) {
-    const int ci = tid + j * NCT, k = ci * 4;
-    xh[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-    xp[j] = xh[j];
+  for (int j = 0; j < NCH; ++j) {   // all loads first: one L2 round trip
+    const int k = (tid + j * NCT) * 4;
+    xh[j] = z4; xp[j] = z4;
     ge[j] = make_uint2(0u, 0u);
     if (k < d) {
-      // every load of this chunk is independent of the others: one L2 round trip
       ge[j] = __ldg((const uint2*)(g + k));
-      float4 hv, pv;
-      if (src.base) {
-        hv = ldcg4(src.base + k);
-        pv = src.p_live ? ldcg4(src.base + d + k) : hv;
-      } else {
+      if (src.emb) {
         const uint2 e = __ldg((const uint2*)(src.emb + k));
-        bf16x2_to_f32(e.x, hv.x, hv.y);
-        bf16x2_to_f32(e.y, hv.z, hv.w);
-        pv = hv;
+        bf16x2_to_f32(e.x, xh[j].x, xh[j].y);
+        bf16x2_to_f32(e.y, xh[j].z, xh[j].w);
+      } else {
+        xh[j] = ldcg4(P.R + k);
+        if (src.p_live) xp[j] = ldcg4(P.R + d + k);
       }
-      if (src.slots) {
-        const int nc = n_contrib(src.n_rt, src.nks, k >> 4, G);
-        float4 sh[3], sp[3];
+    }
+  }
+  float ssh = 0.f, ssp = 0.f;
 #pragma unroll
-        for (int sl = 0; sl < 3; ++sl) {
-          sh[sl] = make_float4(0.f, 0.f, 0.f, 0.f);
-          sp[sl] = sh[sl];
-          if (sl < nc) {
-            sh[sl] = ldcg4(src.slots + (size_t)(sl * 2) * d + k);
-            if (src.p_live) sp[sl] = ldcg4(src.slots + (size_t)(sl * 2 + 1) * d + k);
-          }
-        }
-#pragma unroll
-        for (int sl = 0; sl < 3; ++sl) {
-          if (sl < nc) { hv = f4add(hv, sh[sl]); pv = f4add(pv, sp[sl]); }
-        }
-        for (int sl = 3; sl < nc; ++sl) {
-          hv = f4add(hv, ldcg4(src.slots + (size_t)(sl * 2) * d + k));
-          if (src.p_live) pv = f4add(pv, ldcg4(src.slots + (size_t)(sl * 2 + 1) * d + k));
-        }
-      }
-      if (!src.p_live) pv = hv;
+  for (int j = 0; j < NCH; ++j) {
+    const int ci = tid + j * NCT, k = ci * 4;
+    if (k < d) {
+      const float4 hv = xh[j];
+      float4 pv = src.p_live ? xp[j] : hv;
       const bool owner = (ci % G) == (int)blockIdx.x;
       const float4 pbefore = pv;
-      if (src.gate) {
-        if (owner) st4(P.pexit + (size_t)(src.gate - 1) * d + k, pv);
-        pv = hv;
-      }
+      if (src.gate) pv = hv;
       if (owner && trace_dst) { st4(trace_dst + k, hv); st4(trace_dst + d + k, pbefore); }
-      if (owner && wb) { st4(wb + k, hv); st4(wb + d + k, pv); }
+      if (owner && src.emb) st4(P.R + k, hv);
+      if (owner && (src.emb || src.gate || !src.p_live)) st4(P.R + d + k, pv);
       if (mode == LN_HEAD_P) { xh[j] = pbefore; xp[j] = pbefore; }
-      else if (mode == LN_HEAD_H) { xh[j] = hv; xp[j] = hv; }
-      else { xh[j] = hv; xp[j] = pv; }
+      else if (mode == LN_HEAD_H) { xp[j] = hv; }
+      else { xp[j] = pv; }
       ssh += f4ss(xh[j]);
       ssp += f4ss(xp[j]);
     }
   }
+  TL(65);
   ssh = warp_sum(ssh);
   ssp = warp_sum(ssp);
   if ((tid & 31) == 0) { sred[tid >> 5] = ssh; sred[NCW + (tid >> 5)] = ssp; }
   bar_consumers();
+  TL(66);
   float th = 0.f, tp = 0.f;
 #pragma unroll
   for (int w = 0; w < NCW; ++w) { th += sred[w]; tp += sred[NCW + w]; }
   const float ih = rsqrtf(th / (float)d + P.eps), ip = rsqrtf(tp / (float)d + P.eps);
   bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
 #pragma unroll
-  for (int j = 0; j < NORM_CH; ++j) {
-    const int ci = tid + j * NCT, k = ci * 4;
+  for (int j = 0; j < NCH; ++j) {
+    const int k = (tid + j * NCT) * 4;
     if (k < P.d_pad) {
       float4 a = xh[j], b = xp[j];
       if (k < d) {
@@ -383,125 +386,226 @@ __device__ __forceinline__ void loader_norm(const FParams& P, bf16* x, float* sr
   }
   bar_consumers();
 }
-
-// x <- attention output of both queries: merge of the split partials (m, l, o) in split order (a4)
-__device__ __forceinline__ void loader_attn(const FParams& P, bf16* x, bool accel) {
-  const int tid = threadIdx.x, d = P.d, dh = P.dh, NS = P.ns;
-  bar_consumers();
-  bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
-  for (int idx = tid; idx < 2 * (P.d_pad >> 2); idx += NCT) {
-    const int q = idx >= (P.d_pad >> 2), k = (idx - q * (P.d_pad >> 2)) * 4;
-    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (k < d) {
-      const int head = k / dh, j = k - head * dh;
-      if (q == 0 || (accel && P.sidx[head] >= 0)) {
-        const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
-        float M = -INFINITY;
-        for (int s = 0; s < NS; ++s) {
-          const float* ps = pp + (size_t)s * 2 * (dh + 4);
-          if (ldcg(ps + dh + 1) > 0.f) M = fmaxf(M, ldcg(ps + dh));
-        }
-        float Lsum = 0.f;
-        for (int s = 0; s < NS; ++s) {
-          const float* ps = pp + (size_t)s * 2 * (dh + 4);
-          const float ls = ldcg(ps + dh + 1);
-          if (ls > 0.f) {
-            const float wgt = __expf(ldcg(ps + dh) - M);
-            const float4 v = ldcg4(ps + j);
-            Lsum += ls * wgt;
-            o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
-          }
-        }
-        const float inv = 1.f / Lsum;
-        o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
-      }
-    }
-    if (q == 0) xstore4(c0, c1, k, o); else xstore4(c2, c3, k, o);
-  }
-  bar_consumers();
+__device__ __forceinline__ void loader_norm(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src,
+                                            float* trace_dst, const bf16* g, int G) {
+  const int nch = (P.d_pad >> 2) / NCT;   // d_pad is a multiple of 1024 = 4 * NCT
+  if (nch <= 1) loader_norm_t<1>(P, x, sred, mode, src, trace_dst, g, G);
+  else if (nch == 2) loader_norm_t<2>(P, x, sred, mode, src, trace_dst, g, G);
+  else if (nch == 3) loader_norm_t<3>(P, x, sred, mode, src, trace_dst, g, G);
+  else loader_norm_t<NORM_CH>(P, x, sred, mode, src, trace_dst, g, G);
 }
 
-// x <- SwiGLU activations of both streams (a7 input)
-__device__ __forceinline__ void loader_act(const FParams& P, bf16* x, bool accel) {
+// Merge of the attention split partials (m, l, o) of one query for columns k..k+3 of a head (a4).
+constexpr int MERGE_NS = 4;   // splits merged from registers; more splits take the looped path
+struct MergeRegs {
+  float4 o[MERGE_NS];
+  float2 ml[MERGE_NS];
+};
+__device__ __forceinline__ void merge_load(const FParams& P, MergeRegs& m, int q, int k) {
+  const int dh = P.dh, NS = P.ns, head = k / dh, j = k - head * dh;
+  const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
+#pragma unroll
+  for (int s = 0; s < MERGE_NS; ++s) {
+    m.o[s] = make_float4(0.f, 0.f, 0.f, 0.f);
+    m.ml[s] = make_float2(0.f, 0.f);
+    if (s < NS) {
+      const float* ps = pp + (size_t)s * 2 * (dh + 4);
+      m.o[s] = ldcg4(ps + j);
+      m.ml[s] = __ldcg((const float2*)(ps + dh));
+    }
+  }
+}
+__device__ __forceinline__ float4 merge_finish(const FParams& P, const MergeRegs& m, int q, int k) {
+  const int dh = P.dh, NS = P.ns;
+  float M = -INFINITY, Lsum = 0.f;
+  float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (NS <= MERGE_NS) {
+#pragma unroll
+    for (int s = 0; s < MERGE_NS; ++s) if (s < NS && m.ml[s].y > 0.f) M = fmaxf(M, m.ml[s].x);
+#pragma unroll
+    for (int s = 0; s < MERGE_NS; ++s) {
+      if (s < NS && m.ml[s].y > 0.f) {
+        const float wgt = __expf(m.ml[s].x - M);
+        Lsum += m.ml[s].y * wgt;
+        o.x += m.o[s].x * wgt; o.y += m.o[s].y * wgt; o.z += m.o[s].z * wgt; o.w += m.o[s].w * wgt;
+      }
+    }
+  } else {
+    const int head = k / dh, j = k - head * dh;
+    const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
+    for (int s = 0; s < NS; ++s) {
+      const float* ps = pp + (size_t)s * 2 * (dh + 4);
+      if (ldcg(ps + dh + 1) > 0.f) M = fmaxf(M, ldcg(ps + dh));
+    }
+    for (int s = 0; s < NS; ++s) {
+      const float* ps = pp + (size_t)s * 2 * (dh + 4);
+      const float ls = ldcg(ps + dh + 1);
+      if (ls > 0.f) {
+        const float wgt = __expf(ldcg(ps + dh) - M);
+        const float4 v = ldcg4(ps + j);
+        Lsum += ls * wgt;
+        o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
+      }
+    }
+  }
+  const float inv = 1.f / Lsum;
+  o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+  return o;
+}
+
+// Input slice of a split-K phase: the CTA's stages [s0, s1) of a matrix with nkc k-chunks per row-tile
+// group touch chunks kc0, kc0+1, ... (mod nkc), cnt of them; chunk kc lives in x slot kc % XSLOTS.
+//   OPROJ: merged attention output of both queries (the accelerated stream has columns of S only)
+//   DOWN:  SwiGLU activations of both streams
+__device__ __noinline__ void loader_slice(const FParams& P, bf16* x, int ph, bool accel, int kc0, int cnt, int nkc) {
   const int tid = threadIdx.x;
   bar_consumers();
   bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
-  for (int idx = tid; idx < (P.F_pad >> 2); idx += NCT) {
-    const int k = idx * 4;
-    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
-    if (k < P.F) {
-      a = ldcg4(P.act + k);
-      if (accel) b = ldcg4(P.act + P.F_pad + k);
+  const int items = cnt * 64;   // (chunk, stream, float4)
+  const int K = ph == PH_OPROJ ? P.d : P.F;
+  constexpr int MC = 2;
+  for (int base = 0; base < items; base += NCT * MC) {
+    if (ph == PH_OPROJ) {
+      MergeRegs mr[MC];
+      int kk[MC], xs[MC], qq[MC];
+#pragma unroll
+      for (int c = 0; c < MC; ++c) {
+        const int it = base + tid + c * NCT;
+        kk[c] = -1; xs[c] = 0; qq[c] = 0;
+        if (it < items) {
+          const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
+          int kc = kc0 + i;
+          if (kc >= nkc) kc -= nkc;
+          const int k = kc * SK_K + c4 * 4;
+          xs[c] = (kc % XSLOTS) * SK_K + c4 * 4;
+          qq[c] = q;
+          const bool live = k < K && (q == 0 || (accel && sidx_of(k / P.dh) >= 0));
+          kk[c] = live ? k : -2;
+          if (live && P.ns <= MERGE_NS) merge_load(P, mr[c], q, k);
+        }
+      }
+#pragma unroll
+      for (int c = 0; c < MC; ++c) {
+        if (kk[c] != -1) {
+          float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (kk[c] >= 0) o = merge_finish(P, mr[c], qq[c], kk[c]);
+          if (qq[c] == 0) xstore4(c0, c1, xs[c], o); else xstore4(c2, c3, xs[c], o);
+        }
+      }
+    } else {
+      float4 v[MC];
+      int xs[MC], qq[MC];
+#pragma unroll
+      for (int c = 0; c < MC; ++c) {
+        const int it = base + tid + c * NCT;
+        xs[c] = -1; qq[c] = 0;
+        v[c] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (it < items) {
+          const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
+          int kc = kc0 + i;
+          if (kc >= nkc) kc -= nkc;
+          const int k = kc * SK_K + c4 * 4;
+          xs[c] = (kc % XSLOTS) * SK_K + c4 * 4;
+          qq[c] = q;
+          if (k < K && (q == 0 || accel)) v[c] = ldcg4(P.act + (size_t)q * P.F_pad + k);
+        }
+      }
+#pragma unroll
+      for (int c = 0; c < MC; ++c) {
+        if (xs[c] >= 0) {
+          if (qq[c] == 0) xstore4(c0, c1, xs[c], v[c]); else xstore4(c2, c3, xs[c], v[c]);
+        }
+      }
     }
-    xstore4(c0, c1, k, a);
-    xstore4(c2, c3, k, b);
   }
   bar_consumers();
 }
 
-// Adapter down-projection u = A x^ of the accelerated row, distributed: CTA c computes
-// row j = c / q over k-chunk c % q and publishes it; fetch_u() sums the q chunks of every row in order.
+// ------------------------------------------------------------------ auxiliary warp: adapter down-projections
+// u = A x^ of the accelerated row in the row-owned phases, distributed: CTA c computes row
+// j = c / q over k-chunk c % q and publishes (value, epoch) as ONE 8-byte store; every CTA's fetch_u() polls
+// the nj * q entries until they carry the phase's epoch, then sums the q chunks of every row in chunk order
+// (deterministic).  No counter, no fence: two L2 round trips from "x ready" to "u ready".
 struct UState {
-  unsigned int target;   // publications expected so far in this launch
-  int buf;               // upart buffer of the current phase
+  unsigned int epoch;    // epoch of the current phase (unique per launch and phase, never 0)
   int nj, q;             // geometry of the current phase
-  bool ready;            // warp 0: smem u holds the current phase's u
 };
-__device__ __forceinline__ void publish_u(const FParams& P, const bf16* x, UState& us, const bf16* A, int nj, int Kc,
-                                          const int* cols, int G) {
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int q = min(min(G / nj, UPART_Q), 256 / nj);
-  us.buf ^= 1;
+constexpr int AW = 2;    // A-row chunks (256 inputs each) loaded before the phase's input is ready
+struct APre {
+  uint4 w[AW];
+};
+__device__ __forceinline__ void u_geometry(UState& us, int nj, int G) {
   us.nj = nj;
-  us.q = q;
-  us.target += (unsigned int)(nj * q);
-  us.ready = false;
-  const int c = blockIdx.x;
-  if (warp == 1 && c < nj * q) {
-    const int j = c / q, ch = c - j * q;
-    const int chunk = (((Kc + q - 1) / q) + 7) & ~7;
+  us.q = min(min(G / nj, UPART_Q), 256 / nj);
+}
+__device__ __forceinline__ void publish_prefetch(const UState& us, APre& ap, const bf16* A, int Kc) {
+  const int lane = threadIdx.x & 31, c = blockIdx.x;
+#pragma unroll
+  for (int i = 0; i < AW; ++i) ap.w[i] = make_uint4(0u, 0u, 0u, 0u);
+  if (c < us.nj * us.q) {
+    const int j = c / us.q, ch = c - j * us.q;
+    const int chunk = (((Kc + us.q - 1) / us.q) + 7) & ~7;
+    const int k0 = ch * chunk, k1 = min(Kc, k0 + chunk);
+    const bf16* a = A + (size_t)j * Kc;
+#pragma unroll
+    for (int i = 0; i < AW; ++i) {
+      const int k = k0 + lane * 8 + i * 256;
+      if (k < k1) ap.w[i] = __ldg((const uint4*)(a + k));
+    }
+  }
+}
+__device__ __forceinline__ void publish_u(const FParams& P, const bf16* x, const UState& us, const APre& ap, const bf16* A, int Kc) {
+  const int lane = threadIdx.x & 31, c = blockIdx.x;
+  if (c < us.nj * us.q) {
+    const int j = c / us.q, ch = c - j * us.q;
+    const int chunk = (((Kc + us.q - 1) / us.q) + 7) & ~7;
     const int k0 = ch * chunk, k1 = min(Kc, k0 + chunk);
     const bf16* a = A + (size_t)j * Kc;
     const bf16 *xh = x + 2 * XCOL, *xl = x + 3 * XCOL;
     float acc = 0.f;
-    for (int k = k0 + lane * 8; k < k1; k += 256) {   // chunk and Kc are multiples of 8
-      const uint4 w = __ldg((const uint4*)(a + k));
+    int it = 0;
+    for (int k = k0 + lane * 8; k < k1; k += 256, ++it) {   // chunk and Kc are multiples of 8
+      uint4 w;
+      if (it == 0) w = ap.w[0];
+      else if (it == 1) w = ap.w[1];
+      else w = __ldg((const uint4*)(a + k));
       float f[8];
       bf16x2_to_f32(w.x, f[0], f[1]); bf16x2_to_f32(w.y, f[2], f[3]);
       bf16x2_to_f32(w.z, f[4], f[5]); bf16x2_to_f32(w.w, f[6], f[7]);
 #pragma unroll
-      for (int e = 0; e < 8; ++e) acc += f[e] * xval(xh, xl, cols ? cols[k + e] : k + e);
+      for (int e = 0; e < 8; ++e) acc += f[e] * xval(xh, xl, k + e);
     }
     acc = warp_sum(acc);
     if (lane == 0) {
-      __stcg(P.upart + ((size_t)us.buf * MAX_NJ + j) * UPART_Q + ch, acc);
-      __threadfence();
-      atomicAdd(&P.ctl->ucnt, 1u);
+      const u64 v = ((u64)us.epoch << 32) | (u64)__float_as_uint(acc);
+      asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(P.upart + (size_t)j * UPART_Q + ch), "l"(v) : "memory");
     }
   }
 }
-// warp 0 only
-__device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp, UState& us) {
+__device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp, const UState& us) {
   const int lane = threadIdx.x & 31;
-  if (lane == 0) {
-    long long t0 = clock64();
-    unsigned int n = 0;
-    while ((int)(ld_acquire(&P.ctl->ucnt) - us.target) < 0) {
-      if ((++n & 255u) == 0u) {
-        if (aborted(P.ctl)) break;
-        if (clock64() - t0 > SPIN_LIMIT) { set_abort(P.ctl, 0x500u); break; }
-      }
-    }
-    __threadfence();
-  }
-  __syncwarp();
   const int total = us.nj * us.q;   // <= 256
   float v[8];
+  long long t0 = clock64();
+  unsigned int n = 0;
+  for (;;) {
+    bool ok = true;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
-    const int idx = lane + 32 * i;
-    v[i] = 0.f;
-    if (idx < total) v[i] = ldcg(P.upart + ((size_t)us.buf * MAX_NJ + idx / us.q) * UPART_Q + idx % us.q);
+    for (int i = 0; i < 8; ++i) {
+      const int idx = lane + 32 * i;
+      v[i] = 0.f;
+      if (idx < total) {
+        u64 e;
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(e) : "l"(P.upart + (size_t)(idx / us.q) * UPART_Q + idx % us.q) : "memory");
+        ok = ok && (unsigned int)(e >> 32) == us.epoch;
+        v[i] = __uint_as_float((unsigned int)e);
+      }
+    }
+    if (__all_sync(0xffffffffu, ok)) break;
+    if ((++n & 255u) == 0u) {
+      if (aborted(P.ctl)) break;
+      if (clock64() - t0 > SPIN_LIMIT) { set_abort(P.ctl, 0x500u); break; }
+    }
   }
 #pragma unroll
   for (int i = 0; i < 8; ++i) {
@@ -515,7 +619,6 @@ __device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp,
     u[j] = s;
   }
   __syncwarp();
-  us.ready = true;
 }
 
 __device__ __forceinline__ float lora_dot(const bf16* Brow, const float* u, int r) {
@@ -534,8 +637,136 @@ __device__ __forceinline__ float lora_dot(const bf16* Brow, const float* u, int 
   }
   return s;
 }
+// a row of r <= 8 adapter weights loaded ahead of its use: one 16-byte load when r == 8
+struct RVec {
+  uint4 a;
+  const bf16* p;
+};
+__device__ __forceinline__ RVec rv_load(const bf16* p, int r) {
+  RVec v;
+  v.p = p;
+  v.a = make_uint4(0u, 0u, 0u, 0u);
+  if (r == 8) v.a = __ldg((const uint4*)p);
+  return v;
+}
+__device__ __forceinline__ void rv_unpack(const RVec& v, int r, float (&f)[MAX_R]) {
+  if (r == 8) {
+    bf16x2_to_f32(v.a.x, f[0], f[1]); bf16x2_to_f32(v.a.y, f[2], f[3]);
+    bf16x2_to_f32(v.a.z, f[4], f[5]); bf16x2_to_f32(v.a.w, f[6], f[7]);
+  } else {
+#pragma unroll
+    for (int j = 0; j < MAX_R; ++j) f[j] = j < r ? bf(v.p + j) : 0.f;
+  }
+}
+__device__ __forceinline__ float rv_dot(const RVec& v, const float* u, int r) {
+  float f[MAX_R], s = 0.f;
+  rv_unpack(v, r, f);
+#pragma unroll
+  for (int j = 0; j < MAX_R; ++j) if (j < r) s += f[j] * u[j];
+  return s;
+}
+// split-K phases: u of the adapter from partials the PRODUCING phase left behind (one L2 round trip, no
+// publish / fetch): OPROJ  u = A_o o^ from the attention items' r-vectors and (m, l); DOWN  u = A_d a^ as
+// the sum of the CTAs' r-vectors in CTA order.
+__device__ __forceinline__ void combine_u(const FParams& P, float* u, int ph, int G) {
+  const int lane = threadIdx.x & 31, r = P.r;
+  float acc[MAX_R];
+#pragma unroll
+  for (int i = 0; i < MAX_R; ++i) acc[i] = 0.f;
+  if (ph == PH_OPROJ) {
+    const int NS = P.ns, dh = P.dh;
+    for (int si = lane; si < P.nah; si += 32) {
+      const int head = P.accel_cols[si * dh] / dh;
+      float Lsum = 0.f, part[MAX_R];
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) part[i] = 0.f;
+      if (NS <= MERGE_NS) {
+        // every load first (one L2 round trip), then the merge
+        float2 ml[MERGE_NS];
+        float4 pu[MERGE_NS][MAX_R / 4];
+#pragma unroll
+        for (int s = 0; s < MERGE_NS; ++s) {
+          ml[s] = make_float2(0.f, 0.f);
+#pragma unroll
+          for (int c = 0; c < MAX_R / 4; ++c) pu[s][c] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (s < NS) {
+            ml[s] = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
+            const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
+#pragma unroll
+            for (int c = 0; c < MAX_R / 4; ++c) if (c * 4 < r) pu[s][c] = ldcg4(q + c * 4);
+          }
+        }
+        float M = -INFINITY;
+#pragma unroll
+        for (int s = 0; s < MERGE_NS; ++s) if (s < NS && ml[s].y > 0.f) M = fmaxf(M, ml[s].x);
+#pragma unroll
+        for (int s = 0; s < MERGE_NS; ++s) {
+          if (s < NS && ml[s].y > 0.f) {
+            const float wgt = __expf(ml[s].x - M);
+            Lsum += ml[s].y * wgt;
+#pragma unroll
+            for (int c = 0; c < MAX_R / 4; ++c) {
+              part[c * 4 + 0] += pu[s][c].x * wgt; part[c * 4 + 1] += pu[s][c].y * wgt;
+              part[c * 4 + 2] += pu[s][c].z * wgt; part[c * 4 + 3] += pu[s][c].w * wgt;
+            }
+          }
+        }
+      } else {
+        float M = -INFINITY;
+        for (int s = 0; s < NS; ++s) {
+          const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
+          if (ml.y > 0.f) M = fmaxf(M, ml.x);
+        }
+        for (int s = 0; s < NS; ++s) {
+          const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
+          if (ml.y > 0.f) {
+            const float wgt = __expf(ml.x - M);
+            Lsum += ml.y * wgt;
+            const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
+#pragma unroll
+            for (int i = 0; i < MAX_R; ++i) if (i < r) part[i] += ldcg(q + i) * wgt;
+          }
+        }
+      }
+      const float inv = 1.f / Lsum;
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) acc[i] += part[i] * inv;
+    }
+  } else {
+    for (int c = lane; c < G; c += 32) {
+      const float* pu = P.udpart + (size_t)c * MAX_R;
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) if (i < r) acc[i] += ldcg(pu + i);
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < MAX_R; ++i) {
+    if (i < r) {
+      const float v = warp_sum(acc[i]);
+      if (lane == 0) u[i] = v;
+    }
+  }
+  __syncwarp();
+}
+// split-K phases: R.p[n] += B[n] . u for this CTA's share of the rows (the adapter up-projection)
+struct BPre {
+  RVec row;
+  int n;
+};
+__device__ __forceinline__ void apply_prefetch(const FParams& P, BPre& bp, const bf16* B, int G) {
+  const int lane = threadIdx.x & 31, d = P.d, r = P.r;
+  const int per = (d + G - 1) / G, n0 = (int)blockIdx.x * per, n1 = min(d, n0 + per);
+  bp.n = n0 + lane < n1 ? n0 + lane : -1;
+  bp.row = rv_load(B + (size_t)(bp.n >= 0 ? bp.n : 0) * r, r);
+}
+__device__ __forceinline__ void apply_Bu(const FParams& P, const BPre& bp, const bf16* B, const float* u, int G) {
+  const int lane = threadIdx.x & 31, d = P.d, r = P.r;
+  const int per = (d + G - 1) / G, n0 = (int)blockIdx.x * per, n1 = min(d, n0 + per);
+  if (bp.n >= 0) red_add(P.R + d + bp.n, rv_dot(bp.row, u, r));
+  for (int n = n0 + lane + 32; n < n1; n += 32) red_add(P.R + d + n, lora_dot(B + (size_t)n * r, u, r));
+}
 
-// ------------------------------------------------------------------ phase epilogues (warp 0; one 16-row tile, sums in T[row][stream])
+// ------------------------------------------------------------------ row-owned phase epilogues (one warp per finished 16-row tile, sums in T[row][stream])
 struct PhaseCtx {
   int ph, layer;
   const FLayer* L;
@@ -543,7 +774,8 @@ struct PhaseCtx {
   bool accel;       // stream 1 live
 };
 
-__device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, const float* u, const PhaseCtx& c, int rt, int slot) {
+__device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, const float* u, const PhaseCtx& c, int rt,
+                                              float (&udacc)[MAX_R]) {
   const int lane = threadIdx.x & 31;
   const int d = P.d, dh = P.dh, half = dh >> 1, r = P.r;
   if (c.ph == PH_QKV) {
@@ -556,19 +788,24 @@ __device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, 
         float v0 = T[(2 * m) * 2 + s], v1 = T[(2 * m + 1) * 2 + s];
         int e0, e1;   // element index inside the head of the two packed rows
         if (which < 2) { e0 = i >> 1; e1 = e0 + half; } else { e0 = i; e1 = i + 1; }
-        bool live = true;
-        if (s == 1) {
-          const int si = P.sidx[head];
-          live = si >= 0;
-          if (live) {   // parallel adapters: + B (A x^)   (Q3)
-            const bf16* B = c.L->Bqkv + ((size_t)which * P.da + (size_t)si * dh) * r;
-            v0 += lora_dot(B + (size_t)e0 * r, u + which * r, r);
-            v1 += lora_dot(B + (size_t)e1 * r, u + which * r, r);
-          }
-        }
+        const int si = sidx_of(head);
+        const bool live = s == 0 || si >= 0;
         if (live) {
+          // every global load of the lane first: adapter rows, RoPE pair
+          const bool lora = s == 1 && r > 0;
+          RVec b0, b1;
+          float2 cs = make_float2(1.f, 0.f);
+          if (lora) {
+            const bf16* B = c.L->Bqkv + ((size_t)which * P.da + (size_t)si * dh) * r;
+            b0 = rv_load(B + (size_t)e0 * r, r);
+            b1 = rv_load(B + (size_t)e1 * r, r);
+          }
+          if (which < 2) cs = P.rope_tab[(size_t)c.pos * half + e0];
+          if (lora) {   // parallel adapters: + B (A x^)   (Q3)
+            v0 += rv_dot(b0, u + which * r, r);
+            v1 += rv_dot(b1, u + which * r, r);
+          }
           if (which < 2) {
-            float2 cs = P.rope_tab[(size_t)c.pos * half + e0];
             float a = v0 * cs.x - v1 * cs.y, b = v1 * cs.x + v0 * cs.y;
             v0 = a; v1 = b;
           }
@@ -586,26 +823,47 @@ __device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, 
         }
       }
     }
-  } else if (c.ph == PH_OPROJ || c.ph == PH_DOWN) {
-    // split-K partial of a row-tile -> slot; the contributor of slot 0 adds the adapter term once
-    const int row = lane >> 1, s = lane & 1, n = rt * 16 + row;
-    if (n < d && (s == 0 || c.accel)) {
-      float v = T[lane];
-      if (s == 1 && slot == 0) v += lora_dot((c.ph == PH_OPROJ ? c.L->Bo : c.L->Bd) + (size_t)n * r, u, r);
-      float* S = c.ph == PH_OPROJ ? P.oslots : P.dslots;
-      __stcg(S + (size_t)(slot * 2 + s) * d + n, v);
-    }
   } else if (c.ph == PH_GATEUP) {
     // packed tile: gate rows n..n+7 then up rows n..n+7
+    float a_p = 0.f;
+    RVec at;
+    bool have_p = false;
     if (lane < 16) {
       const int nl = lane >> 1, s = lane & 1, n = rt * 8 + nl;
       if (n < P.F && (s == 0 || c.accel)) {
         float g = T[nl * 2 + s], up = T[(8 + nl) * 2 + s];
-        if (s == 1) {
-          g += lora_dot(c.L->Bg + (size_t)n * r, u, r);
-          up += lora_dot(c.L->Bu + (size_t)n * r, u + r, r);
+        if (s == 1 && r > 0) {
+          // every global load of the lane first: B_g, B_u rows and the A_d column
+          const RVec bg = rv_load(c.L->Bg + (size_t)n * r, r), bu = rv_load(c.L->Bu + (size_t)n * r, r);
+          at = rv_load(c.L->AdT + (size_t)n * r, r);
+          have_p = true;
+          g += rv_dot(bg, u, r);
+          up += rv_dot(bu, u + r, r);
         }
-        __stcg(P.act + s * P.F_pad + n, silu(g) * up);
+        const float a = silu(g) * up;
+        __stcg(P.act + s * P.F_pad + n, a);
+        if (s == 1) a_p = a;
+      }
+    }
+    if (c.accel && r > 0) {
+      // A_d a^ over the tile's 8 activations: the down-projection adapter's u, accumulated per warp and
+      // summed over the CTAs after the barrier (the auxiliary warp of the DOWN phase)
+      float cj[MAX_R];
+#pragma unroll
+      for (int j = 0; j < MAX_R; ++j) cj[j] = 0.f;
+      if (have_p) {
+        rv_unpack(at, r, cj);
+#pragma unroll
+        for (int j = 0; j < MAX_R; ++j) cj[j] *= a_p;
+      }
+#pragma unroll
+      for (int j = 0; j < MAX_R; ++j) {
+        if (j < r) {
+          cj[j] += __shfl_xor_sync(0xffffffffu, cj[j], 2);
+          cj[j] += __shfl_xor_sync(0xffffffffu, cj[j], 4);
+          cj[j] += __shfl_xor_sync(0xffffffffu, cj[j], 8);
+          udacc[j] += cj[j];   // meaningful in lane 1
+        }
       }
     }
   } else {
@@ -638,62 +896,92 @@ __device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, 
 }
 
 // ------------------------------------------------------------------ attention phase (a4): split-K flash-decode, dual query
-// Work item = (head, split), one per CTA.  Keys/values of positions [p0, p1) < pos come from the cache
-// (prefetched into L2 by the producer); both queries share every load.  The last split also takes the
-// token's own key/value: slow = K[pos], V[pos] as stored (rounded), accelerated = k^, v^ from scratch
-// (p_t attends h_<t (+) p_t).  Partials (m, l, o) go to P.apart; the O-proj loader merges.
-__device__ __forceinline__ void attn_phase(const FParams& P, float* red, const FLayer* L, int pos, bool accel, int G) {
+// Work item = (head, split), one per CTA.  The item's keys and values of positions [p0, p1) < pos are two
+// contiguous ranges of the cache ([head][position][dh]): one thread stages them into shared memory with two
+// bulk copies per round (prefetched into L2 by the producer), then every half-warp walks its positions in a
+// rolled loop; both queries share every K/V read.  The last split also takes the token's own key/value:
+// slow = K[pos], V[pos] as stored (rounded), accelerated = k^, v^ from scratch (p_t attends
+// h_<t (+) p_t).  Partials (m, l, o) go to P.apart; the O-proj loader merges them.
+constexpr int KV_BYTES = X_BYTES + RED_FLOATS * 4;   // staging area: the x columns and the parked sums are dead here
+__device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, float* osm, u64* abar, unsigned int& aphase,
+                                        const FLayer* L, int pos, bool accel, int G) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int dh = P.dh, d = P.d, lpp = dh >> 3, NS = P.ns;
-  const int seg = lane >> 4, sl = lane & 15;
+  const int seg = lane >> 4, sl = lane & 15, hw = warp * 2 + seg;
   const bool active = sl < lpp;
-  const int items = P.n_heads * NS;   // red: [2 NCW segments][2 queries][dh + 2]
+  const int items = P.n_heads * NS;
+  const int cap = KV_BYTES / (4 * dh);   // positions per round (K and V rows of dh bf16 each)
+  float* red = (float*)kvbuf;                    // after the rounds: [2 NCW segments][2 queries][dh + 2]
   for (int w = blockIdx.x; w < items; w += G) {
     const int head = w / NS, sp = w - head * NS;
-    const bool q1 = accel && P.sidx[head] >= 0;
+    const bool q1 = accel && sidx_of(head) >= 0;
     const int chunk = (pos + NS - 1) / NS;
     const int p0 = min(pos, sp * chunk), p1 = min(pos, p0 + chunk);
+    const bf16* Kg = L->Kc + (size_t)head * P.max_seq * dh;
+    const bf16* Vg = L->Vc + (size_t)head * P.max_seq * dh;
+    bf16* ks = (bf16*)kvbuf;
+    bf16* vs = ks + (size_t)cap * dh;
+    if (tid == 0 && p1 > p0) {   // first round in flight before the queries are even loaded
+      const int n = min(cap, p1 - p0);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(abar, (uint32_t)(2 * n * dh * 2));
+      bulk_g2s_plain(ks, Kg + (size_t)p0 * dh, (uint32_t)(n * dh * 2), abar);
+      bulk_g2s_plain(vs, Vg + (size_t)p0 * dh, (uint32_t)(n * dh * 2), abar);
+    }
+    // the token's own key/value and the queries: every load issued before anything is used
+    const bool own = sp == NS - 1 && warp == 0;   // this warp adds the token's own key/value (segment 0)
+    uint4 ko = make_uint4(0u, 0u, 0u, 0u), vo = ko;
+    float4 kh0 = make_float4(0.f, 0.f, 0.f, 0.f), kh1 = kh0, vh0 = kh0, vh1 = kh0;
+    if (own && seg == 0 && active) {
+      ko = ldcg16(Kg + (size_t)pos * dh + sl * 8);
+      vo = ldcg16(Vg + (size_t)pos * dh + sl * 8);
+      if (q1) {
+        kh0 = ldcg4(P.khat + head * dh + sl * 8); kh1 = ldcg4(P.khat + head * dh + sl * 8 + 4);
+        vh0 = ldcg4(P.vhat + head * dh + sl * 8); vh1 = ldcg4(P.vhat + head * dh + sl * 8 + 4);
+      }
+    }
     float qa[8], qb[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) { qa[e] = 0.f; qb[e] = 0.f; }
     if (active) {
       const float4 a0 = ldcg4(P.qbuf + head * dh + sl * 8), a1 = ldcg4(P.qbuf + head * dh + sl * 8 + 4);
+      float4 b0 = make_float4(0.f, 0.f, 0.f, 0.f), b1 = b0;
+      if (q1) { b0 = ldcg4(P.qbuf + d + head * dh + sl * 8); b1 = ldcg4(P.qbuf + d + head * dh + sl * 8 + 4); }
       qa[0] = a0.x * P.scale; qa[1] = a0.y * P.scale; qa[2] = a0.z * P.scale; qa[3] = a0.w * P.scale;
       qa[4] = a1.x * P.scale; qa[5] = a1.y * P.scale; qa[6] = a1.z * P.scale; qa[7] = a1.w * P.scale;
-      if (q1) {
-        const float4 b0 = ldcg4(P.qbuf + d + head * dh + sl * 8), b1 = ldcg4(P.qbuf + d + head * dh + sl * 8 + 4);
-        qb[0] = b0.x * P.scale; qb[1] = b0.y * P.scale; qb[2] = b0.z * P.scale; qb[3] = b0.w * P.scale;
-        qb[4] = b1.x * P.scale; qb[5] = b1.y * P.scale; qb[6] = b1.z * P.scale; qb[7] = b1.w * P.scale;
-      }
+      qb[0] = b0.x * P.scale; qb[1] = b0.y * P.scale; qb[2] = b0.z * P.scale; qb[3] = b0.w * P.scale;
+      qb[4] = b1.x * P.scale; qb[5] = b1.y * P.scale; qb[6] = b1.z * P.scale; qb[7] = b1.w * P.scale;
     }
     float m0 = -INFINITY, l0 = 0.f, m1 = -INFINITY, l1 = 0.f, o0[8], o1[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) { o0[e] = 0.f; o1[e] = 0.f; }
-    const bf16* Kb = L->Kc + (size_t)head * P.max_seq * dh + sl * 8;
-    const bf16* Vb = L->Vc + (size_t)head * P.max_seq * dh + sl * 8;
-    // positions of this warp: p0 + 2*warp + seg + 2*NCW*i; AIF iterations in flight
-    constexpr int AIF = 4;
-    for (int ub = p0 + warp * 2; ub < p1; ub += AIF * NCW * 2) {
-      uint4 kk[AIF], vv[AIF];
-      bool valid[AIF];
-#pragma unroll
-      for (int it = 0; it < AIF; ++it) {
-        const int u = ub + it * NCW * 2 + seg;
-        valid[it] = u < p1;
-        kk[it] = make_uint4(0u, 0u, 0u, 0u);
-        vv[it] = kk[it];
-        if (valid[it] && active) {
-          kk[it] = ldcg16(Kb + (size_t)u * dh);
-          vv[it] = ldcg16(Vb + (size_t)u * dh);
+    for (int r0 = p0; r0 < p1; r0 += cap) {
+      const int n = min(cap, p1 - r0);
+      if (r0 > p0) {
+        bar_consumers();   // the previous round's rows are consumed
+        if (tid == 0) {
+          asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+          mbar_expect_tx(abar, (uint32_t)(2 * n * dh * 2));
+          bulk_g2s_plain(ks, Kg + (size_t)r0 * dh, (uint32_t)(n * dh * 2), abar);
+          bulk_g2s_plain(vs, Vg + (size_t)r0 * dh, (uint32_t)(n * dh * 2), abar);
         }
       }
-#pragma unroll
-      for (int it = 0; it < AIF; ++it) {
+      mbar_wait(abar, aphase & 1u, P.ctl, 0x300u);
+      ++aphase;
+#pragma unroll 1
+      for (int ub = warp * 2; ub < n; ub += 2 * NCW) {   // warp-uniform trip count (full-mask shuffles below)
+        const int u = ub + seg;
+        const bool valid = u < n;
+        uint4 kk = make_uint4(0u, 0u, 0u, 0u), vv = kk;
+        if (active && valid) {
+          kk = *(const uint4*)(ks + (size_t)u * dh + sl * 8);
+          vv = *(const uint4*)(vs + (size_t)u * dh + sl * 8);
+        }
         float kf[8], vf[8];
-        bf16x2_to_f32(kk[it].x, kf[0], kf[1]); bf16x2_to_f32(kk[it].y, kf[2], kf[3]);
-        bf16x2_to_f32(kk[it].z, kf[4], kf[5]); bf16x2_to_f32(kk[it].w, kf[6], kf[7]);
-        bf16x2_to_f32(vv[it].x, vf[0], vf[1]); bf16x2_to_f32(vv[it].y, vf[2], vf[3]);
-        bf16x2_to_f32(vv[it].z, vf[4], vf[5]); bf16x2_to_f32(vv[it].w, vf[6], vf[7]);
+        bf16x2_to_f32(kk.x, kf[0], kf[1]); bf16x2_to_f32(kk.y, kf[2], kf[3]);
+        bf16x2_to_f32(kk.z, kf[4], kf[5]); bf16x2_to_f32(kk.w, kf[6], kf[7]);
+        bf16x2_to_f32(vv.x, vf[0], vf[1]); bf16x2_to_f32(vv.y, vf[2], vf[3]);
+        bf16x2_to_f32(vv.z, vf[4], vf[5]); bf16x2_to_f32(vv.w, vf[6], vf[7]);
         float sa = 0.f, sb = 0.f;
 #pragma unroll
         for (int e = 0; e < 8; ++e) { sa += qa[e] * kf[e]; sb += qb[e] * kf[e]; }
@@ -702,7 +990,7 @@ __device__ __forceinline__ void attn_phase(const FParams& P, float* red, const F
           sa += __shfl_xor_sync(0xffffffffu, sa, o);
           sb += __shfl_xor_sync(0xffffffffu, sb, o);
         }
-        if (valid[it]) {
+        if (valid) {
           float mn = fmaxf(m0, sa), corr = __expf(m0 - mn), p = __expf(sa - mn);
           l0 = l0 * corr + p;
 #pragma unroll
@@ -718,24 +1006,16 @@ __device__ __forceinline__ void attn_phase(const FParams& P, float* red, const F
         }
       }
     }
+    TL(70);
     // ---- the token's own key/value (last split, warp 0, segment 0)
-    if (sp == NS - 1 && warp == 0) {
+    if (own) {
       float kf[8], vf[8], k2[8], v2[8];
-#pragma unroll
-      for (int e = 0; e < 8; ++e) { kf[e] = vf[e] = k2[e] = v2[e] = 0.f; }
-      if (seg == 0 && active) {
-        const uint4 kk = ldcg16(Kb + (size_t)pos * dh), vv = ldcg16(Vb + (size_t)pos * dh);
-        bf16x2_to_f32(kk.x, kf[0], kf[1]); bf16x2_to_f32(kk.y, kf[2], kf[3]);
-        bf16x2_to_f32(kk.z, kf[4], kf[5]); bf16x2_to_f32(kk.w, kf[6], kf[7]);
-        bf16x2_to_f32(vv.x, vf[0], vf[1]); bf16x2_to_f32(vv.y, vf[2], vf[3]);
-        bf16x2_to_f32(vv.z, vf[4], vf[5]); bf16x2_to_f32(vv.w, vf[6], vf[7]);
-        if (q1) {
-          const float4 ka = ldcg4(P.khat + head * dh + sl * 8), kb = ldcg4(P.khat + head * dh + sl * 8 + 4);
-          const float4 va = ldcg4(P.vhat + head * dh + sl * 8), vb = ldcg4(P.vhat + head * dh + sl * 8 + 4);
-          k2[0] = ka.x; k2[1] = ka.y; k2[2] = ka.z; k2[3] = ka.w; k2[4] = kb.x; k2[5] = kb.y; k2[6] = kb.z; k2[7] = kb.w;
-          v2[0] = va.x; v2[1] = va.y; v2[2] = va.z; v2[3] = va.w; v2[4] = vb.x; v2[5] = vb.y; v2[6] = vb.z; v2[7] = vb.w;
-        }
-      }
+      bf16x2_to_f32(ko.x, kf[0], kf[1]); bf16x2_to_f32(ko.y, kf[2], kf[3]);
+      bf16x2_to_f32(ko.z, kf[4], kf[5]); bf16x2_to_f32(ko.w, kf[6], kf[7]);
+      bf16x2_to_f32(vo.x, vf[0], vf[1]); bf16x2_to_f32(vo.y, vf[2], vf[3]);
+      bf16x2_to_f32(vo.z, vf[4], vf[5]); bf16x2_to_f32(vo.w, vf[6], vf[7]);
+      k2[0] = kh0.x; k2[1] = kh0.y; k2[2] = kh0.z; k2[3] = kh0.w; k2[4] = kh1.x; k2[5] = kh1.y; k2[6] = kh1.z; k2[7] = kh1.w;
+      v2[0] = vh0.x; v2[1] = vh0.y; v2[2] = vh0.z; v2[3] = vh0.w; v2[4] = vh1.x; v2[5] = vh1.y; v2[6] = vh1.z; v2[7] = vh1.w;
       float sa = 0.f, sb = 0.f;
 #pragma unroll
       for (int e = 0; e < 8; ++e) { sa += qa[e] * kf[e]; sb += qb[e] * k2[e]; }
@@ -759,11 +1039,12 @@ __device__ __forceinline__ void attn_phase(const FParams& P, float* red, const F
         }
       }
     }
+    TL(71);
     // ---- merge the lane segments of the CTA -> one partial per query
+    bar_consumers();   // every half-warp is done with the staged rows: the area becomes the merge scratch
     {
-      const int gseg = warp * 2 + seg;
-      float* dst0 = red + ((size_t)gseg * 2 + 0) * (dh + 2);
-      float* dst1 = red + ((size_t)gseg * 2 + 1) * (dh + 2);
+      float* dst0 = red + ((size_t)hw * 2 + 0) * (dh + 2);
+      float* dst1 = red + ((size_t)hw * 2 + 1) * (dh + 2);
       if (active) {
 #pragma unroll
         for (int e = 0; e < 8; ++e) { dst0[sl * 8 + e] = o0[e]; dst1[sl * 8 + e] = o1[e]; }
@@ -774,11 +1055,13 @@ __device__ __forceinline__ void attn_phase(const FParams& P, float* red, const F
     for (int i = tid; i < 2 * dh; i += NCT) {
       const int q = i / dh, j = i - q * dh;
       float M = -INFINITY;
+#pragma unroll 1
       for (int s = 0; s < 2 * NCW; ++s) {
         const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
         if (src[dh + 1] > 0.f) M = fmaxf(M, src[dh]);
       }
       float Lsum = 0.f, O = 0.f;
+#pragma unroll 1
       for (int s = 0; s < 2 * NCW; ++s) {
         const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
         float ls = src[dh + 1];
@@ -791,54 +1074,108 @@ __device__ __forceinline__ void attn_phase(const FParams& P, float* red, const F
       float* pp = P.apart + ((size_t)(head * NS + sp) * 2 + q) * (dh + 4);
       __stcg(pp + j, O);
       if (j == 0) { __stcg(pp + dh, M); __stcg(pp + dh + 1, Lsum); }
+      if (q == 1) osm[j] = O;
     }
     bar_consumers();
+    TL(72);
+    if (q1 && P.r > 0 && warp == 0) {
+      // O-projection adapter: A_o restricted to this head, applied to the unnormalised partial (linear in the
+      // partials, so the auxiliary warp of the OPROJ phase only combines the splits' r-vectors)
+      const bf16* At = L->AoT + (size_t)sidx_of(head) * dh * P.r;   // [column of the head][r]
+      constexpr int JC = 4;   // dh <= 128
+      RVec av[JC];
+#pragma unroll
+      for (int c = 0; c < JC; ++c) {
+        const int j = lane + 32 * c;
+        av[c] = rv_load(At + (size_t)(j < dh ? j : 0) * P.r, P.r);
+      }
+      float acc[MAX_R];
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) acc[i] = 0.f;
+#pragma unroll
+      for (int c = 0; c < JC; ++c) {
+        const int j = lane + 32 * c;
+        if (j < dh) {
+          float f[MAX_R];
+          rv_unpack(av[c], P.r, f);
+          const float o = osm[j];
+#pragma unroll
+          for (int i = 0; i < MAX_R; ++i) acc[i] += f[i] * o;
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) {
+        if (i < P.r) {
+          const float v = warp_sum(acc[i]);
+          if (lane == 0) __stcg(P.apu + (size_t)(head * NS + sp) * MAX_R + i, v);
+        }
+      }
+    }
   }
 }
 
-// ------------------------------------------------------------------ producer: the CTA's weight-stage stream of the whole pass
+// ------------------------------------------------------------------ the phase sequence of a pass (shared by producer, consumers, auxiliary warp)
 __device__ __forceinline__ bool exit_phase_after(const FParams& P, int layer) {
-  const FLayer* L = P.layers + layer;
+  const FLayer* L = lay(layer);
   return L->gate && L->accel && P.exit_heads && !(P.head_stream == 1 && layer + 1 == P.n_layers_run);
 }
-
-// Walks the CTA's stages of the pass in consumption order (must mirror the consumer loop).
-struct Cursor {
-  int layer, ph;     // ph = -1 before the first phase
-  int s, s1;
+// geometry of a weight phase: stages S = U * gran; the CTA's stage range [s0, s1)
+struct PhaseGeo {
   const unsigned char* W;
-  bool new_layer;    // set when the walk enters a layer's QKV phase
+  int n_units, gran, nkc;    // nkc: k-chunks per row-tile group (split-K) / k-stages per row-tile (row-owned)
+  bool split;
+  int s0, s1;
 };
-__device__ __noinline__ bool cursor_advance(const FParams& P, Cursor& c, int G) {
+__device__ __forceinline__ void phase_geo(const FParams& P, int layer, int ph, int G, PhaseGeo& g) {
   const int n = P.n_layers_run;
-  if (c.ph == PH_HEAD) return false;
+  const FLayer* L = lay(layer < n ? layer : 0);
+  const int nks_d = P.d_pad / STAGE_K;
+  int rot_layer = layer;
+  switch (ph) {
+    case PH_QKV:    g.W = (const unsigned char*)L->Wqkv; g.n_units = P.rt_qkv; g.gran = nks_d; g.nkc = nks_d; g.split = false; break;
+    case PH_OPROJ:  g.W = (const unsigned char*)L->Wo;   g.nkc = (P.d + SK_K - 1) / SK_K; g.n_units = P.ng_d * g.nkc; g.gran = 1; g.split = true; break;
+    case PH_GATEUP: g.W = (const unsigned char*)L->Wgu;  g.n_units = P.rt_gu;  g.gran = nks_d; g.nkc = nks_d; g.split = false; break;
+    case PH_DOWN:   g.W = (const unsigned char*)L->Wd;   g.nkc = P.F_pad / SK_K; g.n_units = P.ng_d * g.nkc; g.gran = 1; g.split = true; break;
+    case PH_EXIT:   g.W = (const unsigned char*)P.Wlm;   g.n_units = P.rt_v;   g.gran = nks_d; g.nkc = nks_d; g.split = false; rot_layer = L->gate - 1; break;
+    default:        g.W = (const unsigned char*)P.Wlm;   g.n_units = P.rt_v;   g.gran = nks_d; g.nkc = nks_d; g.split = false; rot_layer = n; break;
+  }
+  const int v = ((int)blockIdx.x + phase_rot(rot_layer, ph, G)) % G;
+  g.s0 = range_lo(g.n_units, v, G) * g.gran;
+  g.s1 = range_lo(g.n_units, v + 1, G) * g.gran;
+}
+// next weight phase after (layer, ph); ph = -1 before the first.  false at the end of the pass.
+__device__ __forceinline__ bool next_weight_phase(const FParams& P, int& layer, int& ph) {
+  const int n = P.n_layers_run;
+  if (ph == PH_HEAD) return false;
   bool next_layer = false;
-  if (c.ph < 0) { c.layer = -1; next_layer = true; }
-  else if (c.ph == PH_QKV) c.ph = PH_OPROJ;
-  else if (c.ph == PH_OPROJ) c.ph = PH_GATEUP;
-  else if (c.ph == PH_GATEUP) c.ph = PH_DOWN;
-  else if (c.ph == PH_DOWN) { if (exit_phase_after(P, c.layer)) c.ph = PH_EXIT; else next_layer = true; }
+  if (ph < 0) { layer = -1; next_layer = true; }
+  else if (ph == PH_QKV) ph = PH_OPROJ;
+  else if (ph == PH_OPROJ) ph = PH_GATEUP;
+  else if (ph == PH_GATEUP) ph = PH_DOWN;
+  else if (ph == PH_DOWN) { if (exit_phase_after(P, layer)) ph = PH_EXIT; else next_layer = true; }
   else next_layer = true;   // PH_EXIT
   if (next_layer) {
-    ++c.layer;
-    c.ph = c.layer < n ? PH_QKV : PH_HEAD;
-    c.new_layer = c.ph == PH_QKV;
+    ++layer;
+    ph = layer < n ? PH_QKV : PH_HEAD;
   }
-  const int nks_d = P.d_pad / STAGE_K, nks_f = P.F_pad / STAGE_K;
-  int n_rt, nks, gran, rot_layer = c.layer;
-  const FLayer* L = P.layers + (c.layer < n ? c.layer : 0);
-  switch (c.ph) {
-    case PH_QKV:    c.W = (const unsigned char*)L->Wqkv; n_rt = P.rt_qkv; nks = nks_d; gran = nks; break;
-    case PH_OPROJ:  c.W = (const unsigned char*)L->Wo;   n_rt = P.rt_o;   nks = nks_d; gran = 1;   break;
-    case PH_GATEUP: c.W = (const unsigned char*)L->Wgu;  n_rt = P.rt_gu;  nks = nks_d; gran = nks; break;
-    case PH_DOWN:   c.W = (const unsigned char*)L->Wd;   n_rt = P.rt_d;   nks = nks_f; gran = 1;   break;
-    case PH_EXIT:   c.W = (const unsigned char*)P.Wlm;   n_rt = P.rt_v;   nks = nks_d; gran = nks; rot_layer = L->gate - 1; break;
-    default:        c.W = (const unsigned char*)P.Wlm;   n_rt = P.rt_v;   nks = nks_d; gran = nks; rot_layer = n; break;
-  }
-  const int U = n_rt * nks / gran;
-  const int v = ((int)blockIdx.x + phase_rot(rot_layer, c.ph, G)) % G;
-  c.s = range_lo(U, v, G) * gran;
-  c.s1 = range_lo(U, v + 1, G) * gran;
+  return true;
+}
+
+// producer cursor: walks the CTA's stages of the pass in consumption order
+struct Cursor {
+  int layer, ph;
+  int s, s1;
+  const unsigned char* W;
+  bool new_layer;
+};
+__device__ __noinline__ bool cursor_advance(const FParams& P, Cursor& c, int G) {
+  if (!next_weight_phase(P, c.layer, c.ph)) return false;
+  c.new_layer = c.ph == PH_QKV;
+  PhaseGeo g;
+  phase_geo(P, c.layer, c.ph, G, g);
+  c.W = g.W;
+  c.s = g.s0;
+  c.s1 = g.s1;
   return true;
 }
 __device__ __forceinline__ bool cursor_get(const FParams& P, Cursor& c, int G, const unsigned char*& addr) {
@@ -853,7 +1190,7 @@ __device__ __forceinline__ bool cursor_get(const FParams& P, Cursor& c, int G, c
 // L2 prefetch of the K/V positions this CTA will attend to in `layer`
 __device__ __noinline__ void prefetch_kv(const FParams& P, int layer, int G) {
   const int NS = P.ns, pos = P.pos_host, dh = P.dh;
-  const FLayer* L = P.layers + layer;
+  const FLayer* L = lay(layer);
   for (int w = blockIdx.x; w < P.n_heads * NS; w += G) {
     const int head = w / NS, sp = w - head * NS;
     const int chunk = (pos + NS - 1) / NS;
@@ -877,7 +1214,7 @@ __device__ __forceinline__ void prefetch_slice(const void* base, size_t bytes, i
   if (o < bytes) bulk_prefetch_l2((const unsigned char*)base + o, (uint32_t)min(per, ((bytes - o) + 15) & ~(size_t)15));
 }
 __device__ __noinline__ void prefetch_params(const FParams& P, int layer, int G) {
-  const FLayer* L = P.layers + layer;
+  const FLayer* L = lay(layer);
   if ((int)blockIdx.x == layer % G) {
     bulk_prefetch_l2(L->g1, (uint32_t)((P.d * 2 + 15) & ~15));
     bulk_prefetch_l2(L->g2, (uint32_t)((P.d * 2 + 15) & ~15));
@@ -887,16 +1224,36 @@ __device__ __noinline__ void prefetch_params(const FParams& P, int layer, int G)
     }
   }
   if (L->accel && L->ad_bytes) prefetch_slice(L->ad_lo, L->ad_bytes, G);
+  if (L->accel && L->AdT) { prefetch_slice(L->AdT, (size_t)P.F * P.r * 2, G); prefetch_slice(L->AoT, (size_t)P.da * P.r * 2, G); }
   if (layer == 0 && P.lmA && (P.head_stream == 1 || P.exit_heads)) {
     prefetch_slice(P.lmA, (size_t)P.r * P.d * 2, G);
     prefetch_slice(P.lmB, (size_t)P.V * P.r * 2, G);
   }
 }
 
-constexpr int PH_ATTN = N_PH;   // consumer-only phase (no weights)
+// auxiliary work of a weight phase: which adapter, if any
+struct AuxGeo {
+  const bf16 *A, *B;
+  int nj, Kc;
+  bool apply;       // split-K phase: the auxiliary warp adds B u into R.p itself
+};
+__device__ __forceinline__ bool aux_geo(const FParams& P, int layer, int ph, AuxGeo& a) {
+  const int n = P.n_layers_run;
+  const FLayer* L = lay(layer < n ? layer : (n > 0 ? n - 1 : 0));
+  a.B = nullptr; a.apply = false; a.Kc = P.d;
+  if (ph == PH_HEAD || ph == PH_EXIT) {
+    a.A = P.lmA; a.nj = P.r;
+    return P.lmA != nullptr && P.r > 0 && (ph == PH_EXIT || P.head_stream == 1);
+  }
+  if (!L->accel || P.r <= 0) return false;
+  if (ph == PH_QKV) { a.A = L->Aqkv; a.nj = 3 * P.r; }
+  else if (ph == PH_OPROJ) { a.A = L->Ao; a.B = L->Bo; a.nj = P.r; a.Kc = P.da; a.apply = true; }
+  else if (ph == PH_GATEUP) { a.A = L->Agu; a.nj = 2 * P.r; }
+  else { a.A = L->Ad; a.B = L->Bd; a.nj = P.r; a.Kc = P.F; a.apply = true; }
+  return true;
+}
 
 __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __grid_constant__ FParams P) {
-  extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char* const ring = smem_raw;
   bf16* const x = (bf16*)(smem_raw + OFF_X);
   float* const red = (float*)(smem_raw + OFF_RED);
@@ -905,38 +1262,65 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
   float* const sred = (float*)(smem_raw + OFF_SRED);
   u64* const full = (u64*)(smem_raw + OFF_BAR);
   u64* const empty = full + NSTAGE;
+  u64* const abar = full + 2 * NSTAGE;   // attention K/V staging
   float* const utmp = (float*)(smem_raw + OFF_UTMP);
+  int* const frt = (int*)(smem_raw + OFF_FRT);
   const int tid = threadIdx.x, G = gridDim.x;
   if (tid == 0) {
     for (int i = 0; i < NSTAGE; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NCW); }
+    mbar_init(abar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    *(int*)(smem_raw + OFF_TLN) = 0;
+  }
+  for (int i = tid; i < P.n_heads; i += NTHREADS) ((int*)(smem_raw + OFF_SIDX))[i] = P.sidx[i];
+  {
+    const int words = P.n_layers_run * (int)(sizeof(FLayer) / 4);
+    const uint32_t* src = (const uint32_t*)P.layers;
+    uint32_t* dst = (uint32_t*)(smem_raw + OFF_LAYERS);
+    for (int i = tid; i < words; i += NTHREADS) dst[i] = __ldg(src + i);
   }
   __syncthreads();
-  const int nks_d = P.d_pad / STAGE_K, nks_f = P.F_pad / STAGE_K;
   const int n_run = P.n_layers_run;
 
+  if (tid >= NCT + 32) {
+    // ================= auxiliary warp: adapter down-projections (u = A x^) of every phase that has one
+    UState us;
+    us.epoch = P.bar_base; us.nj = 0; us.q = 1;
+    int layer = 0, ph = -1;
+    while (next_weight_phase(P, layer, ph)) {
+      AuxGeo a;
+      if (!aux_geo(P, layer, ph, a)) continue;
+      ++us.epoch;
+      if (a.apply) {
+        BPre bp;
+        apply_prefetch(P, bp, a.B, G);   // B never depends on activations
+        bar_wait(2);   // the grid barrier before this phase has passed: the producing phase's partials are visible
+        combine_u(P, u_s, ph, G);
+        apply_Bu(P, bp, a.B, u_s, G);
+        __threadfence();
+      } else {
+        APre ap;
+        u_geometry(us, a.nj, G);
+        publish_prefetch(us, ap, a.A, a.Kc);   // A never depends on activations
+        bar_wait(2);   // x^ of the phase is in shared memory
+        publish_u(P, x, us, ap, a.A, a.Kc);
+        fetch_u(P, u_s, utmp, us);
+      }
+      __threadfence_block();
+      bar_arrive(3);
+    }
+    return;
+  }
   if (tid >= NCT) {
     // ================= producer warp: one thread streams every weight stage of the pass
     if (tid == NCT) {
       const u64 pol = policy_evict_first();
-      Cursor ld, pf;
+      Cursor ld;
       ld.layer = 0; ld.ph = -1; ld.s = ld.s1 = 0; ld.W = nullptr; ld.new_layer = false;
-      pf = ld;
-      bool pf_live = P.pf_ahead > 0;
       const unsigned char* a;
-      for (int i = 0; i < P.pf_ahead && pf_live; ++i) {
-        pf_live = cursor_get(P, pf, G, a);
-        if (pf_live) bulk_prefetch_l2(a, STAGE_BYTES);
-        if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); prefetch_params(P, pf.layer, G); }
-      }
       unsigned int ctr = 0;
       while (cursor_get(P, ld, G, a)) {
-        if (pf_live) {
-          const unsigned char* b;
-          pf_live = cursor_get(P, pf, G, b);
-          if (pf_live) bulk_prefetch_l2(b, STAGE_BYTES);
-          if (pf.new_layer) { pf.new_layer = false; prefetch_kv(P, pf.layer, G); prefetch_params(P, pf.layer, G); }
-        } else if (P.pf_ahead <= 0 && ld.new_layer) {
+        if (ld.new_layer) {
           ld.new_layer = false;
           prefetch_kv(P, ld.layer, G);
           prefetch_params(P, ld.layer, G);
@@ -951,76 +1335,63 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
     return;
   }
 
-  // ================= consumers: one loop over the phases of the pass (every routine has one call site)
+  // ================= consumers: one loop over the phases of the pass
   const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  unsigned int nbar = 0, stage_ctr = 0, flushes = 0;
-  int tl_n = 0;
-  (void)tl_n;
-  UState us;
-  us.target = 0; us.buf = 0; us.nj = 0; us.q = 1; us.ready = false;
+  unsigned int nbar = 0, stage_ctr = 0, aphase = 0;
   const int d = P.d;
   const int pos = *(volatile int*)P.kv_len + P.joff;
   const int tok = *(volatile const int*)P.tok_in;
   TL(1);
 
-  int layer = 0, ph = n_run > 0 ? PH_QKV : PH_HEAD;
-  for (;;) {
-    const FLayer* L = P.layers + (layer < n_run ? layer : (n_run > 0 ? n_run - 1 : 0));
+  int layer = 0, ph = -1;
+  while (next_weight_phase(P, layer, ph)) {
+    const FLayer* L = lay(layer < n_run ? layer : (n_run > 0 ? n_run - 1 : 0));
     const bool accel = ph == PH_HEAD || ph == PH_EXIT ? true : L->accel != 0;
-    if (ph == PH_ATTN) {
-      // ---- a4: attention
-      attn_phase(P, (float*)x, L, pos, accel, G);
+    if (ph == PH_OPROJ) {
+      // ---- a4: attention (its own phase between QKV and OPROJ; no weights)
+      attn_phase(P, (unsigned char*)x, utmp, abar, aphase, L, pos, accel, G);
       TL(13);
       grid_sync(P.ctl, P.bar_base, nbar, G);
       TL(14);
-      ph = PH_OPROJ;
-      continue;
     }
-    // ---- geometry of the phase
+    PhaseGeo pg;
+    phase_geo(P, layer, ph, G, pg);
     PhaseCtx pc;
     pc.ph = ph; pc.layer = layer; pc.L = L; pc.pos = pos; pc.accel = accel;
-    int n_rt, nks = nks_d, nj = 0, Kc = d;
-    bool split = false, need_u = accel && P.r > 0;
-    const bf16* A = nullptr;
-    const int* cols = nullptr;
-    if (ph == PH_QKV) { n_rt = P.rt_qkv; A = L->Aqkv; nj = 3 * P.r; }
-    else if (ph == PH_OPROJ) { n_rt = P.rt_o; split = true; A = L->Ao; nj = P.r; Kc = P.da; cols = P.accel_cols; }
-    else if (ph == PH_GATEUP) { n_rt = P.rt_gu; A = L->Agu; nj = 2 * P.r; }
-    else if (ph == PH_DOWN) { n_rt = P.rt_d; nks = nks_f; split = true; A = L->Ad; nj = P.r; Kc = P.F; }
-    else {
-      n_rt = P.rt_v; A = P.lmA; nj = P.r;
-      need_u = P.lmA != nullptr && (ph == PH_EXIT || P.head_stream == 1);
-      pc.layer = ph == PH_EXIT ? L->gate - 1 : n_run;
-    }
+    if (ph == PH_EXIT) pc.layer = L->gate - 1;
+    if (ph == PH_HEAD) pc.layer = n_run;
+    AuxGeo ag;
+    const bool need_aux = aux_geo(P, layer, ph, ag);
+    float udacc[MAX_R];
+#pragma unroll
+    for (int j = 0; j < MAX_R; ++j) udacc[j] = 0.f;
     // ---- loader: the phase's input vector(s) -> shared memory
-    if (ph == PH_OPROJ) {
-      loader_attn(P, x, accel);
-    } else if (ph == PH_DOWN) {
-      loader_act(P, x, accel);
+    if (pg.split) {
+      if (need_aux) bar_arrive(2);   // the auxiliary warp reads global partials only: it may start now
+      const int len = pg.s1 - pg.s0;
+      if (len > 0) loader_slice(P, x, ph, accel, pg.s0 % pg.nkc, min(len, pg.nkc), pg.nkc);
     } else {
       LoadSrc src;
       int mode;
-      float *wb = nullptr, *tr = nullptr;
+      float* tr = nullptr;
       const bf16* gn;
-      src.emb = nullptr; src.gate = 0;
+      src.emb = nullptr; src.gate = 0; src.p_live = true;
       if (ph == PH_GATEUP) {
-        // a5-tail: h' = h + O-proj sums
-        src.base = P.RB; src.slots = P.oslots; src.n_rt = P.rt_o; src.nks = nks_d; src.p_live = accel;
-        mode = LN_GU; wb = P.RA; gn = L->g2;
+        src.p_live = accel;
+        mode = LN_GU; gn = L->g2;
       } else if ((ph == PH_QKV && layer == 0) || (ph == PH_HEAD && n_run == 0)) {
         // a1: embedding, p_0 <- h_0 (L82)
-        src.base = nullptr; src.emb = P.embed + (size_t)tok * d; src.slots = nullptr; src.n_rt = 0; src.nks = 1; src.p_live = false;
+        src.emb = P.embed + (size_t)tok * d; src.p_live = false;
         mode = ph == PH_QKV ? LN_QKV : (P.head_stream == 0 ? LN_HEAD_H : LN_HEAD_P);
-        wb = ph == PH_QKV ? P.RB : nullptr;
         gn = ph == PH_QKV ? L->g1 : P.gf;
         tr = P.do_trace ? P.trace : nullptr;
       } else {
-        // a7-tail: residual + down sums of the layer below (accelerated-residual update, Eq. 2), gate
+        // a7-tail: R already holds the accelerated-residual update of the layer below (Eq. 2); gate
         const FLayer* Lp = ph == PH_QKV ? L - 1 : L;
-        src.base = P.RA; src.slots = P.dslots; src.n_rt = P.rt_d; src.nks = nks_f; src.p_live = Lp->accel != 0;
+        src.p_live = Lp->accel != 0;
         if (ph == PH_QKV) {
           src.gate = Lp->accel ? Lp->gate : 0;
-          mode = LN_QKV; wb = P.RB; gn = L->g1;
+          mode = LN_QKV; gn = L->g1;
           tr = P.do_trace ? P.trace + (size_t)layer * 2 * d : nullptr;
         } else if (ph == PH_EXIT) {
           mode = LN_HEAD_P; gn = P.gf;
@@ -1029,20 +1400,61 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
           tr = P.do_trace ? P.trace + (size_t)n_run * 2 * d : nullptr;
         }
       }
-      loader_norm(P, x, sred, mode, src, wb, tr, gn, G);
+      loader_norm(P, x, sred, mode, src, tr, gn, G);
     }
-    if (need_u) publish_u(P, x, us, A, nj, Kc, cols, G);
+    if (need_aux && !pg.split) { __threadfence_block(); bar_arrive(2); }
     TL(10 + ph);
-    // ---- GEMV over this CTA's stages.  Stage (rt, ks): 64 tiles of row-tile rt, inputs [1024 ks, +1024).
-    // Warp w multiplies tiles 8w..8w+7: 8 LDS.128 (A fragments) + 4 LDS.128 (B fragments) + 8 HMMA.
-    {
-      const int S = n_rt * nks, gran = split ? 1 : nks, U = S / gran;
-      const int v = ((int)blockIdx.x + phase_rot(pc.layer, ph, G)) % G;
-      const int s0 = range_lo(U, v, G) * gran, s1 = range_lo(U, v + 1, G) * gran;
+    if (pg.split) {
+      // ---- split-K GEMV: stage (grp, kc) = row-tiles 8 grp .. 8 grp + 7 x inputs [128 kc, +128); warp w owns
+      // row-tile w, accumulates over the k-chunks of a group, then adds its 16 x 2 sums into R.
+      float ca[4] = {0.f, 0.f, 0.f, 0.f}, cb[4] = {0.f, 0.f, 0.f, 0.f};
+      int grp = pg.s0 / pg.nkc, kc = pg.s0 - grp * pg.nkc;
+      for (int s = pg.s0; s < pg.s1; ++s) {
+        const unsigned int slot = stage_ctr % NSTAGE, use = stage_ctr / NSTAGE;
+        ++stage_ctr;
+        uint4 b0 = make_uint4(0u, 0u, 0u, 0u), b1 = b0, b2 = b0, b3 = b0;
+        if (g < 4) {
+          const uint4* xb = (const uint4*)(x + (size_t)g * XCOL + t * 16 + (kc % XSLOTS) * SK_K);
+          b0 = xb[0]; b1 = xb[1]; b2 = xb[8]; b3 = xb[9];
+        }
+        mbar_wait(&full[slot], use & 1u, P.ctl, 0x200u + ph);
+        const uint4* st = (const uint4*)(ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
+        const uint4 a0 = st[0], a1 = st[32], a2 = st[64], a3 = st[96];
+        const uint4 a4 = st[128], a5 = st[160], a6 = st[192], a7 = st[224];
+        mma_bf16(ca, a0, b0.x, b0.y);
+        mma_bf16(cb, a1, b0.z, b0.w);
+        mma_bf16(ca, a2, b1.x, b1.y);
+        mma_bf16(cb, a3, b1.z, b1.w);
+        mma_bf16(ca, a4, b2.x, b2.y);
+        mma_bf16(cb, a5, b2.z, b2.w);
+        mma_bf16(ca, a6, b3.x, b3.y);
+        mma_bf16(cb, a7, b3.z, b3.w);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);   // stage consumed by this warp
+        if (kc == pg.nkc - 1 || s == pg.s1 - 1) {
+          // columns 0,1 = h (hi, lo parts), 2,3 = p: lanes t = 0 / 1 hold the h / p sums of rows g, g + 8
+          if (t < 2 && (t == 0 || accel)) {
+            const int r0 = (grp * SK_RT + warp) * 16 + g;
+            if (r0 < d) red_add(P.R + (size_t)t * d + r0, (ca[0] + ca[1]) + (cb[0] + cb[1]));
+            if (r0 + 8 < d) red_add(P.R + (size_t)t * d + r0 + 8, (ca[2] + ca[3]) + (cb[2] + cb[3]));
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) ca[i] = cb[i] = 0.f;
+        }
+        if (++kc == pg.nkc) { kc = 0; ++grp; }
+      }
+      TL(43);
+      if (need_aux) bar_wait(3);   // the auxiliary warp's adds of B u are issued and fenced
+    } else {
+      // ---- row-owned GEMV: stage (rt, ks) = 64 tiles of row-tile rt, inputs [1024 ks, +1024).  Warp w
+      // multiplies tiles 8w..8w+7.  A finished row-tile leaves 8 x 32 partial sums in shared memory; every
+      // FB finished row-tiles (and at the end) the 8 warps finish one row-tile each.
+      const int nks = pg.nkc;
       float ca[4] = {0.f, 0.f, 0.f, 0.f}, cb[4] = {0.f, 0.f, 0.f, 0.f};
       const bf16* xcol = x + (size_t)(g & 3) * XCOL + t * 16 + warp * 128;
-      int rt = s0 / nks, ks = s0 - rt * nks;
-      for (int s = s0; s < s1; ++s) {
+      int rt = pg.s0 / nks, ks = 0, pending_tiles = 0;
+      bool u_ready = !need_aux;
+      for (int s = pg.s0; s < pg.s1; ++s) {
         const unsigned int slot = stage_ctr % NSTAGE, use = stage_ctr / NSTAGE;
         ++stage_ctr;
         uint4 b0 = make_uint4(0u, 0u, 0u, 0u), b1 = b0, b2 = b0, b3 = b0;
@@ -1064,48 +1476,59 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
         mma_bf16(cb, a7, b3.z, b3.w);
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[slot]);   // stage consumed by this warp
-        if (ks == nks - 1 || s == s1 - 1) {
-          // ---- end of this CTA's segment of row-tile rt: columns 0,1 = h (hi, lo parts), 2,3 = p
-          float* rw = red + (size_t)(flushes & 1u) * NCW * 32 + warp * 32;
+        if (++ks == nks) {
+          // ---- row-tile rt finished in this warp's k range: park the partial sums
+          float* rw = red + ((size_t)pending_tiles * NCW + warp) * 32;
           if (t < 2) {
             rw[g * 2 + t] = (ca[0] + ca[1]) + (cb[0] + cb[1]);
             rw[(g + 8) * 2 + t] = (ca[2] + ca[3]) + (cb[2] + cb[3]);
           }
+          if (tid == 0) frt[pending_tiles] = rt;
 #pragma unroll
           for (int i = 0; i < 4; ++i) ca[i] = cb[i] = 0.f;
+          ks = 0; ++rt; ++pending_tiles;
+        }
+        if (pending_tiles == FB || (s == pg.s1 - 1 && pending_tiles > 0)) {
+          TL(41);
+          if (!u_ready) { bar_wait(3); u_ready = true; }   // u of this phase is in shared memory
           bar_consumers();
-          if (warp == 0) {
-            const float* rb = red + (size_t)(flushes & 1u) * NCW * 32 + lane;
+          TL(42);
+          if (warp < pending_tiles) {
+            const float* rb = red + ((size_t)warp * NCW) * 32 + lane;
             float sum = 0.f;
 #pragma unroll
             for (int w = 0; w < NCW; ++w) sum += rb[w * 32];
-            tile_out[lane] = sum;
+            float* T = tile_out + warp * 32;
+            T[lane] = sum;
             __syncwarp();
-            if (need_u && !us.ready) fetch_u(P, u_s, utmp, us);
-            int sl = 0;
-            if (split) sl = S >= G ? v - unit_owner(S, rt * nks, G) : ks;
-            epilogue_tile(P, tile_out, u_s, pc, rt, sl);
-            __syncwarp();
+            epilogue_tile(P, T, u_s, pc, frt[warp], udacc);
           }
-          ++flushes;
+          TL(44);
+          pending_tiles = 0;
+          if (s != pg.s1 - 1) bar_consumers();   // the parked sums are consumed before the next row-tile parks
           TL(40);
         }
-        if (++ks == nks) { ks = 0; ++rt; }
+      }
+      if (!u_ready) bar_wait(3);   // a CTA without stages in this phase still completes the handshake
+      if (ph == PH_GATEUP && accel && P.r > 0) {
+        // this CTA's share of u = A_d a^ (every CTA writes, also one without row-tiles: the sum runs over all)
+        float* ud_s = (float*)(smem_raw + OFF_UD);
+        if (lane == 1) {
+#pragma unroll
+          for (int j = 0; j < MAX_R; ++j) ud_s[warp * MAX_R + j] = udacc[j];
+        }
+        bar_consumers();
+        if (warp == 0 && lane < P.r) {
+          float sum = 0.f;
+#pragma unroll
+          for (int w = 0; w < NCW; ++w) sum += ud_s[w * MAX_R + lane];
+          __stcg(P.udpart + (size_t)blockIdx.x * MAX_R + lane, sum);
+        }
       }
     }
     TL(20 + ph);
-    if (ph == PH_HEAD) {
-      grid_sync(P.ctl, P.bar_base, nbar, G);
-      break;
-    }
-    if (ph != PH_EXIT) grid_sync(P.ctl, P.bar_base, nbar, G);   // nothing after an exit head depends on it
+    grid_sync(P.ctl, P.bar_base, nbar, G);
     TL(30 + ph);
-    // ---- next phase
-    if (ph == PH_QKV) ph = PH_ATTN;
-    else if (ph == PH_OPROJ) ph = PH_GATEUP;
-    else if (ph == PH_GATEUP) ph = PH_DOWN;
-    else if (ph == PH_DOWN && exit_phase_after(P, layer)) ph = PH_EXIT;
-    else { ++layer; ph = layer < n_run ? PH_QKV : PH_HEAD; }
   }
   TL(50);
   if (blockIdx.x == 0 && tid == 0) {
@@ -1118,16 +1541,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
       if (kj) P.exit_tok[j] = (int)(0xFFFFFFFFu - (unsigned int)(kj & 0xFFFFFFFFull));
       P.ctl->amax[1 + j] = 0ull;
     }
-    P.ctl->ucnt = 0u;
     if (P.advance) { *P.kv_len = pos + 1; *P.pending = tk; }
   }
 }
 
 // ------------------------------------------------------------------ repack: row-major [n_out, K] -> fragment-major stages
 // map 0: natural rows; 1: QKV (RoPE pairs (j, j+dh/2) of q and k made adjacent); 2: gate/up interleaved
-// (16-row tile = gate n..n+7, up n..n+7).  Rows / columns beyond the matrix are zero.
+// (16-row tile = gate n..n+7, up n..n+7): row-owned stages (row-tile, k-stage) of 1 x 1024.
+// map 3: split-K stages (row-tile group, k-chunk) of 8 row-tiles x 128 inputs, natural rows.
+// Rows / columns beyond the matrix are zero.
 __device__ __forceinline__ const bf16* pack_src_row(const bf16* src, const bf16* src2, int map, int r, int n_out, int K, int d, int dh) {
-  if (map == 0) return r < n_out ? src + (size_t)r * K : nullptr;
+  if (map == 0 || map == 3) return r < n_out ? src + (size_t)r * K : nullptr;
   if (map == 1) {
     if (r >= n_out) return nullptr;
     int which = r / d, w = r % d, sr = r;
@@ -1141,15 +1565,24 @@ __device__ __forceinline__ const bf16* pack_src_row(const bf16* src, const bf16*
   if (n >= n_out) return nullptr;
   return ((r & 15) < 8 ? src : src2) + (size_t)n * K;
 }
+__global__ void transpose_kernel(bf16* __restrict__ dst, const bf16* __restrict__ src, int rows, int cols) {
+  // src [rows][cols] -> dst [cols][rows]
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < (size_t)rows * cols; i += (size_t)gridDim.x * blockDim.x) {
+    const int c = (int)(i / rows), r = (int)(i % rows);
+    dst[i] = src[(size_t)r * cols + c];
+  }
+}
 __global__ void pack_kernel(uint4* __restrict__ dst, const bf16* __restrict__ src, const bf16* __restrict__ src2,
-                            int map, int n_out, int K, int n_rt, int nks, int d, int dh) {
-  const size_t total = (size_t)n_rt * nks * (STAGE_BYTES / 16);
+                            int map, int n_out, int K, int n_units, int nks, int d, int dh) {
+  const size_t total = (size_t)n_units * nks * (STAGE_BYTES / 16);
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     const size_t stage = i / (STAGE_BYTES / 16);
     const int within = (int)(i % (STAGE_BYTES / 16));
     const int tile = within >> 5, lane = within & 31, g = lane >> 2, t = lane & 3;
-    const int rt = (int)(stage / nks), ks = (int)(stage % nks);
-    const int k = ks * STAGE_K + tile * 16 + 2 * t;
+    const int un = (int)(stage / nks), ks = (int)(stage % nks);
+    int rt, k;
+    if (map == 3) { rt = un * SK_RT + (tile >> 3); k = ks * SK_K + (tile & 7) * 16 + 2 * t; }
+    else { rt = un; k = ks * STAGE_K + tile * 16 + 2 * t; }
     const bf16* r0 = pack_src_row(src, src2, map, rt * 16 + g, n_out, K, d, dh);
     const bf16* r1 = pack_src_row(src, src2, map, rt * 16 + g + 8, n_out, K, d, dh);
     uint4 v = make_uint4(0u, 0u, 0u, 0u);   // K % 8 == 0: a pair never straddles the end
@@ -1174,66 +1607,75 @@ struct FusedImpl {
   Ctl* h_ctl = nullptr;       // pinned
   bool bound = false;
   u64* d_tl = nullptr;        // debug timeline (M2R2_FUSED_DEBUG builds)
+  std::vector<int> gate_of;   // per layer: 1 + gate index, or 0
+  std::vector<int> accel_of;
   // scratch carve
-  float *RA, *RB, *oslots, *dslots, *act, *qbuf, *khat, *vhat, *pexit, *apart, *upart;
+  float *R, *act, *qbuf, *khat, *vhat, *apart, *apu, *udpart;
+  u64* upart;
   int* accel_cols;
 };
 
 static int pad_to(int v, int m) { return (v + m - 1) / m * m; }
 
-bool fused_config_ok(const m2r2_config& c) {
-  if (c.dtype != M2R2_BF16 || c.n_experts != 0) return false;
-  if (c.head_dim % 8 || c.head_dim > 128) return false;
-  if (c.d_model % 16 || c.d_ff % 8) return false;
-  if (c.accel_enabled && (c.adapter_rank > MAX_R || c.adapter_rank < 1)) return false;
-  if (pad_to(c.d_model, STAGE_K) > NORM_CH * NCT * 4 || pad_to(c.d_ff, STAGE_K) > KMAX) return false;
-  if ((size_t)2 * NCW * 2 * (c.head_dim + 2) * sizeof(float) > (size_t)X_BYTES) return false;
-  return true;
-}
-
 struct PackedDims {
-  int d_pad, F_pad, rt_qkv, rt_o, rt_gu, rt_d, rt_v;
+  int d_pad, F_pad, rt_qkv, rt_gu, rt_v, ng_d, nkc_o, nkc_d;
   size_t st_qkv, st_o, st_gu, st_d, st_v;   // stages
 };
 static PackedDims packed_dims(const m2r2_config& c) {
   PackedDims q;
   q.d_pad = pad_to(c.d_model, STAGE_K);
-  q.F_pad = pad_to(c.d_ff, STAGE_K);
+  q.F_pad = pad_to(c.d_ff, SK_K);
   q.rt_qkv = pad_to(3 * c.d_model, 16) / 16;
-  q.rt_o = pad_to(c.d_model, 16) / 16;
   q.rt_gu = pad_to(c.d_ff, 8) / 8;
-  q.rt_d = q.rt_o;
   q.rt_v = pad_to(c.vocab, 16) / 16;
+  q.ng_d = pad_to(c.d_model, 16 * SK_RT) / (16 * SK_RT);
+  q.nkc_o = pad_to(c.d_model, SK_K) / SK_K;
+  q.nkc_d = q.F_pad / SK_K;
   q.st_qkv = (size_t)q.rt_qkv * (q.d_pad / STAGE_K);
-  q.st_o = (size_t)q.rt_o * (q.d_pad / STAGE_K);
+  q.st_o = (size_t)q.ng_d * q.nkc_o;
   q.st_gu = (size_t)q.rt_gu * (q.d_pad / STAGE_K);
-  q.st_d = (size_t)q.rt_d * (q.F_pad / STAGE_K);
+  q.st_d = (size_t)q.ng_d * q.nkc_d;
   q.st_v = (size_t)q.rt_v * (q.d_pad / STAGE_K);
   return q;
+}
+
+bool fused_config_ok(const m2r2_config& c) {
+  if (c.dtype != M2R2_BF16 || c.n_experts != 0 || c.n_layers > MAXL_S) return false;
+  if (c.head_dim % 8 || c.head_dim > 128) return false;
+  if (c.d_model % 16 || c.d_ff % 8) return false;
+  if (c.accel_enabled && (c.adapter_rank > MAX_R || c.adapter_rank < 1)) return false;
+  if (pad_to(c.d_model, STAGE_K) > XMAX || c.d_ff > KMAX) return false;
+  if ((size_t)2 * NCW * 2 * (c.head_dim + 2) * sizeof(float) > (size_t)KV_BYTES) return false;
+  // a CTA's split-K stage range of the down matrix must fit the x slots (worst case: 100 CTAs)
+  PackedDims q = packed_dims(c);
+  if (q.nkc_d > XSLOTS && (q.st_d + 99) / 100 + 1 > (size_t)XSLOTS) return false;
+  return true;
 }
 
 size_t fused_weights_bytes(const m2r2_config& c) {
   if (!fused_config_ok(c)) return 0;
   PackedDims q = packed_dims(c);
-  return ((q.st_qkv + q.st_o + q.st_gu + q.st_d) * (size_t)c.n_layers + q.st_v) * STAGE_BYTES + 1024;
+  const size_t adt = c.accel_enabled ? (((size_t)c.d_ff * c.adapter_rank * 2 + 255) & ~(size_t)255) + (((size_t)c.n_accel_heads * c.head_dim * c.adapter_rank * 2 + 255) & ~(size_t)255) : 0;
+  return ((q.st_qkv + q.st_o + q.st_gu + q.st_d) * (size_t)c.n_layers + q.st_v) * STAGE_BYTES + adt * c.n_layers + 1024;
 }
 
 void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs) {
   if (!fused_config_ok(c)) return;
   PackedDims q = packed_dims(c);
-  const size_t d = c.d_model, NG = std::max(1, c.n_gates);
+  const size_t d = c.d_model;
   FusedImpl* im = fs ? fs->impl : nullptr;
 #define FTAKE(field, T, n) { T* p_ = cv.take<T>(n); if (im) im->field = p_; }
   FTAKE(d_layers, FLayer, c.n_layers)
   FTAKE(d_ctl, Ctl, 1)
   FTAKE(d_sidx, int, c.n_heads)
   FTAKE(accel_cols, int, std::max(8, c.n_accel_heads * c.head_dim))
-  FTAKE(RA, float, 2 * d) FTAKE(RB, float, 2 * d)
-  FTAKE(oslots, float, (size_t)MAX_SLOTS * 2 * d) FTAKE(dslots, float, (size_t)MAX_SLOTS * 2 * d)
+  FTAKE(R, float, 2 * d)
   FTAKE(act, float, 2 * (size_t)q.F_pad)
-  FTAKE(qbuf, float, 2 * d) FTAKE(khat, float, d) FTAKE(vhat, float, d) FTAKE(pexit, float, NG * d)
+  FTAKE(qbuf, float, 2 * d) FTAKE(khat, float, d) FTAKE(vhat, float, d)
   FTAKE(apart, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * 2 * (c.head_dim + 4))
-  FTAKE(upart, float, (size_t)2 * MAX_NJ * UPART_Q)
+  FTAKE(upart, u64, (size_t)MAX_NJ * UPART_Q)
+  FTAKE(apu, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * MAX_R)
+  FTAKE(udpart, float, (size_t)1024 * MAX_R)
 #undef FTAKE
 }
 
@@ -1246,7 +1688,7 @@ int fused_create(const m2r2_config& c, FusedState* fs) {
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  if (!coop || max_smem < SMEM_BYTES || sms < 2 * MAX_NJ) return 0;   // per-operation kernels serve this device
+  if (!coop || max_smem < SMEM_BYTES || sms < 100) return 0;   // per-operation kernels serve this device
   if (cudaFuncSetAttribute(m2r2_fused_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return 0;
@@ -1275,9 +1717,9 @@ void fused_destroy(FusedState* fs) {
 
 bool fused_supported(const m2r2_config&, const FusedState* fs) { return fs->supported && fs->impl && fs->impl->bound; }
 
-static int pack(cudaStream_t st, void* dst, const void* src, const void* src2, int map, int n_out, int K, int n_rt,
+static int pack(cudaStream_t st, void* dst, const void* src, const void* src2, int map, int n_out, int K, int n_units,
                 int nks, int d, int dh) {
-  pack_kernel<<<1184, 256, 0, st>>>((uint4*)dst, (const bf16*)src, (const bf16*)src2, map, n_out, K, n_rt, nks, d, dh);
+  pack_kernel<<<1184, 256, 0, st>>>((uint4*)dst, (const bf16*)src, (const bf16*)src2, map, n_out, K, n_units, nks, d, dh);
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }
 
@@ -1288,10 +1730,12 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
   const int d = c.d_model, dh = c.head_dim, F = c.d_ff;
-  const int ks_d = q.d_pad / STAGE_K, ks_f = q.F_pad / STAGE_K;
+  const int ks_d = q.d_pad / STAGE_K;
   char* wp = (char*)packed;
   wp = (char*)(((uintptr_t)wp + 1023) & ~(uintptr_t)1023);
   std::vector<FLayer> hl(c.n_layers);
+  im->gate_of.assign(c.n_layers, 0);
+  im->accel_of.assign(c.n_layers, 0);
   const size_t per = (size_t)c.max_batch * c.n_heads * c.max_seq * dh;   // elements per layer of K (or V)
   for (int i = 0; i < c.n_layers; ++i) {
     const DevLayer& L = layers[i];
@@ -1302,9 +1746,9 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     f.Wgu = (const uint4*)wp; wp += q.st_gu * STAGE_BYTES;
     f.Wd = (const uint4*)wp; wp += q.st_d * STAGE_BYTES;
     if (pack(st, (void*)f.Wqkv, L.wqkv, nullptr, 1, 3 * d, d, q.rt_qkv, ks_d, d, dh)) return M2R2_CUDA;
-    if (pack(st, (void*)f.Wo, L.wo, nullptr, 0, d, d, q.rt_o, ks_d, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wo, L.wo, nullptr, 3, d, d, q.ng_d, q.nkc_o, d, dh)) return M2R2_CUDA;
     if (pack(st, (void*)f.Wgu, L.wgate, L.wup, 2, F, d, q.rt_gu, ks_d, d, dh)) return M2R2_CUDA;
-    if (pack(st, (void*)f.Wd, L.wdown, nullptr, 0, d, F, q.rt_d, ks_f, d, dh)) return M2R2_CUDA;
+    if (pack(st, (void*)f.Wd, L.wdown, nullptr, 3, d, F, q.ng_d, q.nkc_d, d, dh)) return M2R2_CUDA;
     f.g1 = (const bf16*)L.g1; f.g2 = (const bf16*)L.g2;
     f.Aqkv = (const bf16*)L.Aqkv; f.Bqkv = (const bf16*)L.Bqkv; f.Ao = (const bf16*)L.Ao; f.Bo = (const bf16*)L.Bo;
     f.Agu = (const bf16*)L.Agu; f.Bg = (const bf16*)L.Bg; f.Bu = (const bf16*)L.Bu; f.Ad = (const bf16*)L.Ad; f.Bd = (const bf16*)L.Bd;
@@ -1317,9 +1761,25 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     }
     f.gate = 0;
     for (int j = 0; j < c.n_gates; ++j) if (c.gates[j] == i + 1) f.gate = j + 1;
+    im->gate_of[i] = f.gate;
+    im->accel_of[i] = f.accel;
   }
   const uint4* Wlm = (const uint4*)wp;
   if (pack(st, (void*)Wlm, lm_head, nullptr, 0, c.vocab, d, q.rt_v, ks_d, d, dh)) return M2R2_CUDA;
+  wp += q.st_v * STAGE_BYTES;
+  if (c.accel_enabled) {
+    const size_t adt = ((size_t)F * c.adapter_rank * 2 + 255) & ~(size_t)255;
+    for (int i = 0; i < c.n_layers; ++i) {
+      if (!hl[i].accel || !layers[i].Ad) continue;
+      transpose_kernel<<<64, 256, 0, st>>>((bf16*)wp, (const bf16*)layers[i].Ad, c.adapter_rank, F);
+      hl[i].AdT = (const bf16*)wp;
+      wp += adt;
+      transpose_kernel<<<16, 256, 0, st>>>((bf16*)wp, (const bf16*)layers[i].Ao, c.adapter_rank, c.n_accel_heads * dh);
+      hl[i].AoT = (const bf16*)wp;
+      wp += ((size_t)c.n_accel_heads * dh * c.adapter_rank * 2 + 255) & ~(size_t)255;
+    }
+    if (cudaGetLastError() != cudaSuccess) return M2R2_CUDA;
+  }
   if (cudaMemcpyAsync(im->d_layers, hl.data(), sizeof(FLayer) * c.n_layers, cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   std::vector<int> sidx(c.n_heads, -1), cols(std::max(8, c.n_accel_heads * dh), 0);
   if (c.accel_enabled)
@@ -1331,7 +1791,9 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   if (cudaMemcpyAsync(im->accel_cols, cols.data(), sizeof(int) * cols.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
   cudaMemsetAsync(im->act, 0, sizeof(float) * 2 * q.F_pad, st);
-  cudaMemsetAsync(im->pexit, 0, sizeof(float) * std::max(1, c.n_gates) * d, st);
+  cudaMemsetAsync(im->R, 0, sizeof(float) * 2 * d, st);
+  cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * MAX_R, st);
+  cudaMemsetAsync(im->upart, 0, sizeof(u64) * MAX_NJ * UPART_Q, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;   // hl / sidx / cols are stack-owned
   im->bar_base = 0;
   FParams& p = im->p;
@@ -1339,18 +1801,18 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   p.d = d; p.n_heads = c.n_heads; p.dh = dh; p.F = F; p.V = c.vocab; p.r = c.accel_enabled ? c.adapter_rank : 0;
   p.da = c.n_accel_heads * dh; p.max_seq = c.max_seq;
   p.d_pad = q.d_pad; p.F_pad = q.F_pad;
-  p.rt_qkv = q.rt_qkv; p.rt_o = q.rt_o; p.rt_gu = q.rt_gu; p.rt_d = q.rt_d; p.rt_v = q.rt_v;
+  p.rt_qkv = q.rt_qkv; p.rt_gu = q.rt_gu; p.rt_v = q.rt_v; p.ng_d = q.ng_d;
   p.eps = c.rms_eps; p.scale = 1.0f / sqrtf((float)dh);
   p.layers = im->d_layers;
   p.embed = (const bf16*)embed; p.gf = (const bf16*)gf; p.lmA = (const bf16*)lm_A; p.lmB = (const bf16*)lm_B;
   p.Wlm = Wlm;
   p.sidx = im->d_sidx; p.accel_cols = im->accel_cols; p.rope_tab = rope_tab;
   p.n_gates = c.n_gates;
-  p.RA = im->RA; p.RB = im->RB; p.oslots = im->oslots; p.dslots = im->dslots;
+  p.R = im->R;
   p.act = im->act; p.qbuf = im->qbuf; p.khat = im->khat; p.vhat = im->vhat;
-  p.pexit = im->pexit; p.apart = im->apart; p.upart = im->upart;
+  p.apart = im->apart; p.upart = im->upart; p.apu = im->apu; p.udpart = im->udpart;
+  p.nah = c.accel_enabled ? c.n_accel_heads : 0;
   p.ctl = im->d_ctl;
-  p.pf_ahead = getenv("M2R2_PF") ? atoi(getenv("M2R2_PF")) : PF_DEFAULT;
   p.tl = nullptr;
 #ifdef M2R2_FUSED_DEBUG
   if (getenv("M2R2_TL_OUT") && !im->d_tl) cudaMalloc((void**)&im->d_tl, sizeof(u64) * TL_MAX * im->G);
@@ -1386,8 +1848,11 @@ int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const Fused
   ns = std::min(ns, (int)M2R2_MAX_SPLITS);
   p.ns = ns;
   p.pos_host = pos;
-  // grid barriers of this launch (must match the kernel's sequence): 5 per layer + the final one
-  const unsigned int nbar = 5u * (unsigned int)run.n_layers + 1u;
+  // grid barriers of this launch (must match the kernel's sequence): per layer 4 weight phases + attention,
+  // one per exit head, one for the final head
+  unsigned int nbar = 5u * (unsigned int)run.n_layers + 1u;
+  for (int i = 0; i < run.n_layers; ++i)
+    if (im->gate_of[i] && im->accel_of[i] && run.exit_heads && !(run.head_stream == 1 && i + 1 == run.n_layers)) ++nbar;
   p.bar_base = im->bar_base;
   im->bar_base += nbar * (unsigned int)G;
   void* args[] = {(void*)&p};
@@ -1415,6 +1880,7 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
     snprintf(msg, n, "fused kernel wait timed out (site 0x%x)", im->h_ctl->abort_where);
     // re-arm: barrier counter and flags back to a clean state
     cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
+    cudaMemsetAsync(im->upart, 0, sizeof(u64) * MAX_NJ * UPART_Q, st);
     cudaStreamSynchronize(st);
     im->bar_base = 0;
     return M2R2_CUDA;
