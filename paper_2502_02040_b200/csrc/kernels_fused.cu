@@ -52,7 +52,7 @@ constexpr int STAGE_TILES = 64;                // m16k16 tiles per stage
 constexpr int STAGE_BYTES = STAGE_TILES * 512; // 32 KB
 constexpr int SK_K = 128;                      // inputs per split-K stage
 constexpr int SK_RT = 8;                       // row-tiles per split-K stage
-constexpr int NSTAGE = 5;
+constexpr int NSTAGE = 4;
 constexpr int NCW = 8;                 // consumer warps
 constexpr int NCT = NCW * 32;          // consumer threads
 constexpr int NTHREADS = NCT + 64;     // + producer warp + auxiliary warp
@@ -67,7 +67,7 @@ constexpr int RED_FLOATS = FB * NCW * 32;
 constexpr int MAX_R = 8;               // adapter rank limit (PAPER.md L399 uses 8); larger ranks take the per-operation kernels
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
-constexpr int NORM_CH = 4;             // float4 chunks per thread in a norm loader (d <= 4096)
+constexpr int MERGE_NS = 4;            // attention splits combined from registers by the auxiliary warp; more take a looped path
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
 
 enum { PH_QKV = 0, PH_OPROJ = 1, PH_GATEUP = 2, PH_DOWN = 3, PH_HEAD = 4, PH_EXIT = 5, N_PH = 6 };
@@ -128,7 +128,8 @@ struct FParams {
 // ------------------------------------------------------------------ shared memory map (fixed offsets)
 constexpr int OFF_X = NSTAGE * STAGE_BYTES;
 constexpr int OFF_RED = OFF_X + X_BYTES;              // [FB][NCW][32] floats
-constexpr int OFF_TILE = OFF_RED + RED_FLOATS * 4;    // [NCW][32] floats
+constexpr int KV_EXTRA = 32 * 1024;                   // with the x columns and the parked sums: the attention K/V staging area
+constexpr int OFF_TILE = OFF_RED + RED_FLOATS * 4 + KV_EXTRA;   // [NCW][32] floats
 constexpr int OFF_U = OFF_TILE + NCW * 32 * 4;        // [MAX_NJ] floats (64 reserved)
 constexpr int OFF_SRED = OFF_U + 256;                 // [64] floats
 constexpr int OFF_BAR = OFF_SRED + 256;               // full[NSTAGE], empty[NSTAGE]
@@ -138,7 +139,8 @@ constexpr int OFF_UD = OFF_FRT + 64;                  // [NCW][MAX_R] floats: pe
 constexpr int OFF_SIDX = OFF_UD + NCW * MAX_R * 4;    // [M2R2_MAX_HEADS] ints: head -> index in S or -1
 constexpr int MAXL_S = 64;                            // layers whose descriptors are cached in shared memory
 constexpr int OFF_LAYERS = OFF_SIDX + M2R2_MAX_HEADS * 4;   // [MAXL_S] FLayer
-constexpr int OFF_TLN = OFF_LAYERS + MAXL_S * (int)sizeof(FLayer); // debug timeline cursor
+constexpr int OFF_GEO = OFF_LAYERS + MAXL_S * (int)sizeof(FLayer);   // [N_PH] int4 {s0, s1, nkc, split}: this CTA's stage range per phase type
+constexpr int OFF_TLN = OFF_GEO + 8 * 16;             // debug timeline cursor
 constexpr int SMEM_BYTES = OFF_TLN + 64;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -223,8 +225,7 @@ __device__ __forceinline__ u64 amax_key(float v, int n) {
 // ------------------------------------------------------------------ static work split
 // A phase has S stages.  Virtual CTA v of G owns units [U*v/G, U*(v+1)/G) where a unit is `gran`
 // consecutive stages (gran = stages per row-tile for row-owned phases, 1 for split-K).
-__device__ __forceinline__ int range_lo(int U, int v, int G) { return (int)(((long long)U * v) / G); }
-__device__ __forceinline__ int phase_rot(int layer, int ph, int G) { return (int)(((unsigned)(layer * 5 + ph) * 29u) % (unsigned)G); }
+__device__ __forceinline__ int range_lo(int U, int v, int G) { return (int)(((unsigned)U * (unsigned)v) / (unsigned)G); }   // U * G < 2^32
 
 #ifdef M2R2_FUSED_DEBUG
 constexpr int TL_MAX = 4096;
@@ -252,7 +253,7 @@ __device__ __forceinline__ void mbar_wait(u64* b, uint32_t parity, Ctl* ctl, uns
 }
 
 // ------------------------------------------------------------------ grid barrier (all CTAs co-resident: cooperative launch)
-__device__ __forceinline__ void grid_sync(Ctl* ctl, unsigned int bar_base, unsigned int& nbar, int G) {
+__device__ __noinline__ void grid_sync(Ctl* ctl, unsigned int bar_base, unsigned int& nbar, int G) {
   bar_consumers();
   ++nbar;
   if (threadIdx.x == 0) {
@@ -311,211 +312,200 @@ struct LoadSrc {
   bool p_live;           // the producing layer carried p
   int gate;              // 1 + gate index: p <- h
 };
-template <int NCH>
-__device__ __noinline__ void loader_norm_t(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src,
-                                           float* trace_dst, const bf16* g, int G) {
-  const int tid = threadIdx.x, d = P.d;
-  bar_consumers();   // x of the previous phase is dead in every warp
+// Staging area of the loaders: raw fp32 / bf16 inputs land here with 16-byte cp.async (LDGSTS through L2,
+// every copy of a thread in flight at once, no registers), then rolled loops convert them into the x columns.
+// Rolled loops keep the code small: the instruction cache holds 32 KB and a layer's code runs once per layer.
+constexpr int STG_BYTES = RED_FLOATS * 4 + KV_EXTRA;   // 40 KB: the parked sums + the K/V extension are dead here
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+__device__ __noinline__ void loader_norm(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src,
+                                         float* trace_dst, const bf16* g, int G) {
+  const int tid = threadIdx.x, d = P.d, nq = d >> 2;
+  float* sh = (float*)(smem_raw + OFF_RED);      // h  [d_pad] fp32
+  float* sp = sh + P.d_pad;                      // p  [d_pad] fp32
+  bf16* sg = (bf16*)(sp + P.d_pad);              // gains [d_pad] bf16 (40 KB in all at d_pad = 4096)
+  bf16* se = x;                                  // embedding row [d] bf16: the x columns are dead until pass 2
+  bar_consumers();   // x and the staging area of the previous phase are dead in every warp
+  if (src.emb) {
+    for (int c = tid; c < (d >> 3); c += NCT) { cp_async16(sg + 8 * c, g + 8 * c); cp_async16(se + 8 * c, src.emb + 8 * c); }
+  } else {
+    for (int c = tid; c < nq; c += NCT) {
+      cp_async16(sh + 4 * c, P.R + 4 * c);
+      if (src.p_live) cp_async16(sp + 4 * c, P.R + d + 4 * c);
+    }
+    for (int c = tid; c < (d >> 3); c += NCT) cp_async16(sg + 8 * c, g + 8 * c);
+  }
+  cp_async_wait_all();
+  bar_consumers();
   TL(64);
-  float4 xh[NCH], xp[NCH];
-  uint2 ge[NCH];
-  const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-  for (int j = 0; j < NCH; ++j) {   // all loads first: one L2 round trip
-    const int k = (tid + j * NCT) * 4;
-    xh[j] = z4; xp[j] = z4;
-    ge[j] = make_uint2(0u, 0u);
-    if (k < d) {
-      ge[j] = __ldg((const uint2*)(g + k));
-      if (src.emb) {
-        const uint2 e = __ldg((const uint2*)(src.emb + k));
-        bf16x2_to_f32(e.x, xh[j].x, xh[j].y);
-        bf16x2_to_f32(e.y, xh[j].z, xh[j].w);
-      } else {
-        xh[j] = ldcg4(P.R + k);
-        if (src.p_live) xp[j] = ldcg4(P.R + d + k);
-      }
-    }
-  }
+  // ---- pass 1: gate, write-back by the chunk's owner CTA, sums of squares of the phase's two inputs
   float ssh = 0.f, ssp = 0.f;
-#pragma unroll
-  for (int j = 0; j < NCH; ++j) {
-    const int ci = tid + j * NCT, k = ci * 4;
-    if (k < d) {
-      const float4 hv = xh[j];
-      float4 pv = src.p_live ? xp[j] : hv;
-      const bool owner = (ci % G) == (int)blockIdx.x;
-      const float4 pbefore = pv;
-      if (src.gate) pv = hv;
-      if (owner && trace_dst) { st4(trace_dst + k, hv); st4(trace_dst + d + k, pbefore); }
-      if (owner && src.emb) st4(P.R + k, hv);
-      if (owner && (src.emb || src.gate || !src.p_live)) st4(P.R + d + k, pv);
-      if (mode == LN_HEAD_P) { xh[j] = pbefore; xp[j] = pbefore; }
-      else if (mode == LN_HEAD_H) { xp[j] = hv; }
-      else { xp[j] = pv; }
-      ssh += f4ss(xh[j]);
-      ssp += f4ss(xp[j]);
+#pragma unroll 1
+  for (int c = tid; c < nq; c += NCT) {
+    const int k = 4 * c;
+    float4 hv, pv;
+    if (src.emb) {
+      const uint2 e = *(const uint2*)(se + k);
+      bf16x2_to_f32(e.x, hv.x, hv.y);
+      bf16x2_to_f32(e.y, hv.z, hv.w);
+    } else {
+      hv = *(const float4*)(sh + k);
     }
+    pv = src.p_live ? *(const float4*)(sp + k) : hv;
+    const float4 pbefore = pv;
+    if (src.gate) pv = hv;
+    if ((c % G) == (int)blockIdx.x) {
+      if (trace_dst) { st4(trace_dst + k, hv); st4(trace_dst + d + k, pbefore); }
+      if (src.emb) st4(P.R + k, hv);
+      if (src.emb || src.gate || !src.p_live) st4(P.R + d + k, pv);
+    }
+    const float4 a = mode == LN_HEAD_P ? pbefore : hv;
+    const float4 b = mode == LN_HEAD_P ? pbefore : (mode == LN_HEAD_H ? hv : pv);
+    if (src.emb || mode != LN_QKV || src.gate || !src.p_live) { *(float4*)(sh + k) = a; *(float4*)(sp + k) = b; }   // what pass 2 reads
+    ssh += f4ss(a);
+    ssp += f4ss(b);
   }
-  TL(65);
   ssh = warp_sum(ssh);
   ssp = warp_sum(ssp);
   if ((tid & 31) == 0) { sred[tid >> 5] = ssh; sred[NCW + (tid >> 5)] = ssp; }
   bar_consumers();
-  TL(66);
   float th = 0.f, tp = 0.f;
 #pragma unroll
   for (int w = 0; w < NCW; ++w) { th += sred[w]; tp += sred[NCW + w]; }
   const float ih = rsqrtf(th / (float)d + P.eps), ip = rsqrtf(tp / (float)d + P.eps);
   bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
-#pragma unroll
-  for (int j = 0; j < NCH; ++j) {
-    const int k = (tid + j * NCT) * 4;
-    if (k < P.d_pad) {
-      float4 a = xh[j], b = xp[j];
-      if (k < d) {
-        float g0, g1, g2, g3;
-        bf16x2_to_f32(ge[j].x, g0, g1);
-        bf16x2_to_f32(ge[j].y, g2, g3);
-        a.x = a.x * ih * g0; a.y = a.y * ih * g1; a.z = a.z * ih * g2; a.w = a.w * ih * g3;
-        b.x = b.x * ip * g0; b.y = b.y * ip * g1; b.z = b.z * ip * g2; b.w = b.w * ip * g3;
-      }
-      xstore4(c0, c1, k, a);
-      xstore4(c2, c3, k, b);
+  // ---- pass 2: x = rms(.; g) as bf16 hi + lo columns; zero padding up to d_pad
+#pragma unroll 1
+  for (int c = tid; c < (P.d_pad >> 2); c += NCT) {
+    const int k = 4 * c;
+    float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a;
+    if (k < d) {
+      a = *(const float4*)(sh + k);
+      b = *(const float4*)(sp + k);
+      const uint2 ge = *(const uint2*)(sg + k);
+      float g0, g1, g2, g3;
+      bf16x2_to_f32(ge.x, g0, g1);
+      bf16x2_to_f32(ge.y, g2, g3);
+      a.x = a.x * ih * g0; a.y = a.y * ih * g1; a.z = a.z * ih * g2; a.w = a.w * ih * g3;
+      b.x = b.x * ip * g0; b.y = b.y * ip * g1; b.z = b.z * ip * g2; b.w = b.w * ip * g3;
     }
+    xstore4(c0, c1, k, a);
+    xstore4(c2, c3, k, b);
   }
   bar_consumers();
 }
-__device__ __forceinline__ void loader_norm(const FParams& P, bf16* x, float* sred, int mode, const LoadSrc& src,
-                                            float* trace_dst, const bf16* g, int G) {
-  const int nch = (P.d_pad >> 2) / NCT;   // d_pad is a multiple of 1024 = 4 * NCT
-  if (nch <= 1) loader_norm_t<1>(P, x, sred, mode, src, trace_dst, g, G);
-  else if (nch == 2) loader_norm_t<2>(P, x, sred, mode, src, trace_dst, g, G);
-  else if (nch == 3) loader_norm_t<3>(P, x, sred, mode, src, trace_dst, g, G);
-  else loader_norm_t<NORM_CH>(P, x, sred, mode, src, trace_dst, g, G);
-}
 
-// Merge of the attention split partials (m, l, o) of one query for columns k..k+3 of a head (a4).
-constexpr int MERGE_NS = 4;   // splits merged from registers; more splits take the looped path
-struct MergeRegs {
-  float4 o[MERGE_NS];
-  float2 ml[MERGE_NS];
-};
-__device__ __forceinline__ void merge_load(const FParams& P, MergeRegs& m, int q, int k) {
+// Input slice of a split-K phase: the CTA's stages [s0, s1) of a matrix with nkc k-chunks per row-tile
+// group touch chunks kc0, kc0+1, ... (mod nkc), cnt of them; chunk kc lives in x slot kc % XSLOTS.
+//   OPROJ: merged attention output of both queries (the accelerated stream has columns of S only): the
+//          split partials (m, l, o) of the heads the chunks touch are staged, then merged in split order
+//   DOWN:  SwiGLU activations of both streams
+__device__ __noinline__ float4 merge_global(const FParams& P, int q, int k) {   // partials do not fit the staging area
   const int dh = P.dh, NS = P.ns, head = k / dh, j = k - head * dh;
   const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
-#pragma unroll
-  for (int s = 0; s < MERGE_NS; ++s) {
-    m.o[s] = make_float4(0.f, 0.f, 0.f, 0.f);
-    m.ml[s] = make_float2(0.f, 0.f);
-    if (s < NS) {
-      const float* ps = pp + (size_t)s * 2 * (dh + 4);
-      m.o[s] = ldcg4(ps + j);
-      m.ml[s] = __ldcg((const float2*)(ps + dh));
-    }
-  }
-}
-__device__ __forceinline__ float4 merge_finish(const FParams& P, const MergeRegs& m, int q, int k) {
-  const int dh = P.dh, NS = P.ns;
   float M = -INFINITY, Lsum = 0.f;
   float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (NS <= MERGE_NS) {
-#pragma unroll
-    for (int s = 0; s < MERGE_NS; ++s) if (s < NS && m.ml[s].y > 0.f) M = fmaxf(M, m.ml[s].x);
-#pragma unroll
-    for (int s = 0; s < MERGE_NS; ++s) {
-      if (s < NS && m.ml[s].y > 0.f) {
-        const float wgt = __expf(m.ml[s].x - M);
-        Lsum += m.ml[s].y * wgt;
-        o.x += m.o[s].x * wgt; o.y += m.o[s].y * wgt; o.z += m.o[s].z * wgt; o.w += m.o[s].w * wgt;
-      }
-    }
-  } else {
-    const int head = k / dh, j = k - head * dh;
-    const float* pp = P.apart + ((size_t)(head * NS) * 2 + q) * (dh + 4);
-    for (int s = 0; s < NS; ++s) {
-      const float* ps = pp + (size_t)s * 2 * (dh + 4);
-      if (ldcg(ps + dh + 1) > 0.f) M = fmaxf(M, ldcg(ps + dh));
-    }
-    for (int s = 0; s < NS; ++s) {
-      const float* ps = pp + (size_t)s * 2 * (dh + 4);
-      const float ls = ldcg(ps + dh + 1);
-      if (ls > 0.f) {
-        const float wgt = __expf(ldcg(ps + dh) - M);
-        const float4 v = ldcg4(ps + j);
-        Lsum += ls * wgt;
-        o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
-      }
+  for (int s = 0; s < NS; ++s) {
+    const float* ps = pp + (size_t)s * 2 * (dh + 4);
+    if (ldcg(ps + dh + 1) > 0.f) M = fmaxf(M, ldcg(ps + dh));
+  }
+  for (int s = 0; s < NS; ++s) {
+    const float* ps = pp + (size_t)s * 2 * (dh + 4);
+    const float ls = ldcg(ps + dh + 1);
+    if (ls > 0.f) {
+      const float wgt = __expf(ldcg(ps + dh) - M);
+      const float4 v = ldcg4(ps + j);
+      Lsum += ls * wgt;
+      o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
     }
   }
   const float inv = 1.f / Lsum;
   o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
   return o;
 }
-
-// Input slice of a split-K phase: the CTA's stages [s0, s1) of a matrix with nkc k-chunks per row-tile
-// group touch chunks kc0, kc0+1, ... (mod nkc), cnt of them; chunk kc lives in x slot kc % XSLOTS.
-//   OPROJ: merged attention output of both queries (the accelerated stream has columns of S only)
-//   DOWN:  SwiGLU activations of both streams
 __device__ __noinline__ void loader_slice(const FParams& P, bf16* x, int ph, bool accel, int kc0, int cnt, int nkc) {
   const int tid = threadIdx.x;
-  bar_consumers();
+  float* stg = (float*)(smem_raw + OFF_RED);
   bf16 *c0 = x, *c1 = x + XCOL, *c2 = x + 2 * XCOL, *c3 = x + 3 * XCOL;
   const int items = cnt * 64;   // (chunk, stream, float4)
-  const int K = ph == PH_OPROJ ? P.d : P.F;
-  constexpr int MC = 2;
-  for (int base = 0; base < items; base += NCT * MC) {
-    if (ph == PH_OPROJ) {
-      MergeRegs mr[MC];
-      int kk[MC], xs[MC], qq[MC];
-#pragma unroll
-      for (int c = 0; c < MC; ++c) {
-        const int it = base + tid + c * NCT;
-        kk[c] = -1; xs[c] = 0; qq[c] = 0;
-        if (it < items) {
-          const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
-          int kc = kc0 + i;
-          if (kc >= nkc) kc -= nkc;
-          const int k = kc * SK_K + c4 * 4;
-          xs[c] = (kc % XSLOTS) * SK_K + c4 * 4;
-          qq[c] = q;
-          const bool live = k < K && (q == 0 || (accel && sidx_of(k / P.dh) >= 0));
-          kk[c] = live ? k : -2;
-          if (live && P.ns <= MERGE_NS) merge_load(P, mr[c], q, k);
+  bar_consumers();
+  if (ph == PH_DOWN) {
+#pragma unroll 1
+    for (int it = tid; it < items; it += NCT) {
+      const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
+      int kc = kc0 + i;
+      if (kc >= nkc) kc -= nkc;
+      const int k = kc * SK_K + c4 * 4;
+      if (k < P.F && (q == 0 || accel)) cp_async16(stg + 4 * it, P.act + (size_t)q * P.F_pad + k);
+      else *(float4*)(stg + 4 * it) = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    cp_async_wait_all();
+    bar_consumers();
+#pragma unroll 1
+    for (int it = tid; it < items; it += NCT) {
+      const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
+      int kc = kc0 + i;
+      if (kc >= nkc) kc -= nkc;
+      const int xs = (kc % XSLOTS) * SK_K + c4 * 4;
+      const float4 v = *(const float4*)(stg + 4 * it);
+      if (q == 0) xstore4(c0, c1, xs, v); else xstore4(c2, c3, xs, v);
+    }
+  } else {
+    // heads touched by the two runs of chunks: [kc0, kcA) and, after the wrap, [0, kcB)
+    const int dh = P.dh, NS = P.ns, rec = NS * 2 * (dh + 4);   // floats of one head's partials
+    const int kcA = min(kc0 + cnt, nkc), kcB = kc0 + cnt - kcA;
+    const int hA0 = (kc0 * SK_K) / dh, hA1 = min(P.n_heads - 1, (kcA * SK_K - 1) / dh);
+    const int nA = hA1 - hA0 + 1, nB = kcB > 0 ? min(P.n_heads - 1, (kcB * SK_K - 1) / dh) + 1 : 0;
+    const bool staged = (size_t)(nA + nB) * rec * 4 <= (size_t)STG_BYTES;
+    if (staged) {
+      const float* srcA = P.apart + (size_t)hA0 * rec;
+#pragma unroll 1
+      for (int i = tid; i < ((nA * rec) >> 2); i += NCT) cp_async16(stg + 4 * i, srcA + 4 * i);
+#pragma unroll 1
+      for (int i = tid; i < ((nB * rec) >> 2); i += NCT) cp_async16(stg + nA * rec + 4 * i, P.apart + 4 * i);
+      cp_async_wait_all();
+      bar_consumers();
+    }
+#pragma unroll 1
+    for (int it = tid; it < items; it += NCT) {
+      const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
+      int kc = kc0 + i;
+      const bool wrapped = kc >= nkc;
+      if (wrapped) kc -= nkc;
+      const int k = kc * SK_K + c4 * 4;
+      const int xs = (kc % XSLOTS) * SK_K + c4 * 4;
+      float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (k < P.d && (q == 0 || (accel && sidx_of(k / dh) >= 0))) {
+        if (staged) {
+          const int head = k / dh, j = k - head * dh;
+          const float* pp = stg + (size_t)(wrapped ? nA + head : head - hA0) * rec + q * (dh + 4);
+          float M = -INFINITY, Lsum = 0.f;
+#pragma unroll 1
+          for (int sp = 0; sp < NS; ++sp) {
+            const float* ps = pp + sp * 2 * (dh + 4);
+            if (ps[dh + 1] > 0.f) M = fmaxf(M, ps[dh]);
+          }
+#pragma unroll 1
+          for (int sp = 0; sp < NS; ++sp) {
+            const float* ps = pp + sp * 2 * (dh + 4);
+            const float ls = ps[dh + 1];
+            if (ls > 0.f) {
+              const float wgt = __expf(ps[dh] - M);
+              const float4 v = *(const float4*)(ps + j);
+              Lsum += ls * wgt;
+              o.x += v.x * wgt; o.y += v.y * wgt; o.z += v.z * wgt; o.w += v.w * wgt;
+            }
+          }
+          const float inv = 1.f / Lsum;
+          o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+        } else {
+          o = merge_global(P, q, k);
         }
       }
-#pragma unroll
-      for (int c = 0; c < MC; ++c) {
-        if (kk[c] != -1) {
-          float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (kk[c] >= 0) o = merge_finish(P, mr[c], qq[c], kk[c]);
-          if (qq[c] == 0) xstore4(c0, c1, xs[c], o); else xstore4(c2, c3, xs[c], o);
-        }
-      }
-    } else {
-      float4 v[MC];
-      int xs[MC], qq[MC];
-#pragma unroll
-      for (int c = 0; c < MC; ++c) {
-        const int it = base + tid + c * NCT;
-        xs[c] = -1; qq[c] = 0;
-        v[c] = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (it < items) {
-          const int i = it >> 6, rem = it & 63, q = rem >> 5, c4 = rem & 31;
-          int kc = kc0 + i;
-          if (kc >= nkc) kc -= nkc;
-          const int k = kc * SK_K + c4 * 4;
-          xs[c] = (kc % XSLOTS) * SK_K + c4 * 4;
-          qq[c] = q;
-          if (k < K && (q == 0 || accel)) v[c] = ldcg4(P.act + (size_t)q * P.F_pad + k);
-        }
-      }
-#pragma unroll
-      for (int c = 0; c < MC; ++c) {
-        if (xs[c] >= 0) {
-          if (qq[c] == 0) xstore4(c0, c1, xs[c], v[c]); else xstore4(c2, c3, xs[c], v[c]);
-        }
-      }
+      if (q == 0) xstore4(c0, c1, xs, o); else xstore4(c2, c3, xs, o);
     }
   }
   bar_consumers();
@@ -578,7 +568,7 @@ __device__ __forceinline__ void publish_u(const FParams& P, const bf16* x, const
     acc = warp_sum(acc);
     if (lane == 0) {
       const u64 v = ((u64)us.epoch << 32) | (u64)__float_as_uint(acc);
-      asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(P.upart + (size_t)j * UPART_Q + ch), "l"(v) : "memory");
+      asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(P.upart + c), "l"(v) : "memory");   // entry index = j * q + ch = c
     }
   }
 }
@@ -596,7 +586,7 @@ __device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp,
       v[i] = 0.f;
       if (idx < total) {
         u64 e;
-        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(e) : "l"(P.upart + (size_t)(idx / us.q) * UPART_Q + idx % us.q) : "memory");
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(e) : "l"(P.upart + idx) : "memory");
         ok = ok && (unsigned int)(e >> 32) == us.epoch;
         v[i] = __uint_as_float((unsigned int)e);
       }
@@ -668,6 +658,25 @@ __device__ __forceinline__ float rv_dot(const RVec& v, const float* u, int r) {
 // split-K phases: u of the adapter from partials the PRODUCING phase left behind (one L2 round trip, no
 // publish / fetch): OPROJ  u = A_o o^ from the attention items' r-vectors and (m, l); DOWN  u = A_d a^ as
 // the sum of the CTAs' r-vectors in CTA order.
+__device__ __noinline__ float combine_slow(const FParams& P, int head, float (&part)[MAX_R]) {
+  const int NS = P.ns, dh = P.dh, r = P.r;
+  float M = -INFINITY, Lsum = 0.f;
+  for (int s = 0; s < NS; ++s) {
+    const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
+    if (ml.y > 0.f) M = fmaxf(M, ml.x);
+  }
+  for (int s = 0; s < NS; ++s) {
+    const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
+    if (ml.y > 0.f) {
+      const float wgt = __expf(ml.x - M);
+      Lsum += ml.y * wgt;
+      const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
+#pragma unroll
+      for (int i = 0; i < MAX_R; ++i) if (i < r) part[i] += ldcg(q + i) * wgt;
+    }
+  }
+  return Lsum;
+}
 __device__ __forceinline__ void combine_u(const FParams& P, float* u, int ph, int G) {
   const int lane = threadIdx.x & 31, r = P.r;
   float acc[MAX_R];
@@ -712,21 +721,7 @@ __device__ __forceinline__ void combine_u(const FParams& P, float* u, int ph, in
           }
         }
       } else {
-        float M = -INFINITY;
-        for (int s = 0; s < NS; ++s) {
-          const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
-          if (ml.y > 0.f) M = fmaxf(M, ml.x);
-        }
-        for (int s = 0; s < NS; ++s) {
-          const float2 ml = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
-          if (ml.y > 0.f) {
-            const float wgt = __expf(ml.x - M);
-            Lsum += ml.y * wgt;
-            const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
-#pragma unroll
-            for (int i = 0; i < MAX_R; ++i) if (i < r) part[i] += ldcg(q + i) * wgt;
-          }
-        }
+        Lsum = combine_slow(P, head, part);
       }
       const float inv = 1.f / Lsum;
 #pragma unroll
@@ -902,8 +897,8 @@ __device__ __forceinline__ void epilogue_tile(const FParams& P, const float* T, 
 // rolled loop; both queries share every K/V read.  The last split also takes the token's own key/value:
 // slow = K[pos], V[pos] as stored (rounded), accelerated = k^, v^ from scratch (p_t attends
 // h_<t (+) p_t).  Partials (m, l, o) go to P.apart; the O-proj loader merges them.
-constexpr int KV_BYTES = X_BYTES + RED_FLOATS * 4;   // staging area: the x columns and the parked sums are dead here
-__device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, float* osm, u64* abar, unsigned int& aphase,
+constexpr int KV_BYTES = X_BYTES + RED_FLOATS * 4 + KV_EXTRA;   // staging area: the x columns and the parked sums are dead here
+__device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, float* osm, float* wsm, u64* abar, unsigned int& aphase,
                                         const FLayer* L, int pos, bool accel, int G) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int dh = P.dh, d = P.d, lpp = dh >> 3, NS = P.ns;
@@ -966,8 +961,10 @@ __device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, 
           bulk_g2s_plain(vs, Vg + (size_t)r0 * dh, (uint32_t)(n * dh * 2), abar);
         }
       }
+      TL(73);
       mbar_wait(abar, aphase & 1u, P.ctl, 0x300u);
       ++aphase;
+      TL(74);
 #pragma unroll 1
       for (int ub = warp * 2; ub < n; ub += 2 * NCW) {   // warp-uniform trip count (full-mask shuffles below)
         const int u = ub + seg;
@@ -1052,28 +1049,30 @@ __device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, 
       if (sl == 0) { dst0[dh] = m0; dst0[dh + 1] = l0; dst1[dh] = m1; dst1[dh + 1] = l1; }
     }
     bar_consumers();
+    if (warp == 0) {
+      // weights of the 16 half-warp partials of each query: lane = (segment, query)
+      const int s_ = lane >> 1, q_ = lane & 1;
+      const float* src = red + ((size_t)s_ * 2 + q_) * (dh + 2);
+      const float ms = src[dh], ls = src[dh + 1];
+      float M = ls > 0.f ? ms : -INFINITY;
+#pragma unroll
+      for (int o = 2; o < 32; o <<= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+      const float wgt = ls > 0.f ? __expf(ms - M) : 0.f;
+      float Lsum = ls * wgt;
+#pragma unroll
+      for (int o = 2; o < 32; o <<= 1) Lsum += __shfl_xor_sync(0xffffffffu, Lsum, o);
+      wsm[lane] = wgt;
+      if (s_ == 0) { wsm[32 + q_] = M; wsm[34 + q_] = Lsum; }
+    }
+    bar_consumers();
     for (int i = tid; i < 2 * dh; i += NCT) {
       const int q = i / dh, j = i - q * dh;
-      float M = -INFINITY;
-#pragma unroll 1
-      for (int s = 0; s < 2 * NCW; ++s) {
-        const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
-        if (src[dh + 1] > 0.f) M = fmaxf(M, src[dh]);
-      }
-      float Lsum = 0.f, O = 0.f;
-#pragma unroll 1
-      for (int s = 0; s < 2 * NCW; ++s) {
-        const float* src = red + ((size_t)s * 2 + q) * (dh + 2);
-        float ls = src[dh + 1];
-        if (ls > 0.f) {
-          float wgt = __expf(src[dh] - M);
-          Lsum += ls * wgt;
-          O += src[j] * wgt;
-        }
-      }
+      float O = 0.f;
+#pragma unroll
+      for (int s = 0; s < 2 * NCW; ++s) O += red[((size_t)s * 2 + q) * (dh + 2) + j] * wsm[s * 2 + q];
       float* pp = P.apart + ((size_t)(head * NS + sp) * 2 + q) * (dh + 4);
       __stcg(pp + j, O);
-      if (j == 0) { __stcg(pp + dh, M); __stcg(pp + dh + 1, Lsum); }
+      if (j == 0) { __stcg(pp + dh, wsm[32 + q]); __stcg(pp + dh + 1, wsm[34 + q]); }
       if (q == 1) osm[j] = O;
     }
     bar_consumers();
@@ -1122,26 +1121,37 @@ __device__ __forceinline__ bool exit_phase_after(const FParams& P, int layer) {
 // geometry of a weight phase: stages S = U * gran; the CTA's stage range [s0, s1)
 struct PhaseGeo {
   const unsigned char* W;
-  int n_units, gran, nkc;    // nkc: k-chunks per row-tile group (split-K) / k-stages per row-tile (row-owned)
+  int nkc;                   // k-chunks per row-tile group (split-K) / k-stages per row-tile (row-owned)
   bool split;
   int s0, s1;
 };
+// The CTA's stage range of every phase TYPE is the same in every layer: computed once per launch into
+// shared memory (thread p < N_PH) so that a phase's set-up is four shared loads, not a page of integer code.
+__device__ __forceinline__ void geo_init(const FParams& P, int ph, int G) {
+  const int nks_d = P.d_pad / STAGE_K;
+  int n_units, gran, nkc, split = 0;
+  switch (ph) {
+    case PH_QKV:    n_units = P.rt_qkv; gran = nks_d; nkc = nks_d; break;
+    case PH_OPROJ:  nkc = (P.d + SK_K - 1) / SK_K; n_units = P.ng_d * nkc; gran = 1; split = 1; break;
+    case PH_GATEUP: n_units = P.rt_gu; gran = nks_d; nkc = nks_d; break;
+    case PH_DOWN:   nkc = P.F_pad / SK_K; n_units = P.ng_d * nkc; gran = 1; split = 1; break;
+    default:        n_units = P.rt_v; gran = nks_d; nkc = nks_d; break;   // PH_HEAD, PH_EXIT
+  }
+  // rotate the owner of the short ranges between phase types
+  const int v = ((int)blockIdx.x + ph * 29) % G;
+  int4 e;
+  e.x = range_lo(n_units, v, G) * gran;
+  e.y = range_lo(n_units, v + 1, G) * gran;
+  e.z = nkc;
+  e.w = split;
+  ((int4*)(smem_raw + OFF_GEO))[ph] = e;
+}
 __device__ __forceinline__ void phase_geo(const FParams& P, int layer, int ph, int G, PhaseGeo& g) {
   const int n = P.n_layers_run;
   const FLayer* L = lay(layer < n ? layer : 0);
-  const int nks_d = P.d_pad / STAGE_K;
-  int rot_layer = layer;
-  switch (ph) {
-    case PH_QKV:    g.W = (const unsigned char*)L->Wqkv; g.n_units = P.rt_qkv; g.gran = nks_d; g.nkc = nks_d; g.split = false; break;
-    case PH_OPROJ:  g.W = (const unsigned char*)L->Wo;   g.nkc = (P.d + SK_K - 1) / SK_K; g.n_units = P.ng_d * g.nkc; g.gran = 1; g.split = true; break;
-    case PH_GATEUP: g.W = (const unsigned char*)L->Wgu;  g.n_units = P.rt_gu;  g.gran = nks_d; g.nkc = nks_d; g.split = false; break;
-    case PH_DOWN:   g.W = (const unsigned char*)L->Wd;   g.nkc = P.F_pad / SK_K; g.n_units = P.ng_d * g.nkc; g.gran = 1; g.split = true; break;
-    case PH_EXIT:   g.W = (const unsigned char*)P.Wlm;   g.n_units = P.rt_v;   g.gran = nks_d; g.nkc = nks_d; g.split = false; rot_layer = L->gate - 1; break;
-    default:        g.W = (const unsigned char*)P.Wlm;   g.n_units = P.rt_v;   g.gran = nks_d; g.nkc = nks_d; g.split = false; rot_layer = n; break;
-  }
-  const int v = ((int)blockIdx.x + phase_rot(rot_layer, ph, G)) % G;
-  g.s0 = range_lo(g.n_units, v, G) * g.gran;
-  g.s1 = range_lo(g.n_units, v + 1, G) * g.gran;
+  const int4 e = ((const int4*)(smem_raw + OFF_GEO))[ph];
+  g.s0 = e.x; g.s1 = e.y; g.nkc = e.z; g.split = e.w != 0;
+  g.W = (const unsigned char*)(ph == PH_QKV ? L->Wqkv : ph == PH_OPROJ ? L->Wo : ph == PH_GATEUP ? L->Wgu : ph == PH_DOWN ? L->Wd : P.Wlm);
 }
 // next weight phase after (layer, ph); ph = -1 before the first.  false at the end of the pass.
 __device__ __forceinline__ bool next_weight_phase(const FParams& P, int& layer, int& ph) {
@@ -1208,10 +1218,10 @@ __device__ __noinline__ void prefetch_kv(const FParams& P, int layer, int G) {
 
 // L2 prefetch of what the consumers will read with plain loads on their critical path: the layer's
 // norm gains and adapter tensors (each CTA one slice: together the whole range), the RoPE row.
-__device__ __forceinline__ void prefetch_slice(const void* base, size_t bytes, int G) {
-  const size_t per = (((bytes + G - 1) / G) + 15) & ~(size_t)15;
-  const size_t o = (size_t)blockIdx.x * per;
-  if (o < bytes) bulk_prefetch_l2((const unsigned char*)base + o, (uint32_t)min(per, ((bytes - o) + 15) & ~(size_t)15));
+__device__ __forceinline__ void prefetch_slice(const void* base, unsigned int bytes, int G) {
+  const unsigned int per = (((bytes + (unsigned)G - 1u) / (unsigned)G) + 15u) & ~15u;
+  const unsigned int o = blockIdx.x * per;
+  if (o < bytes) bulk_prefetch_l2((const unsigned char*)base + o, min(per, ((bytes - o) + 15u) & ~15u));
 }
 __device__ __noinline__ void prefetch_params(const FParams& P, int layer, int G) {
   const FLayer* L = lay(layer);
@@ -1224,10 +1234,10 @@ __device__ __noinline__ void prefetch_params(const FParams& P, int layer, int G)
     }
   }
   if (L->accel && L->ad_bytes) prefetch_slice(L->ad_lo, L->ad_bytes, G);
-  if (L->accel && L->AdT) { prefetch_slice(L->AdT, (size_t)P.F * P.r * 2, G); prefetch_slice(L->AoT, (size_t)P.da * P.r * 2, G); }
+  if (L->accel && L->AdT) { prefetch_slice(L->AdT, (unsigned)(P.F * P.r * 2), G); prefetch_slice(L->AoT, (unsigned)(P.da * P.r * 2), G); }
   if (layer == 0 && P.lmA && (P.head_stream == 1 || P.exit_heads)) {
-    prefetch_slice(P.lmA, (size_t)P.r * P.d * 2, G);
-    prefetch_slice(P.lmB, (size_t)P.V * P.r * 2, G);
+    prefetch_slice(P.lmA, (unsigned)(P.r * P.d * 2), G);
+    prefetch_slice(P.lmB, (unsigned)(P.V * P.r * 2), G);
   }
 }
 
@@ -1272,6 +1282,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     *(int*)(smem_raw + OFF_TLN) = 0;
   }
+  if (tid < N_PH) geo_init(P, tid, G);
   for (int i = tid; i < P.n_heads; i += NTHREADS) ((int*)(smem_raw + OFF_SIDX))[i] = P.sidx[i];
   {
     const int words = P.n_layers_run * (int)(sizeof(FLayer) / 4);
@@ -1349,7 +1360,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
     const bool accel = ph == PH_HEAD || ph == PH_EXIT ? true : L->accel != 0;
     if (ph == PH_OPROJ) {
       // ---- a4: attention (its own phase between QKV and OPROJ; no weights)
-      attn_phase(P, (unsigned char*)x, utmp, abar, aphase, L, pos, accel, G);
+      attn_phase(P, (unsigned char*)x, utmp, sred, abar, aphase, L, pos, accel, G);
       TL(13);
       grid_sync(P.ctl, P.bar_base, nbar, G);
       TL(14);
