@@ -55,7 +55,7 @@ constexpr int SK_RT = 8;                       // row-tiles per split-K stage
 constexpr int NSTAGE = 4;
 constexpr int NCW = 8;                 // consumer warps
 constexpr int NCT = NCW * 32;          // consumer threads
-constexpr int NTHREADS = NCT + 64;     // + producer warp + auxiliary warp
+constexpr int NTHREADS = NCT + 96;     // + producer warp + auxiliary warp + L2 prefetch warp
 constexpr int TPW = STAGE_TILES / NCW; // tiles per warp per stage (8)
 constexpr int XMAX = 4096;             // inputs held in shared memory (d_pad limit; 32 split-K chunks)
 constexpr int XSLOTS = XMAX / SK_K;
@@ -67,6 +67,7 @@ constexpr int RED_FLOATS = FB * NCW * 32;
 constexpr int MAX_R = 8;               // adapter rank limit (PAPER.md L399 uses 8); larger ranks take the per-operation kernels
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
+constexpr int PF_DEFAULT = 6;           // L2 prefetch window of the prefetch warp, in stages (M2R2_PF overrides; 0 = off)
 constexpr int MERGE_NS = 4;            // attention splits combined from registers by the auxiliary warp; more take a looped path
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
 
@@ -122,6 +123,7 @@ struct FParams {
   float ls_beta;
   int ns;        // attention splits
   int pos_host;  // kv_len + joff as the host knows it (producer-side KV prefetch only)
+  int pf_ahead;  // L2 prefetch window in stages beyond the producer's cursor (0 = prefetch warp idle)
   u64* tl;       // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
 };
 
@@ -140,7 +142,8 @@ constexpr int OFF_SIDX = OFF_UD + NCW * MAX_R * 4;    // [M2R2_MAX_HEADS] ints: 
 constexpr int MAXL_S = 64;                            // layers whose descriptors are cached in shared memory
 constexpr int OFF_LAYERS = OFF_SIDX + M2R2_MAX_HEADS * 4;   // [MAXL_S] FLayer
 constexpr int OFF_GEO = OFF_LAYERS + MAXL_S * (int)sizeof(FLayer);   // [N_PH] int4 {s0, s1, nkc, split}: this CTA's stage range per phase type
-constexpr int OFF_TLN = OFF_GEO + 8 * 16;             // debug timeline cursor
+constexpr int OFF_PCTR = OFF_GEO + 8 * 16;            // stages the producer has issued into the ring (read by the prefetch warp)
+constexpr int OFF_TLN = OFF_PCTR + 16;                // debug timeline cursor
 constexpr int SMEM_BYTES = OFF_TLN + 64;
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory budget");
 extern __shared__ __align__(1024) unsigned char smem_raw[];
@@ -1281,6 +1284,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
     mbar_init(abar, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     *(int*)(smem_raw + OFF_TLN) = 0;
+    *(unsigned int*)(smem_raw + OFF_PCTR) = 0u;
   }
   if (tid < N_PH) geo_init(P, tid, G);
   for (int i = tid; i < P.n_heads; i += NTHREADS) ((int*)(smem_raw + OFF_SIDX))[i] = P.sidx[i];
@@ -1293,6 +1297,32 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
   __syncthreads();
   const int n_run = P.n_layers_run;
 
+  if (tid >= NCT + 64) {
+    // ================= L2 prefetch warp: walks the CTA's stage sequence a window ahead of the producer and touches
+    // every 128-byte line with prefetch.global.L2 (requests without return data through the LSU, not the bulk
+    // copy unit), so HBM keeps streaming into L2 while the ring is full and the consumers sit in a gap
+    const int W = P.pf_ahead, lane = tid & 31;
+    if (W <= 0) return;
+    volatile unsigned int* pctr = (volatile unsigned int*)(smem_raw + OFF_PCTR);
+    Cursor pf;
+    pf.layer = 0; pf.ph = -1; pf.s = pf.s1 = 0; pf.W = nullptr; pf.new_layer = false;
+    const unsigned char* a;
+    unsigned int n = 0;
+    while (cursor_get(P, pf, G, a)) {
+      unsigned int spins = 0;
+      while ((int)(n - *pctr) >= W) {
+        __nanosleep(100);
+        if ((++spins & 1023u) == 0u && aborted(P.ctl)) break;
+      }
+      if ((int)(n - *pctr) >= 0) {   // still ahead of the producer: worth fetching
+#pragma unroll
+        for (int i = 0; i < STAGE_BYTES / 128 / 32; ++i)
+          asm volatile("prefetch.global.L2 [%0];" ::"l"(a + (size_t)(lane + 32 * i) * 128));
+      }
+      ++n;
+    }
+    return;
+  }
   if (tid >= NCT + 32) {
     // ================= auxiliary warp: adapter down-projections (u = A x^) of every phase that has one
     UState us;
@@ -1338,6 +1368,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
         }
         const unsigned int slot = ctr % NSTAGE, use = ctr / NSTAGE;
         ++ctr;
+        *(volatile unsigned int*)(smem_raw + OFF_PCTR) = ctr;
         mbar_wait(&empty[slot], (use & 1u) ^ 1u, P.ctl, 0x400u + ld.ph);
         mbar_expect_tx(&full[slot], STAGE_BYTES);
         bulk_g2s(ring + (size_t)slot * STAGE_BYTES, a, STAGE_BYTES, &full[slot], pol);
@@ -1824,6 +1855,7 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   p.apart = im->apart; p.upart = im->upart; p.apu = im->apu; p.udpart = im->udpart;
   p.nah = c.accel_enabled ? c.n_accel_heads : 0;
   p.ctl = im->d_ctl;
+  p.pf_ahead = getenv("M2R2_PF") ? atoi(getenv("M2R2_PF")) : PF_DEFAULT;
   p.tl = nullptr;
 #ifdef M2R2_FUSED_DEBUG
   if (getenv("M2R2_TL_OUT") && !im->d_tl) cudaMalloc((void**)&im->d_tl, sizeof(u64) * TL_MAX * im->G);
