@@ -37,6 +37,9 @@ import numpy as np  # noqa: E402
 METRIC = "decode tokens/s at batch 1 (M2R2 dual-stream decode, 3.8B-class bf16)"
 PROMPT = 512
 HBM_NOMINAL_GBS = 8000.0      # BASELINE.json: "achieved HBM GB/s vs 8 TB/s"
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of m2r2_fused_decode_kernel (one decode step at
+# kv_len ~ 521) from the committed capture profiles/r1_v32_fused_kernel.md (ncu --set full): 7.691 GB + 21.1 MB
+FUSED_TRAFFIC_BYTES = 7.690756e9 + 21.115392e6
 
 
 def measured_peaks():
@@ -291,7 +294,9 @@ def run_ours(args, rk):
     roofline = {"bound": "hbm", "kernel": kernel_names.get(dom, dom), "class": dom,
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
-                "traffic": args.traffic, "step": {"achieved": step_gbs, "frac": step_gbs / peak,
+                "traffic": args.traffic if dom == "fused_step" else None,
+                "traffic_source": "profiles/r1_v32_fused_kernel.md (ncu --set full, one launch)" if dom == "fused_step" else None,
+                "step": {"achieved": step_gbs, "frac": step_gbs / peak,
                                                   "frac_of_nominal_8TBs": step_gbs / HBM_NOMINAL_GBS,
                                                   "algorithmic_bytes_per_step": tot_bytes / K},
                 "per_class": per_class}
@@ -344,7 +349,7 @@ def main():
     ap.add_argument("--exit-heads", type=int, default=0, help="evaluate the exit argmax at every gate (SURVEY Q15 second row)")
     ap.add_argument("--no-fused", action="store_true", help="force the per-operation kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None,
+    ap.add_argument("--traffic", type=float, default=FUSED_TRAFFIC_BYTES,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")
     args = ap.parse_args()
     from paper_2502_02040_b200 import replicas
