@@ -340,6 +340,110 @@ def run_ours(args, rk):
     return 0
 
 
+# ---------------------------------------------------------------------------------------------
+# secondary workloads (BASELINE.json configs[2..4]); not the driver's bench line: `--workload c3|c4|c5`
+# ---------------------------------------------------------------------------------------------
+def run_secondary(args):
+    """C3 self-spec (gamma x alpha), C4 batch-8 long-KV self-spec, C5 MoE expert loading policies.
+    Wall-clock around synchronised library calls (each call returns host results, so it is the e2e number)."""
+    import torch
+    import m2r2_synth as S
+    import paper_2502_02040_b200 as M
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
+    out = {"workload": args.workload, "data": "synthetic", "n_gpus": 1, "runs": []}
+    if args.workload == "c3":
+        cfg = S.config_c3()
+        eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
+        prompt = S.gen_prompt(cfg, PROMPT)
+        for alpha in (0.9, 0.5):
+            for gamma in (2, 4, 6):
+                f, g = S.gen_logit_script(cfg, 400, alpha)
+                eng.set_logit_script(f, g, PROMPT)
+                eng.prefill(prompt)
+                for _ in range(3):
+                    eng.spec_step(gamma)
+                eng.prefill(prompt)
+                torch.cuda.synchronize()
+                t0, emitted, steps, by = time.perf_counter(), 1, 0, 0
+                while emitted < 256:
+                    _, n = eng.spec_step(gamma)
+                    emitted += int(n[0])
+                    steps += 1
+                    by += eng.get_stats()["algorithmic_bytes_last"]
+                torch.cuda.synchronize()
+                dt = time.perf_counter() - t0
+                out["runs"].append({"alpha": alpha, "gamma": gamma, "tokens": emitted - 1, "spec_steps": steps,
+                                    "ms_per_spec_step": 1e3 * dt / steps, "tokens_per_s": (emitted - 1) / dt,
+                                    "tokens_per_spec_step": (emitted - 1) / steps, "algorithmic_GB_per_s": by / dt / 1e9})
+        eng.set_logit_script(None, None, PROMPT)
+        eng.prefill(prompt)
+        for _ in range(3):
+            eng.decode_step()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(128):
+            eng.decode_step()
+        torch.cuda.synchronize()
+        out["plain_decode_control_tokens_per_s"] = 128 / (time.perf_counter() - t0)
+        eng.close()
+    elif args.workload == "c4":
+        cfg = S.config_c4()
+        B, P, gamma = 8, 4096, 4
+        eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
+        prompts = np.stack([S.gen_prompt(cfg, P, seq=b) for b in range(B)])
+        for alpha in (0.9, 0.5):
+            scripts = [S.gen_logit_script(cfg, 1000, alpha, seq=b) for b in range(B)]
+            eng.set_logit_script(np.stack([x[0] for x in scripts]), np.stack([x[1] for x in scripts]), P)
+            eng.prefill(prompts)
+            for _ in range(2):
+                eng.spec_step(gamma)
+            torch.cuda.synchronize()
+            t0, emitted, by = time.perf_counter(), 0, 0
+            for _ in range(128):
+                _, n = eng.spec_step(gamma)
+                emitted += int(n.sum())
+                by += eng.get_stats()["algorithmic_bytes_last"]
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            out["runs"].append({"alpha": alpha, "gamma": gamma, "batch": B, "kv_len_start": P, "spec_steps": 128,
+                                "ms_per_spec_step": 1e3 * dt / 128, "aggregate_tokens_per_s": emitted / dt,
+                                "algorithmic_GB_per_s": by / dt / 1e9, "kv_len_end": list(eng.get_stats()["kv_len"][:B])})
+        eng.close()
+    else:
+        cfg = S.config_c5()
+        P = 256
+        eng = M.Engine(cfg, device="cuda:0")
+        W = S.gen_weights(cfg, expert_alloc=eng.pinned_expert_alloc())   # expert store in pinned host memory
+        eng.load_weights(W)
+        prompt = S.gen_prompt(cfg, P)
+        act, pred = S.gen_router_script(cfg, P + 300, 0.25, 0.9)
+        for pol, name in ((M.POLICY_FIXED, "on-demand"), (M.POLICY_LRU, "LRU"), (M.POLICY_LRU_AOT, "LRU+AoT")):
+            eng.set_policy(pol)
+            eng.set_router_script(act, pred, 0)
+            eng.prefill(prompt)
+            for _ in range(4):
+                eng.decode_step()
+            s0 = eng.get_stats()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(256):
+                eng.decode_step()
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            s1 = eng.get_stats()
+            hits, miss = s1["expert_hits"] - s0["expert_hits"], s1["expert_misses"] - s0["expert_misses"]
+            h2d = s1["h2d_bytes"] - s0["h2d_bytes"]
+            out["runs"].append({"policy": name, "router_script": {"rho": 0.25, "pi": 0.9}, "steps": 256,
+                                "ms_per_step": 1e3 * dt / 256, "tokens_per_s": 256 / dt, "hit_rate": hits / max(1, hits + miss),
+                                "prefetched": s1["expert_prefetched"] - s0["expert_prefetched"],
+                                "on_demand": s1["expert_on_demand"] - s0["expert_on_demand"],
+                                "h2d_GB": h2d / 1e9, "h2d_GB_per_s": h2d / 1e9 / dt})
+        eng.close()
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -348,10 +452,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--exit-heads", type=int, default=0, help="evaluate the exit argmax at every gate (SURVEY Q15 second row)")
     ap.add_argument("--no-fused", action="store_true", help="force the per-operation kernels")
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"],
+                    help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=FUSED_TRAFFIC_BYTES,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")
     args = ap.parse_args()
+    if args.workload != "c2":
+        sys.exit(run_secondary(args))
     from paper_2502_02040_b200 import replicas
     rk = replicas.init_from_env(backend="gloo" if args.impl == "reference" else None)
     if args.gpus != rk.world and rk.world > 1:
