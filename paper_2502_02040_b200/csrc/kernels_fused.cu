@@ -1638,6 +1638,100 @@ __global__ void pack_kernel(uint4* __restrict__ dst, const bf16* __restrict__ sr
   }
 }
 
+// ------------------------------------------------------------------ skinny GEMM on the fragment-major weights (a11)
+// The k-token verify pass (and prefill chunks) multiplies each weight matrix with m <= 8 slow-stream rows.
+// Same fragment-major tiles as the fused kernel, weights as the M operand and the token rows as N: one
+// LDG.128 per lane per tile straight into the A fragment, the rows' bf16 hi + lo parts as two B operands
+// (fp32-class products, as in the fused kernel), fp32 accumulation on the tensor pipe.  One CTA per 16-row
+// tile, its 8 warps split the k-tiles and keep 8 tiles (4 KB per warp) in flight.  HBM-bound: 2 m flop per byte.
+enum { VK_QKV = 0, VK_OPROJ = 1, VK_GATEUP = 2, VK_DOWN = 3, VK_HEAD = 4 };
+struct VArgs {
+  const uint4* W;
+  const float* X;        // [rows][ldx] fp32
+  float* out;            // [rows][ldo]
+  const float* resid;    // O / DOWN: out = resid + W x
+  float* trace;          // DOWN: second copy of out, or nullptr
+  int ldx, ldo, rows, K, n_out, nkt, nstage_k, split, d, dh;
+};
+__device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  const float2 f = __bfloat1622float2(h);
+  const __nv_bfloat162 l = __floats2bfloat162_rn(a - f.x, b - f.y);
+  lo = bf2_u32(l);
+  return bf2_u32(h);
+}
+template <int KIND>
+__global__ void __launch_bounds__(256) gemv_mma_kernel(const VArgs a) {
+  __shared__ float red[8][16][8];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int rt = blockIdx.x;
+  float c[4] = {0.f, 0.f, 0.f, 0.f};
+  const float* xrow = a.X + (size_t)g * a.ldx;
+  const bool row_live = g < a.rows;
+  constexpr int UN = 8;
+  for (int kt0 = warp; kt0 < a.nkt; kt0 += 8 * UN) {
+    uint4 w[UN];
+    float2 x0[UN], x1[UN];
+#pragma unroll
+    for (int u = 0; u < UN; ++u) {
+      const int kt = kt0 + 8 * u;
+      w[u] = make_uint4(0u, 0u, 0u, 0u);
+      x0[u] = make_float2(0.f, 0.f);
+      x1[u] = x0[u];
+      if (kt < a.nkt) {
+        const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
+                                    : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
+        w[u] = ldg_stream(a.W + tile * 32 + lane);
+        const int k = kt * 16 + 2 * t;
+        if (row_live && k < a.K) x0[u] = __ldg((const float2*)(xrow + k));
+        if (row_live && k + 8 < a.K) x1[u] = __ldg((const float2*)(xrow + k + 8));
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < UN; ++u) {
+      uint32_t l0, l1;
+      const uint32_t h0 = pack_hi_lo(x0[u].x, x0[u].y, l0), h1 = pack_hi_lo(x1[u].x, x1[u].y, l1);
+      mma_bf16(c, w[u], h0, h1);
+      mma_bf16(c, w[u], l0, l1);
+    }
+  }
+  red[warp][g][2 * t] = c[0]; red[warp][g][2 * t + 1] = c[1];
+  red[warp][g + 8][2 * t] = c[2]; red[warp][g + 8][2 * t + 1] = c[3];
+  __syncthreads();
+  if (tid < 128) {
+    const int r = tid >> 3, n = tid & 7;
+    if (n < a.rows) {
+      float v = 0.f;
+#pragma unroll
+      for (int w8 = 0; w8 < 8; ++w8) v += red[w8][r][n];
+      const int pr = rt * 16 + r;
+      if (KIND == VK_QKV) {
+        if (pr < a.n_out) {
+          const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
+          const int nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
+          a.out[(size_t)n * a.ldo + nat] = v;
+        }
+      } else if (KIND == VK_GATEUP) {
+        if (r < 8) {
+          float up = 0.f;
+#pragma unroll
+          for (int w8 = 0; w8 < 8; ++w8) up += red[w8][r + 8][n];
+          const int o = rt * 8 + r;
+          if (o < a.n_out) a.out[(size_t)n * a.ldo + o] = silu(v) * up;
+        }
+      } else if (KIND == VK_HEAD) {
+        if (pr < a.n_out) a.out[(size_t)n * a.ldo + pr] = v;
+      } else {
+        if (pr < a.n_out) {
+          const float o = a.resid[(size_t)n * a.ldo + pr] + v;
+          a.out[(size_t)n * a.ldo + pr] = o;
+          if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
+        }
+      }
+    }
+  }
+}
+
 }  // namespace
 
 // ==================================================================================== host side
@@ -1651,6 +1745,8 @@ struct FusedImpl {
   Ctl* h_ctl = nullptr;       // pinned
   bool bound = false;
   u64* d_tl = nullptr;        // debug timeline (M2R2_FUSED_DEBUG builds)
+  std::vector<FLayer> h_layers;   // host copy of the layer descriptors (packed weight pointers)
+  const uint4* h_Wlm = nullptr;
   std::vector<int> gate_of;   // per layer: 1 + gate index, or 0
   std::vector<int> accel_of;
   // scratch carve
@@ -1825,6 +1921,8 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     if (cudaGetLastError() != cudaSuccess) return M2R2_CUDA;
   }
   if (cudaMemcpyAsync(im->d_layers, hl.data(), sizeof(FLayer) * c.n_layers, cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
+  im->h_layers = hl;
+  im->h_Wlm = Wlm;
   std::vector<int> sidx(c.n_heads, -1), cols(std::max(8, c.n_accel_heads * dh), 0);
   if (c.accel_enabled)
     for (int s = 0; s < c.n_accel_heads; ++s) {
@@ -1931,4 +2029,34 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
     return M2R2_CUDA;
   }
   return 0;
+}
+
+// a11 on the fragment-major weights: out = f(W x) for rows <= 8 slow-stream rows (kinds: VK_*).  Returns
+// M2R2_UNSUPPORTED when the fused copy is not bound (the caller then uses the row-major kernels).
+int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
+                    int rows, float* out, int ldo, const float* resid, float* trace) {
+  if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 8) return M2R2_UNSUPPORTED;
+  FusedImpl* im = fs->impl;
+  PackedDims q = packed_dims(c);
+  VArgs a;
+  memset(&a, 0, sizeof(a));
+  a.X = X; a.ldx = ldx; a.rows = rows; a.out = out; a.ldo = ldo; a.resid = resid; a.trace = trace;
+  a.d = c.d_model; a.dh = c.head_dim;
+  int n_rt = 0;
+  const FLayer* L = kind == VK_HEAD ? nullptr : &im->h_layers[layer];
+  switch (kind) {
+    case VK_QKV:    a.W = L->Wqkv; a.K = c.d_model; a.n_out = 3 * c.d_model; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_qkv; break;
+    case VK_OPROJ:  a.W = L->Wo;   a.K = c.d_model; a.n_out = c.d_model; a.nkt = q.nkc_o * 8; a.nstage_k = q.nkc_o; a.split = 1; n_rt = q.ng_d * SK_RT; break;
+    case VK_GATEUP: a.W = L->Wgu;  a.K = c.d_model; a.n_out = c.d_ff; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_gu; break;
+    case VK_DOWN:   a.W = L->Wd;   a.K = c.d_ff; a.n_out = c.d_model; a.nkt = q.nkc_d * 8; a.nstage_k = q.nkc_d; a.split = 1; n_rt = q.ng_d * SK_RT; break;
+    default:        a.W = im->h_Wlm; a.K = c.d_model; a.n_out = c.vocab; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_v; break;
+  }
+  switch (kind) {
+    case VK_QKV:    gemv_mma_kernel<VK_QKV><<<n_rt, 256, 0, st>>>(a); break;
+    case VK_OPROJ:  gemv_mma_kernel<VK_OPROJ><<<n_rt, 256, 0, st>>>(a); break;
+    case VK_GATEUP: gemv_mma_kernel<VK_GATEUP><<<n_rt, 256, 0, st>>>(a); break;
+    case VK_DOWN:   gemv_mma_kernel<VK_DOWN><<<n_rt, 256, 0, st>>>(a); break;
+    default:        gemv_mma_kernel<VK_HEAD><<<n_rt, 256, 0, st>>>(a); break;
+  }
+  return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }

@@ -43,3 +43,8 @@ int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const Fused
               float ls_beta, int64_t* launches);
 // 0 if the last launches completed normally; otherwise a description (device-side timeout)
 int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n);
+// a11: skinny GEMM of <= 8 slow-stream rows on the fragment-major weights (verify pass, prefill chunks).
+// kind: 0 QKV (natural row order out), 1 O-proj (+resid), 2 gate/up + SwiGLU, 3 down (+resid, trace), 4 LM head.
+// Returns M2R2_UNSUPPORTED when the fused weight copy is not bound or rows > 8.
+int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
+                    int rows, float* out, int ldo, const float* resid, float* trace);
