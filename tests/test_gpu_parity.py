@@ -229,6 +229,42 @@ def test_spec_step_zero_equals_decode_step_on_gpu():
     b.close()
 
 
+@pytest.mark.parametrize("gamma", [1, 4, 7])
+def test_verify_rows_on_tensor_cores_match_row_major_kernels(gamma):
+    """a11: the skinny tensor-core GEMM on the fragment-major weights (<= 8 rows; verify pass and prefill
+    chunks) against the row-major fp32-FMA kernels of the same library: prefill + verify logits of every row,
+    accepted tokens and K/V after rollback (ragged d_ff 1000, vocab 3001, head_dim 96).  Both implementations
+    are held to the oracle by the other tests; here they are held to each other.  The bound is not fp32
+    rounding: products with bf16 hi + lo operands differ from fp32 FMAs by ~1e-6, which flips the bf16
+    rounding of about one K/V element in a thousand (measured 1.2e-4 rel-L2 on the layer-0 cache, 1.4e-3 on
+    layer 5, 3.8e-4 on the logits).  Tokens are forced by the logit script so that a near-tie cannot
+    desynchronise the two engines."""
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2, lm_head_adapter=True)
+    W = S.gen_weights(cfg)
+    a, b = M.Engine(cfg, W), M.Engine(cfg, W)
+    b.set_fused(False)          # per-operation kernels everywhere, row-major weights
+    P = 29
+    f, g = S.gen_logit_script(cfg, 120, 0.7)
+    a.set_logit_script(f, g, P)
+    b.set_logit_script(f, g, P)
+    prompt = S.gen_prompt(cfg, P)
+    assert int(a.prefill(prompt)[0]) == int(b.prefill(prompt)[0]) == f[0]
+    assert rel_l2(a.debug_read(M.DBG_LOGITS, (P - 1) % 8), b.debug_read(M.DBG_LOGITS, (P - 1) % 8)) <= 2e-3
+    for _ in range(4):
+        acc_a, n_a = a.spec_step(gamma)
+        acc_b, n_b = b.spec_step(gamma)
+        assert n_a[0] == n_b[0] and acc_a[0][:n_a[0]].tolist() == acc_b[0][:n_b[0]].tolist()
+        for j in range(gamma + 1):
+            assert rel_l2(a.debug_read(M.DBG_LOGITS, j), b.debug_read(M.DBG_LOGITS, j)) <= 2e-3, j
+    T = a.get_stats()["kv_len"][0]
+    assert T == b.get_stats()["kv_len"][0]
+    for i in range(cfg.n_layers):
+        assert rel_l2(a.kcache(i, T), b.kcache(i, T)) <= 5e-3
+        assert rel_l2(a.kcache(i, T, v=True), b.kcache(i, T, v=True)) <= 5e-3
+    a.close()
+    b.close()
+
+
 # ------------------------------------------------------------------ batch (C4 structure, reduced)
 def test_batched_selfspec_per_sequence_divergence():
     """B=3 sequences, per-sequence scripts => per-sequence accepted lengths and kv_len diverge; each
