@@ -10,6 +10,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <map>
 #include <vector>
 
 #include "m2r2_internal.cuh"
@@ -112,6 +113,11 @@ struct m2r2_ctx {
   float *resid, *xn, *U, *qkv, *attn_o, *act, *part_o, *part_ml, *logits, *exit_logits, *trace;
   float *moe_tmp, *route_w, *pred_w;
   int last_rows_per_seq = 1;
+  // CUDA graphs of the verify pass (a11 + a12), keyed by what fixes its launch arguments
+  std::map<unsigned long long, cudaGraphExec_t> vgraph;
+  std::map<unsigned long long, int> vgraph_seen;      // eager runs so far; < 0: capture failed, stay eager
+  std::map<unsigned long long, int> vgraph_launches;  // kernels inside the graph (for the launch counter)
+  unsigned int ls_version = 0;
   float2* rope_tab;
   FusedState fs;
   uint32_t accel_mask[4];
@@ -409,6 +415,7 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
 extern "C" int m2r2_destroy(m2r2_ctx* x) {
   if (!x) return M2R2_INVALID_ARG;
   cudaStreamSynchronize(x->cs);
+  for (auto& kv : x->vgraph) cudaGraphExecDestroy(kv.second);
   if (x->cps != x->cs) cudaStreamSynchronize(x->cps);
   if (x->ods) { cudaStreamSynchronize(x->ods); cudaStreamDestroy(x->ods); }
   for (auto e : x->ev_layer_done) cudaEventDestroy(e);
@@ -1031,24 +1038,64 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
       for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, true, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + j + 1 + 1) * x->esz;
     bytes += (int64_t)c.vocab * c.d_model * x->esz;
   }
-  // a11: k+1-token verify pass, slow stream, all layers
+  // a11: k+1-token verify pass, slow stream, all layers; a12: accept + rollback on the device.
+  // The pass is ~290 dependent launches whose arguments depend only on (k, B, attention splits, script,
+  // implementation): after one eager run it is captured into a CUDA graph and replayed (positions, kv_len,
+  // drafts and tokens are read from device memory inside the kernels).
   {
-    Pass p = {MODE_VERIFY, k + 1, 0, 0, c.n_layers, false, false, false, true, false};
-    rc = run_pass(x, p);
-    if (rc) return rc;
-    // tokens t_j: rows b*(k+1)+j -> d_vtok[b*8 + j]
-    final_head(x, B * (k + 1), x->d_accepted, 1);   // temp: contiguous rows
-    for (int b = 0; b < B; ++b)
-      CU(x, cudaMemcpyAsync(x->d_vtok + b * 8, x->d_accepted + b * (k + 1), sizeof(int) * (k + 1), cudaMemcpyDeviceToDevice, x->cs));
+    int max_len = 0;
+    for (int b = 0; b < B; ++b) max_len = std::max(max_len, x->kv_h[b]);
+    const int splits = n_splits_for(x, B, max_len + k + 1);
+    const unsigned long long key = ((unsigned long long)x->ls_version << 32) | ((unsigned long long)(x->ls_on ? 1 : 0) << 31) |
+                                   ((unsigned long long)(x->fused ? 1 : 0) << 30) | ((unsigned long long)splits << 12) |
+                                   ((unsigned long long)B << 4) | (unsigned long long)k;
+    const bool can_graph = !x->prof;
+    auto it = can_graph ? x->vgraph.find(key) : x->vgraph.end();
+    if (it != x->vgraph.end()) {
+      CU(x, cudaGraphLaunch(it->second, x->cs));
+      x->st.kernel_launches += x->vgraph_launches[key];
+    } else {
+      int& seen = x->vgraph_seen[key];
+      const bool capture = can_graph && seen >= 1;
+      const int64_t l0 = x->st.kernel_launches;
+      if (capture && cudaStreamBeginCapture(x->cs, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); seen = -1000000; }
+      const bool capturing = capture && seen >= 1;
+      Pass p = {MODE_VERIFY, k + 1, 0, 0, c.n_layers, false, false, false, true, false};
+      rc = run_pass(x, p);
+      if (!rc) {
+        // tokens t_j: rows b*(k+1)+j -> d_vtok[b*8 + j]
+        final_head(x, B * (k + 1), x->d_accepted, 1);   // temp: contiguous rows
+        for (int b = 0; b < B; ++b)
+          cudaMemcpyAsync(x->d_vtok + b * 8, x->d_accepted + b * (k + 1), sizeof(int) * (k + 1), cudaMemcpyDeviceToDevice, x->cs);
+        prof_mark(x, M2R2_PROF_OTHER);
+        accept_kernel<<<1, 32, 0, x->cs>>>(B, k, x->d_drafts, x->d_vtok, x->d_accepted, x->d_nacc, x->d_kv_len, x->d_pending);
+        count(x);
+      }
+      if (capturing) {
+        cudaGraph_t g = nullptr;
+        cudaGraphExec_t ex = nullptr;
+        cudaError_t e = cudaStreamEndCapture(x->cs, &g);
+        if (e == cudaSuccess && !rc) e = cudaGraphInstantiate(&ex, g, 0);
+        if (g) cudaGraphDestroy(g);
+        if (rc) return rc;
+        if (e != cudaSuccess || !ex) {
+          cudaGetLastError();
+          seen = -1000000;      // not capturable on this system: stay eager for this key
+          return fail(x, M2R2_CUDA, "verify graph capture failed: %s", cudaGetErrorString(e));
+        }
+        x->vgraph[key] = ex;
+        x->vgraph_launches[key] = (int)(x->st.kernel_launches - l0);
+        CU(x, cudaGraphLaunch(ex, x->cs));   // the captured launches have not run yet
+      } else if (rc) {
+        return rc;
+      }
+      ++seen;
+    }
     for (int i = 0; i < c.n_layers; ++i)
       for (int b = 0; b < B; ++b) bytes += (b == 0 ? layer_bytes(x, i, false, 0) : 0) + 2 * (int64_t)c.d_model * (x->kv_h[b] + k + 1 + k + 1) * x->esz;
     bytes += (int64_t)c.vocab * c.d_model * x->esz;
   }
   x->st.algorithmic_bytes_last = bytes;
-  // a12: accept + rollback on the device
-  prof_mark(x, M2R2_PROF_OTHER);
-  accept_kernel<<<1, 32, 0, x->cs>>>(B, k, x->d_drafts, x->d_vtok, x->d_accepted, x->d_nacc, x->d_kv_len, x->d_pending);
-  count(x);
   prof_resolve(x);
   CU(x, cudaMemcpyAsync(x->h_pinned, x->d_accepted, sizeof(int) * B * 8, cudaMemcpyDeviceToHost, x->cs));
   CU(x, cudaMemcpyAsync(x->h_pinned + 64, x->d_nacc, sizeof(int) * B, cudaMemcpyDeviceToHost, x->cs));
@@ -1194,6 +1241,7 @@ extern "C" int m2r2_set_policy(m2r2_ctx* x, int32_t policy) {
 extern "C" int m2r2_set_logit_script(m2r2_ctx* x, const int32_t* full_tok, const int32_t* draft_tok, int32_t first_pos,
                                      int32_t n, float beta) {
   if (!x) return M2R2_INVALID_ARG;
+  x->ls_version++;
   if (!full_tok) { x->ls_on = false; return M2R2_OK; }
   const m2r2_config& c = x->c;
   if (n < 1 || n > c.max_seq || first_pos < 0) return fail(x, M2R2_INVALID_ARG, "logit script: bad n/first_pos");
