@@ -1652,6 +1652,7 @@ struct VArgs {
   const float* resid;    // O / DOWN: out = resid + W x
   float* trace;          // DOWN: second copy of out, or nullptr
   int ldx, ldo, rows, K, n_out, nkt, nstage_k, split, d, dh;
+  int ksplit;            // O / DOWN: CTAs per row tile along K; > 1 adds into out (= resid, in place) atomically
 };
 __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -1661,7 +1662,7 @@ __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   return bf2_u32(h);
 }
 template <int KIND>
-__global__ void __launch_bounds__(256) gemv_mma_kernel(const VArgs a) {
+__global__ void __launch_bounds__(256, 3) gemv_mma_kernel(const VArgs a) {
   __shared__ float red[8][16][8];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   const int rt = blockIdx.x;
@@ -1669,7 +1670,8 @@ __global__ void __launch_bounds__(256) gemv_mma_kernel(const VArgs a) {
   const float* xrow = a.X + (size_t)g * a.ldx;
   const bool row_live = g < a.rows;
   constexpr int UN = 8;
-  for (int kt0 = warp; kt0 < a.nkt; kt0 += 8 * UN) {
+  const int kt_lo = (int)(((long long)a.nkt * blockIdx.y) / a.ksplit), kt_hi = (int)(((long long)a.nkt * (blockIdx.y + 1)) / a.ksplit);
+  for (int kt0 = kt_lo + warp; kt0 < kt_hi; kt0 += 8 * UN) {
     uint4 w[UN];
     float2 x0[UN], x1[UN];
 #pragma unroll
@@ -1678,7 +1680,7 @@ __global__ void __launch_bounds__(256) gemv_mma_kernel(const VArgs a) {
       w[u] = make_uint4(0u, 0u, 0u, 0u);
       x0[u] = make_float2(0.f, 0.f);
       x1[u] = x0[u];
-      if (kt < a.nkt) {
+      if (kt < kt_hi) {
         const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
                                     : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
         w[u] = ldg_stream(a.W + tile * 32 + lane);
@@ -1723,9 +1725,13 @@ __global__ void __launch_bounds__(256) gemv_mma_kernel(const VArgs a) {
         if (pr < a.n_out) a.out[(size_t)n * a.ldo + pr] = v;
       } else {
         if (pr < a.n_out) {
-          const float o = a.resid[(size_t)n * a.ldo + pr] + v;
-          a.out[(size_t)n * a.ldo + pr] = o;
-          if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
+          if (a.ksplit > 1) {
+            atomicAdd(a.out + (size_t)n * a.ldo + pr, v);   // out == resid (in place): the partial sums land on it
+          } else {
+            const float o = a.resid[(size_t)n * a.ldo + pr] + v;
+            a.out[(size_t)n * a.ldo + pr] = o;
+            if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
+          }
         }
       }
     }
@@ -2043,6 +2049,7 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   a.X = X; a.ldx = ldx; a.rows = rows; a.out = out; a.ldo = ldo; a.resid = resid; a.trace = trace;
   a.d = c.d_model; a.dh = c.head_dim;
   int n_rt = 0;
+  a.ksplit = 1;
   const FLayer* L = kind == VK_HEAD ? nullptr : &im->h_layers[layer];
   switch (kind) {
     case VK_QKV:    a.W = L->Wqkv; a.K = c.d_model; a.n_out = 3 * c.d_model; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_qkv; break;
@@ -2051,12 +2058,18 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     case VK_DOWN:   a.W = L->Wd;   a.K = c.d_ff; a.n_out = c.d_model; a.nkt = q.nkc_d * 8; a.nstage_k = q.nkc_d; a.split = 1; n_rt = q.ng_d * SK_RT; break;
     default:        a.W = im->h_Wlm; a.K = c.d_model; a.n_out = c.vocab; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_v; break;
   }
+  // O / down have few row tiles (d / 16): several CTAs share one along K so that every SM streams (3 CTAs fit an SM)
+  if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
+    const int want = (3 * im->G + n_rt - 1) / n_rt;
+    a.ksplit = std::max(1, std::min(want, a.nkt / 64));
+  }
+  const dim3 grid(n_rt, a.ksplit);
   switch (kind) {
-    case VK_QKV:    gemv_mma_kernel<VK_QKV><<<n_rt, 256, 0, st>>>(a); break;
-    case VK_OPROJ:  gemv_mma_kernel<VK_OPROJ><<<n_rt, 256, 0, st>>>(a); break;
-    case VK_GATEUP: gemv_mma_kernel<VK_GATEUP><<<n_rt, 256, 0, st>>>(a); break;
-    case VK_DOWN:   gemv_mma_kernel<VK_DOWN><<<n_rt, 256, 0, st>>>(a); break;
-    default:        gemv_mma_kernel<VK_HEAD><<<n_rt, 256, 0, st>>>(a); break;
+    case VK_QKV:    gemv_mma_kernel<VK_QKV><<<grid, 256, 0, st>>>(a); break;
+    case VK_OPROJ:  gemv_mma_kernel<VK_OPROJ><<<grid, 256, 0, st>>>(a); break;
+    case VK_GATEUP: gemv_mma_kernel<VK_GATEUP><<<grid, 256, 0, st>>>(a); break;
+    case VK_DOWN:   gemv_mma_kernel<VK_DOWN><<<grid, 256, 0, st>>>(a); break;
+    default:        gemv_mma_kernel<VK_HEAD><<<grid, 256, 0, st>>>(a); break;
   }
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }
