@@ -536,3 +536,32 @@ def test_c3_full_size_long_context_properties():
         assert int(a.decode_step()[0]) == f[pos + 1 - P]
         pos += 1
     a.close()
+
+
+def test_fused_first_steps_repeat_across_engine_instances():
+    """Stress for timing-dependent errors in the fused kernel: 40 fresh engines of a model whose first two layers
+    carry the accelerated stream and whose other layers do not (the C3 structure, where the auxiliary warp
+    retires early), each prefilled and stepped three times under teacher forcing, against the per-operation
+    kernels of the same library.  The two implementations differ by ~5e-4 here (bf16 K/V rounding flips); a
+    lost or late split-K partial sum shows up as >= 1e-2 on the 16 rows of one warp."""
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2)
+    W = S.gen_weights(cfg)
+    prompt = S.gen_prompt(cfg, 11)
+    toks = [5, 77, 1234]
+    r0 = M.Engine(cfg, W)
+    r0.set_fused(False)
+    r0.prefill(prompt)
+    ref = []
+    for s in range(3):
+        r0.decode_step(force_tokens=[toks[s]])
+        ref.append([r0.debug_read(M.DBG_H, i).copy() for i in range(cfg.n_layers + 1)])
+    r0.close()
+    for cyc in range(40):
+        a = M.Engine(cfg, W)
+        a.prefill(prompt)
+        for s in range(3):
+            a.decode_step(force_tokens=[toks[s]])
+            for i in range(cfg.n_layers + 1):
+                e = rel_l2(a.debug_read(M.DBG_H, i), ref[s][i])
+                assert e <= 3e-3, (cyc, s, i, e)
+        a.close()
