@@ -565,3 +565,65 @@ def test_fused_first_steps_repeat_across_engine_instances():
                 e = rel_l2(a.debug_read(M.DBG_H, i), ref[s][i])
                 assert e <= 3e-3, (cyc, s, i, e)
         a.close()
+
+
+@pytest.mark.parametrize("fused", [True, False])
+def test_results_do_not_depend_on_uninitialised_device_memory(fused, monkeypatch):
+    """The weights arena, the KV cache and the scratch arena are handed to the library uninitialised
+    (`torch.empty`).  Each of the three is filled in turn with 0xFF bytes (NaN as bf16 and as fp32, -1 as an
+    index), 0x7F bytes (huge finite values) and seeded random bytes before `m2r2_create`; every hidden state
+    of both streams must come out as with zero-filled arenas.  A read of memory the library never wrote (a
+    padded weight stage the repack skipped, K/V rows past the context, a partial of an empty attention split,
+    a padded activation slot) would show up as NaN or as an O(1) error.  The per-operation kernels are
+    deterministic, so they must agree bit for bit; the fused kernel's fp32 atomics reorder, so it agrees to
+    rounding."""
+    import torch
+    orig_empty = torch.empty
+    state = {"n": 0, "which": -1, "mode": "zero"}
+
+    def poisoned_empty(*a, **k):
+        t = orig_empty(*a, **k)
+        if t.is_cuda and t.dtype == torch.uint8:
+            i = state["n"] % 3   # Engine allocates weights, kv, scratch in this order
+            state["n"] += 1
+            if i != state["which"] or state["mode"] == "zero":
+                t.zero_()
+            elif state["mode"] == "rand":
+                g = torch.Generator(device=t.device).manual_seed(7)
+                t.copy_(torch.randint(0, 256, t.shape, dtype=torch.uint8, device=t.device, generator=g))
+            else:
+                t.fill_(int(state["mode"], 16))
+        return t
+
+    monkeypatch.setattr(torch, "empty", poisoned_empty)
+    toks = [5, 77, 1234, 9, 400]
+
+    def run(cfg, W, prompt):
+        state["n"] = 0
+        e = M.Engine(cfg, W)
+        e.set_fused(fused)
+        e.prefill(prompt)
+        out = []
+        for t in toks:
+            e.decode_step(force_tokens=[t])
+            out.append(np.stack([e.debug_read(M.DBG_H, i) for i in range(cfg.n_layers + 1)] +
+                                [e.debug_read(M.DBG_P, i) for i in range(cfg.n_layers + 1)]))
+        e.close()
+        return out
+
+    for cfg in (S.config_small_bf16(gates=(2,), accel_end_layer=2), S.config_small_bf16()):
+        W = S.gen_weights(cfg)
+        for plen in (11, 70):
+            prompt = S.gen_prompt(cfg, plen)
+            state["which"], state["mode"] = -1, "zero"
+            ref = run(cfg, W, prompt)
+            for which in range(3):
+                for mode in ("ff", "7f", "rand"):
+                    state["which"], state["mode"] = which, mode
+                    out = run(cfg, W, prompt)
+                    for s in range(len(toks)):
+                        assert np.all(np.isfinite(out[s])), (plen, which, mode, s)
+                        if fused:
+                            assert rel_l2(out[s], ref[s]) <= 1e-4, (plen, which, mode, s, rel_l2(out[s], ref[s]))
+                        else:
+                            assert np.array_equal(out[s], ref[s]), (plen, which, mode, s)
