@@ -69,6 +69,12 @@ constexpr int RED_FLOATS = FB * NCW * 32;
 constexpr int MAX_R = 8;               // adapter rank limit (PAPER.md L399 uses 8); larger ranks take the per-operation kernels
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
+// exchanged adapter scratch: every flagged partial (8 bytes) and every r-vector (<= 32 bytes) sits on its own
+// 128-byte line; 148 CTAs poll / read them at once and accesses to one line serialise in L2
+constexpr int UPART_N = 256;           // flagged partials of one phase (n_j * q <= 256)
+constexpr int UPART_STRIDE = 16;       // in 8-byte entries
+constexpr int RV_STRIDE = 32;          // in floats
+static_assert(RV_STRIDE >= MAX_R, "r-vector stride");
 constexpr int PF_DEFAULT = 6;           // L2 prefetch window of the prefetch warp, in stages (M2R2_PF overrides; 0 = off)
 constexpr int MERGE_NS = 4;            // attention splits combined from registers by the auxiliary warp; more take a looped path
 constexpr long long SPIN_LIMIT = 4000000000ll;   // ~2 s of SM clocks before a wait gives up
@@ -113,9 +119,9 @@ struct FParams {
   float* R;                  // residual pair [2][d]: h then p; split-K phases add into it
   float *act, *qbuf, *khat, *vhat;
   float *apart;              // [head][split][2][dh+4]
-  u64 *upart;                // [MAX_NJ][UPART_Q] (epoch << 32 | fp32 bits)
-  float *apu;                // [head][split][MAX_R]: A_o applied to the unnormalised accelerated attention partial
-  float *udpart;             // [CTA][MAX_R]: A_d applied to the CTA's own accelerated SwiGLU activations
+  u64 *upart;                // [UPART_N] entries UPART_STRIDE apart (epoch << 32 | fp32 bits)
+  float *apu;                // [head][split][RV_STRIDE]: A_o applied to the unnormalised accelerated attention partial
+  float *udpart;             // [CTA][RV_STRIDE]: A_d applied to the CTA's own accelerated SwiGLU activations
   int nah;                   // accelerated heads
   float *trace, *logits, *exit_logits;
   Ctl* ctl;
@@ -126,6 +132,7 @@ struct FParams {
   int ns;        // attention splits
   int pos_host;  // kv_len + joff as the host knows it (producer-side KV prefetch only)
   int pf_ahead;  // L2 prefetch window in stages beyond the producer's cursor (0 = prefetch warp idle)
+  unsigned int zero;   // 0 at run time, unknown to the compiler (release_stage)
   u64* tl;       // debug timeline (M2R2_FUSED_DEBUG builds), else nullptr
 };
 
@@ -164,6 +171,16 @@ __device__ __forceinline__ void mbar_expect_tx(u64* b, uint32_t bytes) {
 }
 __device__ __forceinline__ void mbar_arrive(u64* b) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+// A consumer warp hands a ring stage back to the producer.  The arrive must not become visible before the
+// warp's fragment loads of that stage have RETURNED: ptxas schedules a plain mbarrier.arrive right behind the
+// issue of the last LDS (it has no register dependence on the loads), the producer refills the slot as soon as
+// the eighth warp has arrived, and a refill served from L2 was observed to overwrite fragments that were still
+// being read (sporadic errors of ~1e-2 in one warp's 16 rows).  The barrier's address is
+// therefore made to depend, through a run-time zero, on the accumulators the stage's fragments feed.
+__device__ __forceinline__ void release_stage(u64* b, unsigned int zero, float dep) {
+  const uint32_t a = smem_u32(b) + (__float_as_uint(dep) & zero);
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(a) : "memory");
 }
 __device__ __forceinline__ bool mbar_try_wait(u64* b, uint32_t parity) {
   uint32_t ok;
@@ -531,7 +548,7 @@ struct APre {
 };
 __device__ __forceinline__ void u_geometry(UState& us, int nj, int G) {
   us.nj = nj;
-  us.q = min(min(G / nj, UPART_Q), 256 / nj);
+  us.q = min(min(G / nj, UPART_Q), UPART_N / nj);
 }
 __device__ __forceinline__ void publish_prefetch(const UState& us, APre& ap, const bf16* A, int Kc) {
   const int lane = threadIdx.x & 31, c = blockIdx.x;
@@ -573,7 +590,7 @@ __device__ __forceinline__ void publish_u(const FParams& P, const bf16* x, const
     acc = warp_sum(acc);
     if (lane == 0) {
       const u64 v = ((u64)us.epoch << 32) | (u64)__float_as_uint(acc);
-      asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(P.upart + c), "l"(v) : "memory");   // entry index = j * q + ch = c
+      asm volatile("st.global.cg.u64 [%0], %1;" ::"l"(P.upart + (size_t)c * UPART_STRIDE), "l"(v) : "memory");   // entry index = j * q + ch = c
     }
   }
 }
@@ -591,7 +608,7 @@ __device__ __forceinline__ void fetch_u(const FParams& P, float* u, float* utmp,
       v[i] = 0.f;
       if (idx < total) {
         u64 e;
-        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(e) : "l"(P.upart + idx) : "memory");
+        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(e) : "l"(P.upart + (size_t)idx * UPART_STRIDE) : "memory");
         ok = ok && (unsigned int)(e >> 32) == us.epoch;
         v[i] = __uint_as_float((unsigned int)e);
       }
@@ -675,7 +692,7 @@ __device__ __noinline__ float combine_slow(const FParams& P, int head, float (&p
     if (ml.y > 0.f) {
       const float wgt = __expf(ml.x - M);
       Lsum += ml.y * wgt;
-      const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
+      const float* q = P.apu + (size_t)(head * NS + s) * RV_STRIDE;
 #pragma unroll
       for (int i = 0; i < MAX_R; ++i) if (i < r) part[i] += ldcg(q + i) * wgt;
     }
@@ -705,7 +722,7 @@ __device__ __forceinline__ void combine_u(const FParams& P, float* u, int ph, in
           for (int c = 0; c < MAX_R / 4; ++c) pu[s][c] = make_float4(0.f, 0.f, 0.f, 0.f);
           if (s < NS) {
             ml[s] = __ldcg((const float2*)(P.apart + ((size_t)(head * NS + s) * 2 + 1) * (dh + 4) + dh));
-            const float* q = P.apu + (size_t)(head * NS + s) * MAX_R;
+            const float* q = P.apu + (size_t)(head * NS + s) * RV_STRIDE;
 #pragma unroll
             for (int c = 0; c < MAX_R / 4; ++c) if (c * 4 < r) pu[s][c] = ldcg4(q + c * 4);
           }
@@ -734,7 +751,7 @@ __device__ __forceinline__ void combine_u(const FParams& P, float* u, int ph, in
     }
   } else {
     for (int c = lane; c < G; c += 32) {
-      const float* pu = P.udpart + (size_t)c * MAX_R;
+      const float* pu = P.udpart + (size_t)c * RV_STRIDE;
 #pragma unroll
       for (int i = 0; i < MAX_R; ++i) if (i < r) acc[i] += ldcg(pu + i);
     }
@@ -1111,7 +1128,7 @@ __device__ __noinline__ void attn_phase(const FParams& P, unsigned char* kvbuf, 
       for (int i = 0; i < MAX_R; ++i) {
         if (i < P.r) {
           const float v = warp_sum(acc[i]);
-          if (lane == 0) __stcg(P.apu + (size_t)(head * NS + sp) * MAX_R + i, v);
+          if (lane == 0) __stcg(P.apu + (size_t)(head * NS + sp) * RV_STRIDE + i, v);
         }
       }
     }
@@ -1474,7 +1491,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
         mma_bf16(ca, a6, b3.x, b3.y);
         mma_bf16(cb, a7, b3.z, b3.w);
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[slot]);   // stage consumed by this warp
+        if (lane == 0) release_stage(&empty[slot], P.zero, ca[0] + cb[0]);   // stage consumed by this warp
         if (kc == pg.nkc - 1 || s == pg.s1 - 1) {
           // columns 0,1 = h (hi, lo parts), 2,3 = p: lanes t = 0 / 1 hold the h / p sums of rows g, g + 8
           if (t < 2 && (t == 0 || accel)) {
@@ -1519,7 +1536,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
         mma_bf16(ca, a6, b3.x, b3.y);
         mma_bf16(cb, a7, b3.z, b3.w);
         __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[slot]);   // stage consumed by this warp
+        if (lane == 0) release_stage(&empty[slot], P.zero, ca[0] + cb[0]);   // stage consumed by this warp
         if (++ks == nks) {
           // ---- row-tile rt finished in this warp's k range: park the partial sums
           float* rw = red + ((size_t)pending_tiles * NCW + warp) * 32;
@@ -1566,7 +1583,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
           float sum = 0.f;
 #pragma unroll
           for (int w = 0; w < NCW; ++w) sum += ud_s[w * MAX_R + lane];
-          __stcg(P.udpart + (size_t)blockIdx.x * MAX_R + lane, sum);
+          __stcg(P.udpart + (size_t)blockIdx.x * RV_STRIDE + lane, sum);
         }
       }
     }
@@ -1819,9 +1836,9 @@ void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs) {
   FTAKE(act, float, 2 * (size_t)q.F_pad)
   FTAKE(qbuf, float, 2 * d) FTAKE(khat, float, d) FTAKE(vhat, float, d)
   FTAKE(apart, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * 2 * (c.head_dim + 4))
-  FTAKE(upart, u64, (size_t)MAX_NJ * UPART_Q)
-  FTAKE(apu, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * MAX_R)
-  FTAKE(udpart, float, (size_t)1024 * MAX_R)
+  FTAKE(upart, u64, (size_t)UPART_N * UPART_STRIDE)
+  FTAKE(apu, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * RV_STRIDE)
+  FTAKE(udpart, float, (size_t)1024 * RV_STRIDE)
 #undef FTAKE
 }
 
@@ -1940,8 +1957,8 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
   cudaMemsetAsync(im->act, 0, sizeof(float) * 2 * q.F_pad, st);
   cudaMemsetAsync(im->R, 0, sizeof(float) * 2 * d, st);
-  cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * MAX_R, st);
-  cudaMemsetAsync(im->upart, 0, sizeof(u64) * MAX_NJ * UPART_Q, st);
+  cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * RV_STRIDE, st);
+  cudaMemsetAsync(im->upart, 0, sizeof(u64) * UPART_N * UPART_STRIDE, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;   // hl / sidx / cols are stack-owned
   im->bar_base = 0;
   FParams& p = im->p;
@@ -2029,7 +2046,7 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
     snprintf(msg, n, "fused kernel wait timed out (site 0x%x)", im->h_ctl->abort_where);
     // re-arm: barrier counter and flags back to a clean state
     cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
-    cudaMemsetAsync(im->upart, 0, sizeof(u64) * MAX_NJ * UPART_Q, st);
+    cudaMemsetAsync(im->upart, 0, sizeof(u64) * UPART_N * UPART_STRIDE, st);
     cudaStreamSynchronize(st);
     im->bar_base = 0;
     return M2R2_CUDA;
