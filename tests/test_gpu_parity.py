@@ -543,7 +543,8 @@ def test_fused_first_steps_repeat_across_engine_instances():
     carry the accelerated stream and whose other layers do not (the C3 structure, where the auxiliary warp
     retires early), each prefilled and stepped three times under teacher forcing, against the per-operation
     kernels of the same library.  The two implementations differ by ~5e-4 here (bf16 K/V rounding flips); a
-    lost or late split-K partial sum shows up as >= 1e-2 on the 16 rows of one warp."""
+    ring stage refilled while a warp still reads it (the race `release_stage` closes: it hit
+    a third of these cycles once the adapter scratch was padded) shows up as >= 1e-2 on the 16 rows of one warp."""
     cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2)
     W = S.gen_weights(cfg)
     prompt = S.gen_prompt(cfg, 11)
