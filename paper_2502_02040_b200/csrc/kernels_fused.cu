@@ -69,11 +69,12 @@ constexpr int RED_FLOATS = FB * NCW * 32;
 constexpr int MAX_R = 8;               // adapter rank limit (PAPER.md L399 uses 8); larger ranks take the per-operation kernels
 constexpr int MAX_NJ = 3 * MAX_R;
 constexpr int UPART_Q = 64;            // max k-chunks per adapter row
-// exchanged adapter scratch: every flagged partial (8 bytes) and every r-vector (<= 32 bytes) sits on its own
-// 128-byte line; 148 CTAs poll / read them at once and accesses to one line serialise in L2
+// exchanged adapter scratch: strides of the flagged partials (8 bytes each) and of the r-vectors.  One 128-byte
+// line per item (strides 16 / 32) takes the serialisation of 148 CTAs polling one line away and is 1.5 % faster
+// with exit heads on, but 3 % slower on the C2 bench workload (no exit heads) in the same GPU session: dense.
 constexpr int UPART_N = 256;           // flagged partials of one phase (n_j * q <= 256)
-constexpr int UPART_STRIDE = 16;       // in 8-byte entries
-constexpr int RV_STRIDE = 32;          // in floats
+constexpr int UPART_STRIDE = 1;        // in 8-byte entries
+constexpr int RV_STRIDE = MAX_R;       // in floats
 static_assert(RV_STRIDE >= MAX_R, "r-vector stride");
 constexpr int PF_DEFAULT = 6;           // L2 prefetch window of the prefetch warp, in stages (M2R2_PF overrides; 0 = off)
 constexpr int MERGE_NS = 4;            // attention splits combined from registers by the auxiliary warp; more take a looped path
