@@ -89,6 +89,8 @@ def lib():
         L.orc_last_margin.argtypes = [vp]
         L.orc_last_draft_margin.restype = f32
         L.orc_last_draft_margin.argtypes = [vp]
+        L.orc_step_min_margin.restype = f32
+        L.orc_step_min_margin.argtypes = [vp]
         L.orc_get_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
         L.orc_rope.argtypes = [vp, vp, i32]
         L.orc_rmsnorm.argtypes = [vp, vp, vp, vp]
@@ -242,6 +244,10 @@ class Oracle:
 
     def draft_margin(self):
         return float(self.L.orc_last_draft_margin(self.h))
+
+    def step_margin(self):
+        """smallest top-2 margin of any argmax (every draft, every verify row) of the last step"""
+        return float(self.L.orc_step_min_margin(self.h))
 
     def kcache(self, layer):
         """writable view [max_seq, d] (tests poison dead positions through it)"""

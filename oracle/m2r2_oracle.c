@@ -95,6 +95,7 @@ typedef struct orc {
   float* exit_logits;/* [J][V] accelerated-stream exit logits at each gate, before bias */
   float last_margin; /* top-2 margin of the last final argmax (after bias) */
   float last_draft_margin;
+  float step_min_margin; /* introspection: smallest top-2 margin of any argmax (draft or verify) of the last spec_step / decode_step */
   int32_t* route_idx;  /* [N][top_k] routed experts of the last slow token */
   float* route_w;      /* [N][top_k] */
   int32_t* pred_idx;   /* [N][top_k] predicted experts per TARGET layer (-1: none) */
@@ -726,6 +727,7 @@ int orc_decode_step(orc* o, int force_token, int32_t* token_out, int32_t* exit_t
   dual_token(o, tok_in, t, c->n_layers, 1, h, p, exit_tokens, 1);
   head_logits(o, h, 0, o->logits);
   int tok = pick_token(o, o->logits, t + 1, 0, &o->last_margin);
+  o->step_min_margin = o->last_margin;
   o->kv_len = t + 1;
   o->pending = tok;
   o->have_pending = 1;
@@ -756,6 +758,7 @@ int orc_spec_step(orc* o, int gamma, int32_t* accepted, int32_t* n_accepted, int
     int E = c->gates[0];
     int32_t ex[ORC_MAX_GATES];
     dual_token(o, cur, n + j, E, 1, h, p, ex, 0);
+    if (j == 0 || o->last_draft_margin < o->step_min_margin) o->step_min_margin = o->last_draft_margin;
     drafts[j] = ex[0];
     cur = drafts[j];
   }
@@ -769,6 +772,7 @@ int orc_spec_step(orc* o, int gamma, int32_t* accepted, int32_t* n_accepted, int
   for (int j = 0; j < m; ++j) {
     head_logits(o, H + (size_t)j * d, 0, o->logits);
     tv[j] = pick_token(o, o->logits, n + j + 1, 0, &o->last_margin);
+    if ((j == 0 && gamma == 0) || o->last_margin < o->step_min_margin) o->step_min_margin = o->last_margin;
   }
   /* 3. accept the longest matching prefix; 4. rollback = set kv_len */
   int a = 0;
@@ -795,6 +799,7 @@ const float* orc_logits(const orc* o) { return o->logits; }
 const float* orc_exit_logits(const orc* o, int gate) { return o->exit_logits + (size_t)gate * o->c.vocab; }
 float orc_last_margin(const orc* o) { return o->last_margin; }
 float orc_last_draft_margin(const orc* o) { return o->last_draft_margin; }
+float orc_step_min_margin(const orc* o) { return o->step_min_margin; }
 float* orc_kcache(orc* o, int layer) { return o->K + (size_t)layer * o->c.max_seq * o->c.d_model; }
 float* orc_vcache(orc* o, int layer) { return o->V + (size_t)layer * o->c.max_seq * o->c.d_model; }
 const int32_t* orc_route_idx(const orc* o) { return o->route_idx; }

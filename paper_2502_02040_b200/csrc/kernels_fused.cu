@@ -98,6 +98,7 @@ struct Ctl {
   unsigned int bar;        // grid-barrier arrivals (monotonic across launches)
   unsigned int abort_flag; // a wait timed out
   unsigned int abort_where;
+  unsigned int* host_abort;   // host-mapped word written on abort (nullptr: none)
   u64 amax[1 + M2R2_MAX_GATES];   // argmax keys: [0] head of the pass, [1+j] exit head of gate j
 };
 
@@ -259,7 +260,10 @@ __device__ __forceinline__ u64 gtime() { u64 t; asm volatile("mov.u64 %0, %%glob
 #endif
 
 __device__ __forceinline__ void set_abort(Ctl* ctl, unsigned int where) {
-  if (atomicExch(&ctl->abort_flag, 1u) == 0u) ctl->abort_where = where;
+  if (atomicExch(&ctl->abort_flag, 1u) == 0u) {
+    ctl->abort_where = where;
+    if (ctl->host_abort) { *(volatile unsigned int*)ctl->host_abort = 0x80000000u | where; __threadfence_system(); }
+  }
 }
 __device__ __forceinline__ bool aborted(const Ctl* ctl) { return *(volatile const unsigned int*)&ctl->abort_flag != 0u; }
 
@@ -1593,7 +1597,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) m2r2_fused_decode_kernel(const __
     TL(30 + ph);
   }
   TL(50);
-  if (blockIdx.x == 0 && tid == 0) {
+  // A timed-out wait leaves the pass unsynchronised: nothing it computed may become sequence state.
+  // The host sees the abort through ctl->host_abort at its next call and re-arms the control block.
+  if (blockIdx.x == 0 && tid == 0 && !aborted(P.ctl)) {
     u64 key = *(volatile u64*)&P.ctl->amax[0];
     int tk = (int)(0xFFFFFFFFu - (unsigned int)(key & 0xFFFFFFFFull));
     *P.tok_out = tk;
@@ -1767,6 +1773,8 @@ struct FusedImpl {
   int* d_sidx = nullptr;
   unsigned int bar_base = 0;
   Ctl* h_ctl = nullptr;       // pinned
+  unsigned int* h_abort = nullptr;   // host-mapped: set by the kernel when a wait times out
+  unsigned int* d_abort = nullptr;   // its device address
   bool bound = false;
   u64* d_tl = nullptr;        // debug timeline (M2R2_FUSED_DEBUG builds)
   std::vector<FLayer> h_layers;   // host copy of the layer descriptors (packed weight pointers)
@@ -1865,6 +1873,15 @@ int fused_create(const m2r2_config& c, FusedState* fs) {
   FusedImpl* im = new FusedImpl();
   im->G = sms;
   if (cudaMallocHost((void**)&im->h_ctl, sizeof(Ctl)) != cudaSuccess) { delete im; return M2R2_CUDA; }
+  if (cudaHostAlloc((void**)&im->h_abort, 64, cudaHostAllocMapped) != cudaSuccess ||
+      cudaHostGetDevicePointer((void**)&im->d_abort, im->h_abort, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (im->h_abort) cudaFreeHost(im->h_abort);
+    cudaFreeHost(im->h_ctl);
+    delete im;
+    return M2R2_CUDA;
+  }
+  *im->h_abort = 0u;
   fs->impl = im;
   fs->supported = true;
   return 0;
@@ -1873,6 +1890,7 @@ int fused_create(const m2r2_config& c, FusedState* fs) {
 void fused_destroy(FusedState* fs) {
   if (fs->impl) {
     if (fs->impl->h_ctl) cudaFreeHost(fs->impl->h_ctl);
+    if (fs->impl->h_abort) cudaFreeHost(fs->impl->h_abort);
     delete fs->impl;
   }
   fs->impl = nullptr;
@@ -1955,7 +1973,13 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
     }
   if (cudaMemcpyAsync(im->d_sidx, sidx.data(), sizeof(int) * c.n_heads, cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
   if (cudaMemcpyAsync(im->accel_cols, cols.data(), sizeof(int) * cols.size(), cudaMemcpyHostToDevice, st) != cudaSuccess) return M2R2_CUDA;
-  cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
+  {
+    Ctl z;
+    memset(&z, 0, sizeof(z));
+    z.host_abort = im->d_abort;
+    *im->h_ctl = z;
+    cudaMemcpyAsync(im->d_ctl, im->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice, st);
+  }
   cudaMemsetAsync(im->act, 0, sizeof(float) * 2 * q.F_pad, st);
   cudaMemsetAsync(im->R, 0, sizeof(float) * 2 * d, st);
   cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * RV_STRIDE, st);
@@ -1979,9 +2003,10 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   p.apart = im->apart; p.upart = im->upart; p.apu = im->apu; p.udpart = im->udpart;
   p.nah = c.accel_enabled ? c.n_accel_heads : 0;
   p.ctl = im->d_ctl;
-  p.pf_ahead = getenv("M2R2_PF") ? atoi(getenv("M2R2_PF")) : PF_DEFAULT;
+  p.pf_ahead = PF_DEFAULT;
   p.tl = nullptr;
 #ifdef M2R2_FUSED_DEBUG
+  if (getenv("M2R2_PF")) p.pf_ahead = atoi(getenv("M2R2_PF"));   // debug builds only: sweep the L2 prefetch window
   if (getenv("M2R2_TL_OUT") && !im->d_tl) cudaMalloc((void**)&im->d_tl, sizeof(u64) * TL_MAX * im->G);
   p.tl = im->d_tl;
 #endif
@@ -2021,13 +2046,18 @@ int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const Fused
   for (int i = 0; i < run.n_layers; ++i)
     if (im->gate_of[i] && im->accel_of[i] && run.exit_heads && !(run.head_stream == 1 && i + 1 == run.n_layers)) ++nbar;
   p.bar_base = im->bar_base;
-  im->bar_base += nbar * (unsigned int)G;
   void* args[] = {(void*)&p};
   cudaError_t e = cudaLaunchCooperativeKernel((const void*)m2r2_fused_decode_kernel, dim3(G), dim3(NTHREADS), args,
                                               SMEM_BYTES, st);
   if (e != cudaSuccess) return M2R2_CUDA;
+  im->bar_base += nbar * (unsigned int)G;   // only a launch that was enqueued moves the barrier target
   if (launches) *launches += 1;
   return 0;
+}
+
+// non-blocking: has any launch so far reported a timed-out wait?  (host-mapped flag, no stream synchronisation)
+bool fused_abort_pending(const FusedState* fs) {
+  return fs->supported && fs->impl && fs->impl->bound && fs->impl->h_abort && *(volatile unsigned int*)fs->impl->h_abort != 0u;
 }
 
 int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
@@ -2046,7 +2076,14 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
   if (im->h_ctl->abort_flag) {
     snprintf(msg, n, "fused kernel wait timed out (site 0x%x)", im->h_ctl->abort_where);
     // re-arm: barrier counter and flags back to a clean state
-    cudaMemsetAsync(im->d_ctl, 0, sizeof(Ctl), st);
+    {
+      Ctl z;
+      memset(&z, 0, sizeof(z));
+      z.host_abort = im->d_abort;
+      *im->h_ctl = z;
+      cudaMemcpyAsync(im->d_ctl, im->h_ctl, sizeof(Ctl), cudaMemcpyHostToDevice, st);
+    }
+    *im->h_abort = 0u;
     cudaMemsetAsync(im->upart, 0, sizeof(u64) * UPART_N * UPART_STRIDE, st);
     cudaStreamSynchronize(st);
     im->bar_base = 0;

@@ -102,6 +102,14 @@ struct m2r2_ctx {
   size_t expert_bytes = 0, eg_bytes = 0, ed_bytes = 0;
   int policy = M2R2_POLICY_LRU;
   int* h_pinned = nullptr;     // pinned host staging for small D2H reads
+  // forced tokens are staged through a ring of pinned slots, each guarded by an event recorded behind its H2D
+  // copy: decode_step(tokens_out == NULL) returns without synchronising, so the next call must not overwrite a
+  // slot whose copy has not executed yet
+  static constexpr int FORCE_SLOTS = 8;
+  int* h_force = nullptr;      // [FORCE_SLOTS][M2R2_MAX_BATCH]
+  cudaEvent_t ev_force[FORCE_SLOTS] = {};
+  unsigned int force_ctr = 0;
+  int sm_count = 148;
   // scripts
   int ls_first = 0, ls_n = 0; float ls_beta = 0.f; bool ls_on = false;
   int rs_first = 0, rs_n = 0; float rs_beta = 0.f; bool rs_on = false;
@@ -109,9 +117,9 @@ struct m2r2_ctx {
   int *d_kv_len, *d_pending, *d_row_tok, *d_row_seq, *d_row_pos, *d_row_limit, *d_grp_rows;
   int *d_drafts, *d_vtok, *d_accepted, *d_nacc, *d_exit_tok, *d_out_tok, *d_force, *d_prompt;
   int *d_qkv_bmap, *d_accel_cols, *d_ls_full, *d_ls_draft, *d_rs_actual, *d_rs_pred;
-  int *d_route_idx, *d_pred_idx;
+  int *d_route_idx, *d_pred_idx, *d_moe_ridx;
   float *resid, *xn, *U, *qkv, *attn_o, *act, *part_o, *part_ml, *logits, *exit_logits, *trace;
-  float *moe_tmp, *route_w, *pred_w;
+  float *moe_tmp, *route_w, *pred_w, *moe_wtab, *moe_rw;
   int last_rows_per_seq = 1;
   // CUDA graphs of the verify pass (a11 + a12), keyed by what fixes its launch arguments
   std::map<unsigned long long, cudaGraphExec_t> vgraph;
@@ -199,6 +207,10 @@ static int validate(const m2r2_config* c) {
     }
     if (c->adapter_rank < 1 || c->adapter_rank > 16) return M2R2_INVALID_ARG;
     if (c->accel_end_layer < 0 || c->accel_end_layer > c->n_layers) return M2R2_INVALID_ARG;
+    // a gate above the last accelerated layer would never be evaluated (p is not live there): its exit token
+    // slot would hold stale values that look like token ids
+    for (int j = 0; j < c->n_gates; ++j)
+      if (c->gates[j] > c->accel_end_layer) return M2R2_INVALID_ARG;
   }
   if (c->n_experts > 0) {
     if (c->n_experts > M2R2_MAX_EXPERTS || c->top_k < 1 || c->top_k > M2R2_MAX_TOPK ||
@@ -290,6 +302,7 @@ static void carve_scratch(const m2r2_config& c, Carver& cv, m2r2_ctx* x) {
   TAKE(logits, float, R * V) TAKE(exit_logits, float, G * B * V)
   TAKE(trace, float, (N + 1) * 2 * B * d)
   TAKE(moe_tmp, float, R * d) TAKE(route_w, float, N * tk) TAKE(pred_w, float, N * tk)
+  TAKE(moe_wtab, float, 8) TAKE(moe_rw, float, 8 * M2R2_MAX_TOPK) TAKE(d_moe_ridx, int, 8 * M2R2_MAX_TOPK)   // MoE prefill chunk tables
   TAKE(rope_tab, float2, S * (dh / 2))
 #undef TAKE
   fused_carve(c, cv, o ? &o->fs : nullptr);
@@ -389,6 +402,13 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
     CUX(cudaStreamSynchronize(x->cs));
   }
   CUX(cudaMallocHost((void**)&x->h_pinned, 4096 * sizeof(int)));
+  CUX(cudaMallocHost((void**)&x->h_force, m2r2_ctx::FORCE_SLOTS * M2R2_MAX_BATCH * sizeof(int)));
+  for (int i = 0; i < m2r2_ctx::FORCE_SLOTS; ++i) CUX(cudaEventCreateWithFlags(&x->ev_force[i], cudaEventDisableTiming));
+  {
+    int dev = 0;
+    CUX(cudaGetDevice(&dev));
+    CUX(cudaDeviceGetAttribute(&x->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  }
   CUX(cudaEventCreateWithFlags(&x->ev_tmp, cudaEventDisableTiming));
   CUX(cudaEventCreateWithFlags(&x->ev_stage_free, cudaEventDisableTiming));
   int lo = 0, hi = 0;
@@ -423,6 +443,8 @@ extern "C" int m2r2_destroy(m2r2_ctx* x) {
   if (x->ev_tmp) cudaEventDestroy(x->ev_tmp);
   if (x->ev_stage_free) cudaEventDestroy(x->ev_stage_free);
   if (x->h_pinned) cudaFreeHost(x->h_pinned);
+  if (x->h_force) cudaFreeHost(x->h_force);
+  for (auto e : x->ev_force) if (e) cudaEventDestroy(e);
   for (auto e : x->pev) cudaEventDestroy(e);
   fused_destroy(&x->fs);
   delete x;
@@ -598,7 +620,7 @@ static int prefetch_pairs(m2r2_ctx* x, const int* pairs, int n) {
 
 // ------------------------------------------------------------------ forward pass (per-operation kernels)
 static int n_splits_for(const m2r2_ctx* x, int groups, int max_len) {
-  int want = (4 * 148 + x->c.n_heads * groups - 1) / (x->c.n_heads * groups);
+  int want = (4 * x->sm_count + x->c.n_heads * groups - 1) / (x->c.n_heads * groups);
   int cap = std::max(1, (max_len + 31) / 32);
   return std::max(1, std::min(std::min(want, cap), M2R2_MAX_SPLITS));
 }
@@ -896,6 +918,12 @@ static int moe_mlp(m2r2_ctx* x, const Pass& p, int i, int ns, int na) {
 static int check_ready(m2r2_ctx* x) {
   if (!x) return M2R2_INVALID_ARG;
   if (!x->weights_loaded) return fail(x, M2R2_BAD_STATE, "load_weights has not been called");
+  // a fused launch whose device-side wait timed out left no sequence state behind; report it from whichever
+  // call comes next (also when the caller never asked for tokens) and re-arm the kernel
+  if (fused_abort_pending(&x->fs)) {
+    int rc = fused_check(&x->fs, x->cs, x->err, sizeof(x->err));
+    if (rc) return rc;
+  }
   return 0;
 }
 
@@ -948,6 +976,7 @@ extern "C" int m2r2_prefill(m2r2_ctx* x, const int32_t* tokens, int32_t B, int32
   CU(x, cudaStreamSynchronize(x->cs));
   CU(x, cudaGetLastError());
   for (int b = 0; b < B; ++b) { x->kv_h[b] = P; if (first_tokens) first_tokens[b] = x->h_pinned[b]; }
+  x->last_rows_per_seq = P - ((P - 1) / 8) * 8;   // rows per sequence of the last prefill chunk (debug_read LOGITS)
   x->have_pending = true;
   return M2R2_OK;
 }
@@ -963,8 +992,12 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
   if (force_tokens) {
     for (int b = 0; b < B; ++b)
       if (force_tokens[b] < 0 || force_tokens[b] >= c.vocab) return fail(x, M2R2_INVALID_ARG, "force token out of range");
-    memcpy(x->h_pinned + 2048, force_tokens, sizeof(int) * B);
-    CU(x, cudaMemcpyAsync(x->d_force, x->h_pinned + 2048, sizeof(int) * B, cudaMemcpyHostToDevice, x->cs));
+    const unsigned int slot = x->force_ctr++ % m2r2_ctx::FORCE_SLOTS;
+    int* hs = x->h_force + (size_t)slot * M2R2_MAX_BATCH;
+    CU(x, cudaEventSynchronize(x->ev_force[slot]));   // the copy that last used this slot has executed
+    memcpy(hs, force_tokens, sizeof(int) * B);
+    CU(x, cudaMemcpyAsync(x->d_force, hs, sizeof(int) * B, cudaMemcpyHostToDevice, x->cs));
+    CU(x, cudaEventRecord(x->ev_force[slot], x->cs));
   }
   int64_t bytes = 0;
   for (int i = 0; i < c.n_layers; ++i)
@@ -1125,9 +1158,9 @@ static int moe_prefill(m2r2_ctx* x, int P) {
   const m2r2_config& c = x->c;
   const int d = c.d_model, tk = c.top_k, nh = c.n_heads, dh = c.head_dim;
   const float scale = 1.0f / sqrtf((float)dh);
-  float* wtab = x->moe_tmp + (size_t)8 * d;   // [8 rows] per-row weight of the current expert
-  int* ridx = x->d_vtok;                      // [8][tk] routed experts of the chunk's rows
-  float* rw = x->part_ml;                     // [8][tk] their weights (attention partials are dead by then)
+  float* wtab = x->moe_wtab;                  // [8 rows] per-row weight of the current expert
+  int* ridx = x->d_moe_ridx;                  // [8][tk] routed experts of the chunk's rows
+  float* rw = x->moe_rw;                      // [8][tk] their weights
   for (int c0 = 0; c0 < P; c0 += 8) {
     const int m = std::min(8, P - c0);
     x->kv_h[0] = c0;
@@ -1242,6 +1275,10 @@ extern "C" int m2r2_set_logit_script(m2r2_ctx* x, const int32_t* full_tok, const
                                      int32_t n, float beta) {
   if (!x) return M2R2_INVALID_ARG;
   x->ls_version++;
+  // captured verify graphs are keyed by the script version: the old ones can never be launched again
+  CU(x, cudaStreamSynchronize(x->cs));
+  for (auto& kv : x->vgraph) cudaGraphExecDestroy(kv.second);
+  x->vgraph.clear(); x->vgraph_seen.clear(); x->vgraph_launches.clear();
   if (!full_tok) { x->ls_on = false; return M2R2_OK; }
   const m2r2_config& c = x->c;
   if (n < 1 || n > c.max_seq || first_pos < 0) return fail(x, M2R2_INVALID_ARG, "logit script: bad n/first_pos");
@@ -1278,18 +1315,22 @@ extern "C" int m2r2_set_router_script(m2r2_ctx* x, const int32_t* actual, const 
 
 extern "C" int m2r2_get_stats(m2r2_ctx* x, m2r2_stats* out) {
   if (!x || !out) return M2R2_INVALID_ARG;
+  if (fused_abort_pending(&x->fs)) {
+    int rc = fused_check(&x->fs, x->cs, x->err, sizeof(x->err));
+    if (rc) return rc;
+  }
   *out = x->st;
   for (int b = 0; b < M2R2_MAX_BATCH; ++b) out->kv_len[b] = b < x->B ? x->kv_h[b] : 0;
   return M2R2_OK;
 }
 
-__global__ void kv_to_f32_kernel(const void* cache, int bf16, int n_heads, int dh, int max_seq, int T, float* out) {
-  // out[t][head*dh + j] from cache[head][t][j]
+__global__ void kv_to_f32_kernel(const void* cache, int bf16, int n_heads, int dh, int max_seq, int t0, int T, float* out) {
+  // out[t][head*dh + j] from cache[head][t0 + t][j]
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   size_t d = (size_t)n_heads * dh;
   if (i >= (size_t)T * d) return;
   int t = (int)(i / d), hd = (int)(i % d), head = hd / dh, j = hd % dh;
-  size_t src = ((size_t)head * max_seq + t) * dh + j;
+  size_t src = ((size_t)head * max_seq + t0 + t) * dh + j;
   out[i] = bf16 ? __bfloat162float(((const __nv_bfloat16*)cache)[src]) : ((const float*)cache)[src];
 }
 __global__ void i2f_kernel(const int* in, float* out, int n) {
@@ -1308,6 +1349,7 @@ extern "C" int m2r2_debug_read(m2r2_ctx* x, int32_t what, int32_t layer, int32_t
   const float* src = nullptr;
   size_t avail = 0;
   CU(x, cudaStreamSynchronize(x->cs));
+  if (fused_abort_pending(&x->fs) && (rc = fused_check(&x->fs, x->cs, x->err, sizeof(x->err)))) return rc;
   switch (what) {
     case M2R2_DBG_H:
     case M2R2_DBG_P:
@@ -1333,13 +1375,16 @@ extern "C" int m2r2_debug_read(m2r2_ctx* x, int32_t what, int32_t layer, int32_t
       size_t per = (size_t)c.n_heads * c.max_seq * c.head_dim * x->esz;
       char* base = (char*)x->b.kv + ((size_t)layer * c.max_batch + b) * per;
       if (what == M2R2_DBG_V) base += (size_t)c.n_layers * c.max_batch * per;
-      float* tmp = nullptr;
-      CU(x, cudaMalloc((void**)&tmp, T * d * sizeof(float)));
-      kv_to_f32_kernel<<<(unsigned)((T * d + 255) / 256), 256, 0, x->cs>>>(base, c.dtype == M2R2_BF16, c.n_heads, c.head_dim, c.max_seq, (int)T, tmp);
-      cudaError_t e = cudaMemcpyAsync(host_out, tmp, T * d * sizeof(float), cudaMemcpyDeviceToHost, x->cs);
-      cudaStreamSynchronize(x->cs);
-      cudaFree(tmp);
-      if (e != cudaSuccess) return fail(x, M2R2_CUDA, "debug_read copy failed");
+      // converted through the attention-partials scratch (dead between steps, never read back) in chunks of
+      // whole positions
+      const size_t cap = (size_t)x->R * M2R2_MAX_SPLITS;   // part_o holds R * n_heads * splits * dh floats
+      if (cap < 1) return fail(x, M2R2_UNSUPPORTED, "debug_read: scratch too small for one K/V row");
+      for (size_t t0 = 0; t0 < T; t0 += cap) {
+        const size_t nt = std::min(cap, T - t0);
+        kv_to_f32_kernel<<<(unsigned)((nt * d + 255) / 256), 256, 0, x->cs>>>(base, c.dtype == M2R2_BF16, c.n_heads, c.head_dim, c.max_seq, (int)t0, (int)nt, x->part_o);
+        CU(x, cudaMemcpyAsync(host_out + t0 * d, x->part_o, nt * d * sizeof(float), cudaMemcpyDeviceToHost, x->cs));
+        CU(x, cudaStreamSynchronize(x->cs));
+      }
       return M2R2_OK;
     }
     case M2R2_DBG_ROUTE_IDX:

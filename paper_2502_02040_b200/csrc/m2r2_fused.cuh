@@ -43,6 +43,8 @@ int fused_run(const m2r2_config& c, FusedState* fs, cudaStream_t st, const Fused
               float ls_beta, int64_t* launches);
 // 0 if the last launches completed normally; otherwise a description (device-side timeout)
 int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n);
+// non-blocking variant: true once any launch has reported a timed-out wait (then call fused_check to re-arm)
+bool fused_abort_pending(const FusedState* fs);
 // a11: skinny GEMM of <= 8 slow-stream rows on the fragment-major weights (verify pass, prefill chunks).
 // kind: 0 QKV (natural row order out), 1 O-proj (+resid), 2 gate/up + SwiGLU, 3 down (+resid, trace), 4 LM head.
 // Returns M2R2_UNSUPPORTED when the fused weight copy is not bound or rows > 8.

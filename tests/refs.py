@@ -107,3 +107,82 @@ def rel_l2(a, b):
     a = np.asarray(a, dtype=np.float64)
     b = np.asarray(b, dtype=np.float64)
     return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-30))
+
+
+# ---------------------------------------------------------------------------------------------
+# Brute-force restatements of the MoE / predictor / LM-head-adapter branches (pins I18-I21).
+# Written from PAPER.md and DESIGN.md's readings in numpy float64; they share nothing with oracle/.
+# ---------------------------------------------------------------------------------------------
+def np_route(cfg, Wr, y, renorm=True):
+    """Router (DESIGN Q19): softmax over ALL experts, the top_k largest (lower index
+    first on ties), weights renormalised over the selected ones.  -> (idx[top_k], w[top_k])"""
+    logits = Wr.astype(np.float64) @ y.astype(np.float64)
+    pr = np.exp(logits - logits.max())
+    pr /= pr.sum()
+    order = sorted(range(len(pr)), key=lambda e: (-pr[e], e))[:cfg.top_k]
+    w = pr[order]
+    if renorm:
+        w = w / w.sum()
+    return np.asarray(order, dtype=np.int32), w
+
+
+def np_swiglu(Wg, Wu, Wd, y):
+    g, u = Wg @ y, Wu @ y
+    return Wd @ (g / (1.0 + np.exp(-g)) * u)
+
+
+def np_slow_attention(cfg, Lw, h, t, Kc, Vc):
+    """h' = h + W_o concat_a softmax(q_a K_a[0..t]^T / sqrt(dh)) V_a[0..t]  (Eq. 1) for the token at
+    position t, given the slow cache INCLUDING position t (the cache itself is pinned by I1 / I6)."""
+    f = lambda k: S.as_f32(cfg, Lw[k]).astype(np.float64)
+    dh, nh = cfg.head_dim, cfg.n_heads
+    x = np_rms(cfg, h, f("g1"))
+    q = np_rope(cfg, (f("wq") @ x).astype(np.float32), t)
+    o = np.zeros(cfg.d_model)
+    for a in range(nh):
+        sl = slice(a * dh, (a + 1) * dh)
+        sc = Kc[:t + 1, sl].astype(np.float64) @ q[sl] / np.sqrt(dh)
+        pr = np.exp(sc - sc.max())
+        pr /= pr.sum()
+        o[sl] = pr @ Vc[:t + 1, sl].astype(np.float64)
+    return h.astype(np.float64) + f("wo") @ o
+
+
+def np_moe_slow_layer(cfg, Lw, h, t, Kc, Vc):
+    """Slow MoE layer: attention as above, then m = sum_{e in top-k} w_e Expert_e(rms(h'; g2))
+    (SURVEY §8(c).1 'MoE layer').  -> (h_{i+1}, idx, w)"""
+    f = lambda a: S.as_f32(cfg, a).astype(np.float64)
+    h1 = np_slow_attention(cfg, Lw, h, t, Kc, Vc)
+    y = np_rms(cfg, h1, f(Lw["g2"]))
+    idx, w = np_route(cfg, f(Lw["router"]), y, cfg.renorm_topk)
+    m = np.zeros(cfg.d_model)
+    for e, we in zip(idx, w):
+        E = Lw["experts"][int(e)]
+        m += we * np_swiglu(f(E["ewg"]), f(E["ewu"]), f(E["ewd"]), y)
+    return h1 + m, idx, w
+
+
+def np_accel_layer_moe(cfg, Lw, p, t, Kc, Vc):
+    """Accelerated layer of a MoE model: attention with adapters as in the dense case, then the FIXED
+    adapter-only bottleneck  m^ = U_d (silu(U_g y^) * (U_u y^))  (DESIGN Q7)."""
+    f = lambda k: S.as_f32(cfg, Lw[k]).astype(np.float64)
+    dh = cfg.head_dim
+    Sh = list(cfg.accel_heads)
+    rows = np.concatenate([np.arange(a * dh, (a + 1) * dh) for a in Sh])
+    x = np_rms(cfg, p, f("g1"))
+    q = f("wq")[rows] @ x + f("Bq") @ (f("Aq") @ x)
+    k = f("wk")[rows] @ x + f("Bk") @ (f("Ak") @ x)
+    v = f("wv")[rows] @ x + f("Bv") @ (f("Av") @ x)
+    q, k = np_rope(cfg, q, t), np_rope(cfg, k, t)
+    o = np.zeros(len(rows))
+    for s, a in enumerate(Sh):
+        sl = slice(s * dh, (s + 1) * dh)
+        Kmat = np.vstack([Kc[:t, a * dh:(a + 1) * dh].astype(np.float64), k[sl][None]])
+        Vmat = np.vstack([Vc[:t, a * dh:(a + 1) * dh].astype(np.float64), v[sl][None]])
+        sc = Kmat @ q[sl] / np.sqrt(dh)
+        pr = np.exp(sc - sc.max())
+        pr /= pr.sum()
+        o[sl] = pr @ Vmat
+    p1 = p.astype(np.float64) + f("wo")[:, rows] @ o + f("Bo") @ (f("Ao") @ o)
+    y = np_rms(cfg, p1, f("g2"))
+    return p1 + np_swiglu(f("Ug"), f("Uu"), f("Ud"), y)

@@ -139,22 +139,22 @@ def test_gate_reset_and_zero_adapter_invariants_on_gpu():
 
 
 # ------------------------------------------------------------------ self-speculative decoding
-@pytest.mark.parametrize("gamma", [0, 1, 3, 6])
-def test_c1_selfspec_matches_oracle_and_is_lossless(gamma):
-    """a10-a12: accepted tokens, accepted lengths, kv_len bit-exact vs the oracle; emitted stream ==
-    plain greedy stream (lossless)."""
-    cfg = S.config_c1()
-    eng, orc, W = _pair(cfg)
+def _c1_selfspec_run(cfg, W, gamma, prompt_seed):
+    """-> (tokens compared, tied).  Stops at the first step on which the ORACLE's own margin is < 1e-3."""
+    eng, orc = M.Engine(cfg, W), Oracle(cfg, W)
     plain = Oracle(cfg, W)
-    prompt = S.gen_prompt(cfg, 32)
+    prompt = S.gen_prompt(cfg, 32, seed=1000 + prompt_seed)
     first = orc.prefill(prompt)
+    if orc.margin() < MARGIN:
+        eng.close()
+        return 0, True
     assert int(eng.prefill(prompt)[0]) == first
     stream_plain = [plain.prefill(prompt)]
     emitted = [first]
     tie = False
     while len(emitted) < 33:
         acc_o, _ = orc.spec_step(gamma)
-        tie = tie or orc.margin() < MARGIN or orc.draft_margin() < MARGIN
+        tie = orc.step_margin() < MARGIN
         acc_e, n_e = eng.spec_step(gamma)
         if tie:
             break
@@ -163,15 +163,30 @@ def test_c1_selfspec_matches_oracle_and_is_lossless(gamma):
         assert eng.get_stats()["kv_len"][0] == orc.kv_len
         check_logits(cfg, eng.debug_read(M.DBG_LOGITS, gamma), orc.logits(), "verify logits row gamma")
         emitted += acc_o
+        st, so = eng.get_stats(), orc.stats()
+        assert (st["drafted"], st["accepted"], st["emitted"]) == (so["drafted"], so["accepted"], so["emitted"])
     while len(stream_plain) < len(emitted):
         stream_plain.append(plain.decode_step()[0])
-    if not tie:
-        assert emitted == stream_plain[:len(emitted)]
-    st = eng.get_stats()
-    so = orc.stats()
-    if not tie:
-        assert (st["drafted"], st["accepted"], st["emitted"]) == (so["drafted"], so["accepted"], so["emitted"])
+    assert emitted == stream_plain[:len(emitted)]      # lossless up to the tie
     eng.close()
+    return len(emitted) - 1, tie
+
+
+@pytest.mark.parametrize("gamma", [0, 1, 3, 6])
+def test_c1_selfspec_matches_oracle_and_is_lossless(gamma):
+    """a10-a12: accepted tokens, accepted lengths, kv_len bit-exact vs the oracle; emitted stream ==
+    plain greedy stream (lossless).  A near-tie in the oracle (margin < 1e-3, Q23) ends the
+    comparison for that prompt only; further prompts are run until at least 32 tokens have been compared, so
+    the test cannot pass vacuously."""
+    cfg = S.config_c1()
+    W = S.gen_weights(cfg)
+    total = 0
+    for prompt_seed in range(6):
+        n, tied = _c1_selfspec_run(cfg, W, gamma, prompt_seed)
+        total += n
+        if total >= 32:
+            break
+    assert total >= 32, total
 
 
 @pytest.mark.parametrize("alpha", [0.5, 0.9])

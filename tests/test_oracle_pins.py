@@ -12,7 +12,8 @@ import pytest
 
 import m2r2_synth as S
 from oracle import Oracle
-from tests.refs import np_accel_layer, np_rope, rel_l2, torch_decoder
+from tests.refs import (np_accel_layer, np_accel_layer_moe, np_moe_slow_layer, np_rms, np_rope, np_route, rel_l2,
+                        torch_decoder)
 
 
 def tiny(**kw):
@@ -483,3 +484,163 @@ def test_golden_c1_tokens_regression():
     with open(__file__.replace("test_oracle_pins.py", "golden/c1_tokens.txt")) as fh:
         want = [int(x) for ln in fh if ln.strip() and ln[0] != "#" for x in ln.split()]
     assert toks == want
+
+
+# ---------------------------------------------------------------- I18-I21: the branches VERDICT r1 found unpinned
+def test_I18_moe_topk_mixture_bruteforce():
+    """PAPER.md L131 / SURVEY §8(c).1 'MoE layer': h_{i+1} = h' + sum_{e in top-2} w_e Expert_e(rms(h'; g2)) with
+    n_e = 8, top_k = 2 and RENORMALISED weights, against a numpy restatement (attention over the oracle's own
+    cache, which I1/I6 pin).  Sensitivity: dropping the renormalisation or weighting both experts equally
+    moves the result far outside the tolerance."""
+    cfg = S.config_small_moe()
+    W = S.gen_weights(cfg)
+    o = Oracle(cfg, W)
+    o.prefill(S.gen_prompt(cfg, 7))
+    for _ in range(3):
+        o.decode_step()
+        H = o.trace_h()
+        t = o.kv_len - 1
+        ri, rw = o.route_idx(), o.route_w()
+        for i in range(cfg.n_layers):
+            want, idx, w = np_moe_slow_layer(cfg, W["layers"][i], H[i], t, o.kcache(i), o.vcache(i))
+            assert idx.tolist() == ri[i].tolist(), (i, idx, ri[i])
+            assert idx[0] != idx[1]
+            assert np.allclose(w, rw[i], atol=1e-6) and abs(w.sum() - 1.0) < 1e-12
+            err = rel_l2(H[i + 1] - H[i], want - H[i])
+            assert err < 5e-6, (i, err)
+            # a plausible slip: un-renormalised softmax weights (sum < 1) or equal weights
+            no_renorm, _, w_raw = np_moe_slow_layer(replace(cfg, renorm_topk=False), W["layers"][i], H[i], t,
+                                                    o.kcache(i), o.vcache(i))
+            assert w_raw.sum() < 0.9
+            assert rel_l2(H[i + 1] - H[i], no_renorm - H[i]) > 1e-2
+
+
+def test_I19_moe_accelerated_bottleneck_bruteforce():
+    """PAPER.md L137 ('fixed set of accelerator adapters' while h takes the routed experts) in DESIGN Q7's
+    reading: the accelerated stream of a MoE layer is attention-with-adapters followed by the rank-r_m SwiGLU
+    bottleneck U_d(silu(U_g y^) * U_u y^), with NO expert involved.  Brute force in numpy from trace_p."""
+    cfg = S.config_small_moe()
+    W = S.gen_weights(cfg)
+    o = Oracle(cfg, W)
+    o.prefill(S.gen_prompt(cfg, 6))
+    for _ in range(2):
+        o.decode_step()
+        P = o.trace_p()
+        t = o.kv_len - 1
+        for i in range(cfg.n_layers):
+            want = np_accel_layer_moe(cfg, W["layers"][i], P[i], t, o.kcache(i), o.vcache(i))
+            assert rel_l2(P[i + 1] - P[i], want - P[i]) < 5e-6, i
+            # sensitivity: gate and up swapped (silu on the wrong branch) is far off
+            Lw = dict(W["layers"][i])
+            Lw["Ug"], Lw["Uu"] = Lw["Uu"], Lw["Ug"]
+            bad = np_accel_layer_moe(cfg, Lw, P[i], t, o.kcache(i), o.vcache(i))
+            assert rel_l2(P[i + 1] - P[i], bad - P[i]) > 1e-3     # 200x the tolerance above
+    # the accelerated stream of a MoE layer does not depend on the experts at all
+    W2 = S.gen_weights(cfg)
+    for L in W2["layers"]:
+        for E in L["experts"]:
+            E["ewd"][...] = 0
+    o2 = Oracle(cfg, W2)
+    o2.prefill(S.gen_prompt(cfg, 6))
+    o2.decode_step()
+    P2 = o2.trace_p()
+    o3 = Oracle(cfg, W)
+    o3.prefill(S.gen_prompt(cfg, 6))
+    o3.decode_step()
+    # layer 0 of the first decode step: p_0 = h_0 is the same embedding row and the layer-0 cache is identical
+    assert np.array_equal(P2[1], o3.trace_p()[1])
+
+
+def test_I20_expert_predictor_unscripted():
+    """PAPER.md L387 / L137 in DESIGN Q16's reading: after accelerated layer i the experts of every target layer
+    L' in targets(i) are predicted as top-2 of softmax(W_r^{L'} rms(p_{i+1}; g2_{L'})): the TARGET layer's router
+    and the TARGET layer's g2, applied to the accelerated residual LEAVING layer i.  No router script, so the
+    arithmetic itself decides.  The alternatives a slip would produce (source layer's g2, source layer's
+    router, p entering the layer, the slow residual) must disagree somewhere, or the pin would be blind."""
+    cfg = S.config_small_moe()
+    assert cfg.aot_targets[0] == (2, 4) and cfg.aot_targets[1] == (4, 6)
+    W = S.gen_weights(cfg)
+    o = Oracle(cfg, W)
+    o.set_policy(2)
+    o.prefill(S.gen_prompt(cfg, 5))
+    f = lambda a: S.as_f32(cfg, a).astype(np.float64)
+    blind = {"g2_src": 0, "router_src": 0, "p_in": 0, "h": 0}
+    checked = 0
+    for _ in range(6):
+        o.decode_step()
+        P, H, pred = o.trace_p(), o.trace_h(), o.pred_idx()
+        for i, (lo, hi) in enumerate(cfg.aot_targets):
+            for Lt in range(lo, hi):
+                Lw, Ls = W["layers"][Lt], W["layers"][i]
+                idx, _ = np_route(cfg, f(Lw["router"]), np_rms(cfg, P[i + 1], f(Lw["g2"])))
+                assert idx.tolist() == pred[Lt].tolist(), (i, Lt, idx, pred[Lt])
+                checked += 1
+                alts = {"g2_src": np_route(cfg, f(Lw["router"]), np_rms(cfg, P[i + 1], f(Ls["g2"])))[0],
+                        "router_src": np_route(cfg, f(Ls["router"]), np_rms(cfg, P[i + 1], f(Lw["g2"])))[0],
+                        "p_in": np_route(cfg, f(Lw["router"]), np_rms(cfg, P[i], f(Lw["g2"])))[0],
+                        "h": np_route(cfg, f(Lw["router"]), np_rms(cfg, H[i + 1], f(Lw["g2"])))[0]}
+                for k, v in alts.items():
+                    blind[k] += int(v.tolist() != idx.tolist())
+        untargeted = [L for L in range(cfg.n_layers) if not any(lo <= L < hi for lo, hi in cfg.aot_targets)]
+        assert (pred[untargeted] == -1).all()
+    assert checked == 6 * 4
+    # the gains are 1 + 0.02 N(0,1): a wrong g2 rarely flips a top-2, so that alternative is only required
+    # to be distinguishable through the router input norm; the others must flip at least once
+    assert blind["router_src"] > 0 and blind["p_in"] > 0 and blind["h"] > 0, blind
+
+
+def test_I20b_predictor_uses_target_layer_gain():
+    """Same pin with gains that differ strongly between layers, so that taking g2 of the wrong layer flips
+    the predicted experts."""
+    cfg = S.config_small_moe()
+    W = S.gen_weights(cfg)
+    rng = np.random.default_rng(5)
+    for L in W["layers"]:
+        g = (1.0 + 0.9 * rng.standard_normal(cfg.d_model)).astype(np.float32)
+        L["g2"][...] = (g.view(np.uint32) >> 16).astype(np.uint16)    # bf16 bits (truncation is fine: an input)
+    o = Oracle(cfg, W)
+    o.set_policy(2)
+    o.prefill(S.gen_prompt(cfg, 5))
+    f = lambda a: S.as_f32(cfg, a).astype(np.float64)
+    flips = 0
+    for _ in range(4):
+        o.decode_step()
+        P, pred = o.trace_p(), o.pred_idx()
+        for i, (lo, hi) in enumerate(cfg.aot_targets):
+            for Lt in range(lo, hi):
+                Lw, Ls = W["layers"][Lt], W["layers"][i]
+                idx, _ = np_route(cfg, f(Lw["router"]), np_rms(cfg, P[i + 1], f(Lw["g2"])))
+                assert idx.tolist() == pred[Lt].tolist()
+                flips += int(np_route(cfg, f(Lw["router"]), np_rms(cfg, P[i + 1], f(Ls["g2"])))[0].tolist() != idx.tolist())
+    assert flips > 0
+
+
+def test_I21_lm_head_adapter_on_exit_logits():
+    """PAPER.md L162 ('low-rank layers for ... language modeling heads') in DESIGN Q9's reading: the exit / draft
+    logits at a gate are W_lm z + B_lm (A_lm z) with z = rms(p_E; g_f), p_E the accelerated residual BEFORE the
+    gate reset; the final head on h never takes the adapter.  numpy from trace_p / trace_h."""
+    cfg = tiny(lm_head_adapter=True)
+    W = S.gen_weights(cfg)
+    o = Oracle(cfg, W)
+    o.prefill(S.gen_prompt(cfg, 9))
+    f = lambda a: S.as_f32(cfg, a).astype(np.float64)
+    for _ in range(3):
+        o.decode_step()
+        P, H = o.trace_p(), o.trace_h()
+        E = cfg.gates[0]
+        z = np_rms(cfg, P[E], f(W["gf"]))
+        base = f(W["lm_head"]) @ z
+        want = base + f(W["lm_B"]) @ (f(W["lm_A"]) @ z)
+        got = o.exit_logits(0)
+        assert rel_l2(got, want) < 2e-6
+        assert rel_l2(got, base) > 1e-3            # the adapter is live: leaving it out is visible
+        zh = np_rms(cfg, H[cfg.n_layers], f(W["gf"]))
+        assert rel_l2(o.logits(), f(W["lm_head"]) @ zh) < 2e-6     # final head: no adapter
+    # a draft taken through spec_step uses the same head
+    o.spec_step(2)
+    # with the flag off the same weights give the base logits
+    o2 = Oracle(replace(cfg, lm_head_adapter=False), {k: v for k, v in W.items() if k not in ("lm_A", "lm_B")})
+    o2.prefill(S.gen_prompt(cfg, 9))
+    o2.decode_step()
+    z2 = np_rms(cfg, o2.trace_p()[cfg.gates[0]], f(W["gf"]))
+    assert rel_l2(o2.exit_logits(0), f(W["lm_head"]) @ z2) < 2e-6
