@@ -34,7 +34,7 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-METRIC = "decode tokens/s at batch 1 (M2R2 dual-stream decode, 3.8B-class bf16)"
+METRIC = "decode tokens/s at batch 1 (M2R2 self-spec); achieved HBM GB/s vs 8 TB/s"   # BASELINE.json wording
 PROMPT = 512
 HBM_NOMINAL_GBS = 8000.0      # BASELINE.json: "achieved HBM GB/s vs 8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of m2r2_fused_decode_kernel (one decode step at
@@ -324,20 +324,88 @@ def run_ours(args, rk):
     line = {"metric": METRIC, "value": value, "unit": "tokens/s", "n_gpus": rk.world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 arithmetic (bf16 weights + KV cache)", "data": "synthetic",
-            "config": config_json(cfg, {"exit_heads_at_gates": exit_heads, "kv_len_start": kv0,
-                                        "implementation": "per-operation kernels" if args.no_fused else "default"}),
+            "config": config_json(cfg),
+            "run": {"exit_heads_at_gates": exit_heads, "kv_len_start": kv0,
+                    "implementation": "per-operation kernels" if args.no_fused else "default",
+                    "value_is": "plain M2R2 dual-stream decode steps of C2 (the workload the roofline target is stated on); "
+                                "the self-speculative tokens/s of the same model are in `selfspec`"},
             "clocks": clk, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline}
 
     # ---- cpu_baseline: oracle on this box's host cores (rank 0, N = 1 only)
     eng.close()
     del eng
     torch.cuda.empty_cache()
+    if rk.rank == 0 and rk.world == 1 and not args.no_selfspec:
+        line["selfspec"] = selfspec_record(peak)
+        torch.cuda.empty_cache()
     if rk.rank == 0 and rk.world == 1 and not args.no_cpu_baseline:
         tps, n, dt, desc = time_oracle(cfg, W, 12, 1, budget_s=25.0)
         line["cpu_baseline"] = {"value": tps, "unit": "tokens/s", "cores": host_cores(), "kind": "oracle", "sample": desc}
     if rk.rank == 0:
         print(json.dumps(line), flush=True)
     return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# self-speculative decoding of the same 3.8B model (BASELINE.json configs[2], "C3"): the metric's "M2R2 self-spec"
+# ---------------------------------------------------------------------------------------------
+def selfspec_record(peak, gamma=4, alphas=(0.9, 0.5), n_tokens=256):
+    """C3: drafts from the accelerated stream at layer 8 (gamma draft passes of layers 0..7 + draft head), one
+    gamma+1-token verify pass of the full model with greedy acceptance and KV rollback, acceptance forced to alpha
+    by the seeded logit script.  Device-timed (CUDA events on the library's compute stream) over the
+    whole generation of n_tokens tokens after a 512-token prompt; spec_step returns the accepted tokens to the host
+    every step, so this is also the end-to-end number."""
+    import torch
+    import m2r2_synth as S
+    import paper_2502_02040_b200 as M
+    cfg = S.config_c3()
+    eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
+    prompt = S.gen_prompt(cfg, PROMPT)
+    stream = eng.compute_stream
+    rec = {"workload": "C3 (BASELINE.json configs[2]): the C2 model under self-speculative decoding, drafts from the "
+                       "accelerated stream at layer 8 (E = 8, LM-head adapter rank 8), draft length gamma = %d, "
+                       "prompt %d, %d generated tokens, acceptance forced by seeded logit biasing" % (gamma, PROMPT, n_tokens),
+           "gamma": gamma, "runs": []}
+    for alpha in alphas:
+        f, g = S.gen_logit_script(cfg, n_tokens + 160, alpha)
+        eng.set_logit_script(f, g, PROMPT)
+        eng.prefill(prompt)
+        for _ in range(3):
+            eng.spec_step(gamma)
+        eng.prefill(prompt)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        emitted, steps, by = 1, 0, 0
+        l0 = eng.get_stats()["kernel_launches"]
+        e0.record(stream)
+        while emitted < n_tokens:
+            _, n = eng.spec_step(gamma)
+            emitted += int(n[0])
+            steps += 1
+            by += eng.get_stats()["algorithmic_bytes_last"]
+        e1.record(stream)
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+        gbs = by / (ms * 1e-3) / 1e9
+        rec["runs"].append({"alpha": alpha, "tokens": emitted - 1, "spec_steps": steps, "tokens_per_s": (emitted - 1) / (ms * 1e-3),
+                            "ms_per_spec_step": ms / steps, "tokens_per_spec_step": (emitted - 1) / steps,
+                            "algorithmic_bytes_per_spec_step": by / steps, "GB/s": gbs, "frac_of_measured_peak": gbs / peak,
+                            "frac_of_nominal_8TBs": gbs / HBM_NOMINAL_GBS,
+                            "gpu_launches_per_spec_step": (eng.get_stats()["kernel_launches"] - l0) / steps})
+    eng.set_logit_script(None, None, PROMPT)
+    eng.prefill(prompt)
+    for _ in range(3):
+        eng.decode_step(want_tokens=False)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(128):
+        eng.decode_step(want_tokens=False)
+    e1.record(stream)
+    e1.synchronize()
+    rec["plain_decode_control_tokens_per_s"] = 128 / (e0.elapsed_time(e1) * 1e-3)
+    eng.close()
+    return rec
 
 
 # ---------------------------------------------------------------------------------------------
@@ -455,6 +523,7 @@ def main():
     ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"],
                     help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-selfspec", action="store_true", help="skip the C3 self-speculative sub-record of the bench line")
     ap.add_argument("--traffic", type=float, default=FUSED_TRAFFIC_BYTES,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")
     args = ap.parse_args()

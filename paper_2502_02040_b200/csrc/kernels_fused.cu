@@ -1677,6 +1677,7 @@ struct VArgs {
   float* trace;          // DOWN: second copy of out, or nullptr
   int ldx, ldo, rows, K, n_out, nkt, nstage_k, split, d, dh;
   int ksplit;            // O / DOWN: CTAs per row tile along K; > 1 adds into out (= resid, in place) atomically
+  int n_rt;              // row tiles of the matrix (rows_mma_kernel)
 };
 __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -1756,6 +1757,102 @@ __global__ void __launch_bounds__(256, 3) gemv_mma_kernel(const VArgs a) {
             a.out[(size_t)n * a.ldo + pr] = o;
             if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
           }
+        }
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ skinny GEMM for 9..64 slow-stream rows (a11 at batch > 1, prefill chunks)
+// Same fragment-major weights.  A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows
+// of a 256-input chunk are staged ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row
+// tiles, so every weight is read from HBM once for all rows (the fp32-FMA kernel reads it once per 8 rows) and the
+// replicated activation traffic from L2 stays near the weight traffic.  NG groups of 8 rows = NG n8 MMA tiles (x2:
+// hi, lo) per weight tile, fp32 accumulators; epilogues as in gemv_mma_kernel.
+constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
+constexpr int RM_LD = RM_KC + 8;         // bf16 elements per staged row (+8: bank spread)
+template <int KIND, int NG>
+__global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
+  extern __shared__ __align__(16) unsigned char rm_smem[];
+  bf16* xh = (bf16*)rm_smem;                       // [NG * 8][RM_LD] hi parts
+  bf16* xl = xh + (size_t)NG * 8 * RM_LD;          // lo parts
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int rt = blockIdx.x * 4 + warp;
+  const bool mine = rt < a.n_rt;
+  float c[NG][4];
+#pragma unroll
+  for (int i = 0; i < NG; ++i)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) c[i][e] = 0.f;
+  const int nch = (a.nkt + 15) / 16;               // chunks of the whole K
+  const int ch_lo = (int)(((long long)nch * blockIdx.y) / a.ksplit), ch_hi = (int)(((long long)nch * (blockIdx.y + 1)) / a.ksplit);
+  for (int ch = ch_lo; ch < ch_hi; ++ch) {
+    const int kbase = ch * RM_KC;
+    // weights of the chunk for this warp's row tile: 16 LDG.128 per lane in flight while the activations are staged
+    uint4 w[16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      const int kt = ch * 16 + u;
+      w[u] = make_uint4(0u, 0u, 0u, 0u);
+      if (mine && kt < a.nkt) {
+        const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
+                                    : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
+        w[u] = ldg_stream(a.W + tile * 32 + lane);
+      }
+    }
+    __syncthreads();   // the previous chunk's staged rows are consumed
+    for (int i = tid; i < NG * 8 * (RM_KC / 4); i += 128) {
+      const int row = i / (RM_KC / 4), q = i - row * (RM_KC / 4), k = kbase + 4 * q;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (row < a.rows && k < a.K) v = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));   // K % 4 == 0
+      uint32_t l0, l1;
+      const uint32_t h0 = pack_hi_lo(v.x, v.y, l0), h1 = pack_hi_lo(v.z, v.w, l1);
+      *(uint2*)(xh + (size_t)row * RM_LD + 4 * q) = make_uint2(h0, h1);
+      *(uint2*)(xl + (size_t)row * RM_LD + 4 * q) = make_uint2(l0, l1);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi) {
+        const bf16* ph = xh + (size_t)(gi * 8 + g) * RM_LD + u * 16 + 2 * t;
+        const bf16* pl = xl + (size_t)(gi * 8 + g) * RM_LD + u * 16 + 2 * t;
+        mma_bf16(c[gi], w[u], *(const uint32_t*)ph, *(const uint32_t*)(ph + 8));
+        mma_bf16(c[gi], w[u], *(const uint32_t*)pl, *(const uint32_t*)(pl + 8));
+      }
+    }
+  }
+  if (!mine) return;
+  // c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2], c[gi][3] = weight row g + 8
+#pragma unroll
+  for (int gi = 0; gi < NG; ++gi) {
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+      const int n = gi * 8 + 2 * t + s;
+      if (n >= a.rows) continue;
+      const float v0 = c[gi][s], v1 = c[gi][2 + s];
+      if (KIND == VK_GATEUP) {
+        const int o = rt * 8 + g;
+        if (o < a.n_out) a.out[(size_t)n * a.ldo + o] = silu(v0) * v1;
+        continue;
+      }
+#pragma unroll
+      for (int hh = 0; hh < 2; ++hh) {
+        const int pr = rt * 16 + g + 8 * hh;
+        const float v = hh ? v1 : v0;
+        if (pr >= a.n_out) continue;
+        if (KIND == VK_QKV) {
+          const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
+          const int nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
+          a.out[(size_t)n * a.ldo + nat] = v;
+        } else if (KIND == VK_HEAD) {
+          a.out[(size_t)n * a.ldo + pr] = v;
+        } else if (a.ksplit > 1) {
+          atomicAdd(a.out + (size_t)n * a.ldo + pr, v);   // out == resid (in place)
+        } else {
+          const float o = a.resid[(size_t)n * a.ldo + pr] + v;
+          a.out[(size_t)n * a.ldo + pr] = o;
+          if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
         }
       }
     }
@@ -2094,9 +2191,25 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
 
 // a11 on the fragment-major weights: out = f(W x) for rows <= 8 slow-stream rows (kinds: VK_*).  Returns
 // M2R2_UNSUPPORTED when the fused copy is not bound (the caller then uses the row-major kernels).
+template <int KIND>
+static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) {
+  const size_t sh = (size_t)2 * ng * 8 * RM_LD * sizeof(bf16);
+#define RM_CASE(NG)                                                                                   \
+  case NG: {                                                                                          \
+    static bool attr_set = false;                                                                     \
+    if (!attr_set) {                                                                                  \
+      cudaFuncSetAttribute(rows_mma_kernel<KIND, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024); \
+      attr_set = true;                                                                                \
+    }                                                                                                 \
+    rows_mma_kernel<KIND, NG><<<grid, 128, sh, st>>>(a);                                              \
+  } break;
+  switch (ng) { RM_CASE(2) RM_CASE(3) RM_CASE(4) RM_CASE(5) RM_CASE(6) RM_CASE(7) RM_CASE(8) default: break; }
+#undef RM_CASE
+}
+
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
                     int rows, float* out, int ldo, const float* resid, float* trace) {
-  if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 8) return M2R2_UNSUPPORTED;
+  if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 64 || (c.d_model % 4) || (c.d_ff % 4)) return M2R2_UNSUPPORTED;
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
   VArgs a;
@@ -2112,6 +2225,24 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     case VK_GATEUP: a.W = L->Wgu;  a.K = c.d_model; a.n_out = c.d_ff; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_gu; break;
     case VK_DOWN:   a.W = L->Wd;   a.K = c.d_ff; a.n_out = c.d_model; a.nkt = q.nkc_d * 8; a.nstage_k = q.nkc_d; a.split = 1; n_rt = q.ng_d * SK_RT; break;
     default:        a.W = im->h_Wlm; a.K = c.d_model; a.n_out = c.vocab; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_v; break;
+  }
+  a.n_rt = n_rt;
+  if (rows > 8) {
+    // 9..64 rows: rows_mma_kernel, 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual)
+    const int ng = (rows + 7) / 8, gx = (n_rt + 3) / 4, nch = (a.nkt + 15) / 16;
+    if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
+      const int want = (4 * im->G + gx - 1) / gx;
+      a.ksplit = std::max(1, std::min(want, nch));
+    }
+    const dim3 grid(gx, a.ksplit);
+    switch (kind) {
+      case VK_QKV:    launch_rows_mma<VK_QKV>(a, grid, ng, st); break;
+      case VK_OPROJ:  launch_rows_mma<VK_OPROJ>(a, grid, ng, st); break;
+      case VK_GATEUP: launch_rows_mma<VK_GATEUP>(a, grid, ng, st); break;
+      case VK_DOWN:   launch_rows_mma<VK_DOWN>(a, grid, ng, st); break;
+      default:        launch_rows_mma<VK_HEAD>(a, grid, ng, st); break;
+    }
+    return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
   }
   // O / down have few row tiles (d / 16): several CTAs share one along K so that every SM streams (3 CTAs fit an SM)
   if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {

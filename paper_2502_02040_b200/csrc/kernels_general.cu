@@ -335,16 +335,19 @@ __device__ __forceinline__ void load_kv<float>(const float* p, float out[8]) {
   out[4] = out[5] = out[6] = out[7] = 0.f;
 }
 
-template <typename KT, int SEG>
+// NQ = query rows compiled in (the group's live rows are packed from slot 0); UN positions per segment are
+// loaded before any is used, so a warp keeps 2 * UN 16-byte loads per lane in flight (the K/V stream is the bound).
+template <typename KT, int SEG, int NQ>
 __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
   constexpr int EPL = KVec<KT>::EPL;
   constexpr int NSEG = 4 * (32 / SEG);           // segments per CTA
+  constexpr int UN = 4;
   extern __shared__ float sm[];
   const int head = blockIdx.x, grp = blockIdx.y, split = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int dh = a.dh, lpp = dh / EPL;
-  float* qs = sm;                                // [MAXQ][dh], pre-scaled
-  float* red = sm + M2R2_MAXQ * dh;              // [NSEG][MAXQ][dh + 2]
+  float* qs = sm;                                // [NQ][dh], pre-scaled
+  float* red = sm + NQ * dh;                     // [NSEG][NQ][dh + 2]
   __shared__ int s_row[M2R2_MAXQ], s_lim[M2R2_MAXQ];
   __shared__ int s_seq, s_maxlim;
   const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
@@ -357,12 +360,12 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
   __syncthreads();
   if (tid == 0) {
     int mx = 0, sq = 0;
-    for (int q = 0; q < M2R2_MAXQ; ++q)
+    for (int q = 0; q < NQ; ++q)
       if (s_row[q] >= 0) { mx = max(mx, s_lim[q]); sq = a.row_seq[s_row[q]]; }
     s_maxlim = mx;
     s_seq = sq;
   }
-  for (int i = tid; i < M2R2_MAXQ * dh; i += 128) {
+  for (int i = tid; i < NQ * dh; i += 128) {
     int q = i / dh, j = i % dh, r = s_row[q];
     qs[i] = r >= 0 ? a.qkv[(size_t)r * 3 * a.d + head * dh + j] * a.scale : 0.f;
   }
@@ -375,49 +378,54 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
 
   const int seg = lane / SEG, sl = lane % SEG;   // segment in warp, lane in segment
   const bool active = sl < lpp;
-  float m[M2R2_MAXQ], l[M2R2_MAXQ], o[M2R2_MAXQ][EPL];
-  int lim[M2R2_MAXQ];
+  float m[NQ], l[NQ], o[NQ][EPL], qr[NQ][EPL];
+  int lim[NQ];
 #pragma unroll
-  for (int q = 0; q < M2R2_MAXQ; ++q) {
+  for (int q = 0; q < NQ; ++q) {
     m[q] = -INFINITY; l[q] = 0.f; lim[q] = s_lim[q];
 #pragma unroll
-    for (int e = 0; e < EPL; ++e) o[q][e] = 0.f;
+    for (int e = 0; e < EPL; ++e) { o[q][e] = 0.f; qr[q][e] = active ? qs[q * dh + sl * EPL + e] : 0.f; }
   }
   constexpr int PPW = 32 / SEG;
-  for (int ub = u0 + warp * PPW; ub < u1; ub += 4 * PPW) {
-    const int u = ub + seg;
-    const bool valid = u < u1;
-    float kv[8], vv[8];
+  for (int ub = u0 + warp * PPW; ub < u1; ub += 4 * PPW * UN) {
+    float kv[UN][8], vv[UN][8];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) { kv[e] = 0.f; vv[e] = 0.f; }
-    if (valid && active) {
-      load_kv<KT>(Kb + (size_t)u * dh + sl * EPL, kv);
-      load_kv<KT>(Vb + (size_t)u * dh + sl * EPL, vv);
+    for (int i = 0; i < UN; ++i) {
+      const int u = ub + i * 4 * PPW + seg;
+#pragma unroll
+      for (int e = 0; e < 8; ++e) { kv[i][e] = 0.f; vv[i][e] = 0.f; }
+      if (u < u1 && active) {
+        load_kv<KT>(Kb + (size_t)u * dh + sl * EPL, kv[i]);
+        load_kv<KT>(Vb + (size_t)u * dh + sl * EPL, vv[i]);
+      }
     }
 #pragma unroll
-    for (int q = 0; q < M2R2_MAXQ; ++q) {
-      float s = 0.f;
-      if (active) {
+    for (int i = 0; i < UN; ++i) {
+      const int u = ub + i * 4 * PPW + seg;
+      const bool valid = u < u1;
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) s += qs[q * dh + sl * EPL + e] * kv[e];
-      }
+      for (int q = 0; q < NQ; ++q) {
+        float s = 0.f;
 #pragma unroll
-      for (int off = SEG / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
-      if (valid && u < lim[q]) {
-        float mn = fmaxf(m[q], s);
-        float corr = __expf(m[q] - mn), p = __expf(s - mn);
-        l[q] = l[q] * corr + p;
+        for (int e = 0; e < EPL; ++e) s += qr[q][e] * kv[i][e];
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) o[q][e] = o[q][e] * corr + p * vv[e];
-        m[q] = mn;
+        for (int off = SEG / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+        if (valid && u < lim[q]) {
+          float mn = fmaxf(m[q], s);
+          float corr = __expf(m[q] - mn), p = __expf(s - mn);
+          l[q] = l[q] * corr + p;
+#pragma unroll
+          for (int e = 0; e < EPL; ++e) o[q][e] = o[q][e] * corr + p * vv[i][e];
+          m[q] = mn;
+        }
       }
     }
   }
   // merge the NSEG running states through shared memory
   const int gseg = warp * PPW + seg;
 #pragma unroll
-  for (int q = 0; q < M2R2_MAXQ; ++q) {
-    float* dst = red + ((size_t)gseg * M2R2_MAXQ + q) * (dh + 2);
+  for (int q = 0; q < NQ; ++q) {
+    float* dst = red + ((size_t)gseg * NQ + q) * (dh + 2);
     if (active) {
 #pragma unroll
       for (int e = 0; e < EPL; ++e) dst[sl * EPL + e] = o[q][e];
@@ -425,14 +433,14 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
     if (sl == 0) { dst[dh] = m[q]; dst[dh + 1] = l[q]; }
   }
   __syncthreads();
-  for (int i = tid; i < M2R2_MAXQ * dh; i += 128) {
+  for (int i = tid; i < NQ * dh; i += 128) {
     int q = i / dh, j = i % dh, r = s_row[q];
     if (r < 0) continue;
     float M = -INFINITY;
-    for (int s = 0; s < NSEG; ++s) M = fmaxf(M, red[((size_t)s * M2R2_MAXQ + q) * (dh + 2) + dh]);
+    for (int s = 0; s < NSEG; ++s) M = fmaxf(M, red[((size_t)s * NQ + q) * (dh + 2) + dh]);
     float L = 0.f, O = 0.f;
     for (int s = 0; s < NSEG; ++s) {
-      const float* src = red + ((size_t)s * M2R2_MAXQ + q) * (dh + 2);
+      const float* src = red + ((size_t)s * NQ + q) * (dh + 2);
       float ls = src[dh + 1];
       if (ls > 0.f) {
         float w = __expf(src[dh] - M);
@@ -446,30 +454,40 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
   }
 }
 
-void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups) {
+template <typename KT, int SEG>
+static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq) {
+  const int nseg = 4 * (32 / SEG);
+#define ATTN_CASE(NQ)                                                                          \
+  {                                                                                            \
+    static bool attr_set = false;                                                              \
+    if (!attr_set) {                                                                           \
+      cudaFuncSetAttribute(attn_kernel<KT, SEG, NQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024); \
+      attr_set = true;                                                                         \
+    }                                                                                          \
+    size_t sh = ((size_t)NQ * a.dh + (size_t)nseg * NQ * (a.dh + 2)) * sizeof(float);          \
+    attn_kernel<KT, SEG, NQ><<<grid, 128, sh, st>>>(a);                                        \
+  }
+  if (nq <= 2) ATTN_CASE(2) else if (nq <= 4) ATTN_CASE(4) else ATTN_CASE(8)
+#undef ATTN_CASE
+}
+
+// rows_per_group: live query rows of a group (<= M2R2_MAXQ), packed from slot 0 of grp_rows
+void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group) {
   dim3 grid(a.n_heads, n_groups, a.n_splits);
   int epl = dtype == M2R2_FP32 ? 4 : 8;
   int lpp = a.dh / epl;
   int seg = lpp <= 4 ? 4 : lpp <= 8 ? 8 : lpp <= 16 ? 16 : 32;
-  int nseg = 4 * (32 / seg);
-  size_t sh = ((size_t)M2R2_MAXQ * a.dh + (size_t)nseg * M2R2_MAXQ * (a.dh + 2)) * sizeof(float);
-#define ATTN_CASE(KT, S)                                                                       \
-  {                                                                                            \
-    static bool attr_set = false;                                                              \
-    if (!attr_set) {                                                                           \
-      cudaFuncSetAttribute(attn_kernel<KT, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024); \
-      attr_set = true;                                                                         \
-    }                                                                                          \
-    attn_kernel<KT, S><<<grid, 128, sh, st>>>(a);                                              \
-  }
   if (dtype == M2R2_FP32) {
-    if (seg == 4) ATTN_CASE(float, 4) else if (seg == 8) ATTN_CASE(float, 8)
-    else if (seg == 16) ATTN_CASE(float, 16) else ATTN_CASE(float, 32)
+    if (seg == 4) launch_attn_nq<float, 4>(st, a, grid, rows_per_group);
+    else if (seg == 8) launch_attn_nq<float, 8>(st, a, grid, rows_per_group);
+    else if (seg == 16) launch_attn_nq<float, 16>(st, a, grid, rows_per_group);
+    else launch_attn_nq<float, 32>(st, a, grid, rows_per_group);
   } else {
-    if (seg == 4) ATTN_CASE(__nv_bfloat16, 4) else if (seg == 8) ATTN_CASE(__nv_bfloat16, 8)
-    else if (seg == 16) ATTN_CASE(__nv_bfloat16, 16) else ATTN_CASE(__nv_bfloat16, 32)
+    if (seg == 4) launch_attn_nq<__nv_bfloat16, 4>(st, a, grid, rows_per_group);
+    else if (seg == 8) launch_attn_nq<__nv_bfloat16, 8>(st, a, grid, rows_per_group);
+    else if (seg == 16) launch_attn_nq<__nv_bfloat16, 16>(st, a, grid, rows_per_group);
+    else launch_attn_nq<__nv_bfloat16, 32>(st, a, grid, rows_per_group);
   }
-#undef ATTN_CASE
 }
 
 // merge of the split partials; accelerated rows add their own (k^_t, v^_t) as one more key:

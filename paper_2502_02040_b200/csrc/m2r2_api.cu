@@ -677,7 +677,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   const bool any_accel = dual && p.accel && c.accel_enabled && c.accel_end_layer > 0;
   // slow-stream rows only, at most 8 of them, bf16 dense model with the fragment-major copy bound: the skinny
   // tensor-core GEMM (kernels_fused.cu) reads each weight once for all rows (a11)
-  const bool mma_rows = !dual && ns <= 8 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
+  const bool mma_rows = !dual && ns <= 64 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
   float* tr0 = p.trace ? x->trace : nullptr;
   launch_embed(x->cs, c.dtype, x->embed, x->d_row_tok, ns, d, x->resid, any_accel ? x->resid + (size_t)ns * d : nullptr,
                tr0, (tr0 && dual) ? tr0 + (size_t)B * d : nullptr);
@@ -719,7 +719,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       a.slow_rows = ns;
       memset(a.accel_head_mask, 0, sizeof(a.accel_head_mask));
     }
-    launch_attn(x->cs, c.dtype, a, B);
+    launch_attn(x->cs, c.dtype, a, B, dual ? 2 : p.m);
     MergeArgs mg;
     memset(&mg, 0, sizeof(mg));
     mg.qkv = x->qkv; mg.part_o = x->part_o; mg.part_ml = x->part_ml; mg.row_limit = x->d_row_limit; mg.out = x->attn_o;
@@ -786,7 +786,7 @@ static int final_head(m2r2_ctx* x, int ns, int* tok_out, int tok_stride) {
   GemvArgs g;
   memset(&g, 0, sizeof(g));
   g.W = x->lm_head; g.X = x->xn; g.ldx = d; g.n_rows = ns; g.K = d; g.n_out = V; g.out = x->logits; g.ldo = V;
-  const bool mma_rows = ns <= 8 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
+  const bool mma_rows = ns <= 64 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
   if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, 0, 4, x->xn, d, ns, x->logits, V, nullptr, nullptr)) launch_gemv(x->cs, c.dtype, g, false);
   launch_argmax(x->cs, x->logits, V, ns, V, x->d_row_seq, x->d_row_pos, x->ls_on ? x->d_ls_full : nullptr,
                 x->ls_first, x->ls_n, x->ls_beta, tok_out, tok_stride);
@@ -1184,7 +1184,7 @@ static int moe_prefill(m2r2_ctx* x, int P) {
       a.qkv = x->qkv; a.Kc = Kc; a.Vc = Vc; a.row_seq = x->d_row_seq; a.row_limit = x->d_row_limit; a.grp_rows = x->d_grp_rows;
       a.part_o = x->part_o; a.part_ml = x->part_ml; a.n_heads = nh; a.dh = dh; a.d = d; a.max_seq = c.max_seq; a.n_splits = splits;
       a.slow_rows = 1 << 30; a.scale = scale;
-      launch_attn(x->cs, c.dtype, a, 1);
+      launch_attn(x->cs, c.dtype, a, 1, m);
       MergeArgs mg;
       memset(&mg, 0, sizeof(mg));
       mg.qkv = x->qkv; mg.part_o = x->part_o; mg.part_ml = x->part_ml; mg.row_limit = x->d_row_limit; mg.out = x->attn_o;

@@ -134,7 +134,7 @@ void launch_gemv(cudaStream_t st, int dtype, const GemvArgs& a, bool swiglu);
 void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int slow_rows, const int* row_seq,
                         const int* row_pos, const float2* rope_tab, void* Kc, void* Vc, int n_heads,
                         int dh, int max_seq);
-void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups);
+void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group);
 void launch_merge(cudaStream_t st, const MergeArgs& a, int rows);
 void launch_argmax(cudaStream_t st, const float* logits, int ldl, int rows, int V, const int* row_seq,
                    const int* row_pos, const int* script, int script_first, int script_n, float beta,
