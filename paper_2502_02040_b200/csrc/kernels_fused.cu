@@ -1678,6 +1678,11 @@ struct VArgs {
   int ldx, ldo, rows, K, n_out, nkt, nstage_k, split, d, dh;
   int ksplit;            // O / DOWN: CTAs per row tile along K; > 1 adds into out (= resid, in place) atomically
   int n_rt;              // row tiles of the matrix (rows_mma_kernel)
+  // parallel adapters of the accelerated rows (rows_mma_kernel): rows >= lora_row0 get + B[bmap(n)] . U[row][usel * r ..)
+  const bf16 *Bm, *Bm2;  // Bm2: the up projection's B (gate/up)
+  const int* bmap;       // nullable -> identity; -1 = no adapter row for this output
+  const float* U;
+  int ldu, r, lora_row0, usel_div;
 };
 __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -1830,23 +1835,41 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
     for (int s = 0; s < 2; ++s) {
       const int n = gi * 8 + 2 * t + s;
       if (n >= a.rows) continue;
-      const float v0 = c[gi][s], v1 = c[gi][2 + s];
+      float v0 = c[gi][s], v1 = c[gi][2 + s];
+      const bool lora = a.Bm != nullptr && n >= a.lora_row0 && blockIdx.y == 0;   // + B (A x^) on accelerated rows
+      const float* urow = a.U + (size_t)n * a.ldu;
       if (KIND == VK_GATEUP) {
         const int o = rt * 8 + g;
-        if (o < a.n_out) a.out[(size_t)n * a.ldo + o] = silu(v0) * v1;
+        if (o < a.n_out) {
+          if (lora) {
+            for (int q = 0; q < a.r; ++q) {
+              v0 += bf(a.Bm + (size_t)o * a.r + q) * urow[q];
+              v1 += bf(a.Bm2 + (size_t)o * a.r + q) * urow[a.r + q];
+            }
+          }
+          a.out[(size_t)n * a.ldo + o] = silu(v0) * v1;
+        }
         continue;
       }
 #pragma unroll
       for (int hh = 0; hh < 2; ++hh) {
         const int pr = rt * 16 + g + 8 * hh;
-        const float v = hh ? v1 : v0;
+        float v = hh ? v1 : v0;
         if (pr >= a.n_out) continue;
+        int nat = pr;
         if (KIND == VK_QKV) {
           const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
-          const int nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
+          nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
+        }
+        if (lora) {
+          const int bn = a.bmap ? a.bmap[nat] : nat;
+          if (bn >= 0) {
+            const float* u = urow + (a.usel_div ? nat / a.usel_div : 0) * a.r;
+            for (int q = 0; q < a.r; ++q) v += bf(a.Bm + (size_t)bn * a.r + q) * u[q];
+          }
+        }
+        if (KIND == VK_QKV || KIND == VK_HEAD) {
           a.out[(size_t)n * a.ldo + nat] = v;
-        } else if (KIND == VK_HEAD) {
-          a.out[(size_t)n * a.ldo + pr] = v;
         } else if (a.ksplit > 1) {
           atomicAdd(a.out + (size_t)n * a.ldo + pr, v);   // out == resid (in place)
         } else {
@@ -2208,8 +2231,9 @@ static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) 
 }
 
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
-                    int rows, float* out, int ldo, const float* resid, float* trace) {
+                    int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora) {
   if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 64 || (c.d_model % 4) || (c.d_ff % 4)) return M2R2_UNSUPPORTED;
+  if (lora && rows <= 8) return M2R2_UNSUPPORTED;   // gemv_mma_kernel carries no adapters
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
   VArgs a;
@@ -2227,6 +2251,10 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     default:        a.W = im->h_Wlm; a.K = c.d_model; a.n_out = c.vocab; a.nkt = q.d_pad / 16; a.nstage_k = q.d_pad / STAGE_K; a.split = 0; n_rt = q.rt_v; break;
   }
   a.n_rt = n_rt;
+  if (lora && lora->Bm) {
+    a.Bm = (const bf16*)lora->Bm; a.Bm2 = (const bf16*)lora->Bm2; a.bmap = lora->bmap; a.U = lora->U;
+    a.ldu = lora->ldu; a.r = lora->r; a.lora_row0 = lora->lora_row0; a.usel_div = lora->usel_div;
+  }
   if (rows > 8) {
     // 9..64 rows: rows_mma_kernel, 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual)
     const int ng = (rows + 7) / 8, gx = (n_rt + 3) / 4, nch = (a.nkt + 15) / 16;

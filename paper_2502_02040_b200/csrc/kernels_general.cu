@@ -315,8 +315,24 @@ void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int sl
 // SEG = next power of two >= LPP lanes form a segment; a warp handles 32/SEG positions at once.
 // =====================================================================================
 template <typename KT> struct KVec;
-template <> struct KVec<__nv_bfloat16> { static constexpr int EPL = 8; };
-template <> struct KVec<float> { static constexpr int EPL = 4; };
+template <> struct KVec<__nv_bfloat16> {
+  static constexpr int EPL = 8;
+  typedef uint4 Raw;
+  static __device__ __forceinline__ Raw zero() { return make_uint4(0u, 0u, 0u, 0u); }
+  static __device__ __forceinline__ void unpack(const Raw& u, float out[8]) {
+    bf16x2_to_f32(u.x, out[0], out[1]); bf16x2_to_f32(u.y, out[2], out[3]);
+    bf16x2_to_f32(u.z, out[4], out[5]); bf16x2_to_f32(u.w, out[6], out[7]);
+  }
+};
+template <> struct KVec<float> {
+  static constexpr int EPL = 4;
+  typedef float4 Raw;
+  static __device__ __forceinline__ Raw zero() { return make_float4(0.f, 0.f, 0.f, 0.f); }
+  static __device__ __forceinline__ void unpack(const Raw& u, float out[8]) {
+    out[0] = u.x; out[1] = u.y; out[2] = u.z; out[3] = u.w;
+    out[4] = out[5] = out[6] = out[7] = 0.f;
+  }
+};
 
 template <typename KT>
 __device__ __forceinline__ void load_kv(const KT* p, float out[8]);
@@ -338,7 +354,7 @@ __device__ __forceinline__ void load_kv<float>(const float* p, float out[8]) {
 // NQ = query rows compiled in (the group's live rows are packed from slot 0); UN positions per segment are
 // loaded before any is used, so a warp keeps 2 * UN 16-byte loads per lane in flight (the K/V stream is the bound).
 template <typename KT, int SEG, int NQ>
-__global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
+__global__ void __launch_bounds__(128, NQ <= 5 ? 4 : 3) attn_kernel(AttnArgs a) {
   constexpr int EPL = KVec<KT>::EPL;
   constexpr int NSEG = 4 * (32 / SEG);           // segments per CTA
   constexpr int UN = 4;
@@ -378,36 +394,46 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
 
   const int seg = lane / SEG, sl = lane % SEG;   // segment in warp, lane in segment
   const bool active = sl < lpp;
-  float m[NQ], l[NQ], o[NQ][EPL], qr[NQ][EPL];
+  float m[NQ], l[NQ], o[NQ][EPL];
   int lim[NQ];
 #pragma unroll
   for (int q = 0; q < NQ; ++q) {
     m[q] = -INFINITY; l[q] = 0.f; lim[q] = s_lim[q];
 #pragma unroll
-    for (int e = 0; e < EPL; ++e) { o[q][e] = 0.f; qr[q][e] = active ? qs[q * dh + sl * EPL + e] : 0.f; }
+    for (int e = 0; e < EPL; ++e) o[q][e] = 0.f;
   }
+  // the lane's slice of every query stays in shared memory (broadcast reads): registers hold the running
+  // outputs and the raw K/V loads in flight, so that several CTAs fit an SM
+  const float* ql = qs + (active ? sl * EPL : 0);
   constexpr int PPW = 32 / SEG;
+  typedef typename KVec<KT>::Raw Raw;
   for (int ub = u0 + warp * PPW; ub < u1; ub += 4 * PPW * UN) {
-    float kv[UN][8], vv[UN][8];
+    Raw kraw[UN], vraw[UN];
 #pragma unroll
     for (int i = 0; i < UN; ++i) {
       const int u = ub + i * 4 * PPW + seg;
-#pragma unroll
-      for (int e = 0; e < 8; ++e) { kv[i][e] = 0.f; vv[i][e] = 0.f; }
+      kraw[i] = KVec<KT>::zero(); vraw[i] = kraw[i];
       if (u < u1 && active) {
-        load_kv<KT>(Kb + (size_t)u * dh + sl * EPL, kv[i]);
-        load_kv<KT>(Vb + (size_t)u * dh + sl * EPL, vv[i]);
+        kraw[i] = *(const Raw*)(Kb + (size_t)u * dh + sl * EPL);
+        vraw[i] = *(const Raw*)(Vb + (size_t)u * dh + sl * EPL);
       }
     }
 #pragma unroll
     for (int i = 0; i < UN; ++i) {
       const int u = ub + i * 4 * PPW + seg;
       const bool valid = u < u1;
+      float kv[8], vv[8];
+      KVec<KT>::unpack(kraw[i], kv);
+      KVec<KT>::unpack(vraw[i], vv);
 #pragma unroll
       for (int q = 0; q < NQ; ++q) {
         float s = 0.f;
 #pragma unroll
-        for (int e = 0; e < EPL; ++e) s += qr[q][e] * kv[i][e];
+        for (int e = 0; e < EPL; e += 4) {
+          const float4 qv = *(const float4*)(ql + q * dh + e);
+          s += qv.x * kv[e] + qv.y * kv[e + 1] + qv.z * kv[e + 2] + qv.w * kv[e + 3];
+        }
+        if (!active) s = 0.f;
 #pragma unroll
         for (int off = SEG / 2; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
         if (valid && u < lim[q]) {
@@ -415,7 +441,7 @@ __global__ void __launch_bounds__(128) attn_kernel(AttnArgs a) {
           float corr = __expf(m[q] - mn), p = __expf(s - mn);
           l[q] = l[q] * corr + p;
 #pragma unroll
-          for (int e = 0; e < EPL; ++e) o[q][e] = o[q][e] * corr + p * vv[i][e];
+          for (int e = 0; e < EPL; ++e) o[q][e] = o[q][e] * corr + p * vv[e];
           m[q] = mn;
         }
       }
@@ -467,7 +493,7 @@ static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq
     size_t sh = ((size_t)NQ * a.dh + (size_t)nseg * NQ * (a.dh + 2)) * sizeof(float);          \
     attn_kernel<KT, SEG, NQ><<<grid, 128, sh, st>>>(a);                                        \
   }
-  if (nq <= 2) ATTN_CASE(2) else if (nq <= 4) ATTN_CASE(4) else ATTN_CASE(8)
+  if (nq <= 2) ATTN_CASE(2) else if (nq <= 4) ATTN_CASE(4) else if (nq <= 5) ATTN_CASE(5) else if (nq <= 6) ATTN_CASE(6) else ATTN_CASE(8)
 #undef ATTN_CASE
 }
 

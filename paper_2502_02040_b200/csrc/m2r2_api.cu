@@ -677,7 +677,8 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   const bool any_accel = dual && p.accel && c.accel_enabled && c.accel_end_layer > 0;
   // slow-stream rows only, at most 8 of them, bf16 dense model with the fragment-major copy bound: the skinny
   // tensor-core GEMM (kernels_fused.cu) reads each weight once for all rows (a11)
-  const bool mma_rows = !dual && ns <= 64 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
+  // (dual passes at batch >= 5 have 9..32 rows: the same kernel carries the accelerated rows' adapters)
+  const bool mma_rows = ((!dual && ns <= 64) || (dual && 2 * B > 8 && 2 * B <= 64)) && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
   float* tr0 = p.trace ? x->trace : nullptr;
   launch_embed(x->cs, c.dtype, x->embed, x->d_row_tok, ns, d, x->resid, any_accel ? x->resid + (size_t)ns * d : nullptr,
                tr0, (tr0 && dual) ? tr0 + (size_t)B * d : nullptr);
@@ -701,7 +702,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     memset(&g, 0, sizeof(g));
     g.W = L.wqkv; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = 3 * d; g.out = x->qkv; g.ldo = 3 * d;
     if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
-    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
     // a3: RoPE + KV append
     prof_mark(x, M2R2_PROF_ROPE);
     launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
@@ -734,7 +735,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     memset(&g, 0, sizeof(g));
     g.W = L.wo; g.X = x->attn_o; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
     if (acc_on) { g.Bm = L.Bo; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
     count(x);
     float* trl = p.trace ? x->trace + (size_t)(i + 1) * 2 * B * d : nullptr;
     if (!c.n_experts) {
@@ -744,14 +745,14 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       memset(&g, 0, sizeof(g));
       g.W = L.wgate; g.W2 = L.wup; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = c.d_ff; g.out = x->act; g.ldo = c.d_ff;
       if (acc_on) { g.Bm = L.Bg; g.Bm2 = L.Bu; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr)) launch_gemv(x->cs, c.dtype, g, true);
+      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, true);
       prof_mark(x, M2R2_PROF_DOWN);
       if (acc_on) { launch_lora_down(x->cs, c.dtype, x->act, c.d_ff, ns, na, c.d_ff, nullptr, L.Ad, r, x->U, 64); count(x); }
       memset(&g, 0, sizeof(g));
       g.W = L.wdown; g.X = x->act; g.ldx = c.d_ff; g.n_rows = rows; g.K = c.d_ff; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
       g.trace = trl;
       if (acc_on) { g.Bm = L.Bd; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl)) launch_gemv(x->cs, c.dtype, g, false);
+      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
       count(x, 3);
     } else {
       int rc = moe_mlp(x, p, i, ns, na);

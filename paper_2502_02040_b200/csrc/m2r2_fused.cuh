@@ -47,6 +47,8 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n);
 bool fused_abort_pending(const FusedState* fs);
 // a11: skinny GEMM of <= 8 slow-stream rows on the fragment-major weights (verify pass, prefill chunks).
 // kind: 0 QKV (natural row order out), 1 O-proj (+resid), 2 gate/up + SwiGLU, 3 down (+resid, trace), 4 LM head.
-// Returns M2R2_UNSUPPORTED when the fused weight copy is not bound or rows > 8.
+// Returns M2R2_UNSUPPORTED when the fused weight copy is not bound or rows > 64.
+// rows 9..64 (rows_mma_kernel) may carry the accelerated rows' parallel adapters: `lora` supplies Bm / Bm2 / bmap / U /
+// ldu / r / lora_row0 / usel_div with the meaning they have in GemvArgs (nullptr: none).
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
-                    int rows, float* out, int ldo, const float* resid, float* trace);
+                    int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora = nullptr);
