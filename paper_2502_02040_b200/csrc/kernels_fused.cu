@@ -1662,12 +1662,11 @@ __global__ void pack_kernel(uint4* __restrict__ dst, const bf16* __restrict__ sr
   }
 }
 
-// ------------------------------------------------------------------ skinny GEMM on the fragment-major weights (a11)
-// The k-token verify pass (and prefill chunks) multiplies each weight matrix with m <= 8 slow-stream rows.
-// Same fragment-major tiles as the fused kernel, weights as the M operand and the token rows as N: one
-// LDG.128 per lane per tile straight into the A fragment, the rows' bf16 hi + lo parts as two B operands
-// (fp32-class products, as in the fused kernel), fp32 accumulation on the tensor pipe.  One CTA per 16-row
-// tile, its 8 warps split the k-tiles and keep 8 tiles (4 KB per warp) in flight.  HBM-bound: 2 m flop per byte.
+// ------------------------------------------------------------------ skinny GEMM on the fragment-major weights (a11, a18, batched a10)
+// The k-token verify pass, prefill chunks and batched draft passes multiply each weight matrix with 1..64 activation
+// rows.  Same fragment-major tiles as the fused kernel, weights as the M operand and the rows as N of mma.sync.m16n8k16:
+// one LDG.128 per lane per tile straight into the A fragment, the rows' bf16 hi + lo parts as two B operands (fp32-class
+// products, as in the fused kernel), fp32 accumulation on the tensor pipe.  HBM-bound: 2 m flop per byte.
 enum { VK_QKV = 0, VK_OPROJ = 1, VK_GATEUP = 2, VK_DOWN = 3, VK_HEAD = 4 };
 struct VArgs {
   const uint4* W;
@@ -1691,89 +1690,13 @@ __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   lo = bf2_u32(l);
   return bf2_u32(h);
 }
-template <int KIND>
-__global__ void __launch_bounds__(256, 3) gemv_mma_kernel(const VArgs a) {
-  __shared__ float red[8][16][8];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  const int rt = blockIdx.x;
-  float c[4] = {0.f, 0.f, 0.f, 0.f};
-  const float* xrow = a.X + (size_t)g * a.ldx;
-  const bool row_live = g < a.rows;
-  constexpr int UN = 8;
-  const int kt_lo = (int)(((long long)a.nkt * blockIdx.y) / a.ksplit), kt_hi = (int)(((long long)a.nkt * (blockIdx.y + 1)) / a.ksplit);
-  for (int kt0 = kt_lo + warp; kt0 < kt_hi; kt0 += 8 * UN) {
-    uint4 w[UN];
-    float2 x0[UN], x1[UN];
-#pragma unroll
-    for (int u = 0; u < UN; ++u) {
-      const int kt = kt0 + 8 * u;
-      w[u] = make_uint4(0u, 0u, 0u, 0u);
-      x0[u] = make_float2(0.f, 0.f);
-      x1[u] = x0[u];
-      if (kt < kt_hi) {
-        const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
-                                    : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
-        w[u] = ldg_stream(a.W + tile * 32 + lane);
-        const int k = kt * 16 + 2 * t;
-        if (row_live && k < a.K) x0[u] = __ldg((const float2*)(xrow + k));
-        if (row_live && k + 8 < a.K) x1[u] = __ldg((const float2*)(xrow + k + 8));
-      }
-    }
-#pragma unroll
-    for (int u = 0; u < UN; ++u) {
-      uint32_t l0, l1;
-      const uint32_t h0 = pack_hi_lo(x0[u].x, x0[u].y, l0), h1 = pack_hi_lo(x1[u].x, x1[u].y, l1);
-      mma_bf16(c, w[u], h0, h1);
-      mma_bf16(c, w[u], l0, l1);
-    }
-  }
-  red[warp][g][2 * t] = c[0]; red[warp][g][2 * t + 1] = c[1];
-  red[warp][g + 8][2 * t] = c[2]; red[warp][g + 8][2 * t + 1] = c[3];
-  __syncthreads();
-  if (tid < 128) {
-    const int r = tid >> 3, n = tid & 7;
-    if (n < a.rows) {
-      float v = 0.f;
-#pragma unroll
-      for (int w8 = 0; w8 < 8; ++w8) v += red[w8][r][n];
-      const int pr = rt * 16 + r;
-      if (KIND == VK_QKV) {
-        if (pr < a.n_out) {
-          const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
-          const int nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
-          a.out[(size_t)n * a.ldo + nat] = v;
-        }
-      } else if (KIND == VK_GATEUP) {
-        if (r < 8) {
-          float up = 0.f;
-#pragma unroll
-          for (int w8 = 0; w8 < 8; ++w8) up += red[w8][r + 8][n];
-          const int o = rt * 8 + r;
-          if (o < a.n_out) a.out[(size_t)n * a.ldo + o] = silu(v) * up;
-        }
-      } else if (KIND == VK_HEAD) {
-        if (pr < a.n_out) a.out[(size_t)n * a.ldo + pr] = v;
-      } else {
-        if (pr < a.n_out) {
-          if (a.ksplit > 1) {
-            atomicAdd(a.out + (size_t)n * a.ldo + pr, v);   // out == resid (in place): the partial sums land on it
-          } else {
-            const float o = a.resid[(size_t)n * a.ldo + pr] + v;
-            a.out[(size_t)n * a.ldo + pr] = o;
-            if (a.trace) a.trace[(size_t)n * a.ldo + pr] = o;
-          }
-        }
-      }
-    }
-  }
-}
-
-// ------------------------------------------------------------------ skinny GEMM for 9..64 slow-stream rows (a11 at batch > 1, prefill chunks)
-// Same fragment-major weights.  A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows
-// of a 256-input chunk are staged ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row
-// tiles, so every weight is read from HBM once for all rows (the fp32-FMA kernel reads it once per 8 rows) and the
-// replicated activation traffic from L2 stays near the weight traffic.  NG groups of 8 rows = NG n8 MMA tiles (x2:
-// hi, lo) per weight tile, fp32 accumulators; epilogues as in gemv_mma_kernel.
+// A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows of a 256-input chunk are staged
+// ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row tiles, so every weight is read from HBM
+// once for all rows and the replicated activation traffic from L2 stays near the weight traffic; each warp keeps the
+// chunk's 16 weight tiles (8 KB) in flight while the rows are staged.  NG groups of 8 rows = NG n8 MMA tiles (x2: hi, lo)
+// per weight tile.  Epilogues: QKV undoes the RoPE row permutation of the packed matrix, gate/up applies SwiGLU on the
+// lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
+// writes logits; accelerated rows add their parallel adapter term B u.
 constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
 constexpr int RM_LD = RM_KC + 8;         // bf16 elements per staged row (+8: bank spread)
 template <int KIND, int NG>
@@ -2226,14 +2149,13 @@ static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) 
     }                                                                                                 \
     rows_mma_kernel<KIND, NG><<<grid, 128, sh, st>>>(a);                                              \
   } break;
-  switch (ng) { RM_CASE(2) RM_CASE(3) RM_CASE(4) RM_CASE(5) RM_CASE(6) RM_CASE(7) RM_CASE(8) default: break; }
+  switch (ng) { RM_CASE(1) RM_CASE(2) RM_CASE(3) RM_CASE(4) RM_CASE(5) RM_CASE(6) RM_CASE(7) RM_CASE(8) default: break; }
 #undef RM_CASE
 }
 
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
                     int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora) {
   if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 64 || (c.d_model % 4) || (c.d_ff % 4)) return M2R2_UNSUPPORTED;
-  if (lora && rows <= 8) return M2R2_UNSUPPORTED;   // gemv_mma_kernel carries no adapters
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
   VArgs a;
@@ -2255,8 +2177,8 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     a.Bm = (const bf16*)lora->Bm; a.Bm2 = (const bf16*)lora->Bm2; a.bmap = lora->bmap; a.U = lora->U;
     a.ldu = lora->ldu; a.r = lora->r; a.lora_row0 = lora->lora_row0; a.usel_div = lora->usel_div;
   }
-  if (rows > 8) {
-    // 9..64 rows: rows_mma_kernel, 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual)
+  {
+    // 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual) so that every SM streams
     const int ng = (rows + 7) / 8, gx = (n_rt + 3) / 4, nch = (a.nkt + 15) / 16;
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
       const int want = (4 * im->G + gx - 1) / gx;
@@ -2270,20 +2192,6 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
       case VK_DOWN:   launch_rows_mma<VK_DOWN>(a, grid, ng, st); break;
       default:        launch_rows_mma<VK_HEAD>(a, grid, ng, st); break;
     }
-    return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
-  }
-  // O / down have few row tiles (d / 16): several CTAs share one along K so that every SM streams (3 CTAs fit an SM)
-  if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
-    const int want = (3 * im->G + n_rt - 1) / n_rt;
-    a.ksplit = std::max(1, std::min(want, a.nkt / 64));
-  }
-  const dim3 grid(n_rt, a.ksplit);
-  switch (kind) {
-    case VK_QKV:    gemv_mma_kernel<VK_QKV><<<grid, 256, 0, st>>>(a); break;
-    case VK_OPROJ:  gemv_mma_kernel<VK_OPROJ><<<grid, 256, 0, st>>>(a); break;
-    case VK_GATEUP: gemv_mma_kernel<VK_GATEUP><<<grid, 256, 0, st>>>(a); break;
-    case VK_DOWN:   gemv_mma_kernel<VK_DOWN><<<grid, 256, 0, st>>>(a); break;
-    default:        gemv_mma_kernel<VK_HEAD><<<grid, 256, 0, st>>>(a); break;
   }
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }

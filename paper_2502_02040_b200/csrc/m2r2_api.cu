@@ -621,7 +621,7 @@ static int prefetch_pairs(m2r2_ctx* x, const int* pairs, int n) {
 // ------------------------------------------------------------------ forward pass (per-operation kernels)
 static int n_splits_for(const m2r2_ctx* x, int groups, int max_len) {
   int want = (4 * x->sm_count + x->c.n_heads * groups - 1) / (x->c.n_heads * groups);
-  int cap = std::max(1, (max_len + 31) / 32);
+  int cap = std::max(1, (max_len + 127) / 128);   // >= 128 positions per split: shorter items are all prologue and merge
   return std::max(1, std::min(std::min(want, cap), M2R2_MAX_SPLITS));
 }
 

@@ -14,9 +14,12 @@ from tests.refs import rel_l2
 # Two CUDA implementations of the same step (persistent fused kernel vs per-operation kernels) are
 # cross-checked on bf16 models.  The fused kernel feeds activations to the tensor pipe as bf16
 # hi + lo pairs (relative error <= 2^-17 per element), the
-# per-operation kernels use fp32 activations, so they agree to a few 1e-5, not to fp32 rounding.
+# per-operation kernels use fp32 activations, so they agree to a few 1e-5, not to fp32 rounding.  Two RUNS of the
+# same implementation differ as well: split-K partial sums are added onto the residual with fp32 atomics in launch
+# order (1e-7), and where such a difference crosses a bf16 rounding boundary of a cached K/V element that element
+# moves by 2^-9; over a few layers the logits of two engines agree to 1-2e-4 (observed), so the bound is 5e-4.
 # (Oracle parity keeps BASELINE.json's tolerances; this constant is not used there.)
-XIMPL_TOL = 1e-4
+XIMPL_TOL = 5e-4
 
 pytestmark = pytest.mark.gpu
 
@@ -640,6 +643,6 @@ def test_results_do_not_depend_on_uninitialised_device_memory(fused, monkeypatch
                     for s in range(len(toks)):
                         assert np.all(np.isfinite(out[s])), (plen, which, mode, s)
                         if fused:
-                            assert rel_l2(out[s], ref[s]) <= 1e-4, (plen, which, mode, s, rel_l2(out[s], ref[s]))
+                            assert rel_l2(out[s], ref[s]) <= XIMPL_TOL, (plen, which, mode, s, rel_l2(out[s], ref[s]))
                         else:
                             assert np.array_equal(out[s], ref[s]), (plen, which, mode, s)
