@@ -424,8 +424,8 @@ def run_secondary(args):
         cfg = S.config_c3()
         eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
         prompt = S.gen_prompt(cfg, PROMPT)
-        for alpha in (0.9, 0.5):
-            for gamma in (2, 4, 6):
+        for alpha in ((args.alpha,) if args.alpha else (0.9, 0.5)):
+            for gamma in ((args.gamma,) if args.gamma else (2, 4, 6)):
                 f, g = S.gen_logit_script(cfg, 400, alpha)
                 eng.set_logit_script(f, g, PROMPT)
                 eng.prefill(prompt)
@@ -433,14 +433,16 @@ def run_secondary(args):
                     eng.spec_step(gamma)
                 eng.prefill(prompt)
                 torch.cuda.synchronize()
+                torch.cuda.profiler.start()     # `ncu --profile-from-start off` captures the timed region only
                 t0, emitted, steps, by = time.perf_counter(), 1, 0, 0
-                while emitted < 256:
+                while emitted < args.tokens:
                     _, n = eng.spec_step(gamma)
                     emitted += int(n[0])
                     steps += 1
                     by += eng.get_stats()["algorithmic_bytes_last"]
                 torch.cuda.synchronize()
                 dt = time.perf_counter() - t0
+                torch.cuda.profiler.stop()
                 out["runs"].append({"alpha": alpha, "gamma": gamma, "tokens": emitted - 1, "spec_steps": steps,
                                     "ms_per_spec_step": 1e3 * dt / steps, "tokens_per_s": (emitted - 1) / dt,
                                     "tokens_per_spec_step": (emitted - 1) / steps, "algorithmic_GB_per_s": by / dt / 1e9})
@@ -523,6 +525,9 @@ def main():
     ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"],
                     help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gamma", type=int, default=0, help="--workload c3: one draft length instead of 2, 4, 6")
+    ap.add_argument("--alpha", type=float, default=0.0, help="--workload c3: one acceptance rate instead of 0.9, 0.5")
+    ap.add_argument("--tokens", type=int, default=256, help="--workload c3: tokens to generate per run")
     ap.add_argument("--no-selfspec", action="store_true", help="skip the C3 self-speculative sub-record of the bench line")
     ap.add_argument("--traffic", type=float, default=FUSED_TRAFFIC_BYTES,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")

@@ -1698,29 +1698,34 @@ __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
 // lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
 // writes logits; accelerated rows add their parallel adapter term B u.
 constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
-constexpr int RM_LD = RM_KC + 8;         // bf16 elements per staged row (+8: bank spread)
-template <int KIND, int NG>
+// SW (NG <= 2): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
+// takes its w-th quarter) and their sums meet in shared memory: four times the CTAs for matrices with few row tiles.
+template <int KIND, int NG, bool SW>
 __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
+  constexpr int NQ = SW ? 4 : 1;                   // 256-input chunks staged per iteration
+  constexpr int LD = NQ * RM_KC + 8;               // bf16 elements per staged row (+8: bank spread)
   extern __shared__ __align__(16) unsigned char rm_smem[];
-  bf16* xh = (bf16*)rm_smem;                       // [NG * 8][RM_LD] hi parts
-  bf16* xl = xh + (size_t)NG * 8 * RM_LD;          // lo parts
+  bf16* xh = (bf16*)rm_smem;                       // [NG * 8][LD] hi parts
+  bf16* xl = xh + (size_t)NG * 8 * LD;             // lo parts
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  const int rt = blockIdx.x * 4 + warp;
+  const int rt = SW ? blockIdx.x : blockIdx.x * 4 + warp;
   const bool mine = rt < a.n_rt;
   float c[NG][4];
 #pragma unroll
   for (int i = 0; i < NG; ++i)
 #pragma unroll
     for (int e = 0; e < 4; ++e) c[i][e] = 0.f;
-  const int nch = (a.nkt + 15) / 16;               // chunks of the whole K
+  const int nch = (a.nkt + 16 * NQ - 1) / (16 * NQ);   // (super-)chunks of the whole K
   const int ch_lo = (int)(((long long)nch * blockIdx.y) / a.ksplit), ch_hi = (int)(((long long)nch * (blockIdx.y + 1)) / a.ksplit);
+  const int wq = SW ? warp : 0;                    // the warp's quarter of the staged inputs
   for (int ch = ch_lo; ch < ch_hi; ++ch) {
-    const int kbase = ch * RM_KC;
-    // weights of the chunk for this warp's row tile: 16 LDG.128 per lane in flight while the activations are staged
+    const int kbase = ch * NQ * RM_KC;
+    // the warp's 16 weight tiles of this iteration: 16 LDG.128 per lane in flight while the activations are staged
+    // (requesting the next iteration's tiles before the MMAs as well costs 60 registers and an SM's third CTA: slower)
     uint4 w[16];
 #pragma unroll
     for (int u = 0; u < 16; ++u) {
-      const int kt = ch * 16 + u;
+      const int kt = (ch * NQ + wq) * 16 + u;
       w[u] = make_uint4(0u, 0u, 0u, 0u);
       if (mine && kt < a.nkt) {
         const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
@@ -1728,27 +1733,46 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
         w[u] = ldg_stream(a.W + tile * 32 + lane);
       }
     }
-    __syncthreads();   // the previous chunk's staged rows are consumed
-    for (int i = tid; i < NG * 8 * (RM_KC / 4); i += 128) {
-      const int row = i / (RM_KC / 4), q = i - row * (RM_KC / 4), k = kbase + 4 * q;
+    __syncthreads();   // the previous iteration's staged rows are consumed
+    for (int i = tid; i < NG * 8 * (NQ * RM_KC / 4); i += 128) {
+      const int row = i / (NQ * RM_KC / 4), q = i - row * (NQ * RM_KC / 4), k = kbase + 4 * q;
       float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
       if (row < a.rows && k < a.K) v = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));   // K % 4 == 0
       uint32_t l0, l1;
       const uint32_t h0 = pack_hi_lo(v.x, v.y, l0), h1 = pack_hi_lo(v.z, v.w, l1);
-      *(uint2*)(xh + (size_t)row * RM_LD + 4 * q) = make_uint2(h0, h1);
-      *(uint2*)(xl + (size_t)row * RM_LD + 4 * q) = make_uint2(l0, l1);
+      *(uint2*)(xh + (size_t)row * LD + 4 * q) = make_uint2(h0, h1);
+      *(uint2*)(xl + (size_t)row * LD + 4 * q) = make_uint2(l0, l1);
     }
     __syncthreads();
 #pragma unroll
     for (int u = 0; u < 16; ++u) {
 #pragma unroll
       for (int gi = 0; gi < NG; ++gi) {
-        const bf16* ph = xh + (size_t)(gi * 8 + g) * RM_LD + u * 16 + 2 * t;
-        const bf16* pl = xl + (size_t)(gi * 8 + g) * RM_LD + u * 16 + 2 * t;
+        const bf16* ph = xh + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
+        const bf16* pl = xl + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
         mma_bf16(c[gi], w[u], *(const uint32_t*)ph, *(const uint32_t*)(ph + 8));
         mma_bf16(c[gi], w[u], *(const uint32_t*)pl, *(const uint32_t*)(pl + 8));
       }
     }
+  }
+  if (SW) {
+    // the four warps' partial sums of the row tile -> warp 0
+    __syncthreads();
+    float* red = (float*)rm_smem;                  // [3][NG * 4][32]
+    if (warp > 0) {
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) red[((warp - 1) * NG * 4 + gi * 4 + e) * 32 + lane] = c[gi][e];
+    }
+    __syncthreads();
+    if (warp > 0) return;
+#pragma unroll
+    for (int ww = 0; ww < 3; ++ww)
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) c[gi][e] += red[(ww * NG * 4 + gi * 4 + e) * 32 + lane];
   }
   if (!mine) return;
   // c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2], c[gi][3] = weight row g + 8
@@ -2137,20 +2161,28 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
 
 // a11 on the fragment-major weights: out = f(W x) for rows <= 8 slow-stream rows (kinds: VK_*).  Returns
 // M2R2_UNSUPPORTED when the fused copy is not bound (the caller then uses the row-major kernels).
+template <int KIND, int NG, bool SW>
+static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
+  const size_t sh = (size_t)2 * NG * 8 * ((SW ? 4 : 1) * RM_KC + 8) * sizeof(bf16);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(rows_mma_kernel<KIND, NG, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
+    attr_set = true;
+  }
+  rows_mma_kernel<KIND, NG, SW><<<grid, 128, sh, st>>>(a);
+}
 template <int KIND>
 static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) {
-  const size_t sh = (size_t)2 * ng * 8 * RM_LD * sizeof(bf16);
-#define RM_CASE(NG)                                                                                   \
-  case NG: {                                                                                          \
-    static bool attr_set = false;                                                                     \
-    if (!attr_set) {                                                                                  \
-      cudaFuncSetAttribute(rows_mma_kernel<KIND, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024); \
-      attr_set = true;                                                                                \
-    }                                                                                                 \
-    rows_mma_kernel<KIND, NG><<<grid, 128, sh, st>>>(a);                                              \
-  } break;
-  switch (ng) { RM_CASE(1) RM_CASE(2) RM_CASE(3) RM_CASE(4) RM_CASE(5) RM_CASE(6) RM_CASE(7) RM_CASE(8) default: break; }
-#undef RM_CASE
+  switch (ng) {
+    case 1: launch_rows_mma_t<KIND, 1, true>(a, grid, st); break;
+    case 2: launch_rows_mma_t<KIND, 2, true>(a, grid, st); break;
+    case 3: launch_rows_mma_t<KIND, 3, false>(a, grid, st); break;
+    case 4: launch_rows_mma_t<KIND, 4, false>(a, grid, st); break;
+    case 5: launch_rows_mma_t<KIND, 5, false>(a, grid, st); break;
+    case 6: launch_rows_mma_t<KIND, 6, false>(a, grid, st); break;
+    case 7: launch_rows_mma_t<KIND, 7, false>(a, grid, st); break;
+    default: launch_rows_mma_t<KIND, 8, false>(a, grid, st); break;
+  }
 }
 
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
@@ -2179,7 +2211,9 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   }
   {
     // 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual) so that every SM streams
-    const int ng = (rows + 7) / 8, gx = (n_rt + 3) / 4, nch = (a.nkt + 15) / 16;
+    const int ng = (rows + 7) / 8;
+    const bool sw = ng <= 2;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW)
+    const int gx = sw ? n_rt : (n_rt + 3) / 4, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
       const int want = (4 * im->G + gx - 1) / gx;
       a.ksplit = std::max(1, std::min(want, nch));
