@@ -1698,7 +1698,7 @@ __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
 // lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
 // writes logits; accelerated rows add their parallel adapter term B u.
 constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
-// SW (NG <= 2): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
+// SW (NG == 1): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
 // takes its w-th quarter) and their sums meet in shared memory: four times the CTAs for matrices with few row tiles.
 template <int KIND, int NG, bool SW>
 __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
@@ -2175,7 +2175,7 @@ template <int KIND>
 static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) {
   switch (ng) {
     case 1: launch_rows_mma_t<KIND, 1, true>(a, grid, st); break;
-    case 2: launch_rows_mma_t<KIND, 2, true>(a, grid, st); break;
+    case 2: launch_rows_mma_t<KIND, 2, false>(a, grid, st); break;
     case 3: launch_rows_mma_t<KIND, 3, false>(a, grid, st); break;
     case 4: launch_rows_mma_t<KIND, 4, false>(a, grid, st); break;
     case 5: launch_rows_mma_t<KIND, 5, false>(a, grid, st); break;
@@ -2212,7 +2212,8 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   {
     // 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual) so that every SM streams
     const int ng = (rows + 7) / 8;
-    const bool sw = ng <= 2;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW)
+    const bool sw = ng <= 1;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW); with more
+                                                   // rows the replicated activation reads would exceed the weight stream
     const int gx = sw ? n_rt : (n_rt + 3) / 4, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
       const int want = (4 * im->G + gx - 1) / gx;
