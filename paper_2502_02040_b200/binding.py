@@ -85,11 +85,21 @@ EXPORTS = ["m2r2_query_sizes", "m2r2_create", "m2r2_destroy", "m2r2_load_weights
 _lib = None
 
 
+_lib_path = None   # tests may point the binding at a variant build of the library (use_library)
+
+
+def use_library(path):
+    """Load `path` instead of the in-tree libm2r2.so from now on (None: back to the default).  Test hook for variant
+    builds (build.build_variant); engines created earlier keep the library they were created with."""
+    global _lib, _lib_path
+    _lib, _lib_path = None, path
+
+
 def lib():
     """Load libm2r2.so (building it with nvcc if the in-tree copy is missing or stale)."""
     global _lib
     if _lib is None:
-        path = _build.build()
+        path = _lib_path or _build.build()
         L = ctypes.CDLL(path)
         L.m2r2_query_sizes.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(Sizes)]
         L.m2r2_create.argtypes = [ctypes.POINTER(Config), ctypes.POINTER(Buffers), vp, vp, ctypes.POINTER(vp)]

@@ -53,5 +53,23 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_variant(tag: str, defines) -> str:
+    """A test build of the library with extra -D defines -> paper_2502_02040_b200/libm2r2_<tag>.so (git-ignored).
+    Used by the ring-race stress test (M2R2_PAD_SCRATCH; M2R2_PLAIN_ARRIVE to show what the guard prevents)."""
+    out = os.path.join(_HERE, "libm2r2_%s.so" % tag)
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if not f.endswith(".o")]
+    if os.path.exists(out) and all(os.path.getmtime(d) <= os.path.getmtime(out) for d in deps):
+        return out
+    nvcc = _nvcc()
+    flags = [f for f in NVCC_FLAGS if not f.startswith("--use_fast_math")] + ["-D" + d for d in defines]
+    objs = []
+    for s in SOURCES:
+        o = os.path.join(CSRC, s.replace(".cu", ".%s.o" % tag))
+        objs.append(o)
+        subprocess.check_call([nvcc] + flags + ["-c", os.path.join(CSRC, s), "-o", o])
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", out] + objs + ["-lcudart"])
+    return out
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -73,8 +73,13 @@ constexpr int UPART_Q = 64;            // max k-chunks per adapter row
 // line per item (strides 16 / 32) takes the serialisation of 148 CTAs polling one line away and is 1.5 % faster
 // with exit heads on, but 3 % slower on the C2 bench workload (no exit heads) in the same GPU session: dense.
 constexpr int UPART_N = 256;           // flagged partials of one phase (n_j * q <= 256)
+#ifdef M2R2_PAD_SCRATCH                // test builds only: the layout under which the ring race of DESIGN.md 6.3 fired
+constexpr int UPART_STRIDE = 16;       // in 8-byte entries: one 128-byte line per partial
+constexpr int RV_STRIDE = 32;          // in floats: one 128-byte line per r-vector
+#else
 constexpr int UPART_STRIDE = 1;        // in 8-byte entries
 constexpr int RV_STRIDE = MAX_R;       // in floats
+#endif
 static_assert(RV_STRIDE >= MAX_R, "r-vector stride");
 constexpr int PF_DEFAULT = 6;           // L2 prefetch window of the prefetch warp, in stages (M2R2_PF overrides; 0 = off)
 constexpr int MERGE_NS = 4;            // attention splits combined from registers by the auxiliary warp; more take a looped path
@@ -181,7 +186,12 @@ __device__ __forceinline__ void mbar_arrive(u64* b) {
 // being read (sporadic errors of ~1e-2 in one warp's 16 rows).  The barrier's address is
 // therefore made to depend, through a run-time zero, on the accumulators the stage's fragments feed.
 __device__ __forceinline__ void release_stage(u64* b, unsigned int zero, float dep) {
+#ifdef M2R2_PLAIN_ARRIVE               // test builds only: the unguarded arrive, to show that the stress test catches the race
+  const uint32_t a = smem_u32(b);
+  (void)zero; (void)dep;
+#else
   const uint32_t a = smem_u32(b) + (__float_as_uint(dep) & zero);
+#endif
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(a) : "memory");
 }
 __device__ __forceinline__ bool mbar_try_wait(u64* b, uint32_t parity) {

@@ -556,6 +556,56 @@ def test_c3_full_size_long_context_properties():
     a.close()
 
 
+def _first_steps_stress(cycles):
+    """-> number of (cycle, step, layer) checks that exceeded the bound, and the worst error"""
+    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2)
+    W = S.gen_weights(cfg)
+    prompt = S.gen_prompt(cfg, 11)
+    toks = [5, 77, 1234]
+    r0 = M.Engine(cfg, W)
+    r0.set_fused(False)
+    r0.prefill(prompt)
+    ref = []
+    for s in range(3):
+        r0.decode_step(force_tokens=[toks[s]])
+        ref.append([r0.debug_read(M.DBG_H, i).copy() for i in range(cfg.n_layers + 1)])
+    r0.close()
+    bad, worst = 0, 0.0
+    for cyc in range(cycles):
+        a = M.Engine(cfg, W)
+        a.prefill(prompt)
+        for s in range(3):
+            a.decode_step(force_tokens=[toks[s]])
+            for i in range(cfg.n_layers + 1):
+                e = rel_l2(a.debug_read(M.DBG_H, i), ref[s][i])
+                worst = max(worst, e)
+                bad += e > 3e-3
+        a.close()
+    return bad, worst
+
+
+def test_ring_race_guard_under_the_padded_scratch_layout():
+    """The write-after-read race on the weight ring fired about once per ten launches, but only with
+    the adapter scratch padded to one 128-byte line per item; the committed layout is dense and never showed it.
+    This test therefore runs the stress on a VARIANT BUILD of the library with that padded layout
+    (-DM2R2_PAD_SCRATCH): the committed `release_stage` must hold there.  With M2R2_RACE_DEMO=1 in the environment
+    it also builds the variant whose `release_stage` is the plain arrive (-DM2R2_PLAIN_ARRIVE) and requires the
+    stress to FAIL on it, i.e. that this test can see the race at all (recorded in profiles/r2_ring_race_guard.md)."""
+    import os
+    from paper_2502_02040_b200 import binding, build
+    try:
+        binding.use_library(build.build_variant("pad", ["M2R2_PAD_SCRATCH"]))
+        bad, worst = _first_steps_stress(40)
+        assert bad == 0, (bad, worst)
+        if os.environ.get("M2R2_RACE_DEMO"):
+            binding.use_library(build.build_variant("padplain", ["M2R2_PAD_SCRATCH", "M2R2_PLAIN_ARRIVE"]))
+            bad, worst = _first_steps_stress(100)
+            print("plain arrive + padded scratch: %d checks above the bound, worst rel-L2 %.3g" % (bad, worst))
+            assert bad > 0, "the unguarded arrive did not reproduce the race on this box"
+    finally:
+        binding.use_library(None)
+
+
 def test_fused_first_steps_repeat_across_engine_instances():
     """Stress for timing-dependent errors in the fused kernel: 40 fresh engines of a model whose first two layers
     carry the accelerated stream and whose other layers do not (the C3 structure, where the auxiliary warp
