@@ -38,8 +38,8 @@ METRIC = "decode tokens/s at batch 1 (M2R2 self-spec); achieved HBM GB/s vs 8 TB
 PROMPT = 512
 HBM_NOMINAL_GBS = 8000.0      # BASELINE.json: "achieved HBM GB/s vs 8 TB/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of m2r2_fused_decode_kernel (one decode step at
-# kv_len ~ 521) from the committed capture profiles/r1_v33_fused_kernel.md (ncu --set full): 7.690 GB + 22.9 MB
-FUSED_TRAFFIC_BYTES = 7.689782e9 + 22.862592e6
+# kv_len ~ 521) from the committed capture profiles/r2_v33_fused_kernel.md (ncu --set full): 7.690 GB + 21.8 MB
+FUSED_TRAFFIC_BYTES = 7.690290e9 + 21.755648e6
 
 
 def measured_peaks():
@@ -295,7 +295,7 @@ def run_ours(args, rk):
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "peak_source": peak_src, "bytes_per_launch": dom_bytes, "ms_per_launch": dom_ms,
                 "traffic": args.traffic if dom == "fused_step" else None,
-                "traffic_source": "profiles/r1_v33_fused_kernel.md (ncu --set full, one launch)" if dom == "fused_step" else None,
+                "traffic_source": "profiles/r2_v33_fused_kernel.md (ncu --set full, one launch)" if dom == "fused_step" else None,
                 "step": {"achieved": step_gbs, "frac": step_gbs / peak,
                                                   "frac_of_nominal_8TBs": step_gbs / HBM_NOMINAL_GBS,
                                                   "algorithmic_bytes_per_step": tot_bytes / K},
