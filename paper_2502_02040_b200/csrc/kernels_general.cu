@@ -480,6 +480,183 @@ __global__ void __launch_bounds__(128, NQ <= 5 ? 4 : 3) attn_kernel(AttnArgs a) 
   }
 }
 
+// ------------------------------------------------------------------ a11: k-token verification attention on the tensor pipe
+// Three to eight query rows of a sequence (the rows of a verify pass or a prefill chunk) against the bf16 K/V cache:
+// the scores of 16 positions are one m16n8k16 contraction over d_h per 8 positions (A = the queries, rows 0..7 of the
+// tile; B = K rows straight from the cache: each lane's 16-byte loads are its B fragments because the SAME permutation
+// of d_h is applied to the queries), P V is a second contraction over the 16 positions (A = the probabilities from the
+// score accumulators, B = V through ldmatrix.trans from a staged tile).  Queries and probabilities enter as bf16 hi + lo
+// parts (two MMAs, fp32 accumulation): products exact to ~2^-17, as everywhere else on this path.  A warp owns the
+// positions u0 + 16 (warp + 4 i); the four warps' online-softmax states meet in shared memory and leave one (m, l, o)
+// partial per (row, head, split), exactly what attn_kernel leaves (merge_kernel is shared).
+__device__ __forceinline__ void mma_a02(float c[4], uint32_t a0, uint32_t a2, uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a0), "r"(0u), "r"(a2), "r"(0u), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_bf16_hi_lo(float a, float b, uint32_t& lo) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  const float2 f = __bfloat1622float2(h);
+  const __nv_bfloat162 l = __floats2bfloat162_rn(a - f.x, b - f.y);
+  lo = *(const uint32_t*)&l;
+  return *(const uint32_t*)&h;
+}
+template <int DH>
+__global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
+  constexpr int NCC = DH / 32;        // 16-byte chunks of a K row per lane
+  constexpr int NKS = DH / 16;        // k-steps of Q K^T
+  constexpr int NB = DH / 8;          // n8 column blocks of the output
+  constexpr int VLD = DH + 8;         // staged V row stride in elements (+16 bytes: conflict-free ldmatrix)
+  extern __shared__ __align__(16) unsigned char am_smem[];
+  const int head = blockIdx.x, grp = blockIdx.y, split = blockIdx.z;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  __nv_bfloat16* vt = (__nv_bfloat16*)am_smem + (size_t)warp * 16 * VLD;   // the warp's staged V tile [16][VLD]
+  float* red = (float*)(am_smem + 4 * 16 * VLD * 2);                      // [4 warps][8 rows][DH + 2]
+  __shared__ int s_row[M2R2_MAXQ], s_lim[M2R2_MAXQ];
+  __shared__ int s_seq, s_maxlim;
+  const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
+  if (tid < M2R2_MAXQ) {
+    int r = a.grp_rows[grp * M2R2_MAXQ + tid];
+    if (r >= a.slow_rows && !accel_head) r = -1;
+    s_row[tid] = r;
+    s_lim[tid] = r >= 0 ? a.row_limit[r] : 0;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int mx = 0, sq = 0;
+    for (int q = 0; q < M2R2_MAXQ; ++q)
+      if (s_row[q] >= 0) { mx = max(mx, s_lim[q]); sq = a.row_seq[s_row[q]]; }
+    s_maxlim = mx;
+    s_seq = sq;
+  }
+  __syncthreads();
+  const int maxlim = s_maxlim;
+  const int chunk = (maxlim + a.n_splits - 1) / a.n_splits;
+  const int u0 = split * chunk, u1 = min(maxlim, u0 + chunk);
+  const __nv_bfloat16* Kb = (const __nv_bfloat16*)a.Kc + ((size_t)s_seq * a.n_heads + head) * a.max_seq * DH;
+  const __nv_bfloat16* Vb = (const __nv_bfloat16*)a.Vc + ((size_t)s_seq * a.n_heads + head) * a.max_seq * DH;
+  // the lane's query row g: A fragments (a0, a2) of every k-step, hi and lo parts.  k-step j, slots (2t, 2t+1 | 2t+8,
+  // 2t+9) <-> elements 8 (t + 4 (j / 2)) + 4 (j % 2) + {0, 1 | 2, 3} of d_h: the K chunks a lane loads are its B fragments
+  const int qrow = s_row[g], lim = s_lim[g];
+  uint32_t qh[NKS][2], ql[NKS][2];
+#pragma unroll
+  for (int j = 0; j < NKS; ++j) {
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (qrow >= 0) v = *(const float4*)(a.qkv + (size_t)qrow * 3 * a.d + head * DH + 8 * (t + 4 * (j >> 1)) + 4 * (j & 1));
+    qh[j][0] = pack_bf16_hi_lo(v.x * a.scale, v.y * a.scale, ql[j][0]);
+    qh[j][1] = pack_bf16_hi_lo(v.z * a.scale, v.w * a.scale, ql[j][1]);
+  }
+  float m = -INFINITY, l = 0.f, o[NB][4];
+#pragma unroll
+  for (int nb = 0; nb < NB; ++nb)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) o[nb][e] = 0.f;
+  for (int p0 = u0 + 16 * warp; p0 < u1; p0 += 64) {
+    // ---- stage V[p0 .. p0+15] (rows past the split are zero: they meet probability 0, which must not meet a NaN)
+    __syncwarp();
+#pragma unroll
+    for (int i = lane; i < 16 * (DH / 8); i += 32) {
+      const int r = i / (DH / 8), c8 = i - r * (DH / 8);
+      __nv_bfloat16* dst = vt + r * VLD + 8 * c8;
+      if (p0 + r < u1) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(Vb + (size_t)(p0 + r) * DH + 8 * c8) : "memory");
+      else *(uint4*)dst = make_uint4(0u, 0u, 0u, 0u);
+    }
+    // ---- K rows of the two 8-position blocks: lane (g, t) loads chunks t, t + 4, .. of row p0 + 8 b + g
+    uint4 kr[2][NCC];
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int cc = 0; cc < NCC; ++cc) {
+        kr[b][cc] = make_uint4(0u, 0u, 0u, 0u);
+        if (p0 + 8 * b + g < u1) kr[b][cc] = *(const uint4*)(Kb + (size_t)(p0 + 8 * b + g) * DH + 8 * (t + 4 * cc));
+      }
+    // ---- scores: s[b][0], s[b][1] = query g x positions p0 + 8 b + 2 t, + 1
+    float s[2][4];
+#pragma unroll
+    for (int b = 0; b < 2; ++b) {
+      s[b][0] = s[b][1] = s[b][2] = s[b][3] = 0.f;
+#pragma unroll
+      for (int j = 0; j < NKS; ++j) {
+        const uint32_t b0 = (j & 1) ? kr[b][j >> 1].z : kr[b][j >> 1].x, b1 = (j & 1) ? kr[b][j >> 1].w : kr[b][j >> 1].y;
+        mma_a02(s[b], qh[j][0], qh[j][1], b0, b1);
+        mma_a02(s[b], ql[j][0], ql[j][1], b0, b1);
+      }
+    }
+    // ---- online softmax of row g (its four lanes hold four positions each)
+    float mt = -INFINITY;
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const int u = p0 + 8 * b + 2 * t + e;
+        if (!(u < u1 && u < lim)) s[b][e] = -INFINITY;
+        mt = fmaxf(mt, s[b][e]);
+      }
+    mt = fmaxf(mt, __shfl_xor_sync(0xffffffffu, mt, 1));
+    mt = fmaxf(mt, __shfl_xor_sync(0xffffffffu, mt, 2));
+    const float mn = fmaxf(m, mt);
+    const float corr = mn == -INFINITY ? 1.f : __expf(m - mn);
+    float p[2][2];
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) p[b][e] = s[b][e] == -INFINITY ? 0.f : __expf(s[b][e] - mn);
+    l = l * corr + (p[0][0] + p[0][1]) + (p[1][0] + p[1][1]);
+    m = mn;
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) { o[nb][0] *= corr; o[nb][1] *= corr; }
+    uint32_t pl0, pl1;
+    const uint32_t ph0 = pack_bf16_hi_lo(p[0][0], p[0][1], pl0), ph1 = pack_bf16_hi_lo(p[1][0], p[1][1], pl1);
+    // ---- o += P V: B fragments of V through ldmatrix.trans (rows 0-7 | 8-15 of the tile, 8 columns)
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncwarp();
+    const uint32_t vaddr = (uint32_t)__cvta_generic_to_shared(vt + (lane & 15) * VLD);
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) {
+      uint32_t b0, b1;
+      asm volatile("ldmatrix.sync.aligned.m8n8.x2.trans.shared.b16 {%0, %1}, [%2];" : "=r"(b0), "=r"(b1) : "r"(vaddr + nb * 16));
+      mma_a02(o[nb], ph0, ph1, b0, b1);
+      mma_a02(o[nb], pl0, pl1, b0, b1);
+    }
+  }
+  // ---- the four warps' states -> one partial per query row
+  l += __shfl_xor_sync(0xffffffffu, l, 1);
+  l += __shfl_xor_sync(0xffffffffu, l, 2);
+  __syncthreads();   // every warp is done with its staged tile (red does not alias it, but s_row / s_lim stay live)
+  {
+    float* dst = red + ((size_t)warp * 8 + g) * (DH + 2);
+#pragma unroll
+    for (int nb = 0; nb < NB; ++nb) { dst[8 * nb + 2 * t] = o[nb][0]; dst[8 * nb + 2 * t + 1] = o[nb][1]; }
+    if (t == 0) { dst[DH] = m; dst[DH + 1] = l; }
+  }
+  __syncthreads();
+  for (int i = tid; i < 8 * DH; i += 128) {
+    const int q = i / DH, j = i % DH, r = s_row[q];
+    if (r < 0) continue;
+    float M = -INFINITY;
+    for (int w = 0; w < 4; ++w) M = fmaxf(M, red[((size_t)w * 8 + q) * (DH + 2) + DH]);
+    float L = 0.f, O = 0.f;
+    for (int w = 0; w < 4; ++w) {
+      const float* src = red + ((size_t)w * 8 + q) * (DH + 2);
+      const float ls = src[DH + 1];
+      if (ls > 0.f) {
+        const float wgt = __expf(src[DH] - M);
+        L += ls * wgt;
+        O += src[j] * wgt;
+      }
+    }
+    const size_t pidx = ((size_t)r * a.n_heads + head) * a.n_splits + split;
+    a.part_o[pidx * DH + j] = O;
+    if (j == 0) { a.part_ml[pidx * 2] = M; a.part_ml[pidx * 2 + 1] = L; }
+  }
+}
+template <int DH>
+static void launch_attn_mma(cudaStream_t st, const AttnArgs& a, dim3 grid) {
+  const size_t sh = (size_t)4 * 16 * (DH + 8) * 2 + (size_t)4 * 8 * (DH + 2) * sizeof(float);
+  attn_mma_kernel<DH><<<grid, 128, sh, st>>>(a);
+}
+
 template <typename KT, int SEG>
 static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq) {
   const int nseg = 4 * (32 / SEG);
@@ -500,6 +677,11 @@ static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq
 // rows_per_group: live query rows of a group (<= M2R2_MAXQ), packed from slot 0 of grp_rows
 void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group) {
   dim3 grid(a.n_heads, n_groups, a.n_splits);
+  if (dtype != M2R2_FP32 && rows_per_group > 2) {   // k-token verification attention: tensor pipe (bf16 cache)
+    if (a.dh == 64) { launch_attn_mma<64>(st, a, grid); return; }
+    if (a.dh == 96) { launch_attn_mma<96>(st, a, grid); return; }
+    if (a.dh == 128) { launch_attn_mma<128>(st, a, grid); return; }
+  }
   int epl = dtype == M2R2_FP32 ? 4 : 8;
   int lpp = a.dh / epl;
   int seg = lpp <= 4 ? 4 : lpp <= 8 ? 8 : lpp <= 16 ? 16 : 32;
