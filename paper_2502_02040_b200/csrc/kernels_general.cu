@@ -511,8 +511,8 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
   extern __shared__ __align__(16) unsigned char am_smem[];
   const int head = blockIdx.x, grp = blockIdx.y, split = blockIdx.z;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  __nv_bfloat16* vt = (__nv_bfloat16*)am_smem + (size_t)warp * 16 * VLD;   // the warp's staged V tile [16][VLD]
-  float* red = (float*)(am_smem + 4 * 16 * VLD * 2);                      // [4 warps][8 rows][DH + 2]
+  __nv_bfloat16* vt = (__nv_bfloat16*)am_smem + (size_t)warp * 16 * VLD;   // the warp's staged V tiles [2 buffers][4 warps][16][VLD]
+  float* red = (float*)(am_smem + 2 * 4 * 16 * VLD * 2);                  // [4 warps][8 rows][DH + 2]
   __shared__ int s_row[M2R2_MAXQ], s_lim[M2R2_MAXQ];
   __shared__ int s_seq, s_maxlim;
   const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
@@ -552,18 +552,20 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
   for (int nb = 0; nb < NB; ++nb)
 #pragma unroll
     for (int e = 0; e < 4; ++e) o[nb][e] = 0.f;
-  for (int p0 = u0 + 16 * warp; p0 < u1; p0 += 64) {
-    // ---- stage V[p0 .. p0+15] (rows past the split are zero: they meet probability 0, which must not meet a NaN)
-    __syncwarp();
+  // software pipeline: the NEXT tile's V rows (cp.async into the other buffer) and K chunks (registers) are requested
+  // before this tile is computed
+  auto stage_v = [&](int p0, int buf) {   // rows past the split are zero: they meet probability 0, which must not meet a NaN
+    __nv_bfloat16* vb = vt + (size_t)buf * 4 * 16 * VLD;
 #pragma unroll
     for (int i = lane; i < 16 * (DH / 8); i += 32) {
       const int r = i / (DH / 8), c8 = i - r * (DH / 8);
-      __nv_bfloat16* dst = vt + r * VLD + 8 * c8;
+      __nv_bfloat16* dst = vb + r * VLD + 8 * c8;
       if (p0 + r < u1) asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(Vb + (size_t)(p0 + r) * DH + 8 * c8) : "memory");
       else *(uint4*)dst = make_uint4(0u, 0u, 0u, 0u);
     }
-    // ---- K rows of the two 8-position blocks: lane (g, t) loads chunks t, t + 4, .. of row p0 + 8 b + g
-    uint4 kr[2][NCC];
+    asm volatile("cp.async.commit_group;" ::: "memory");
+  };
+  auto load_k = [&](int p0, uint4 (&kr)[2][NCC]) {   // lane (g, t) loads chunks t, t + 4, .. of row p0 + 8 b + g
 #pragma unroll
     for (int b = 0; b < 2; ++b)
 #pragma unroll
@@ -571,6 +573,18 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
         kr[b][cc] = make_uint4(0u, 0u, 0u, 0u);
         if (p0 + 8 * b + g < u1) kr[b][cc] = *(const uint4*)(Kb + (size_t)(p0 + 8 * b + g) * DH + 8 * (t + 4 * cc));
       }
+  };
+  uint4 kr[2][NCC], kn[2][NCC];
+  int buf = 0;
+  if (u0 + 16 * warp < u1) { stage_v(u0 + 16 * warp, 0); load_k(u0 + 16 * warp, kn); }
+  for (int p0 = u0 + 16 * warp; p0 < u1; p0 += 64, buf ^= 1) {
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+      for (int cc = 0; cc < NCC; ++cc) kr[b][cc] = kn[b][cc];
+    const bool more = p0 + 64 < u1;
+    __syncwarp();   // the other buffer's ldmatrix reads (previous tile) are done in every lane
+    if (more) { stage_v(p0 + 64, buf ^ 1); load_k(p0 + 64, kn); }
     // ---- scores: s[b][0], s[b][1] = query g x positions p0 + 8 b + 2 t, + 1
     float s[2][4];
 #pragma unroll
@@ -609,9 +623,9 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
     uint32_t pl0, pl1;
     const uint32_t ph0 = pack_bf16_hi_lo(p[0][0], p[0][1], pl0), ph1 = pack_bf16_hi_lo(p[1][0], p[1][1], pl1);
     // ---- o += P V: B fragments of V through ldmatrix.trans (rows 0-7 | 8-15 of the tile, 8 columns)
-    asm volatile("cp.async.wait_all;" ::: "memory");
+    if (more) asm volatile("cp.async.wait_group 1;" ::: "memory"); else asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncwarp();
-    const uint32_t vaddr = (uint32_t)__cvta_generic_to_shared(vt + (lane & 15) * VLD);
+    const uint32_t vaddr = (uint32_t)__cvta_generic_to_shared(vt + (size_t)buf * 4 * 16 * VLD + (lane & 15) * VLD);
 #pragma unroll
     for (int nb = 0; nb < NB; ++nb) {
       uint32_t b0, b1;
@@ -653,7 +667,12 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
 }
 template <int DH>
 static void launch_attn_mma(cudaStream_t st, const AttnArgs& a, dim3 grid) {
-  const size_t sh = (size_t)4 * 16 * (DH + 8) * 2 + (size_t)4 * 8 * (DH + 2) * sizeof(float);
+  const size_t sh = (size_t)2 * 4 * 16 * (DH + 8) * 2 + (size_t)4 * 8 * (DH + 2) * sizeof(float);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(attn_mma_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    attr_set = true;
+  }
   attn_mma_kernel<DH><<<grid, 128, sh, st>>>(a);
 }
 
@@ -677,7 +696,7 @@ static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq
 // rows_per_group: live query rows of a group (<= M2R2_MAXQ), packed from slot 0 of grp_rows
 void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group) {
   dim3 grid(a.n_heads, n_groups, a.n_splits);
-  if (dtype != M2R2_FP32 && rows_per_group > 2) {   // k-token verification attention: tensor pipe (bf16 cache)
+  if (dtype != M2R2_FP32 && rows_per_group >= 2) {   // k-token verification attention: tensor pipe (bf16 cache)
     if (a.dh == 64) { launch_attn_mma<64>(st, a, grid); return; }
     if (a.dh == 96) { launch_attn_mma<96>(st, a, grid); return; }
     if (a.dh == 128) { launch_attn_mma<128>(st, a, grid); return; }
