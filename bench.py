@@ -462,22 +462,25 @@ def run_secondary(args):
         B, P, gamma = 8, 4096, 4
         eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
         prompts = np.stack([S.gen_prompt(cfg, P, seq=b) for b in range(B)])
-        for alpha in (0.9, 0.5):
+        for alpha in ((args.alpha,) if args.alpha else (0.9, 0.5)):
             scripts = [S.gen_logit_script(cfg, 1000, alpha, seq=b) for b in range(B)]
             eng.set_logit_script(np.stack([x[0] for x in scripts]), np.stack([x[1] for x in scripts]), P)
             eng.prefill(prompts)
             for _ in range(2):
                 eng.spec_step(gamma)
             torch.cuda.synchronize()
+            nsteps = 128 if args.tokens == 256 else args.tokens     # --tokens N: N spec steps (short profiled runs)
+            torch.cuda.profiler.start()     # `ncu --profile-from-start off` captures the timed region only
             t0, emitted, by = time.perf_counter(), 0, 0
-            for _ in range(128):
+            for _ in range(nsteps):
                 _, n = eng.spec_step(gamma)
                 emitted += int(n.sum())
                 by += eng.get_stats()["algorithmic_bytes_last"]
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-            out["runs"].append({"alpha": alpha, "gamma": gamma, "batch": B, "kv_len_start": P, "spec_steps": 128,
-                                "ms_per_spec_step": 1e3 * dt / 128, "aggregate_tokens_per_s": emitted / dt,
+            torch.cuda.profiler.stop()
+            out["runs"].append({"alpha": alpha, "gamma": gamma, "batch": B, "kv_len_start": P, "spec_steps": nsteps,
+                                "ms_per_spec_step": 1e3 * dt / nsteps, "aggregate_tokens_per_s": emitted / dt,
                                 "algorithmic_GB_per_s": by / dt / 1e9, "kv_len_end": list(eng.get_stats()["kv_len"][:B])})
         eng.close()
     else:
