@@ -557,6 +557,47 @@ def run_secondary(args):
     return 0
 
 
+def run_olmoe(args):
+    """the paper's five expert-loading strategies on an OLMoE-shaped model with half of
+    the experts resident, natural (un-scripted) routing of the random-init routers.  Reports per-step latency (Fig. 9b's
+    metric), hit rate at use (Fig. 9a's), bytes loaded and the link rate."""
+    import torch
+    import m2r2_synth as S
+    import paper_2502_02040_b200 as M
+    cfg = S.config_olmoe_shaped()
+    P, STEPS = 64, 128 if args.tokens == 256 else args.tokens
+    eng = M.Engine(cfg, device="cuda:0")
+    W = S.gen_weights(cfg, expert_alloc=eng.pinned_expert_alloc())
+    eng.load_weights(W)
+    prompt = S.gen_prompt(cfg, P)
+    out = {"workload": "olmoe-shaped (f-2)", "data": "synthetic", "n_gpus": 1, "config": {"n_layers": cfg.n_layers, "d_model": cfg.d_model,
+           "n_experts": cfg.n_experts, "top_k": cfg.top_k, "d_ff_expert": cfg.d_ff_expert, "cache_slots_per_layer": cfg.cache_slots,
+           "expert_bytes": 3 * cfg.d_model * cfg.d_ff_expert * 2, "aot_schedule": "layer i -> {2i+2, 2i+3}, i < 8"}, "runs": []}
+    names = {M.POLICY_FIXED: "fixed + on-demand", M.POLICY_LRU: "LRU", M.POLICY_LRU_RANDOM: "LRU + random speculation",
+             M.POLICY_LRU_PREV: "LRU + previous-layer residual", M.POLICY_LRU_AOT: "LRU + accelerated residual (M2R2 AoT)"}
+    for pol in (M.POLICY_FIXED, M.POLICY_LRU, M.POLICY_LRU_RANDOM, M.POLICY_LRU_PREV, M.POLICY_LRU_AOT):
+        eng.set_policy(pol)
+        eng.prefill(prompt)
+        for _ in range(4):
+            eng.decode_step()
+        s0 = eng.get_stats()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(STEPS):
+            eng.decode_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        s1 = eng.get_stats()
+        d = {k: s1[k] - s0[k] for k in ("expert_hits", "expert_misses", "expert_prefetched", "expert_on_demand", "h2d_bytes")}
+        out["runs"].append({"policy": names[pol], "steps": STEPS, "ms_per_step": 1e3 * dt / STEPS, "tokens_per_s": STEPS / dt,
+                            "hit_rate_at_use": d["expert_hits"] / max(1, d["expert_hits"] + d["expert_misses"]),
+                            "prefetched": d["expert_prefetched"], "on_demand": d["expert_on_demand"],
+                            "h2d_GB": d["h2d_bytes"] / 1e9, "h2d_GB_per_s": d["h2d_bytes"] / 1e9 / dt})
+    eng.close()
+    print(json.dumps(out), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -565,8 +606,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--exit-heads", type=int, default=0, help="evaluate the exit argmax at every gate (SURVEY Q15 second row)")
     ap.add_argument("--no-fused", action="store_true", help="force the per-operation kernels")
-    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"],
-                    help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]")
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5", "olmoe"],
+                    help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]; "
+                         "olmoe = the five expert-loading strategies on an OLMoE-shaped model (SURVEY 8(f) f-2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--gamma", type=int, default=0, help="--workload c3: one draft length instead of 2, 4, 6")
     ap.add_argument("--alpha", type=float, default=0.0, help="--workload c3: one acceptance rate instead of 0.9, 0.5")
@@ -575,6 +617,8 @@ def main():
     ap.add_argument("--traffic", type=float, default=FUSED_TRAFFIC_BYTES,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/)")
     args = ap.parse_args()
+    if args.workload == "olmoe":
+        sys.exit(run_olmoe(args))
     if args.workload != "c2":
         sys.exit(run_secondary(args))
     from paper_2502_02040_b200 import replicas

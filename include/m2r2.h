@@ -39,7 +39,7 @@ extern "C" {
 #define M2R2_MAX_LAYERS 128
 #define M2R2_MAX_BATCH 8
 #define M2R2_MAX_DRAFT 7   /* spec_step k <= 7  =>  k+1 <= 8 verify rows per sequence */
-#define M2R2_MAX_TOPK 4
+#define M2R2_MAX_TOPK 8
 #define M2R2_MAX_EXPERTS 64
 
 typedef enum {
@@ -53,8 +53,14 @@ typedef enum {
 
 enum { M2R2_FP32 = 0, M2R2_BF16 = 1 };
 
-/* MoE expert-loading policy (PAPER.md L242 strategies 1, 2, 5) */
-enum { M2R2_POLICY_FIXED = 0, M2R2_POLICY_LRU = 1, M2R2_POLICY_LRU_AOT = 2 };
+/* MoE expert-loading policy: the five strategies of PAPER.md L242.
+ *   FIXED       experts 0..C-1 of a layer stay resident, every other expert is loaded on demand each time
+ *   LRU         least-recently-used replacement, loads on demand only
+ *   LRU_AOT     LRU + ahead-of-time speculation from the accelerated residual (L137-139, L244, App. B: the paper's)
+ *   LRU_RANDOM  LRU + top_k uniformly drawn experts pre-loaded one layer ahead (seeded counter-based generator)
+ *   LRU_PREV    LRU + speculation one layer ahead from the previous layer's slow residual: the router of layer i + 1
+ *               applied to rms(h_{i+1}; g2_{i+1})                                                                        */
+enum { M2R2_POLICY_FIXED = 0, M2R2_POLICY_LRU = 1, M2R2_POLICY_LRU_AOT = 2, M2R2_POLICY_LRU_RANDOM = 3, M2R2_POLICY_LRU_PREV = 4 };
 
 typedef struct m2r2_config {
   uint32_t struct_size;          /* = sizeof(m2r2_config); versions the struct */

@@ -156,6 +156,18 @@ def config_c5() -> ModelConfig:
                        aot_targets=tuple(tg), seed=0x4D325232 + 5)
 
 
+def config_olmoe_shaped() -> ModelConfig:
+    """an OLMoE-shaped MoE decoder for the paper's five expert-loading strategies:
+    16 layers, d 2048, 16 x 128 heads, 64 experts of FFN 1024 per layer, top-8, HALF of the experts resident (32 slots
+    per layer), accelerated stream in layers 0..7 predicting with the paper's 2x schedule (layer i -> {2i+2, 2i+3})."""
+    n = 16
+    return ModelConfig(name="OLMoE-shaped-bf16", n_layers=n, d_model=2048, n_heads=16, head_dim=128,
+                       d_ff=0, vocab=32064, dtype=BF16, max_seq=768,
+                       accel_heads=(0, 1, 2, 3), gates=(8,), accel_end_layer=8,
+                       n_experts=64, top_k=8, d_ff_expert=1024, cache_slots=32, accel_mlp_rank=64,
+                       aot_targets=aot_targets_for_rate(n, 2, 8), seed=0x4D325232 + 6)
+
+
 def config_small_bf16(**kw) -> ModelConfig:
     """Reduced bf16 dense model for parity tests: same structure as C2/C3 (head_dim 96,
     ragged row counts), sized so the oracle finishes in seconds."""

@@ -249,7 +249,8 @@ static int lru_insert(orc* o, int L, int e, const int32_t* keep, int nk) {
 }
 
 /* policy 0: fixed residency (experts 0..C-1 stay; others are loaded on demand every time).
- * policy 1: LRU.  policy 2: LRU + ahead-of-time speculation. */
+ * policy 1: LRU.  policy 2: LRU + ahead-of-time speculation from the accelerated residual.  policy 3: LRU + random
+ * speculation.  policy 4: LRU + speculation from the previous layer's (slow) residual.  (the five strategies) */
 static void moe_use_event(orc* o, int L, const int32_t* idx) {
   for (int k = 0; k < o->c.top_k; ++k) {
     if (o->policy == 0) {
@@ -262,9 +263,33 @@ static void moe_use_event(orc* o, int L, const int32_t* idx) {
   }
 }
 static void moe_predict_event(orc* o, int L, const int32_t* idx) {
-  if (o->policy != 2) return;
+  if (o->policy < 2) return;
   for (int k = 0; k < o->c.top_k; ++k)
     if (lru_insert(o, L, idx[k], idx, o->c.top_k)) o->st.prefetched++;
+}
+/* counter-based generator of the random-speculation policy (the CUDA side implements the same function) */
+static uint64_t spec_mix(uint64_t counter) {
+  uint64_t x = 0x5EC0DE5EEDull + 0x9E3779B97F4A7C15ull * (counter + 1);
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+/* policy 3 (third strategy: "LRU ... adding speculative caching and randomly pre-loading experts"):
+ * before layer Lt is reached, top_k distinct experts drawn uniformly are pre-loaded into its cache.  DESIGN.md Q24:
+ * one layer ahead, top_k experts, draw d of (position t, layer Lt) = spec_mix((t * N + Lt) * 256 + d) mod n_experts,
+ * duplicates skipped. */
+static void random_speculation(orc* o, int Lt, int t) {
+  const orc_config* c = &o->c;
+  int32_t idx[ORC_MAX_TOPK];
+  int n = 0;
+  for (int dr = 0; n < c->top_k && dr < 256; ++dr) {
+    int e = (int)(spec_mix(((uint64_t)t * (uint64_t)c->n_layers + (uint64_t)Lt) * 256u + (uint64_t)dr) % (uint64_t)c->n_experts);
+    int dup = 0;
+    for (int k = 0; k < n; ++k) dup |= idx[k] == e;
+    if (!dup) idx[n++] = e;
+  }
+  for (int k = 0; k < c->top_k; ++k) o->pred_idx[Lt * c->top_k + k] = idx[k];
+  moe_predict_event(o, Lt, idx);
 }
 
 /* router: softmax over all experts, top-k (lower index wins ties), renormalise (Q19) */
@@ -549,8 +574,27 @@ static void predict_experts(orc* o, int src_layer, const float* p, int t) {
     rmsnorm(o, p, o->L[Lt].t[T_G2], y);
     route(o, o->L[Lt].t[T_ROUTER], y, sp, o->rs_beta, idx, w);
     for (int k = 0; k < c->top_k; ++k) o->pred_idx[Lt * c->top_k + k] = idx[k];
-    moe_predict_event(o, Lt, idx);
+    if (o->policy == 2) moe_predict_event(o, Lt, idx);
   }
+  free(y);
+}
+
+/* policy 4 (fourth strategy: "speculative loading based on residual states from the previous layer";
+ * L244: started "only one layer before the current layer"): the router of layer Lt = i + 1 applied to the SLOW residual
+ * entering that layer, rms(h_{i+1}; g2_{Lt}) (Q25). */
+static void prev_layer_speculation(orc* o, int Lt, const float* h, int t) {
+  const orc_config* c = &o->c;
+  int d = c->d_model;
+  float* y = (float*)malloc(sizeof(float) * d);
+  int32_t idx[ORC_MAX_TOPK];
+  float w[ORC_MAX_TOPK];
+  const int32_t* sp = NULL;
+  if (o->rs_pred && t >= o->rs_first && t < o->rs_first + o->rs_n)
+    sp = o->rs_pred + ((size_t)(t - o->rs_first) * c->n_layers + Lt) * 2;
+  rmsnorm(o, h, o->L[Lt].t[T_G2], y);
+  route(o, o->L[Lt].t[T_ROUTER], y, sp, o->rs_beta, idx, w);
+  for (int k = 0; k < c->top_k; ++k) o->pred_idx[Lt * c->top_k + k] = idx[k];
+  moe_predict_event(o, Lt, idx);
   free(y);
 }
 
@@ -571,9 +615,13 @@ static void dual_token(orc* o, int token, int t, int n_run, int accel, float* h,
   for (int i = 0; i < n_run; ++i) {
     int acc_on = accel && c->accel_enabled && i < c->accel_end_layer;
     slow_layer(o, i, h, 1, t, 1);
+    if (c->n_experts && i + 1 < c->n_layers) {
+      if (o->policy == 3) random_speculation(o, i + 1, t);
+      if (o->policy == 4) prev_layer_speculation(o, i + 1, h, t);
+    }
     if (acc_on) {
       accel_layer(o, i, p, t);
-      if (c->n_experts) predict_experts(o, i, p, t);
+      if (c->n_experts && o->policy <= 2) predict_experts(o, i, p, t);   /* acts on the cache under policy 2 only */
     }
     if (trace) {
       memcpy(o->trH + (size_t)(i + 1) * d, h, sizeof(float) * d);
@@ -688,7 +736,7 @@ int orc_set_router_script(orc* o, const int32_t* actual, const int32_t* pred, in
 }
 
 int orc_set_policy(orc* o, int policy) {
-  if (policy < 0 || policy > 2) return -1;
+  if (policy < 0 || policy > 4) return -1;
   o->policy = policy;
   return 0;
 }

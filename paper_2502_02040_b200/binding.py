@@ -17,7 +17,7 @@ from . import build as _build
 MAX_HEADS, MAX_GATES, MAX_LAYERS, MAX_BATCH, MAX_DRAFT = 128, 16, 128, 8, 7
 OK, INVALID_ARG, BAD_STATE, CAPACITY, CUDA, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 FP32, BF16 = 0, 1
-POLICY_FIXED, POLICY_LRU, POLICY_LRU_AOT = 0, 1, 2
+POLICY_FIXED, POLICY_LRU, POLICY_LRU_AOT, POLICY_LRU_RANDOM, POLICY_LRU_PREV = 0, 1, 2, 3, 4
 DBG_H, DBG_P, DBG_LOGITS, DBG_EXIT_LOGITS, DBG_K, DBG_V, DBG_ROUTE_IDX, DBG_ROUTE_W, DBG_PRED_IDX = range(9)
 
 i32, i64, u32, u64, f32, vp = (ctypes.c_int32, ctypes.c_int64, ctypes.c_uint32, ctypes.c_uint64,

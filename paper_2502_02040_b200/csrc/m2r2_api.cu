@@ -565,6 +565,14 @@ extern "C" int m2r2_reset(m2r2_ctx* x) {
   return M2R2_OK;
 }
 
+// counter-based generator of the random-speculation policy (the oracle implements the same function on its side)
+static uint64_t spec_mix(uint64_t counter) {
+  uint64_t v = 0x5EC0DE5EEDull + 0x9E3779B97F4A7C15ull * (counter + 1);
+  v = (v ^ (v >> 30)) * 0xBF58476D1CE4E5B9ull;
+  v = (v ^ (v >> 27)) * 0x94D049BB133111EBull;
+  return v ^ (v >> 31);
+}
+
 // ------------------------------------------------------------------ MoE cache (host side, A15/A16)
 static void lru_touch(std::vector<int>& q, int e) {
   auto it = std::find(q.begin(), q.end(), e);
@@ -912,6 +920,38 @@ static int moe_mlp(m2r2_ctx* x, const Pass& p, int i, int ns, int na) {
     expert_ffn(x, blob[k], 0, 1, x->route_w + i * tk + k, 0, k == 0, k == tk - 1);
   CU(x, cudaEventRecord(x->ev_layer_done[i], x->cs));
   if (x->policy == M2R2_POLICY_FIXED) CU(x, cudaEventRecord(x->ev_stage_free, x->cs));
+  // the two comparison strategies of PAPER.md L242 that speculate ONE layer ahead (L244), through the same prefetch machinery
+  if (p.count_events && i + 1 < c.n_layers && (x->policy == M2R2_POLICY_LRU_RANDOM || x->policy == M2R2_POLICY_LRU_PREV)) {
+    const int Lt = i + 1;
+    int pairs[2 * M2R2_MAX_TOPK];
+    if (x->policy == M2R2_POLICY_LRU_RANDOM) {
+      // top_k distinct experts, draw d of (position t, layer Lt) = spec_mix((t * N + Lt) * 256 + d) mod n_experts
+      const uint64_t t = (uint64_t)x->kv_h[0] + (uint64_t)p.joff;
+      int n = 0;
+      for (int dr = 0; n < tk && dr < 256; ++dr) {
+        const int e = (int)(spec_mix((t * (uint64_t)c.n_layers + (uint64_t)Lt) * 256u + (uint64_t)dr) % (uint64_t)c.n_experts);
+        bool dup = false;
+        for (int k = 0; k < n; ++k) dup |= pairs[2 * k + 1] == e;
+        if (!dup) { pairs[2 * n] = Lt; pairs[2 * n + 1] = e; ++n; }
+      }
+      for (int k = 0; k < tk; ++k) x->h_pinned[2048 + k] = pairs[2 * k + 1];
+      CU(x, cudaMemcpyAsync(x->d_pred_idx + Lt * tk, x->h_pinned + 2048, sizeof(int) * tk, cudaMemcpyHostToDevice, x->cs));
+      CU(x, cudaEventRecord(x->ev_tmp, x->cs));
+      CU(x, cudaEventSynchronize(x->ev_tmp));   // the pinned staging words are reused by the next layer
+    } else {
+      // the router of layer i + 1 on the slow residual h_{i+1} this layer just produced
+      launch_route(x->cs, c.dtype, x->resid, d, 1, d, x->L[Lt].g2, c.rms_eps, 1, x->L[Lt].router, c.n_experts, tk, c.renorm_topk,
+                   x->d_row_pos, x->rs_on ? x->d_rs_pred : nullptr, x->rs_first, x->rs_n, c.n_layers, Lt, x->rs_beta,
+                   x->d_pred_idx + Lt * tk, x->pred_w + Lt * tk);
+      count(x);
+      CU(x, cudaMemcpyAsync(x->h_pinned + 1024, x->d_pred_idx + Lt * tk, sizeof(int) * tk, cudaMemcpyDeviceToHost, x->cs));
+      CU(x, cudaEventRecord(x->ev_tmp, x->cs));
+      CU(x, cudaEventSynchronize(x->ev_tmp));
+      for (int k = 0; k < tk; ++k) { pairs[2 * k] = Lt; pairs[2 * k + 1] = x->h_pinned[1024 + k]; }
+    }
+    int rc = prefetch_pairs(x, pairs, tk);
+    if (rc < 0) return fail(x, rc, "prefetch failed");
+  }
   return 0;
 }
 
@@ -1265,7 +1305,7 @@ extern "C" int m2r2_moe_prefetch(m2r2_ctx* x, int32_t src_layer, const int32_t* 
 
 extern "C" int m2r2_set_policy(m2r2_ctx* x, int32_t policy) {
   if (!x) return M2R2_INVALID_ARG;
-  if (policy < 0 || policy > 2) return fail(x, M2R2_INVALID_ARG, "bad policy");
+  if (policy < 0 || policy > M2R2_POLICY_LRU_PREV) return fail(x, M2R2_INVALID_ARG, "bad policy");
   if (!x->c.n_experts) return fail(x, M2R2_UNSUPPORTED, "policy on a dense model");
   x->policy = policy;
   if (x->weights_loaded) return reset_expert_cache(x);

@@ -343,10 +343,11 @@ def _moe_pair(cfg):
     return eng, Oracle(cfg, W), W
 
 
-@pytest.mark.parametrize("policy", [M.POLICY_FIXED, M.POLICY_LRU, M.POLICY_LRU_AOT])
+@pytest.mark.parametrize("policy", [M.POLICY_FIXED, M.POLICY_LRU, M.POLICY_LRU_AOT, M.POLICY_LRU_RANDOM, M.POLICY_LRU_PREV])
 def test_small_moe_decode_matches_oracle(policy):
-    """a13-a17: hidden states, routed / predicted expert indices, router weights and the cache counters
-    (hits, misses, prefetched, on-demand) equal the oracle's logical LRU model (I15), natural routing."""
+    """a13-a17 and the five expert-loading strategies of PAPER.md L242: hidden states, routed / predicted expert
+    indices, router weights and the cache counters (hits, misses, prefetched, on-demand) equal the oracle's logical
+    LRU model (I15, I22, I23), natural routing."""
     cfg = S.config_small_moe()
     eng, orc, _ = _moe_pair(cfg)
     eng.set_policy(policy)
@@ -361,7 +362,7 @@ def test_small_moe_decode_matches_oracle(policy):
         ri = eng.debug_read(M.DBG_ROUTE_IDX).reshape(cfg.n_layers, cfg.top_k).astype(np.int32)
         assert np.array_equal(ri, orc.route_idx()), (s, ri, orc.route_idx())
         assert np.allclose(eng.debug_read(M.DBG_ROUTE_W).reshape(cfg.n_layers, cfg.top_k), orc.route_w(), atol=2e-3)
-        if policy == M.POLICY_LRU_AOT:
+        if policy >= M.POLICY_LRU_AOT:
             pi = eng.debug_read(M.DBG_PRED_IDX).reshape(cfg.n_layers, cfg.top_k).astype(np.int32)
             po = orc.pred_idx()
             mask = po >= 0

@@ -360,7 +360,7 @@ def _lru_sim(C, events, policy):
         cache[s] = -s
     stamp, hits, misses, pref = 1, 0, 0, 0
     for kind, idx in events:
-        if kind == "pred" and policy != 2:
+        if kind == "pred" and policy < 2:
             continue
         for e in idx:
             if e in cache:
@@ -379,7 +379,7 @@ def _lru_sim(C, events, policy):
     return hits, misses, pref, sorted(cache, key=lambda x: -cache[x])
 
 
-@pytest.mark.parametrize("policy", [1, 2])
+@pytest.mark.parametrize("policy", [1, 2, 3, 4])
 @pytest.mark.parametrize("C", [2, 3, 5])
 def test_I15_lru_model_vs_bruteforce(policy, C):
     """PAPER.md L139/L242 (LRU replaced by speculated experts), Fig. 5 L121 (only
@@ -487,6 +487,97 @@ def test_golden_c1_tokens_regression():
 
 
 # ---------------------------------------------------------------- I18-I21: the branches VERDICT r1 found unpinned
+# ---------------------------------------------------------------- I22, I23: the comparison strategies of PAPER.md L242
+def _spec_mix(counter):
+    """the counter-based generator of the random-speculation policy, restated (64-bit wrap-around arithmetic)"""
+    M = (1 << 64) - 1
+    x = (0x5EC0DE5EED + 0x9E3779B97F4A7C15 * (counter + 1)) & M
+    x = ((x ^ (x >> 30)) * 0xBF58476D1CE4E5B9) & M
+    x = ((x ^ (x >> 27)) * 0x94D049BB133111EB) & M
+    return x ^ (x >> 31)
+
+
+def test_I22_random_speculation_draws_and_counters():
+    """Policy 3 (L242: LRU + random pre-loading, Q24): before layer L+1 the top_k experts
+    spec_mix((t N + L+1) 256 + draw) mod n_e (duplicates skipped) are pre-loaded.  The oracle's predicted indices
+    equal the restated draws, the draws are distinct and roughly uniform, and its counters equal the brute-force LRU
+    simulation fed with the (pred, use) event sequence."""
+    cfg = S.config_small_moe()
+    W = S.gen_weights(cfg)
+    P, steps = 5, 10
+    o = Oracle(cfg, W)
+    o.set_policy(3)
+    o.prefill(S.gen_prompt(cfg, P))
+    events = {L: [] for L in range(cfg.n_layers)}
+    seen = np.zeros(cfg.n_experts, int)
+    for s in range(steps):
+        o.decode_step()
+        t = P + s
+        pred, use = o.pred_idx(), o.route_idx()
+        assert pred[0].tolist() == [-1] * cfg.top_k          # nothing speculates for layer 0
+        for L in range(1, cfg.n_layers):
+            want, dr = [], 0
+            while len(want) < cfg.top_k:
+                e = _spec_mix((t * cfg.n_layers + L) * 256 + dr) % cfg.n_experts
+                dr += 1
+                if e not in want:
+                    want.append(e)
+            assert pred[L].tolist() == want and len(set(want)) == cfg.top_k
+            seen[want] += 1
+        for L in range(cfg.n_layers):
+            # within a step: layer L is used, then layer L + 1 is speculated
+            if L >= 1:
+                events[L].insert(len(events[L]), ("pred", pred[L].tolist()))
+            events[L].append(("use", use[L].tolist()))
+    assert seen.min() > 0
+    hits = misses = pref = 0
+    for L in range(cfg.n_layers):
+        h, m, pf, order = _lru_sim(cfg.cache_slots, events[L], 3)
+        hits += h; misses += m; pref += pf
+        assert o.lru()[L].tolist() == order
+    st = o.stats()
+    assert (st["expert_hits"], st["expert_misses"], st["prefetched"]) == (hits, misses, pref)
+
+
+def test_I23_previous_layer_speculation_is_the_next_router_on_h():
+    """Policy 4 (L242: speculation from the previous layer's residual; L244: one layer ahead; Q25): the
+    predicted experts of layer L+1 are route(W_r^{L+1}, rms(h_{L+1}; g2_{L+1})) with h_{L+1} the slow residual entering
+    that layer, recomputed here in numpy from trace_h; counters equal the brute-force LRU simulation."""
+    cfg = S.config_small_moe()
+    W = S.gen_weights(cfg)
+    P, steps = 5, 8
+    o = Oracle(cfg, W)
+    o.set_policy(4)
+    o.prefill(S.gen_prompt(cfg, P))
+    events = {L: [] for L in range(cfg.n_layers)}
+    agree = 0
+    for s in range(steps):
+        o.decode_step()
+        H, pred, use = o.trace_h(), o.pred_idx(), o.route_idx()
+        for L in range(1, cfg.n_layers):
+            g2 = S.as_f32(cfg, W["layers"][L]["g2"]).astype(np.float64)
+            Wr = S.as_f32(cfg, W["layers"][L]["router"]).astype(np.float64)
+            h = H[L].astype(np.float64)
+            y = h / np.sqrt(np.mean(h * h) + cfg.rms_eps) * g2
+            lg = Wr @ y
+            want = list(np.argsort(-lg, kind="stable")[:cfg.top_k])
+            assert pred[L].tolist() == [int(e) for e in want], (s, L)
+            agree += len(set(want) & set(use[L].tolist()))
+        for L in range(cfg.n_layers):
+            if L >= 1:
+                events[L].append(("pred", pred[L].tolist()))
+            events[L].append(("use", use[L].tolist()))
+    hits = misses = pref = 0
+    for L in range(cfg.n_layers):
+        h_, m_, pf, order = _lru_sim(cfg.cache_slots, events[L], 4)
+        hits += h_; misses += m_; pref += pf
+        assert o.lru()[L].tolist() == order
+    st = o.stats()
+    assert (st["expert_hits"], st["expert_misses"], st["prefetched"]) == (hits, misses, pref)
+    # the previous-layer residual is an informative predictor (PAPER.md Fig. 9a): far above chance (top_k / n_e per slot)
+    assert agree > 1.5 * steps * (cfg.n_layers - 1) * cfg.top_k * cfg.top_k / cfg.n_experts
+
+
 def test_I18_moe_topk_mixture_bruteforce():
     """PAPER.md L131 / SURVEY §8(c).1 'MoE layer': h_{i+1} = h' + sum_{e in top-2} w_e Expert_e(rms(h'; g2)) with
     n_e = 8, top_k = 2 and RENORMALISED weights, against a numpy restatement (attention over the oracle's own
