@@ -575,8 +575,14 @@ def run_olmoe(args):
            "expert_bytes": 3 * cfg.d_model * cfg.d_ff_expert * 2, "aot_schedule": "layer i -> {2i+2, 2i+3}, i < 8"}, "runs": []}
     names = {M.POLICY_FIXED: "fixed + on-demand", M.POLICY_LRU: "LRU", M.POLICY_LRU_RANDOM: "LRU + random speculation",
              M.POLICY_LRU_PREV: "LRU + previous-layer residual", M.POLICY_LRU_AOT: "LRU + accelerated residual (M2R2 AoT)"}
+    # random-init routers on random-init hidden states pick almost the same experts every step (LRU hit rate 0.995), so
+    # two of the eight routed experts per layer and step follow the seeded router script (reused from the previous step
+    # with probability rho = 0.25, predicted correctly with probability pi = 0.9); the other six stay natural
+    act, pred = S.gen_router_script(cfg, P + STEPS + 44, 0.25, 0.9)
+    out["router_script"] = {"rho": 0.25, "pi": 0.9, "scripted_experts_per_layer": 2}
     for pol in (M.POLICY_FIXED, M.POLICY_LRU, M.POLICY_LRU_RANDOM, M.POLICY_LRU_PREV, M.POLICY_LRU_AOT):
         eng.set_policy(pol)
+        eng.set_router_script(act, pred, 0)
         eng.prefill(prompt)
         for _ in range(4):
             eng.decode_step()
