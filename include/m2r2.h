@@ -85,6 +85,10 @@ typedef struct m2r2_config {
   int32_t renorm_topk;
   int32_t aot_lo[M2R2_MAX_LAYERS];       /* source layer i predicts experts of layers        */
   int32_t aot_hi[M2R2_MAX_LAYERS];       /* [aot_lo[i], aot_hi[i]); R=2 -> {2i+2, 2i+3} L137 */
+  /* Attention FLOPs optimisation (footnote 4 L170: k = 64): per head, the accelerated stream attends only the
+   * k cached positions with the largest attention coefficients of the slow stream (same head, same token; ties: lower
+   * position), plus its own k^_t.  0 = every cached position.  With k > 0 a step runs the per-operation kernels. */
+  int32_t accel_topk_tokens;
 } m2r2_config;
 
 typedef struct m2r2_sizes {

@@ -87,6 +87,7 @@ class ModelConfig:
     accel_mlp_rank: int = 0
     renorm_topk: bool = True
     aot_targets: Tuple[Tuple[int, int], ...] = ()   # per source layer: [lo, hi) target layers
+    accel_topk_tokens: int = 0                      # p attends the slow stream's top-k cached positions (0 = all)
     seed: int = 0x4D325232
 
     @property

@@ -39,7 +39,8 @@ class _Config(ctypes.Structure):
                 ("n_experts", ctypes.c_int32), ("top_k", ctypes.c_int32),
                 ("d_ff_expert", ctypes.c_int32), ("cache_slots", ctypes.c_int32),
                 ("accel_mlp_rank", ctypes.c_int32), ("renorm_topk", ctypes.c_int32),
-                ("aot_lo", ctypes.c_int32 * MAX_LAYERS), ("aot_hi", ctypes.c_int32 * MAX_LAYERS)]
+                ("aot_lo", ctypes.c_int32 * MAX_LAYERS), ("aot_hi", ctypes.c_int32 * MAX_LAYERS),
+                ("accel_topk_tokens", ctypes.c_int32)]
 
 
 class _Stats(ctypes.Structure):
@@ -91,6 +92,8 @@ def lib():
         L.orc_last_draft_margin.argtypes = [vp]
         L.orc_step_min_margin.restype = f32
         L.orc_step_min_margin.argtypes = [vp]
+        L.orc_topk_margin.restype = f32
+        L.orc_topk_margin.argtypes = [vp]
         L.orc_get_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
         L.orc_rope.argtypes = [vp, vp, i32]
         L.orc_rmsnorm.argtypes = [vp, vp, vp, vp]
@@ -122,6 +125,7 @@ def _fill_config(c) -> _Config:
     s.renorm_topk = int(c.renorm_topk)
     for i, (lo, hi) in enumerate(c.aot_targets):
         s.aot_lo[i], s.aot_hi[i] = lo, hi
+    s.accel_topk_tokens = int(getattr(c, "accel_topk_tokens", 0))
     return s
 
 
@@ -244,6 +248,10 @@ class Oracle:
 
     def draft_margin(self):
         return float(self.L.orc_last_draft_margin(self.h))
+
+    def topk_margin(self):
+        """smallest gap between the k-th and (k+1)-th slow attention score of any top-k token selection of the last step"""
+        return float(self.L.orc_topk_margin(self.h))
 
     def step_margin(self):
         """smallest top-2 margin of any argmax (every draft, every verify row) of the last step"""

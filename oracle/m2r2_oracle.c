@@ -49,6 +49,7 @@ typedef struct {
   int32_t accel_end_layer, lm_head_adapter;
   int32_t n_experts, top_k, d_ff_expert, cache_slots, accel_mlp_rank, renorm_topk;
   int32_t aot_lo[ORC_MAX_LAYERS], aot_hi[ORC_MAX_LAYERS];
+  int32_t accel_topk_tokens; /* p attends only the top-k cached positions of the slow stream (0 = all) */
 } orc_config;
 
 /* tensor ids for orc_set_tensor (same names as m2r2_synth.KIND_ID, own numbering) */
@@ -90,6 +91,8 @@ typedef struct orc {
   orc_stats st;
   /* traces of the last decode_step (or last verify row) */
   float* trH;        /* [(N+1)][d]: h_0 .. h_N */
+  float* slow_q;     /* [d]: rotated slow query of the last single-row slow_layer call */
+  float topk_margin; /* smallest gap between the k-th and (k+1)-th slow score of any top-k selection of the last step */
   float* trP;        /* [(N+1)][d]: p_0 .. ; p_{i+1} is the value BEFORE a gate reset */
   float* logits;     /* [V] final-head logits, before script bias */
   float* exit_logits;/* [J][V] accelerated-stream exit logits at each gate, before bias */
@@ -431,6 +434,7 @@ static void slow_layer(orc* o, int i, float* H, int m, int t0, int use_events) {
     free(U);
     free(Z);
   }
+  if (m == 1 && o->slow_q) memcpy(o->slow_q, Q, sizeof(float) * d); /* rotated slow query of this token (top-k token selection of the accelerated stream) */
   free(X); free(Q); free(Kn); free(Vn); free(O); free(Y);
 }
 
@@ -467,8 +471,36 @@ static void accel_layer(orc* o, int i, float* p, int t) {
   double scale = 1.0 / sqrt((double)dh);
   float* sc = (float*)malloc(sizeof(float) * (size_t)(t + 1));
   double* ex = (double*)malloc(sizeof(double) * (size_t)(t + 1));
+  const int topk = c->accel_topk_tokens;
+  float* ssc = (float*)malloc(sizeof(float) * (size_t)(t + 1));   /* slow scores (selection) */
+  char* keep = (char*)malloc((size_t)(t + 1));
   for (int s = 0; s < ns; ++s) {
     int a = c->accel_heads[s];
+    /* Attention FLOPs optimisation (footnote 4 L170; Q21): per head, the accelerated stream
+     * attends only the `topk` cached positions with the largest attention coefficients of the SLOW stream (same head,
+     * same token; softmax is monotone, so: the largest scores q_h . K_h[u]; ties: lower position first) plus its own
+     * k^_t, and assigns its own coefficients to them. */
+    for (int u = 0; u <= t; ++u) keep[u] = 1;
+    if (topk > 0 && t > topk) {
+      for (int u = 0; u < t; ++u) {
+        double acc = 0;
+        for (int j = 0; j < dh; ++j) acc += (double)o->slow_q[a * dh + j] * Kc[(size_t)u * d + a * dh + j];
+        ssc[u] = (float)(acc * scale);
+        keep[u] = 0;
+      }
+      float last = 0.f;
+      for (int r2 = 0; r2 < topk; ++r2) {
+        int best = -1;
+        for (int u = 0; u < t; ++u)
+          if (!keep[u] && (best < 0 || ssc[u] > ssc[best])) best = u;
+        keep[best] = 1;
+        last = ssc[best];
+      }
+      float next = -INFINITY;
+      for (int u = 0; u < t; ++u)
+        if (!keep[u] && ssc[u] > next) next = ssc[u];
+      if (last - next < o->topk_margin) o->topk_margin = last - next;
+    }
     for (int u = 0; u < t; ++u) {
       double acc = 0;
       for (int j = 0; j < dh; ++j) acc += (double)q[s * dh + j] * Kc[(size_t)u * d + a * dh + j];
@@ -479,10 +511,10 @@ static void accel_layer(orc* o, int i, float* p, int t) {
       for (int j = 0; j < dh; ++j) acc += (double)q[s * dh + j] * k[s * dh + j];
       sc[t] = (float)(acc * scale);
     }
-    float mx = sc[0];
-    for (int u = 1; u <= t; ++u) if (sc[u] > mx) mx = sc[u];
+    float mx = sc[t];
+    for (int u = 0; u < t; ++u) if (keep[u] && sc[u] > mx) mx = sc[u];
     double sum = 0;
-    for (int u = 0; u <= t; ++u) { ex[u] = exp((double)(sc[u] - mx)); sum += ex[u]; }
+    for (int u = 0; u <= t; ++u) { ex[u] = keep[u] ? exp((double)(sc[u] - mx)) : 0.0; sum += ex[u]; }
     for (int j = 0; j < dh; ++j) {
       double acc = 0;
       for (int u = 0; u < t; ++u) acc += ex[u] * Vc[(size_t)u * d + a * dh + j];
@@ -492,6 +524,8 @@ static void accel_layer(orc* o, int i, float* p, int t) {
   }
   free(sc);
   free(ex);
+  free(ssc);
+  free(keep);
   /* 4. p' = p + W_o[:, S] o^ + B_o(A_o o^) */
   for (int n = 0; n < d; ++n) {
     double acc = 0;
@@ -657,6 +691,7 @@ orc* orc_create(const orc_config* cfg) {
   o->K = (float*)calloc((size_t)N * c->max_seq * d, sizeof(float));
   o->V = (float*)calloc((size_t)N * c->max_seq * d, sizeof(float));
   o->trH = (float*)calloc((size_t)(N + 1) * d, sizeof(float));
+  o->slow_q = (float*)calloc((size_t)d, sizeof(float));
   o->trP = (float*)calloc((size_t)(N + 1) * d, sizeof(float));
   o->logits = (float*)calloc((size_t)c->vocab, sizeof(float));
   o->exit_logits = (float*)calloc((size_t)(c->n_gates > 0 ? c->n_gates : 1) * c->vocab, sizeof(float));
@@ -683,7 +718,7 @@ void orc_reset(orc* o) {
 void orc_destroy(orc* o) {
   if (!o) return;
   for (int i = 0; i < o->c.n_layers; ++i) { free(o->L[i].ewg); free(o->L[i].ewu); free(o->L[i].ewd); }
-  free(o->L); free(o->K); free(o->V); free(o->trH); free(o->trP); free(o->logits);
+  free(o->L); free(o->K); free(o->V); free(o->trH); free(o->slow_q); free(o->trP); free(o->logits);
   free(o->exit_logits); free(o->route_idx); free(o->route_w); free(o->pred_idx); free(o->lru);
   free(o->ls_full); free(o->ls_draft); free(o->rs_actual); free(o->rs_pred);
   free(o);
@@ -764,6 +799,7 @@ int orc_prefill(orc* o, const int32_t* tokens, int P, int32_t* first_token) {
 
 /* decode_step: both streams through all layers for the pending (or forced) token */
 int orc_decode_step(orc* o, int force_token, int32_t* token_out, int32_t* exit_tokens) {
+  o->topk_margin = INFINITY;
   const orc_config* c = &o->c;
   if (!o->have_pending && force_token < 0) return -2;
   if (o->kv_len + 1 > c->max_seq) return -3;
@@ -791,6 +827,7 @@ int orc_decode_step(orc* o, int force_token, int32_t* token_out, int32_t* exit_t
  * (§2.3.2), verify gamma+1 positions with the slow stream, accept the longest
  * matching prefix plus the verifier's own token, roll kv_len back (Q10-Q13). */
 int orc_spec_step(orc* o, int gamma, int32_t* accepted, int32_t* n_accepted, int32_t* drafts_out) {
+  o->topk_margin = INFINITY;
   const orc_config* c = &o->c;
   if (!o->have_pending) return -2;
   if (gamma < 0 || gamma > 16) return -1;
@@ -848,6 +885,8 @@ const float* orc_exit_logits(const orc* o, int gate) { return o->exit_logits + (
 float orc_last_margin(const orc* o) { return o->last_margin; }
 float orc_last_draft_margin(const orc* o) { return o->last_draft_margin; }
 float orc_step_min_margin(const orc* o) { return o->step_min_margin; }
+/* smallest gap between the k-th and (k+1)-th slow score over the top-k token selections of the last step (INFINITY: none) */
+float orc_topk_margin(const orc* o) { return o->topk_margin; }
 float* orc_kcache(orc* o, int layer) { return o->K + (size_t)layer * o->c.max_seq * o->c.d_model; }
 float* orc_vcache(orc* o, int layer) { return o->V + (size_t)layer * o->c.max_seq * o->c.d_model; }
 const int32_t* orc_route_idx(const orc* o) { return o->route_idx; }

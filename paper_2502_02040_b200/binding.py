@@ -34,7 +34,7 @@ class Config(ctypes.Structure):
                 ("accel_end_layer", i32), ("lm_head_adapter", i32), ("exit_heads_enabled", i32),
                 ("n_experts", i32), ("top_k", i32), ("d_ff_expert", i32),
                 ("cache_slots_per_layer", i32), ("accel_mlp_rank", i32), ("renorm_topk", i32),
-                ("aot_lo", i32 * MAX_LAYERS), ("aot_hi", i32 * MAX_LAYERS)]
+                ("aot_lo", i32 * MAX_LAYERS), ("aot_hi", i32 * MAX_LAYERS), ("accel_topk_tokens", i32)]
 
 
 class Sizes(ctypes.Structure):
@@ -147,6 +147,7 @@ def make_config(c) -> Config:
     s.renorm_topk = int(c.renorm_topk)
     for i, (lo, hi) in enumerate(c.aot_targets):
         s.aot_lo[i], s.aot_hi[i] = lo, hi
+    s.accel_topk_tokens = int(getattr(c, "accel_topk_tokens", 0))
     return s
 
 

@@ -717,6 +717,118 @@ void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, in
   }
 }
 
+// ------------------------------------------------------------------ accelerated attention over the slow stream's top-k positions
+// PAPER.md L158, footnote 4 L170 (k = 64), Q21.  One CTA per (accelerated head, sequence):
+//   1. the SLOW query's scores q_h . K_h[u] / sqrt(d_h) over the cached positions u < t,
+//   2. the k largest (ties: lower position) by k rounds of a block-wide arg-max,
+//   3. the accelerated query's own softmax over those positions plus its own k^_t, v^_t (L76), written to attn_o.
+// A correctness path: on this hardware the dense accelerated query rides on the slow query's K/V tiles for free, so the
+// fused kernel keeps it dense and a model with accel_topk_tokens > 0 runs the per-operation kernels.
+struct TopkAttnArgs {
+  const float* qkv;      // [rows][3d], rotated; slow row b, accelerated row B + b
+  const void *Kc, *Vc;   // this layer's cache [B][n_heads][max_seq][dh]
+  const int* row_limit;  // [rows]: cached positions visible to the accelerated row = t
+  const int* accel_heads;// [n_accel] head ids (device)
+  float* out;            // attn_o [rows][d]
+  int B, n_heads, dh, d, max_seq, topk;
+  float scale;
+};
+template <typename KT>
+__global__ void __launch_bounds__(256) accel_topk_attn_kernel(TopkAttnArgs a) {
+  extern __shared__ float tk_sm[];
+  const int head = a.accel_heads[blockIdx.x], b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int dh = a.dh, t = a.row_limit[a.B + b], k = a.topk;
+  float* sc = tk_sm;                       // [max(t, 1)] slow scores
+  float* qs = sc + ((t + 3) & ~3) + 4;     // [dh] slow query, [dh] accelerated query
+  float* qa = qs + dh;
+  float* p = qa + dh;                      // [k + 1] accelerated scores / probabilities
+  int* sel = (int*)(p + k + 1);            // [k] selected positions
+  __shared__ float rv[8];
+  __shared__ int ri[8];
+  __shared__ float s_bc[2];
+  const KT* Kb = (const KT*)a.Kc + ((size_t)b * a.n_heads + head) * a.max_seq * dh;
+  const KT* Vb = (const KT*)a.Vc + ((size_t)b * a.n_heads + head) * a.max_seq * dh;
+  const float* qrow = a.qkv + (size_t)b * 3 * a.d + head * dh;
+  const float* arow = a.qkv + (size_t)(a.B + b) * 3 * a.d + head * dh;
+  for (int j = tid; j < dh; j += 256) { qs[j] = qrow[j]; qa[j] = arow[j]; }
+  __syncthreads();
+  const int nsel = min(t, k);
+  if (t > k) {
+    for (int u = tid; u < t; u += 256) {
+      float acc = 0.f;
+      for (int j = 0; j < dh; ++j) acc += qs[j] * to_f32(Kb[(size_t)u * dh + j]);
+      sc[u] = acc * a.scale;
+    }
+    __syncthreads();
+    for (int r = 0; r < k; ++r) {
+      float bv = -INFINITY;
+      int bi = 0x7fffffff;
+      for (int u = tid; u < t; u += 256) {
+        const float v = sc[u];
+        if (v > bv || (v == bv && u < bi)) { bv = v; bi = u; }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+      }
+      if (lane == 0) { rv[warp] = bv; ri[warp] = bi; }
+      __syncthreads();
+      if (tid == 0) {
+        for (int w = 1; w < 8; ++w)
+          if (rv[w] > rv[0] || (rv[w] == rv[0] && ri[w] < ri[0])) { rv[0] = rv[w]; ri[0] = ri[w]; }
+        sel[r] = ri[0];
+        sc[ri[0]] = -INFINITY;   // taken (scores are finite: -inf never competes)
+      }
+      __syncthreads();
+    }
+  } else {
+    for (int u = tid; u < t; u += 256) sel[u] = u;
+    __syncthreads();
+  }
+  // accelerated scores on the selected positions and on the token's own key
+  for (int i = tid; i <= nsel; i += 256) {
+    float acc = 0.f;
+    if (i < nsel) { for (int j = 0; j < dh; ++j) acc += qa[j] * to_f32(Kb[(size_t)sel[i] * dh + j]); }
+    else { for (int j = 0; j < dh; ++j) acc += qa[j] * arow[a.d + j]; }
+    p[i] = acc * a.scale;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    float mx = p[0];
+    for (int i = 1; i <= nsel; ++i) mx = fmaxf(mx, p[i]);
+    float sum = 0.f;
+    for (int i = 0; i <= nsel; ++i) { p[i] = __expf(p[i] - mx); sum += p[i]; }
+    s_bc[0] = 1.f / sum;
+  }
+  __syncthreads();
+  for (int j = tid; j < dh; j += 256) {
+    float acc = 0.f;
+    for (int i = 0; i < nsel; ++i) acc += p[i] * to_f32(Vb[(size_t)sel[i] * dh + j]);
+    acc += p[nsel] * arow[2 * a.d + j];
+    a.out[(size_t)(a.B + b) * a.d + head * dh + j] = acc * s_bc[0];
+  }
+}
+void launch_accel_topk_attn(cudaStream_t st, int dtype, const float* qkv, const void* Kc, const void* Vc, const int* row_limit,
+                            const int* accel_heads, int n_accel, float* out, int B, int n_heads, int dh, int d, int max_seq,
+                            int topk, float scale) {
+  TopkAttnArgs a;
+  a.qkv = qkv; a.Kc = Kc; a.Vc = Vc; a.row_limit = row_limit; a.accel_heads = accel_heads; a.out = out;
+  a.B = B; a.n_heads = n_heads; a.dh = dh; a.d = d; a.max_seq = max_seq; a.topk = topk; a.scale = scale;
+  const size_t sh = ((size_t)((max_seq + 3) & ~3) + 4 + 2 * dh + topk + 1 + topk) * sizeof(float);
+  dim3 grid(n_accel, B);
+  if (dtype == M2R2_FP32) {
+    static bool set = false;
+    if (!set) { cudaFuncSetAttribute(accel_topk_attn_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); set = true; }
+    accel_topk_attn_kernel<float><<<grid, 256, sh, st>>>(a);
+  } else {
+    static bool set = false;
+    if (!set) { cudaFuncSetAttribute(accel_topk_attn_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); set = true; }
+    accel_topk_attn_kernel<__nv_bfloat16><<<grid, 256, sh, st>>>(a);
+  }
+}
+
 // merge of the split partials; accelerated rows add their own (k^_t, v^_t) as one more key:
 //   MHA(p_t, h_<t (+) p_t, h_<t (+) p_t)
 __global__ void merge_kernel(MergeArgs a) {

@@ -116,7 +116,7 @@ struct m2r2_ctx {
   // scratch
   int *d_kv_len, *d_pending, *d_row_tok, *d_row_seq, *d_row_pos, *d_row_limit, *d_grp_rows;
   int *d_drafts, *d_vtok, *d_accepted, *d_nacc, *d_exit_tok, *d_out_tok, *d_force, *d_prompt;
-  int *d_qkv_bmap, *d_accel_cols, *d_ls_full, *d_ls_draft, *d_rs_actual, *d_rs_pred;
+  int *d_qkv_bmap, *d_accel_cols, *d_accel_heads, *d_ls_full, *d_ls_draft, *d_rs_actual, *d_rs_pred;
   int *d_route_idx, *d_pred_idx, *d_moe_ridx;
   float *resid, *xn, *U, *qkv, *attn_o, *act, *part_o, *part_ml, *logits, *exit_logits, *trace;
   float *moe_tmp, *route_w, *pred_w, *moe_wtab, *moe_rw;
@@ -194,6 +194,8 @@ static int validate(const m2r2_config* c) {
   if (c->dtype != M2R2_FP32 && c->dtype != M2R2_BF16) return M2R2_INVALID_ARG;
   if (c->max_batch < 1 || c->max_batch > M2R2_MAX_BATCH || c->max_seq < 1) return M2R2_INVALID_ARG;
   if (c->vocab < 2) return M2R2_INVALID_ARG;
+  if (c->accel_topk_tokens < 0 || c->accel_topk_tokens > 4096) return M2R2_INVALID_ARG;
+  if (c->accel_topk_tokens > 0 && ((size_t)c->max_seq + 8 + 2 * (size_t)c->head_dim + 2 * (size_t)c->accel_topk_tokens + 1) * 4 > (size_t)200 * 1024) return M2R2_INVALID_ARG;
   if (c->n_gates < 0 || c->n_gates > M2R2_MAX_GATES) return M2R2_INVALID_ARG;
   for (int j = 0; j < c->n_gates; ++j) {
     if (c->gates[j] < 1 || c->gates[j] > c->n_layers) return M2R2_INVALID_ARG;
@@ -292,7 +294,7 @@ static void carve_scratch(const m2r2_config& c, Carver& cv, m2r2_ctx* x) {
   TAKE(d_drafts, int, B * 8) TAKE(d_vtok, int, B * 8) TAKE(d_accepted, int, B * 8) TAKE(d_nacc, int, B)
   TAKE(d_exit_tok, int, B * G) TAKE(d_out_tok, int, B) TAKE(d_force, int, B)
   TAKE(d_prompt, int, B * S)
-  TAKE(d_qkv_bmap, int, 3 * d) TAKE(d_accel_cols, int, da)
+  TAKE(d_qkv_bmap, int, 3 * d) TAKE(d_accel_cols, int, da) TAKE(d_accel_heads, int, M2R2_MAX_HEADS)
   TAKE(d_ls_full, int, B * S) TAKE(d_ls_draft, int, B * S)
   TAKE(d_rs_actual, int, c.n_experts ? S * N * 2 : 1) TAKE(d_rs_pred, int, c.n_experts ? S * N * 2 : 1)
   TAKE(d_route_idx, int, N * tk) TAKE(d_pred_idx, int, N * tk)
@@ -399,6 +401,8 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
         for (int j = 0; j < dh; ++j) cols[s * dh + j] = c.accel_heads[s] * dh + j;
     CUX(cudaMemcpyAsync(x->d_qkv_bmap, bmap.data(), bmap.size() * sizeof(int), cudaMemcpyHostToDevice, x->cs));
     CUX(cudaMemcpyAsync(x->d_accel_cols, cols.data(), cols.size() * sizeof(int), cudaMemcpyHostToDevice, x->cs));
+    if (c.accel_enabled && c.n_accel_heads > 0)
+      CUX(cudaMemcpyAsync(x->d_accel_heads, c.accel_heads, sizeof(int) * c.n_accel_heads, cudaMemcpyHostToDevice, x->cs));
     CUX(cudaStreamSynchronize(x->cs));
   }
   CUX(cudaMallocHost((void**)&x->h_pinned, 4096 * sizeof(int)));
@@ -723,7 +727,9 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     a.n_heads = nh; a.dh = dh; a.d = d; a.max_seq = c.max_seq; a.n_splits = splits; a.slow_rows = acc_on ? ns : (1 << 30);
     memcpy(a.accel_head_mask, x->accel_mask, sizeof(a.accel_head_mask));
     a.scale = scale;
-    if (!acc_on && dual) {
+    // PAPER.md L158 / L170: with accel_topk_tokens the accelerated rows attend the slow stream's top-k positions in their own kernel
+    const bool topk_accel = acc_on && c.accel_topk_tokens > 0;
+    if ((!acc_on && dual) || topk_accel) {
       // groups still list the accelerated rows; hide them by marking every row as slow-limited
       a.slow_rows = ns;
       memset(a.accel_head_mask, 0, sizeof(a.accel_head_mask));
@@ -734,8 +740,14 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     mg.qkv = x->qkv; mg.part_o = x->part_o; mg.part_ml = x->part_ml; mg.row_limit = x->d_row_limit; mg.out = x->attn_o;
     mg.n_heads = nh; mg.dh = dh; mg.d = d; mg.n_splits = splits; mg.slow_rows = ns;
     memcpy(mg.accel_head_mask, x->accel_mask, sizeof(mg.accel_head_mask));
+    if (topk_accel) memset(mg.accel_head_mask, 0, sizeof(mg.accel_head_mask));   // accelerated rows: zero here, S heads written below
     mg.scale = scale;
     launch_merge(x->cs, mg, rows);
+    if (topk_accel) {
+      launch_accel_topk_attn(x->cs, c.dtype, x->qkv, Kc, Vc, x->d_row_limit, x->d_accel_heads, c.n_accel_heads, x->attn_o, B, nh, dh, d,
+                             c.max_seq, c.accel_topk_tokens, scale);
+      count(x);
+    }
     count(x, 5);
     // a5: O-proj + residual
     prof_mark(x, M2R2_PROF_OPROJ);
@@ -1046,7 +1058,7 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
   bytes += (int64_t)c.vocab * c.d_model * x->esz * (1 + (c.exit_heads_enabled ? c.n_gates : 0)) + (int64_t)c.d_model * x->esz * B;
   x->st.algorithmic_bytes_last = bytes;
 
-  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1;
+  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1 && c.accel_topk_tokens == 0;   // the fused kernel keeps p's attention dense
   if (use_fused) {
     prof_mark(x, M2R2_PROF_FUSED_STEP);
     FusedRun fr = {c.n_layers, 0, force_tokens ? x->d_force : x->d_pending, 0, x->d_out_tok, 1, c.exit_heads_enabled, 1};
@@ -1094,7 +1106,7 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
     if (x->kv_h[b] + k + 1 > c.max_seq) return fail(x, M2R2_CAPACITY, "kv cache full");
   int64_t bytes = 0;
   // a10: draft loop — k dependent passes of layers 0..E-1 (both streams) + draft head
-  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1;
+  const bool use_fused = x->fused && fused_supported(c, &x->fs) && B == 1 && c.accel_topk_tokens == 0;
   for (int j = 0; j < k; ++j) {
     if (use_fused) {
       prof_mark(x, M2R2_PROF_FUSED_STEP);

@@ -136,6 +136,9 @@ void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int sl
                         int dh, int max_seq);
 void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group);
 void launch_merge(cudaStream_t st, const MergeArgs& a, int rows);
+void launch_accel_topk_attn(cudaStream_t st, int dtype, const float* qkv, const void* Kc, const void* Vc, const int* row_limit,
+                            const int* accel_heads, int n_accel, float* out, int B, int n_heads, int dh, int d, int max_seq,
+                            int topk, float scale);
 void launch_argmax(cudaStream_t st, const float* logits, int ldl, int rows, int V, const int* row_seq,
                    const int* row_pos, const int* script, int script_first, int script_n, float beta,
                    int* out, int out_stride);

@@ -75,8 +75,11 @@ def np_rope(cfg, v, t):
     return v.reshape(-1)
 
 
-def np_accel_layer(cfg, Lw, p, t, Kc, Vc):
-    """Brute-force accelerated layer for a dense model.  Kc/Vc: slow cache [>=t, d]."""
+def np_accel_layer(cfg, Lw, p, t, Kc, Vc, h=None, topk=0):
+    """Brute-force accelerated layer for a dense model.  Kc/Vc: slow cache [>=t, d].
+    topk > 0: per head the accelerated query attends only the `topk` cached positions with the
+    largest SLOW attention scores (slow query of the same token = rope(W_q rms(h; g1)) with `h` the slow residual
+    entering the layer; ties: lower position) plus its own key."""
     f = lambda k: S.as_f32(cfg, Lw[k]).astype(np.float64)
     dh = cfg.head_dim
     Sh = list(cfg.accel_heads)
@@ -92,6 +95,14 @@ def np_accel_layer(cfg, Lw, p, t, Kc, Vc):
         Kmat = np.vstack([Kc[:t, a * dh:(a + 1) * dh].astype(np.float64), k[sl][None]])   # (t+1, dh)
         Vmat = np.vstack([Vc[:t, a * dh:(a + 1) * dh].astype(np.float64), v[sl][None]])
         sc = Kmat @ q[sl] / np.sqrt(dh)
+        if topk and t > topk:
+            qs = np_rope(cfg, (f("wq") @ np_rms(cfg, h, f("g1"))).astype(np.float32), t)[a * dh:(a + 1) * dh].astype(np.float64)
+            ss = Kc[:t, a * dh:(a + 1) * dh].astype(np.float64) @ qs / np.sqrt(dh)
+            chosen = sorted(range(t), key=lambda u: (-ss[u], u))[:topk]
+            mask = np.full(t + 1, -np.inf)
+            mask[chosen] = 0.0
+            mask[t] = 0.0
+            sc = sc + mask
         pr = np.exp(sc - sc.max())
         pr /= pr.sum()
         o[sl] = pr @ Vmat

@@ -155,6 +155,62 @@ def test_I5_accelerated_attention_bruteforce(dtype):
     assert rel_l2(o0.accel_layer(0, p, 0), want0) < 2e-6
 
 
+# ---------------------------------------------------------------- I24
+@pytest.mark.parametrize("dtype", [S.FP32, S.BF16])
+def test_I24_topk_token_subset_accelerated_attention(dtype):
+    """PAPER.md L158, footnote 4 L170 (Q21): per head, p attends only the k cached positions with the largest
+    slow-stream attention coefficients (same head, same token) plus its own key.
+    (a) brute force in numpy float64 from the traces, the slow cache and the weights (selection from the SLOW query);
+    (b) k >= t is the dense accelerated attention, bit for bit; the slow stream never changes;
+    (c) with k < t the result differs from the dense one (the restriction is real) and perturbing a NON-selected cached
+        position's V leaves the accelerated output unchanged while a selected one changes it."""
+    k = 6
+    cfg = tiny(dtype=dtype, accel_topk_tokens=k)
+    dense = tiny(dtype=dtype)
+    W = S.gen_weights(cfg)
+    o, od = Oracle(cfg, W), Oracle(dense, W)
+    prompt = S.gen_prompt(cfg, 19)
+    assert o.prefill(prompt) == od.prefill(prompt)
+    for step in range(3):
+        tok = od.pending
+        o.decode_step(force_token=tok)
+        od.decode_step(force_token=tok)
+        H, P = o.trace_h(), o.trace_p()
+        assert np.array_equal(H, od.trace_h())                       # the slow stream is untouched
+        t = o.kv_len - 1
+        assert t > k and np.isfinite(o.topk_margin()) and o.topk_margin() > 0
+        differs = False
+        for i in range(cfg.accel_end_layer):
+            gated = i in cfg.gates
+            p_in = H[i] if (i == 0 or gated) else P[i]
+            want = np_accel_layer(cfg, W["layers"][i], p_in, t, o.kcache(i), o.vcache(i), h=H[i], topk=k)
+            assert rel_l2(P[i + 1], want) < 2e-6, (step, i)
+            differs |= rel_l2(P[i + 1], od.trace_p()[i + 1]) > 1e-6
+        assert differs
+    # (b) k >= t: identical to dense
+    big = Oracle(tiny(dtype=dtype, accel_topk_tokens=64), W)
+    od2 = Oracle(dense, W)
+    big.prefill(prompt); od2.prefill(prompt)
+    big.decode_step(); od2.decode_step()
+    assert np.array_equal(big.trace_p(), od2.trace_p()) and not np.isfinite(big.topk_margin())
+    # (c) selection is what restricts: layer 0, head S[0]
+    t = o.kv_len - 1
+    H = o.trace_h()
+    a, dh = cfg.accel_heads[0], cfg.head_dim
+    from tests.refs import np_rms, np_rope
+    f = lambda key: S.as_f32(cfg, W["layers"][0][key]).astype(np.float64)
+    qs = np_rope(cfg, (f("wq") @ np_rms(cfg, H[0], f("g1"))).astype(np.float32), t)[a * dh:(a + 1) * dh]
+    ss = o.kcache(0)[:t, a * dh:(a + 1) * dh].astype(np.float64) @ qs
+    order = sorted(range(t), key=lambda u: (-ss[u], u))
+    chosen, dropped = order[0], order[-1]
+    o.slow_layer(0, H[0], t)             # re-runs slow layer 0 of this token: the oracle now holds ITS slow query again
+    base = o.accel_layer(0, H[0], t)
+    o.vcache(0)[dropped, a * dh:(a + 1) * dh] += 7.0
+    assert np.array_equal(o.accel_layer(0, H[0], t), base)
+    o.vcache(0)[chosen, a * dh:(a + 1) * dh] += 7.0
+    assert not np.array_equal(o.accel_layer(0, H[0], t), base)
+
+
 # ---------------------------------------------------------------- I6
 def test_I6_incremental_equals_recompute():
     """KV-cache indexing: prefill(P) + q decode steps == prefill(P+q) at every position."""
