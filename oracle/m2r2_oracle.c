@@ -20,11 +20,18 @@
  * adapters + all heads => p == h; I4 gate reset; I5 brute-force h_{<t} (+) p_t attention;
  * I6 incremental == recompute; I7 lossless self-spec; I8 rollback; I9 spec(0)==decode;
  * I10 closed-form acceptance under the logit script; I12 RoPE relativity; I13 softmax /
- * top-k ties; I14 MoE n_e=1 == dense; I15 LRU vs brute force; I16 AoT targets {2i+2,2i+3}.
- * PARITY UNPINNED (the paper is silent; the oracle is the definition — DESIGN.md): adapter
- * parameterisation W x + B(A x) (Q3-Q5), accelerated MLP form (Q7), LM-head adapter (Q9),
- * gate placement for plain decode (Q15), which p feeds the expert predictor (Q16), router
- * normalisation (Q19), RoPE pairing / eps (Q1), gain init (Q22).
+ * top-k ties; I14 MoE n_e=1 == dense; I15 LRU vs brute force; I16 AoT targets {2i+2,2i+3};
+ * I18 top-2 expert mixture, I19 MoE accelerated bottleneck, I20 un-scripted expert predictor,
+ * I21 LM-head adapter (numpy brute force from the traces); I22 random speculation, I23
+ * previous-layer-residual speculation (PAPER.md L242 strategies 3 and 4: draws / router restated,
+ * counters vs the brute-force cache simulation); I24 top-k token-subset accelerated attention
+ * (L158, L170: numpy brute force, k >= t == dense, invisible non-selected positions).
+ * PARITY UNPINNED (the paper is silent ON THE CHOICE; the arithmetic of each choice is pinned above
+ * — DESIGN.md): adapter parameterisation W x + B(A x) (Q3-Q5), accelerated MLP form (Q7), LM-head
+ * adapter form (Q9), gate placement for plain decode (Q15), which p feeds the expert predictor
+ * (Q16), router normalisation (Q19), RoPE pairing / eps (Q1), gain init (Q22), how many experts and
+ * how far ahead the two comparison strategies speculate (Q24, Q25), the granularity of the top-k
+ * token selection (Q21).
  */
 #include <math.h>
 #include <stdint.h>
