@@ -420,12 +420,14 @@ def run_secondary(args):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the product has no CPU fallback")
     out = {"workload": args.workload, "data": "synthetic", "n_gpus": 1, "runs": []}
-    if args.workload == "c3":
-        cfg = S.config_c3()
+    if args.workload in ("c3", "gemma"):
+        # gemma: SURVEY 8(f) f-4, the paper's self-spec regime (Gemma-7B-class shape, E = 4, gamma = 3)
+        cfg = S.config_c3() if args.workload == "c3" else S.config_gemma7b_class()
+        out["model"] = cfg.name
         eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
         prompt = S.gen_prompt(cfg, PROMPT)
         for alpha in ((args.alpha,) if args.alpha else (0.9, 0.5)):
-            for gamma in ((args.gamma,) if args.gamma else (2, 4, 6)):
+            for gamma in ((args.gamma,) if args.gamma else ((2, 4, 6) if args.workload == "c3" else (3,))):
                 f, g = S.gen_logit_script(cfg, 400, alpha)
                 eng.set_logit_script(f, g, PROMPT)
                 eng.prefill(prompt)
@@ -612,9 +614,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--exit-heads", type=int, default=0, help="evaluate the exit argmax at every gate (SURVEY Q15 second row)")
     ap.add_argument("--no-fused", action="store_true", help="force the per-operation kernels")
-    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5", "olmoe"],
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5", "olmoe", "gemma"],
                     help="c2 = the bench line (default); c3/c4/c5 = secondary workloads of BASELINE.json configs[2..4]; "
-                         "olmoe = the five expert-loading strategies on an OLMoE-shaped model (SURVEY 8(f) f-2)")
+                         "olmoe = the five expert-loading strategies on an OLMoE-shaped model (SURVEY 8(f) f-2); gemma = self-spec on a "
+                         "Gemma-7B-class shape, E = 4, gamma = 3 (f-4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--gamma", type=int, default=0, help="--workload c3: one draft length instead of 2, 4, 6")
     ap.add_argument("--alpha", type=float, default=0.0, help="--workload c3: one acceptance rate instead of 0.9, 0.5")

@@ -157,6 +157,17 @@ def config_c5() -> ModelConfig:
                        aot_targets=tuple(tg), seed=0x4D325232 + 5)
 
 
+def config_gemma7b_class() -> ModelConfig:
+    """the regime of the paper's 2.8x (footnote 3 L133: Gemma-7B, drafts from the
+    first 4 layers' accelerated stream, draft length 3): a 7B-class decoder whose 256k-row LM head dominates a draft.
+    28 layers, d 3072, FFN 16384, vocab 256000, E = 4; 24 heads x 128 instead of Gemma's 16 x 256 and FFN 16384 instead
+    of 24576 (the fused kernel's limits: d_h <= 128, F <= 16384) -- 6.9 B parameters."""
+    return ModelConfig(name="Gemma7B-class-bf16", n_layers=28, d_model=3072, n_heads=24, head_dim=128,
+                       d_ff=16384, vocab=256000, dtype=BF16, max_seq=1024,
+                       accel_heads=tuple(range(6)), gates=(4,), accel_end_layer=4, lm_head_adapter=True,
+                       seed=0x4D325232 + 7)
+
+
 def config_olmoe_shaped() -> ModelConfig:
     """an OLMoE-shaped MoE decoder for the paper's five expert-loading strategies:
     16 layers, d 2048, 16 x 128 heads, 64 experts of FFN 1024 per layer, top-8, HALF of the experts resident (32 slots

@@ -75,14 +75,22 @@ def test_four_heads_long_context_unstaged_merge(P):
     assert worst <= 1e-2
 
 
-def test_unscripted_selfspec_draft_head_and_lm_adapter_match_oracle():
-    """a8/a10 on the path C3 runs: bf16 model with a single draft gate and the LM-head adapter, spec_step WITHOUT
+@pytest.mark.parametrize("shape", ["c3", "gemma"])
+def test_unscripted_selfspec_draft_head_and_lm_adapter_match_oracle(shape):
+    """(shape "gemma": SURVEY 8(f) f-4, the structure of `config_gemma7b_class` reduced: 128-wide heads, the draft gate
+    after ONE of six layers and a vocabulary 50x the model width, so the LM head dominates the draft as the 256k-row
+    head does at full size.)
+    a8/a10 on the path C3 runs: bf16 model with a single draft gate and the LM-head adapter, spec_step WITHOUT
     a logit script, so the draft tokens are decided by the fused draft pass itself (PH_HEAD with head_stream = 1:
     `LN_HEAD_P` loader, `lmA`/`lmB` adapter, joff > 0 positions).  After every step the draft logits of the LAST
     draft pass, the verify logits of the last accepted row, the accepted tokens and kv_len are compared with the
     oracle.  A token may differ only where the oracle's own margin (draft or verify) is below 1e-3 (Q23); that
     ends the comparison for the prompt, and further prompts run until 8 spec steps have been compared."""
-    cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2, lm_head_adapter=True)
+    if shape == "c3":
+        cfg = S.config_small_bf16(gates=(2,), accel_end_layer=2, lm_head_adapter=True)
+    else:
+        cfg = replace(S.config_small_bf16(gates=(1,), accel_end_layer=1, lm_head_adapter=True), name="S-gemma", d_model=384,
+                      n_heads=3, head_dim=128, accel_heads=(0,), vocab=19997)
     W = S.gen_weights(cfg)
     compared = 0
     for prompt_seed in range(4):
