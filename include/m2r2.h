@@ -89,6 +89,10 @@ typedef struct m2r2_config {
    * k cached positions with the largest attention coefficients of the slow stream (same head, same token; ties: lower
    * position), plus its own k^_t.  0 = every cached position.  With k > 0 a step runs the per-operation kernels. */
   int32_t accel_topk_tokens;
+  /* Accelerated Residual Latent Attention (footnote 2: d^s = 64): latent dimension of the exit router that
+   * scores each gate from the accelerated residuals of its whole interval.  0 = none.  Mechanics only: decode_step reports the
+   * scores (m2r2_debug_read M2R2_DBG_EXIT_SCORE); no layer is skipped. */
+  int32_t arla_dim;
 } m2r2_config;
 
 typedef struct m2r2_sizes {
@@ -130,6 +134,7 @@ typedef struct m2r2_weight_table {
   const void* lm_A;       /* host [r, d]  or NULL */
   const void* lm_B;       /* host [V, r]  or NULL */
   const m2r2_layer_weights* layers;   /* host array [n_layers] */
+  const void* arla;       /* host [n_gates * (3 d^s + 1), d] or NULL: per gate W_q^s, W_k^s, W_v^s [d^s, d], then one row = w_o[0..d^s), b */
 } m2r2_weight_table;
 
 typedef struct m2r2_stats {
@@ -225,7 +230,8 @@ enum {
   M2R2_DBG_V = 5,
   M2R2_DBG_ROUTE_IDX = 6,  /* routed experts of the last step, all layers -> [N][top_k]     */
   M2R2_DBG_ROUTE_W = 7,
-  M2R2_DBG_PRED_IDX = 8    /* predicted experts per target layer (-1 none) -> [N][top_k]    */
+  M2R2_DBG_PRED_IDX = 8,   /* predicted experts per target layer (-1 none) -> [N][top_k]    */
+  M2R2_DBG_EXIT_SCORE = 9  /* ARLA exit score of every gate, last decode_step      -> [J]    */
 };
 /* Copy n floats of an internal tensor of sequence b to host_out (integers as floats). */
 int m2r2_debug_read(m2r2_ctx* ctx, int32_t what, int32_t layer, int32_t b, float* host_out,

@@ -88,6 +88,7 @@ class ModelConfig:
     renorm_topk: bool = True
     aot_targets: Tuple[Tuple[int, int], ...] = ()   # per source layer: [lo, hi) target layers
     accel_topk_tokens: int = 0                      # p attends the slow stream's top-k cached positions (0 = all)
+    arla_dim: int = 0                               # latent dimension d^s of the exit router (0 = no ARLA)
     seed: int = 0x4D325232
 
     @property
@@ -208,9 +209,9 @@ def config_small_moe(**kw) -> ModelConfig:
 _KINDS = ["embed", "gf", "lm_head", "lm_A", "lm_B",
           "g1", "g2", "wq", "wk", "wv", "wo", "wgate", "wup", "wdown",
           "Aq", "Bq", "Ak", "Bk", "Av", "Bv", "Ao", "Bo", "Ag", "Bg", "Au", "Bu", "Ad", "Bd",
-          "router", "Ug", "Uu", "Ud", "ewg", "ewu", "ewd"]
+          "router", "Ug", "Uu", "Ud", "ewg", "ewu", "ewd", "arla"]
 KIND_ID = {k: i for i, k in enumerate(_KINDS)}
-GLOBAL_KINDS = ("embed", "gf", "lm_head", "lm_A", "lm_B")
+GLOBAL_KINDS = ("embed", "gf", "lm_head", "lm_A", "lm_B", "arla")
 EXPERT_KINDS = ("ewg", "ewu", "ewd")
 
 
@@ -223,6 +224,9 @@ def global_shapes(c: ModelConfig) -> Dict[str, Tuple[int, ...]]:
     if c.lm_head_adapter:
         s["lm_A"] = (c.adapter_rank, c.d_model)
         s["lm_B"] = (c.vocab, c.adapter_rank)
+    if c.arla_dim and c.accel_enabled and len(c.gates):
+        # ARLA exit router, one block per gate: W_q^s, W_k^s, W_v^s [d^s, d] each, then one row holding w_o[0..d^s) and b
+        s["arla"] = (len(c.gates) * (3 * c.arla_dim + 1), c.d_model)
     return s
 
 

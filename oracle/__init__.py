@@ -23,7 +23,7 @@ MAX_HEADS, MAX_GATES, MAX_LAYERS = 128, 16, 128
 _TENSORS = ["embed", "gf", "lm_head", "lm_A", "lm_B",
             "g1", "g2", "wq", "wk", "wv", "wo", "wgate", "wup", "wdown",
             "Aq", "Bq", "Ak", "Bk", "Av", "Bv", "Ao", "Bo", "Ag", "Bg", "Au", "Bu", "Ad", "Bd",
-            "router", "Ug", "Uu", "Ud", "ewg", "ewu", "ewd"]
+            "router", "Ug", "Uu", "Ud", "ewg", "ewu", "ewd", "arla"]
 _TID = {k: i for i, k in enumerate(_TENSORS)}
 
 
@@ -40,7 +40,7 @@ class _Config(ctypes.Structure):
                 ("d_ff_expert", ctypes.c_int32), ("cache_slots", ctypes.c_int32),
                 ("accel_mlp_rank", ctypes.c_int32), ("renorm_topk", ctypes.c_int32),
                 ("aot_lo", ctypes.c_int32 * MAX_LAYERS), ("aot_hi", ctypes.c_int32 * MAX_LAYERS),
-                ("accel_topk_tokens", ctypes.c_int32)]
+                ("accel_topk_tokens", ctypes.c_int32), ("arla_dim", ctypes.c_int32)]
 
 
 class _Stats(ctypes.Structure):
@@ -94,6 +94,8 @@ def lib():
         L.orc_step_min_margin.argtypes = [vp]
         L.orc_topk_margin.restype = f32
         L.orc_topk_margin.argtypes = [vp]
+        L.orc_exit_score.restype = f32
+        L.orc_exit_score.argtypes = [vp, ctypes.c_int32]
         L.orc_get_stats.argtypes = [vp, ctypes.POINTER(_Stats)]
         L.orc_rope.argtypes = [vp, vp, i32]
         L.orc_rmsnorm.argtypes = [vp, vp, vp, vp]
@@ -126,6 +128,7 @@ def _fill_config(c) -> _Config:
     for i, (lo, hi) in enumerate(c.aot_targets):
         s.aot_lo[i], s.aot_hi[i] = lo, hi
     s.accel_topk_tokens = int(getattr(c, "accel_topk_tokens", 0))
+    s.arla_dim = int(getattr(c, "arla_dim", 0))
     return s
 
 
@@ -139,7 +142,7 @@ class Oracle:
         self.L = lib()
         self._c = _fill_config(cfg)
         self.h = self.L.orc_create(ctypes.byref(self._c))
-        for k in ("embed", "gf", "lm_head", "lm_A", "lm_B"):
+        for k in ("embed", "gf", "lm_head", "lm_A", "lm_B", "arla"):
             if k in weights:
                 self._set(k, -1, 0, weights[k])
         for l, Lw in enumerate(weights["layers"]):
@@ -248,6 +251,10 @@ class Oracle:
 
     def draft_margin(self):
         return float(self.L.orc_last_draft_margin(self.h))
+
+    def exit_scores(self):
+        """ARLA exit score of every gate for the last decode_step"""
+        return np.array([self.L.orc_exit_score(self.h, j) for j in range(len(self.cfg.gates))], dtype=np.float32)
 
     def topk_margin(self):
         """smallest gap between the k-th and (k+1)-th slow attention score of any top-k token selection of the last step"""

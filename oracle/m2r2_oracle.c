@@ -25,13 +25,14 @@
  * I21 LM-head adapter (numpy brute force from the traces); I22 random speculation, I23
  * previous-layer-residual speculation (PAPER.md L242 strategies 3 and 4: draws / router restated,
  * counters vs the brute-force cache simulation); I24 top-k token-subset accelerated attention
- * (L158, L170: numpy brute force, k >= t == dense, invisible non-selected positions).
+ * (L158, L170: numpy brute force, k >= t == dense, invisible non-selected positions); I25 ARLA exit
+ * scores (L105-117: numpy brute force, W_v = 0 and W_q = 0 special cases).
  * PARITY UNPINNED (the paper is silent ON THE CHOICE; the arithmetic of each choice is pinned above
  * — DESIGN.md): adapter parameterisation W x + B(A x) (Q3-Q5), accelerated MLP form (Q7), LM-head
  * adapter form (Q9), gate placement for plain decode (Q15), which p feeds the expert predictor
  * (Q16), router normalisation (Q19), RoPE pairing / eps (Q1), gain init (Q22), how many experts and
  * how far ahead the two comparison strategies speculate (Q24, Q25), the granularity of the top-k
- * token selection (Q21).
+ * token selection (Q21), ARLA's states, normalisation and output map (Q26).
  */
 #include <math.h>
 #include <stdint.h>
@@ -57,6 +58,7 @@ typedef struct {
   int32_t n_experts, top_k, d_ff_expert, cache_slots, accel_mlp_rank, renorm_topk;
   int32_t aot_lo[ORC_MAX_LAYERS], aot_hi[ORC_MAX_LAYERS];
   int32_t accel_topk_tokens; /* p attends only the top-k cached positions of the slow stream (0 = all) */
+  int32_t arla_dim;          /* latent dimension d^s of the ARLA exit router (0 = none) */
 } orc_config;
 
 /* tensor ids for orc_set_tensor (same names as m2r2_synth.KIND_ID, own numbering) */
@@ -64,7 +66,7 @@ enum {
   T_EMBED = 0, T_GF, T_LM_HEAD, T_LM_A, T_LM_B,
   T_G1, T_G2, T_WQ, T_WK, T_WV, T_WO, T_WGATE, T_WUP, T_WDOWN,
   T_AQ, T_BQ, T_AK, T_BK, T_AV, T_BV, T_AO, T_BO, T_AG, T_BG, T_AU, T_BU, T_AD, T_BD,
-  T_ROUTER, T_UG, T_UU, T_UD, T_EWG, T_EWU, T_EWD, T_COUNT
+  T_ROUTER, T_UG, T_UU, T_UD, T_EWG, T_EWU, T_EWD, T_ARLA, T_COUNT
 };
 
 typedef struct {
@@ -103,6 +105,7 @@ typedef struct orc {
   float* trP;        /* [(N+1)][d]: p_0 .. ; p_{i+1} is the value BEFORE a gate reset */
   float* logits;     /* [V] final-head logits, before script bias */
   float* exit_logits;/* [J][V] accelerated-stream exit logits at each gate, before bias */
+  float exit_score[ORC_MAX_GATES]; /* ARLA exit scores of the last decode_step */
   float last_margin; /* top-2 margin of the last final argmax (after bias) */
   float last_draft_margin;
   float step_min_margin; /* introspection: smallest top-2 margin of any argmax (draft or verify) of the last spec_step / decode_step */
@@ -682,6 +685,50 @@ static void dual_token(orc* o, int token, int t, int n_run, int accel, float* h,
   }
 }
 
+/* Accelerated Residual Latent Attention (Fig. 4a; Q26): the exit decision at gate E_j looks at
+ * the accelerated residuals of the whole interval, z_i for i = E_{j-1} .. E_j (z at the interval's start = the slow residual p
+ * was re-initialised from, L82; z_{E_j} = p before the reset).  The states are projected into a latent space of dimension d^s
+ * (footnote 2: 64), Q^s = W_q z, K^s = W_k z, V^s = W_v z; the query of the state AT the gate attends the keys of all states
+ * of the interval; the exit score is sigma(w_o . (softmax(q K^T / sqrt(d^s)) V) + b).  Mechanics only: the score is reported,
+ * no layer is skipped (the paper does not say how skipped layers' K/V are filled, L248). */
+static void arla_scores(orc* o) {
+  const orc_config* c = &o->c;
+  const int ds = c->arla_dim, d = c->d_model;
+  if (ds <= 0 || !o->g[T_ARLA]) return;
+  for (int j = 0; j < c->n_gates; ++j) {
+    const int lo = j ? c->gates[j - 1] : 0, hi = c->gates[j], n = hi - lo + 1;
+    const size_t r0 = (size_t)j * (3 * ds + 1);
+    float* q = (float*)malloc(sizeof(float) * ds);
+    float* K = (float*)malloc(sizeof(float) * (size_t)n * ds);
+    float* V = (float*)malloc(sizeof(float) * (size_t)n * ds);
+    for (int s = 0; s < n; ++s) {
+      const int i = lo + s;
+      const float* z = (s == 0) ? o->trH + (size_t)i * d : o->trP + (size_t)i * d;
+      for (int e = 0; e < ds; ++e) {
+        K[(size_t)s * ds + e] = (float)dot_row(o, o->g[T_ARLA], r0 + ds + e, (size_t)d, 0, (size_t)d, z);
+        V[(size_t)s * ds + e] = (float)dot_row(o, o->g[T_ARLA], r0 + 2 * ds + e, (size_t)d, 0, (size_t)d, z);
+        if (s == n - 1) q[e] = (float)dot_row(o, o->g[T_ARLA], r0 + e, (size_t)d, 0, (size_t)d, z);
+      }
+    }
+    double sc[ORC_MAX_LAYERS + 1], mx = -INFINITY, sum = 0;
+    for (int s = 0; s < n; ++s) {
+      double acc = 0;
+      for (int e = 0; e < ds; ++e) acc += (double)q[e] * K[(size_t)s * ds + e];
+      sc[s] = acc / sqrt((double)ds);
+      if (sc[s] > mx) mx = sc[s];
+    }
+    for (int s = 0; s < n; ++s) { sc[s] = exp(sc[s] - mx); sum += sc[s]; }
+    double logit = wld(o, o->g[T_ARLA], (r0 + 3 * ds) * (size_t)d + ds); /* bias */
+    for (int e = 0; e < ds; ++e) {
+      double ce = 0;
+      for (int s = 0; s < n; ++s) ce += sc[s] / sum * V[(size_t)s * ds + e];
+      logit += (double)wld(o, o->g[T_ARLA], (r0 + 3 * ds) * (size_t)d + e) * (float)ce;
+    }
+    o->exit_score[j] = (float)(1.0 / (1.0 + exp(-logit)));
+    free(q); free(K); free(V);
+  }
+}
+
 /* ------------------------------------------------------------------ public API */
 orc* orc_create(const orc_config* cfg) {
   orc* o = (orc*)calloc(1, sizeof(orc));
@@ -733,7 +780,7 @@ void orc_destroy(orc* o) {
 
 int orc_set_tensor(orc* o, int id, int layer, int expert, const void* ptr) {
   if (id < 0 || id >= T_COUNT) return -1;
-  if (id <= T_LM_B) { o->g[id] = ptr; return 0; }
+  if (id <= T_LM_B || id == T_ARLA) { o->g[id] = ptr; return 0; }
   if (layer < 0 || layer >= o->c.n_layers) return -1;
   if (id >= T_EWG) {
     if (expert < 0 || expert >= o->c.n_experts) return -1;
@@ -816,6 +863,7 @@ int orc_decode_step(orc* o, int force_token, int32_t* token_out, int32_t* exit_t
   float* p = (float*)malloc(sizeof(float) * d);
   int t = o->kv_len;
   dual_token(o, tok_in, t, c->n_layers, 1, h, p, exit_tokens, 1);
+  arla_scores(o);
   head_logits(o, h, 0, o->logits);
   int tok = pick_token(o, o->logits, t + 1, 0, &o->last_margin);
   o->step_min_margin = o->last_margin;
@@ -894,6 +942,7 @@ float orc_last_draft_margin(const orc* o) { return o->last_draft_margin; }
 float orc_step_min_margin(const orc* o) { return o->step_min_margin; }
 /* smallest gap between the k-th and (k+1)-th slow score over the top-k token selections of the last step (INFINITY: none) */
 float orc_topk_margin(const orc* o) { return o->topk_margin; }
+float orc_exit_score(const orc* o, int gate) { return (gate >= 0 && gate < o->c.n_gates) ? o->exit_score[gate] : -1.f; }
 float* orc_kcache(orc* o, int layer) { return o->K + (size_t)layer * o->c.max_seq * o->c.d_model; }
 float* orc_vcache(orc* o, int layer) { return o->V + (size_t)layer * o->c.max_seq * o->c.d_model; }
 const int32_t* orc_route_idx(const orc* o) { return o->route_idx; }

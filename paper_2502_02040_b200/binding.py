@@ -18,7 +18,7 @@ MAX_HEADS, MAX_GATES, MAX_LAYERS, MAX_BATCH, MAX_DRAFT = 128, 16, 128, 8, 7
 OK, INVALID_ARG, BAD_STATE, CAPACITY, CUDA, UNSUPPORTED = 0, -1, -2, -3, -4, -5
 FP32, BF16 = 0, 1
 POLICY_FIXED, POLICY_LRU, POLICY_LRU_AOT, POLICY_LRU_RANDOM, POLICY_LRU_PREV = 0, 1, 2, 3, 4
-DBG_H, DBG_P, DBG_LOGITS, DBG_EXIT_LOGITS, DBG_K, DBG_V, DBG_ROUTE_IDX, DBG_ROUTE_W, DBG_PRED_IDX = range(9)
+DBG_H, DBG_P, DBG_LOGITS, DBG_EXIT_LOGITS, DBG_K, DBG_V, DBG_ROUTE_IDX, DBG_ROUTE_W, DBG_PRED_IDX, DBG_EXIT_SCORE = range(10)
 
 i32, i64, u32, u64, f32, vp = (ctypes.c_int32, ctypes.c_int64, ctypes.c_uint32, ctypes.c_uint64,
                                ctypes.c_float, ctypes.c_void_p)
@@ -34,7 +34,7 @@ class Config(ctypes.Structure):
                 ("accel_end_layer", i32), ("lm_head_adapter", i32), ("exit_heads_enabled", i32),
                 ("n_experts", i32), ("top_k", i32), ("d_ff_expert", i32),
                 ("cache_slots_per_layer", i32), ("accel_mlp_rank", i32), ("renorm_topk", i32),
-                ("aot_lo", i32 * MAX_LAYERS), ("aot_hi", i32 * MAX_LAYERS), ("accel_topk_tokens", i32)]
+                ("aot_lo", i32 * MAX_LAYERS), ("aot_hi", i32 * MAX_LAYERS), ("accel_topk_tokens", i32), ("arla_dim", i32)]
 
 
 class Sizes(ctypes.Structure):
@@ -59,7 +59,7 @@ class LayerWeights(ctypes.Structure):
 
 class WeightTable(ctypes.Structure):
     _fields_ = [("embed", vp), ("gf", vp), ("lm_head", vp), ("lm_A", vp), ("lm_B", vp),
-                ("layers", ctypes.POINTER(LayerWeights))]
+                ("layers", ctypes.POINTER(LayerWeights)), ("arla", vp)]
 
 
 class Stats(ctypes.Structure):
@@ -148,6 +148,7 @@ def make_config(c) -> Config:
     for i, (lo, hi) in enumerate(c.aot_targets):
         s.aot_lo[i], s.aot_hi[i] = lo, hi
     s.accel_topk_tokens = int(getattr(c, "accel_topk_tokens", 0))
+    s.arla_dim = int(getattr(c, "arla_dim", 0))
     return s
 
 
@@ -237,7 +238,7 @@ class Engine:
                     keep.append(arr)
                     setattr(layers[i], field, ctypes.cast(arr, ctypes.POINTER(vp)))
         t = WeightTable()
-        for n in ("embed", "gf", "lm_head", "lm_A", "lm_B"):
+        for n in ("embed", "gf", "lm_head", "lm_A", "lm_B", "arla"):
             if n in W:
                 setattr(t, n, W[n].ctypes.data)
         t.layers = ctypes.cast(layers, ctypes.POINTER(LayerWeights))
@@ -321,7 +322,7 @@ class Engine:
         if n is None:
             n = {DBG_H: cfg.d_model, DBG_P: cfg.d_model, DBG_LOGITS: cfg.vocab, DBG_EXIT_LOGITS: cfg.vocab,
                  DBG_ROUTE_IDX: cfg.n_layers * max(1, cfg.top_k), DBG_ROUTE_W: cfg.n_layers * max(1, cfg.top_k),
-                 DBG_PRED_IDX: cfg.n_layers * max(1, cfg.top_k)}[what]
+                 DBG_PRED_IDX: cfg.n_layers * max(1, cfg.top_k), DBG_EXIT_SCORE: max(1, len(cfg.gates))}[what]
         out = np.zeros(n, dtype=np.float32)
         self._chk(self.L.m2r2_debug_read(self.h, what, layer, b, self._ptr(out), n), "debug_read")
         return out

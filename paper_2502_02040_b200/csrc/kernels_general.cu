@@ -881,6 +881,82 @@ void launch_merge(cudaStream_t st, const MergeArgs& a, int rows) {
 }
 
 // =====================================================================================
+// f-3  Accelerated Residual Latent Attention (Fig. 4a; Q26): one CTA per (gate, sequence).
+// States of the interval [E_{j-1}, E_j]: the residual p was re-initialised from at its start (h), then p_i, the last
+// one before the gate reset -- all in the step's trace.  K^s, V^s of every state and Q^s of the last one are d^s dot
+// products of length d each (a warp per dot product), then a softmax over <= N + 1 states and the sigmoid score.
+// =====================================================================================
+struct ArlaArgs {
+  const float* trace;    // [layer][2][B][d]
+  const void* W;         // [n_gates][3 ds + 1][d]
+  float* score;          // [B][M2R2_MAX_GATES]
+  int gates[M2R2_MAX_GATES];
+  int n_gates, ds, d, B;
+};
+template <typename WT>
+__global__ void __launch_bounds__(256) arla_kernel(ArlaArgs a) {
+  extern __shared__ float ar_sm[];   // K [n][ds], V [n][ds], q [ds], sc [n]
+  const int j = blockIdx.x, b = blockIdx.y, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int lo = j ? a.gates[j - 1] : 0, hi = a.gates[j], n = hi - lo + 1, ds = a.ds, d = a.d;
+  float* K = ar_sm;
+  float* V = K + (size_t)n * ds;
+  float* q = V + (size_t)n * ds;
+  float* sc = q + ds;
+  const WT* W = (const WT*)a.W + (size_t)j * (3 * ds + 1) * d;
+  // dot products: item = (state s, which in {K, V, Q-of-last-state}, e)
+  const int items = (2 * n + 1) * ds;
+  for (int it = warp; it < items; it += 8) {
+    int s, which, e;
+    if (it < 2 * n * ds) { s = it / (2 * ds); which = (it / ds) & 1; e = it % ds; } else { s = n - 1; which = 2; e = it - 2 * n * ds; }
+    const float* z = a.trace + (((size_t)(lo + s) * 2 + (s == 0 ? 0 : 1)) * a.B + b) * d;
+    const WT* w = W + (size_t)((which == 2 ? 0 : (which == 0 ? ds : 2 * ds)) + e) * d;
+    float acc = 0.f;
+    for (int k = lane; k < d; k += 32) acc += to_f32(w[k]) * z[k];
+    acc = warp_sum(acc);
+    if (lane == 0) { if (which == 0) K[(size_t)s * ds + e] = acc; else if (which == 1) V[(size_t)s * ds + e] = acc; else q[e] = acc; }
+  }
+  __syncthreads();
+  if (tid < n) {
+    float acc = 0.f;
+    for (int e = 0; e < ds; ++e) acc += q[e] * K[(size_t)tid * ds + e];
+    sc[tid] = acc * rsqrtf((float)ds);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    float mx = sc[0];
+    for (int s = 1; s < n; ++s) mx = fmaxf(mx, sc[s]);
+    float sum = 0.f;
+    for (int s = 0; s < n; ++s) { sc[s] = expf(sc[s] - mx); sum += sc[s]; }
+    const WT* wo = W + (size_t)(3 * ds) * d;
+    float logit = to_f32(wo[ds]);
+    for (int e = 0; e < ds; ++e) {
+      float ce = 0.f;
+      for (int s = 0; s < n; ++s) ce += sc[s] / sum * V[(size_t)s * ds + e];
+      logit += to_f32(wo[e]) * ce;
+    }
+    a.score[(size_t)b * M2R2_MAX_GATES + j] = 1.f / (1.f + expf(-logit));
+  }
+}
+void launch_arla(cudaStream_t st, int dtype, const float* trace, const void* W, const int* gates, int n_gates, int ds, int d, int B,
+                 float* score_out) {
+  if (n_gates <= 0 || ds <= 0) return;
+  ArlaArgs a;
+  a.trace = trace; a.W = W; a.score = score_out; a.n_gates = n_gates; a.ds = ds; a.d = d; a.B = B;
+  int nmax = 1;
+  for (int j = 0; j < n_gates; ++j) { a.gates[j] = gates[j]; nmax = max(nmax, gates[j] - (j ? gates[j - 1] : 0) + 1); }
+  const size_t sh = ((size_t)2 * nmax * ds + ds + nmax) * sizeof(float);
+  dim3 grid(n_gates, B);
+  static bool set = false;
+  if (!set) {
+    cudaFuncSetAttribute(arla_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    cudaFuncSetAttribute(arla_kernel<__nv_bfloat16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    set = true;
+  }
+  if (dtype == M2R2_FP32) arla_kernel<float><<<grid, 256, sh, st>>>(a);
+  else arla_kernel<__nv_bfloat16><<<grid, 256, sh, st>>>(a);
+}
+
+// =====================================================================================
 // a8/a9  greedy argmax with the logit-script bias hook; lowest index wins ties.
 // =====================================================================================
 __global__ void __launch_bounds__(1024) argmax_kernel(const float* __restrict__ logits, int ldl, int V,

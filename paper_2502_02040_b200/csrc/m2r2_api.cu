@@ -88,7 +88,7 @@ struct m2r2_ctx {
   int kv_h[M2R2_MAX_BATCH];    // host mirror of kv_len
   size_t esz = 0;              // bytes per element
   // resident weights
-  const void *embed = nullptr, *gf = nullptr, *lm_head = nullptr, *lm_A = nullptr, *lm_B = nullptr;
+  const void *embed = nullptr, *gf = nullptr, *lm_head = nullptr, *lm_A = nullptr, *lm_B = nullptr, *arla = nullptr;
   void* packed = nullptr;      // tile-major copy of the big matrices for the fused kernel
   std::vector<DevLayer> L;
   // MoE
@@ -119,7 +119,7 @@ struct m2r2_ctx {
   int *d_qkv_bmap, *d_accel_cols, *d_accel_heads, *d_ls_full, *d_ls_draft, *d_rs_actual, *d_rs_pred;
   int *d_route_idx, *d_pred_idx, *d_moe_ridx;
   float *resid, *xn, *U, *qkv, *attn_o, *act, *part_o, *part_ml, *logits, *exit_logits, *trace;
-  float *moe_tmp, *route_w, *pred_w, *moe_wtab, *moe_rw;
+  float *moe_tmp, *route_w, *pred_w, *moe_wtab, *moe_rw, *exit_score;
   int last_rows_per_seq = 1;
   // CUDA graphs of the verify pass (a11 + a12), keyed by what fixes its launch arguments
   std::map<unsigned long long, cudaGraphExec_t> vgraph;
@@ -195,6 +195,8 @@ static int validate(const m2r2_config* c) {
   if (c->max_batch < 1 || c->max_batch > M2R2_MAX_BATCH || c->max_seq < 1) return M2R2_INVALID_ARG;
   if (c->vocab < 2) return M2R2_INVALID_ARG;
   if (c->accel_topk_tokens < 0 || c->accel_topk_tokens > 4096) return M2R2_INVALID_ARG;
+  if (c->arla_dim < 0 || c->arla_dim > 128) return M2R2_INVALID_ARG;
+  if (c->arla_dim > 0 && ((size_t)2 * (c->n_layers + 1) * c->arla_dim + c->arla_dim + c->n_layers + 1) * 4 > (size_t)160 * 1024) return M2R2_INVALID_ARG;
   if (c->accel_topk_tokens > 0 && ((size_t)c->max_seq + 8 + 2 * (size_t)c->head_dim + 2 * (size_t)c->accel_topk_tokens + 1) * 4 > (size_t)200 * 1024) return M2R2_INVALID_ARG;
   if (c->n_gates < 0 || c->n_gates > M2R2_MAX_GATES) return M2R2_INVALID_ARG;
   for (int j = 0; j < c->n_gates; ++j) {
@@ -255,6 +257,9 @@ static void walk_weights(const m2r2_config& c, WeightWalk& w, m2r2_ctx* ctx) {
     p = w.take(r * d); if (ctx) ctx->lm_A = p;
     p = w.take(V * r); if (ctx) ctx->lm_B = p;
   }
+  if (c.arla_dim > 0 && c.accel_enabled && c.n_gates > 0) {
+    p = w.take((size_t)c.n_gates * (3 * c.arla_dim + 1) * d); if (ctx) ctx->arla = p;
+  }
   for (int i = 0; i < c.n_layers; ++i) {
     DevLayer L;
     memset(&L, 0, sizeof(L));
@@ -297,7 +302,7 @@ static void carve_scratch(const m2r2_config& c, Carver& cv, m2r2_ctx* x) {
   TAKE(d_qkv_bmap, int, 3 * d) TAKE(d_accel_cols, int, da) TAKE(d_accel_heads, int, M2R2_MAX_HEADS)
   TAKE(d_ls_full, int, B * S) TAKE(d_ls_draft, int, B * S)
   TAKE(d_rs_actual, int, c.n_experts ? S * N * 2 : 1) TAKE(d_rs_pred, int, c.n_experts ? S * N * 2 : 1)
-  TAKE(d_route_idx, int, N * tk) TAKE(d_pred_idx, int, N * tk)
+  TAKE(d_route_idx, int, N * tk) TAKE(d_pred_idx, int, N * tk) TAKE(exit_score, float, M2R2_MAX_BATCH * M2R2_MAX_GATES)
   TAKE(resid, float, R * d) TAKE(xn, float, R * d) TAKE(U, float, R * 64)
   TAKE(qkv, float, R * 3 * d) TAKE(attn_o, float, R * d) TAKE(act, float, R * (size_t)fmax_act(c))
   TAKE(part_o, float, R * nh * M2R2_MAX_SPLITS * dh) TAKE(part_ml, float, R * nh * M2R2_MAX_SPLITS * 2)
@@ -514,6 +519,10 @@ extern "C" int m2r2_load_weights(m2r2_ctx* x, const m2r2_weight_table* t) {
 #define UP(dst, src, n) if ((rc = up(x, dst, src, n))) return rc
   UP(x->embed, t->embed, V * d); UP(x->gf, t->gf, d); UP(x->lm_head, t->lm_head, V * d);
   if (x->lm_A) { UP(x->lm_A, t->lm_A, r * d); UP(x->lm_B, t->lm_B, V * r); }
+  if (x->arla) {
+    if (!t->arla) return fail(x, M2R2_INVALID_ARG, "arla_dim > 0 but the weight table has no ARLA router");
+    UP(x->arla, t->arla, (size_t)c.n_gates * (3 * c.arla_dim + 1) * d);
+  }
   if (c.n_experts) { x->eg.assign(c.n_layers, {}); x->eu.assign(c.n_layers, {}); x->ed.assign(c.n_layers, {}); }
   for (int i = 0; i < c.n_layers; ++i) {
     const m2r2_layer_weights& h = t->layers[i];
@@ -1074,6 +1083,11 @@ extern "C" int m2r2_decode_step(m2r2_ctx* x, const int32_t* force_tokens, int32_
     advance_kernel<<<1, 32, 0, x->cs>>>(B, x->d_kv_len, x->d_pending, x->d_out_tok);
     count(x);
   }
+  if (x->arla) {
+    // f-3 ARLA mechanics: exit score of every gate from the step's traced accelerated residuals
+    launch_arla(x->cs, c.dtype, x->trace, x->arla, c.gates, c.n_gates, c.arla_dim, c.d_model, B, x->exit_score);
+    count(x);
+  }
   prof_resolve(x);
   for (int b = 0; b < B; ++b) x->kv_h[b] += 1;
   x->st.steps++;
@@ -1450,6 +1464,11 @@ extern "C" int m2r2_debug_read(m2r2_ctx* x, int32_t what, int32_t layer, int32_t
       CU(x, cudaStreamSynchronize(x->cs));
       return M2R2_OK;
     }
+    case M2R2_DBG_EXIT_SCORE:
+      if (!x->arla) return fail(x, M2R2_UNSUPPORTED, "debug_read: the config has no ARLA router");
+      src = x->exit_score + (size_t)b * M2R2_MAX_GATES;
+      avail = (size_t)c.n_gates;
+      break;
     case M2R2_DBG_ROUTE_W:
       src = x->route_w;
       avail = (size_t)c.n_layers * tk;

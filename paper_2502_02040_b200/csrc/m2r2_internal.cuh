@@ -142,6 +142,9 @@ void launch_accel_topk_attn(cudaStream_t st, int dtype, const float* qkv, const 
 void launch_argmax(cudaStream_t st, const float* logits, int ldl, int rows, int V, const int* row_seq,
                    const int* row_pos, const int* script, int script_first, int script_n, float beta,
                    int* out, int out_stride);
+// f-3: ARLA exit scores from the traced residuals [layer][2][B][d] (h then p); gates: host array [n_gates]
+void launch_arla(cudaStream_t st, int dtype, const float* trace, const void* W, const int* gates, int n_gates, int ds, int d, int B,
+                 float* score_out);
 void launch_copy_rows(cudaStream_t st, const float* src, float* dst, int rows, int d);
 void launch_route(cudaStream_t st, int dtype, const float* X, int ldx, int rows, int d, const void* g,
                   float eps, int do_norm, const void* Wr, int n_experts, int top_k, int renorm,

@@ -283,3 +283,32 @@ def test_topk_token_subset_selfspec_is_lossless_on_gpu():
         plain.append(int(b.decode_step()[0]))
     assert spec == plain[:len(spec)] and n_ok >= 3
     a.close(); b.close()
+
+
+# ------------------------------------------------------------------ f-3: ARLA mechanics
+@pytest.mark.parametrize("which", ["c1-fp32", "small-bf16-fused", "small-bf16-per-op"])
+def test_arla_exit_scores_match_oracle(which):
+    """the exit score of every gate, sigma(w_o . softmax(q K^T / sqrt(d^s)) V + b)
+    over the latent projections (d^s = 64, footnote 2) of the interval's accelerated residuals, computed by `arla_kernel`
+    from the traces of the decode step (fused kernel or per-operation kernels), against the oracle under teacher forcing."""
+    if which == "c1-fp32":
+        cfg, tol = replace(S.config_c1(), arla_dim=64), 2e-5
+    else:
+        cfg, tol = S.config_small_bf16(arla_dim=64), 2e-3
+    W = S.gen_weights(cfg)
+    eng, orc = M.Engine(cfg, W), Oracle(cfg, W)
+    if which == "small-bf16-per-op":
+        eng.set_fused(False)
+    prompt = S.gen_prompt(cfg, 21)
+    eng.prefill(prompt); orc.prefill(prompt)
+    seen = []
+    for s in range(5):
+        tok_in = orc.pending
+        orc.decode_step()
+        eng.decode_step(force_tokens=[tok_in])
+        got, want = eng.debug_read(M.DBG_EXIT_SCORE), orc.exit_scores()
+        assert got.shape == want.shape == (len(cfg.gates),)
+        assert np.max(np.abs(got - want)) <= tol, (s, got, want)
+        seen.append(want.copy())
+    assert np.ptp(np.stack(seen)) > 1e-4          # the scores depend on the token
+    eng.close()

@@ -211,6 +211,57 @@ def test_I24_topk_token_subset_accelerated_attention(dtype):
     assert not np.array_equal(o.accel_layer(0, H[0], t), base)
 
 
+# ---------------------------------------------------------------- I25
+@pytest.mark.parametrize("gates", [(2,), (1, 3)])
+def test_I25_arla_exit_scores_bruteforce(gates):
+    """PAPER.md L105-117, Fig. 4a (Q26): the exit score of gate E_j = sigma(w_o . softmax(q K^T / sqrt(d^s)) V + b)
+    with K, V the latent projections of the interval's residuals (the state p was re-initialised from, then every p_i up
+    to the one before the reset) and q the projection of the LAST one.  (a) numpy float64 brute force from the traces;
+    (b) W_v = 0 => sigma(b); (c) W_q = 0 => uniform attention => the value is the mean of the interval's V."""
+    ds = 8
+    cfg = tiny(arla_dim=ds, gates=gates)
+    W = S.gen_weights(cfg)
+    d = cfg.d_model
+
+    def brute(Wm, H, P):
+        A = S.as_f32(cfg, Wm["arla"]).astype(np.float64).reshape(len(gates), 3 * ds + 1, d)
+        out = []
+        for j, hi in enumerate(gates):
+            lo = gates[j - 1] if j else 0
+            Z = np.stack([H[lo]] + [P[i] for i in range(lo + 1, hi + 1)]).astype(np.float64)
+            Wq, Wk, Wv, wo, b = A[j, :ds], A[j, ds:2 * ds], A[j, 2 * ds:3 * ds], A[j, 3 * ds, :ds], A[j, 3 * ds, ds]
+            q, K, V = Wq @ Z[-1], Z @ Wk.T, Z @ Wv.T
+            sc = K @ q / np.sqrt(ds)
+            a = np.exp(sc - sc.max()); a /= a.sum()
+            out.append(1.0 / (1.0 + np.exp(-(wo @ (a @ V) + b))))
+        return np.array(out)
+
+    o = Oracle(cfg, W)
+    o.prefill(S.gen_prompt(cfg, 7))
+    for _ in range(3):
+        o.decode_step()
+        got = o.exit_scores()
+        want = brute(W, o.trace_h(), o.trace_p())
+        assert np.allclose(got, want, atol=2e-6), (got, want)
+        assert np.all((got > 0) & (got < 1)) and np.ptp(got) > 0 or len(gates) == 1
+    # (b), (c): edited copies of the router
+    A = W["arla"].reshape(len(gates), 3 * ds + 1, d)
+    Wb = dict(W); Ab = A.copy(); Ab[:, 2 * ds:3 * ds] = 0; Wb["arla"] = np.ascontiguousarray(Ab.reshape(-1, d))
+    ob = Oracle(cfg, Wb); ob.prefill(S.gen_prompt(cfg, 7)); ob.decode_step()
+    bias = S.as_f32(cfg, W["arla"]).reshape(len(gates), 3 * ds + 1, d)[:, 3 * ds, ds].astype(np.float64)
+    assert np.allclose(ob.exit_scores(), 1.0 / (1.0 + np.exp(-bias)), atol=1e-6)
+    Wc = dict(W); Ac = A.copy(); Ac[:, :ds] = 0; Wc["arla"] = np.ascontiguousarray(Ac.reshape(-1, d))
+    oc = Oracle(cfg, Wc); oc.prefill(S.gen_prompt(cfg, 7)); oc.decode_step()
+    Af = S.as_f32(cfg, W["arla"]).astype(np.float64).reshape(len(gates), 3 * ds + 1, d)
+    H, P = oc.trace_h(), oc.trace_p()
+    for j, hi in enumerate(gates):
+        lo = gates[j - 1] if j else 0
+        Z = np.stack([H[lo]] + [P[i] for i in range(lo + 1, hi + 1)]).astype(np.float64)
+        v = (Z @ Af[j, 2 * ds:3 * ds].T).mean(axis=0)
+        want = 1.0 / (1.0 + np.exp(-(Af[j, 3 * ds, :ds] @ v + Af[j, 3 * ds, ds])))
+        assert abs(oc.exit_scores()[j] - want) < 2e-6
+
+
 # ---------------------------------------------------------------- I6
 def test_I6_incremental_equals_recompute():
     """KV-cache indexing: prefill(P) + q decode steps == prefill(P+q) at every position."""
