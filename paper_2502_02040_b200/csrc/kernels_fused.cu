@@ -1728,6 +1728,7 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
   const int nch = (a.nkt + 16 * NQ - 1) / (16 * NQ);   // (super-)chunks of the whole K
   const int ch_lo = (int)(((long long)nch * blockIdx.y) / a.ksplit), ch_hi = (int)(((long long)nch * (blockIdx.y + 1)) / a.ksplit);
   const int wq = SW ? warp : 0;                    // the warp's quarter of the staged inputs
+  pdl_launch_dependents();                         // the next kernel of the chain may begin to launch
   for (int ch = ch_lo; ch < ch_hi; ++ch) {
     const int kbase = ch * NQ * RM_KC;
     // the warp's 16 weight tiles of this iteration: 16 LDG.128 per lane in flight while the activations are staged
@@ -1743,6 +1744,9 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
         w[u] = ldg_stream(a.W + tile * 32 + lane);
       }
     }
+    // weights never depend on the previous kernel: under programmatic dependent launch the first iteration's tiles are
+    // already in flight while the producer of the activation rows finishes
+    if (ch == ch_lo) pdl_wait();
     __syncthreads();   // the previous iteration's staged rows are consumed
     for (int i = tid; i < NG * 8 * (NQ * RM_KC / 4); i += 128) {
       const int row = i / (NQ * RM_KC / 4), q = i - row * (NQ * RM_KC / 4), k = kbase + 4 * q;
@@ -1765,6 +1769,7 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
       }
     }
   }
+  if (ch_lo >= ch_hi) pdl_wait();                  // (a CTA without chunks still orders its epilogue behind the predecessor)
   if (SW) {
     // the four warps' partial sums of the row tile -> warp 0
     __syncthreads();
@@ -2179,7 +2184,16 @@ static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
     cudaFuncSetAttribute(rows_mma_kernel<KIND, NG, SW>, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024);
     attr_set = true;
   }
-  rows_mma_kernel<KIND, NG, SW><<<grid, 128, sh, st>>>(a);
+  // programmatic dependent launch: the kernel starts while its predecessor in the stream drains and prefetches its first
+  // weight tiles; it reads activations only behind pdl_wait()
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = sh; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, rows_mma_kernel<KIND, NG, SW>, a);
 }
 template <int KIND>
 static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) {

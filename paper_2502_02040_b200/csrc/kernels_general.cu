@@ -47,6 +47,8 @@ __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict_
                                                         float* __restrict__ U, int ldu) {
   extern __shared__ float sx[];
   __shared__ float red[8];
+  pdl_launch_dependents();   // the GEMM that consumes xn may begin to launch and prefetch its weights
+  pdl_wait();
   int row = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const float* x = X + (size_t)row * d;
   float ss = 0.f;
@@ -88,9 +90,9 @@ void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int 
                       int ldu) {
   size_t sh = (size_t)d * sizeof(float);
   if (dtype == M2R2_FP32)
-    norm_lora_kernel<float><<<rows, 256, sh, st>>>(X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<float>, dim3(rows), dim3(256), sh, st, X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
   else
-    norm_lora_kernel<__nv_bfloat16><<<rows, 256, sh, st>>>(X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<__nv_bfloat16>, dim3(rows), dim3(256), sh, st, X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
 }
 
 // u[row][j] = A[j, :] . x[row][xmap(:)]   (no norm; A_o on the compact o^, A_d on the activations)
@@ -271,6 +273,8 @@ __global__ void rope_append_kernel(float* __restrict__ qkv, int slow_rows, const
                                    const int* __restrict__ row_pos, const float2* __restrict__ rope_tab,
                                    KT* __restrict__ Kc, KT* __restrict__ Vc, int n_heads, int dh,
                                    int max_seq) {
+  pdl_launch_dependents();
+  pdl_wait();
   int row = blockIdx.x, head = blockIdx.y, half = dh / 2, d = n_heads * dh;
   int pos = row_pos[row], seq = row_seq[row];
   float* q = qkv + (size_t)row * 3 * d + head * dh;
@@ -301,9 +305,9 @@ void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int sl
                         int dh, int max_seq) {
   dim3 grid(rows, n_heads);
   if (dtype == M2R2_FP32)
-    rope_append_kernel<float><<<grid, 64, 0, st>>>(qkv, slow_rows, row_seq, row_pos, rope_tab, (float*)Kc, (float*)Vc, n_heads, dh, max_seq);
+    launch_pdl(rope_append_kernel<float>, grid, dim3(64), 0, st, qkv, slow_rows, row_seq, row_pos, rope_tab, (float*)Kc, (float*)Vc, n_heads, dh, max_seq);
   else
-    rope_append_kernel<__nv_bfloat16><<<grid, 64, 0, st>>>(qkv, slow_rows, row_seq, row_pos, rope_tab, (__nv_bfloat16*)Kc, (__nv_bfloat16*)Vc, n_heads, dh, max_seq);
+    launch_pdl(rope_append_kernel<__nv_bfloat16>, grid, dim3(64), 0, st, qkv, slow_rows, row_seq, row_pos, rope_tab, (__nv_bfloat16*)Kc, (__nv_bfloat16*)Vc, n_heads, dh, max_seq);
 }
 
 // =====================================================================================
@@ -504,6 +508,8 @@ __device__ __forceinline__ uint32_t pack_bf16_hi_lo(float a, float b, uint32_t& 
 }
 template <int DH>
 __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
+  pdl_launch_dependents();
+  pdl_wait();
   constexpr int NCC = DH / 32;        // 16-byte chunks of a K row per lane
   constexpr int NKS = DH / 16;        // k-steps of Q K^T
   constexpr int NB = DH / 8;          // n8 column blocks of the output
@@ -673,7 +679,7 @@ static void launch_attn_mma(cudaStream_t st, const AttnArgs& a, dim3 grid) {
     cudaFuncSetAttribute(attn_mma_kernel<DH>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
     attr_set = true;
   }
-  attn_mma_kernel<DH><<<grid, 128, sh, st>>>(a);
+  launch_pdl(attn_mma_kernel<DH>, grid, dim3(128), sh, st, a);
 }
 
 template <typename KT, int SEG>
@@ -832,6 +838,8 @@ void launch_accel_topk_attn(cudaStream_t st, int dtype, const float* qkv, const 
 // merge of the split partials; accelerated rows add their own (k^_t, v^_t) as one more key:
 //   MHA(p_t, h_<t (+) p_t, h_<t (+) p_t)
 __global__ void merge_kernel(MergeArgs a) {
+  pdl_launch_dependents();
+  pdl_wait();
   const int row = blockIdx.x, head = blockIdx.y, j = threadIdx.x, dh = a.dh;
   const bool is_accel = row >= a.slow_rows;
   const bool accel_head = (a.accel_head_mask[head >> 5] >> (head & 31)) & 1u;
@@ -877,7 +885,7 @@ __global__ void merge_kernel(MergeArgs a) {
 
 void launch_merge(cudaStream_t st, const MergeArgs& a, int rows) {
   dim3 grid(rows, a.n_heads);
-  merge_kernel<<<grid, 128, 0, st>>>(a);
+  launch_pdl(merge_kernel, grid, dim3(128), 0, st, a);
 }
 
 // =====================================================================================

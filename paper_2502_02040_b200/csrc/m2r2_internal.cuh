@@ -50,6 +50,26 @@ __device__ __forceinline__ void load8(const float* p, float w[8]) {
   w[6] = __uint_as_float(b.z); w[7] = __uint_as_float(b.w);
 }
 
+// programmatic dependent launch (sm_90+): a kernel lets the NEXT kernel of the stream start launching early; a kernel
+// launched with the programmatic-serialization attribute blocks in pdl_wait() until its predecessor has completed and
+// flushed.  Both are no-ops in a kernel that was launched normally / whose successor was.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// host: launch `kernel` so that it may start while its predecessor in the stream drains; the kernel must call pdl_wait()
+// before it reads anything the predecessor wrote
+template <typename... KArgs, typename... Args>
+static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg;
+  cfg = cudaLaunchConfig_t();
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
