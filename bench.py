@@ -4,8 +4,9 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
         --master-port P bench.py --gpus N --steps K --warmup W
+    python bench.py --workload c3|c4|c5|olmoe|gemma [--gamma G] [--alpha A] [--tokens T]     # secondary workloads
 
-Workload (BASELINE.json configs[1], "C2"): 3.8B-class bf16 decoder (32 layers, d 3072, 32x96 heads,
+Workload of the bench line (BASELINE.json configs[1], "C2"): 3.8B-class bf16 decoder (32 layers, d 3072, 32x96 heads,
 FFN 8192, vocab 32064), batch 1, 512-token random prompt, then K dual-stream M2R2 decode steps (slow
 and accelerated residual streams both carried through all 32 layers).  A "step" = one
 m2r2_decode_step = one generated token.  Synthetic seeded weights N(0, 0.02) and uniform-random
@@ -15,8 +16,14 @@ Prints ONE JSON line (rank 0).  `value` is device-timed (CUDA events on the libr
 stream, inputs resident in HBM, tokens stay on the device); `e2e` is the same metric through the C
 ABI with host buffers (the forced input token goes host->device, the produced token device->host,
 every step, inside the timed region).  `roofline` is for the dominant kernel class measured live by
-the library's event profile; `cpu_baseline` is the oracle timed on this box's host cores.
+the library's event profile; `selfspec` is the metric's other half, the same model under self-speculative
+decoding (BASELINE.json configs[2], "C3": gamma 4, acceptance 0.9 and 0.5, 256 tokens, device-timed over the whole
+generation); `cpu_baseline` is the oracle timed on this box's host cores.
 `--impl reference` times the oracle (CPU) on the same config and metric.
+
+Secondary workloads (one JSON line each): c3 = self-spec sweep (gamma x alpha), c4 = batch 8 x 4096-token KV self-spec,
+c5 = MoE expert-loading policies with copy/compute overlap accounting, olmoe = the paper's five strategies on an
+OLMoE-shaped model, gemma = self-spec on a Gemma-7B-class shape (f-4).
 """
 from __future__ import annotations
 
