@@ -1692,6 +1692,14 @@ struct VArgs {
   const int* bmap;       // nullable -> identity; -1 = no adapter row for this output
   const float* U;
   int ldu, r, lora_row0, usel_div;
+  // neighbours absorbed by rows_ring_kernel (RowsFuse)
+  const bf16* gain;      // row-owned: X is the raw residual; RMSNorm(x; gain, eps) applied inside
+  float eps;
+  int n_heads;
+  const int *row_seq, *row_pos;    // QKV: RoPE on q, k and the K/V cache append in the epilogue
+  const float2* rope_tab;
+  bf16 *Kc, *Vc;
+  int max_seq;
 };
 __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -2176,6 +2184,337 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
 
 // a11 on the fragment-major weights: out = f(W x) for rows <= 8 slow-stream rows (kinds: VK_*).  Returns
 // M2R2_UNSUPPORTED when the fused copy is not bound (the caller then uses the row-major kernels).
+// ------------------------------------------------------------------ <= 8 rows: the same GEMM as a persistent ring kernel
+// For the k-token verify pass and prefill chunks at batch 1 the matrices are streamed exactly as the fused decode kernel
+// streams them: one CTA per SM owns a contiguous range of the matrix's 32 KB stages, a producer thread moves them through a
+// shared-memory ring with cp.async.bulk + mbarriers, eight consumer warps multiply.  Under programmatic dependent launch
+// the producer starts BEFORE the previous kernel of the chain has finished (weights do not depend on it), so the ring is
+// full when the activation rows arrive; the rows (<= 8) are staged once per CTA as (bf16 hi pair, bf16 lo pair) words, so
+// that one LDS.64 yields a B fragment register of both MMAs.
+//   row-owned matrices (QKV, gate/up, LM head): stage = one 16-row tile x 1024 inputs; the warps split the inputs and add
+//     their partial sums of a finished row tile into one of RR_NB shared-memory accumulators; the warp that arrives last
+//     runs the epilogue (no CTA barrier in the stream);
+//   split-K matrices (O, down): stage = 8 row tiles x 128 inputs; warp w owns row tile w, accumulates over the k-chunks of
+//     a group inside the CTA's range and adds onto the in-place residual atomically.
+// The kernel can absorb its neighbours in the layer (RowsFuse): RMSNorm of the rows while they are staged (the sums of
+// squares are collected on the way, 1 / rms multiplies the finished sums: W (g (.) x / rms) = (W (g (.) x)) / rms), and
+// RoPE + the K/V cache append in the QKV epilogue.
+#ifdef M2R2_RING_TL
+__device__ unsigned long long rr_tl[5][160][16];
+__device__ __forceinline__ u64 rr_time() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define RTL(i) (rr_tl[KIND][blockIdx.x][i] = rr_time())
+#else
+#define RTL(i) do { } while (0)
+#endif
+constexpr int RR_THREADS = NCT + 32;
+constexpr int RR_NB = 8;   // row-tile accumulators; a warp runs at most nst (<= 6) stages ahead of the slowest one
+template <int KIND>
+__global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a, int nst, int ld2, int xs_chunks, unsigned int zero) {
+  extern __shared__ __align__(1024) unsigned char rr_smem[];
+  unsigned char* const ring = rr_smem;
+  uint2* const xp = (uint2*)(rr_smem + (size_t)nst * STAGE_BYTES);    // [rows + 1][ld2]: inputs 2p, 2p + 1 as (hi, lo); last row zeros
+  float* const acc = (float*)(xp + (size_t)(a.rows + 1) * ld2);       // [RR_NB][4][32]
+  u64* const full = (u64*)(acc + RR_NB * 4 * 32);
+  u64* const empty = full + 8;
+  float* const ssq = (float*)(empty + 8);                             // [8][NCW] sums of squares (fused RMSNorm)
+  unsigned int* const cnt = (unsigned int*)(ssq + 8 * NCW);           // [RR_NB] warps that have added their part
+  float2* const rope_s = (float2*)(cnt + RR_NB);                      // [8][dh / 2] RoPE (cos, sin) of the rows' positions (QKV)
+  int* const seq_s = (int*)(rope_s + 8 * (a.dh >> 1));                // [8] row -> sequence, [8] row -> position
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int G = gridDim.x, v = blockIdx.x;
+  const bool split = a.split != 0;
+  const int nks = a.nstage_k;
+  int s0, s1;
+  if (!split) { s0 = range_lo(a.n_rt, v, G) * nks; s1 = range_lo(a.n_rt, v + 1, G) * nks; }
+  else { const int S = (a.n_rt / SK_RT) * nks; s0 = range_lo(S, v, G); s1 = range_lo(S, v + 1, G); }
+  if (tid == 0) {
+    RTL(0);
+    for (int i = 0; i < nst; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NCW); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0) RTL(1);
+  pdl_launch_dependents();
+  if (tid >= NCT) {
+    if (tid == NCT) {   // producer: every stage of the CTA's range, independent of the previous kernel
+      // (requesting further stages into L2 while the consumers stage the rows was measured: the rows' loads slow down
+      // by more than the stream gains, 4.80 -> 4.91 ms per C3 spec_step)
+      const u64 pol = policy_evict_first();
+      for (int s = s0, i = 0; s < s1; ++s, ++i) {
+        const int slot = i % nst, use = i / nst;
+        while (!mbar_try_wait(&empty[slot], (use & 1u) ^ 1u)) { }
+        mbar_expect_tx(&full[slot], STAGE_BYTES);
+        bulk_g2s(ring + (size_t)slot * STAGE_BYTES, a.W + (size_t)s * (STAGE_BYTES / 16), STAGE_BYTES, &full[slot], pol);
+      }
+      RTL(6);
+    }
+    return;
+  }
+  // ---- consumers
+  for (int i = tid; i < RR_NB * 4 * 32; i += NCT) acc[i] = 0.f;
+  if (tid < RR_NB) cnt[tid] = 0u;
+  for (int i = tid; i < ld2; i += NCT) xp[(size_t)a.rows * ld2 + i] = make_uint2(0u, 0u);   // rows >= a.rows read zeros
+  pdl_wait();
+  if (tid == 0) RTL(2);
+  if (KIND == VK_QKV && a.rope_tab) {
+    const int half = a.dh >> 1;
+    for (int i = tid; i < a.rows * half; i += NCT) {
+      const int n = i / half, j = i - n * half;
+      rope_s[n * half + j] = a.rope_tab[(size_t)a.row_pos[n] * half + j];
+    }
+    if (tid < a.rows) { seq_s[tid] = a.row_seq[tid]; seq_s[8 + tid] = a.row_pos[tid]; }
+  }
+  if (!split) {
+    // all inputs of every row: two column groups x eight rows of loads in flight per thread; every CTA starts its sweep
+    // at another column (all CTAs read the same rows: in step they would queue on the same L2 lines)
+    const int nq = nks * (STAGE_K / 4), nit = nq / NCT;   // STAGE_K / 4 == NCT
+    const int rot = (int)((unsigned)v * 37u % (unsigned)nq);
+    float ss[8];
+#pragma unroll
+    for (int row = 0; row < 8; ++row) ss[row] = 0.f;
+    for (int it = 0; it < nit; it += 2) {
+      float4 xr[2][8];
+      int qq[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        int q = (it + u) * NCT + tid + rot;
+        if (q >= nq) q -= nq;
+        qq[u] = (it + u) < nit ? q : -1;
+        const int k = 4 * q;
+#pragma unroll
+        for (int row = 0; row < 8; ++row) {
+          xr[u][row] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (qq[u] >= 0 && row < a.rows && k < a.K) xr[u][row] = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        if (qq[u] < 0) continue;
+        const int q = qq[u], k = 4 * q;
+        float4 g4 = make_float4(1.f, 1.f, 1.f, 1.f);
+        if (a.gain && k < a.K) {
+          const uint2 gr = __ldg((const uint2*)(a.gain + k));
+          const float2 g01 = __bfloat1622float2(*(const __nv_bfloat162*)&gr.x), g23 = __bfloat1622float2(*(const __nv_bfloat162*)&gr.y);
+          g4 = make_float4(g01.x, g01.y, g23.x, g23.y);
+        }
+#pragma unroll
+        for (int row = 0; row < 8; ++row) {
+          if (row < a.rows) {
+            const float4 x4 = xr[u][row];
+            ss[row] += x4.x * x4.x + x4.y * x4.y + x4.z * x4.z + x4.w * x4.w;
+            uint32_t l0, l1;
+            const uint32_t h0 = pack_hi_lo(x4.x * g4.x, x4.y * g4.y, l0), h1 = pack_hi_lo(x4.z * g4.z, x4.w * g4.w, l1);
+            *(uint4*)(xp + (size_t)row * ld2 + 2 * q) = make_uint4(h0, l0, h1, l1);
+          }
+        }
+      }
+      if (tid == 0 && it == 0) RTL(10);
+    }
+    if (tid == 0) RTL(11);
+    if (a.gain) {
+#pragma unroll
+      for (int row = 0; row < 8; ++row) {
+        const float tot = warp_sum(ss[row]);
+        if (lane == 0) ssq[row * NCW + warp] = tot;
+      }
+    }
+  } else if (s1 > s0) {
+    // the k-chunks of the CTA's range (slots by chunk index modulo xs_chunks), eight loads in flight per thread
+    const int kc0 = s0 % nks, cnt_c = min(s1 - s0, nks), items = a.rows * cnt_c * (SK_K / 4);   // SK_K / 4 == 32
+    for (int i0 = tid; i0 < items; i0 += 8 * NCT) {
+      float4 xr[8];
+      int xo[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int i = i0 + u * NCT;
+        xr[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        xo[u] = -1;
+        if (i < items) {
+          const int q = i & 31, j = i >> 5, row = j / cnt_c, ci = j - row * cnt_c;
+          int kc = kc0 + ci;
+          if (kc >= nks) kc -= nks;
+          const int k = kc * SK_K + 4 * q;
+          if (k < a.K) xr[u] = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));
+          xo[u] = row * ld2 + (((kc % xs_chunks) * SK_K + 4 * q) >> 1);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        if (xo[u] >= 0) {
+          uint32_t l0, l1;
+          const uint32_t h0 = pack_hi_lo(xr[u].x, xr[u].y, l0), h1 = pack_hi_lo(xr[u].z, xr[u].w, l1);
+          *(uint4*)(xp + xo[u]) = make_uint4(h0, l0, h1, l1);
+        }
+      }
+    }
+  }
+  if (tid == 0) RTL(12);
+  bar_consumers();
+  if (tid == 0) RTL(3);
+#ifdef M2R2_RING_TL
+  u64 spin = 0;
+#endif
+  const uint2* bp = xp + (size_t)min(g, a.rows) * ld2 + t;
+  float c[4] = {0.f, 0.f, 0.f, 0.f}, cl[4] = {0.f, 0.f, 0.f, 0.f};
+  float rs[2] = {1.f, 1.f};   // 1 / rms of activation rows 2t, 2t + 1
+  if (!split && a.gain) {
+#pragma unroll
+    for (int sx = 0; sx < 2; ++sx) {
+      float tot = 0.f;
+#pragma unroll
+      for (int w8 = 0; w8 < NCW; ++w8) tot += ssq[(2 * t + sx) * NCW + w8];
+      rs[sx] = rsqrtf(tot / (float)a.K + a.eps);
+    }
+  }
+  for (int s = s0, i = 0; s < s1; ++s, ++i) {
+    const int slot = i % nst, use = i / nst;
+#ifdef M2R2_RING_TL
+    const u64 tw0 = rr_time();
+#endif
+    while (!mbar_try_wait(&full[slot], use & 1u)) { }
+#ifdef M2R2_RING_TL
+    if (tid == 0) { spin += rr_time() - tw0; if (i == 0) RTL(4); }
+#endif
+    const uint4* A = (const uint4*)(ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
+    int p0;   // first input pair of the warp's eight tiles, in staged coordinates
+    if (!split) p0 = ((s % nks) * STAGE_K + warp * (TPW * 16)) >> 1;
+    else p0 = (((s % nks) % xs_chunks) * SK_K) >> 1;
+    uint32_t dep = 0u;
+#pragma unroll
+    for (int u = 0; u < TPW; ++u) {
+      const uint4 w = A[u * 32];
+      const uint2 b0 = bp[p0 + u * 8], b1 = bp[p0 + u * 8 + 4];   // inputs 16u + 2t (+1) and + 8: (hi, lo)
+      mma_bf16(c, w, b0.x, b1.x);
+      mma_bf16(cl, w, b0.y, b1.y);   // the lo parts' products: a second, independent accumulation chain
+      dep ^= w.x;
+    }
+    __syncwarp();
+    if (lane == 0) release_stage(&empty[slot], zero, __uint_as_float(dep));
+#ifdef M2R2_RING_TL
+    if (tid == 0 && s == s1 - 1) { RTL(5); rr_tl[KIND][blockIdx.x][8] = spin; rr_tl[KIND][blockIdx.x][9] = (u64)(s1 - s0); }
+#endif
+    if (!split) {
+      if ((s % nks) != nks - 1) continue;
+      // the row tile is finished in this warp's k range: add the partial sums into the tile's accumulator; the warp that
+      // arrives last holds the complete sums and finishes the tile
+      const int rt = s / nks, b = (i / nks) % RR_NB;
+      float* ab = acc + b * 4 * 32;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { atomicAdd(ab + e * 32 + lane, c[e] + cl[e]); c[e] = 0.f; cl[e] = 0.f; }
+      __syncwarp();
+      unsigned int old = 0u;
+      if (lane == 0) { __threadfence_block(); old = atomicAdd(&cnt[b], 1u); }
+      old = __shfl_sync(0xffffffffu, old, 0);
+      if (old != NCW - 1) continue;
+      __threadfence_block();
+      float r4[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) { r4[e] = ab[e * 32 + lane] * rs[e & 1]; ab[e * 32 + lane] = 0.f; }
+      if (lane == 0) cnt[b] = 0u;
+      // r4[0], r4[1] = weight row g x activation rows 2t, 2t + 1; r4[2], r4[3] = weight row g + 8
+      if (KIND == VK_QKV && a.rope_tab) {
+        // RoPE on q and k (packed rows 2i, 2i + 1 = the pair (i, i + dh / 2): the partner sits in lane ^ 4) and the
+        // append of k, v to the cache (a3, rope_append_kernel's arithmetic)
+        const int half = a.dh >> 1;
+#pragma unroll
+        for (int sx = 0; sx < 2; ++sx) {
+          const int n = 2 * t + sx;
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            const float val = r4[2 * hh + sx];
+            const float pv = __shfl_xor_sync(0xffffffffu, val, 4);
+            const int pr = rt * 16 + g + 8 * hh;
+            if (n >= a.rows || pr >= a.n_out) continue;
+            const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
+            const int pos = seq_s[8 + n], seq = seq_s[n];
+            const size_t cbase = (((size_t)seq * a.n_heads + head) * a.max_seq + pos) * a.dh;
+            if (which < 2) {
+              const int j = e >> 1;
+              const float2 cs = rope_s[n * half + j];
+              const float o = (e & 1) ? val * cs.x + pv * cs.y : val * cs.x - pv * cs.y;
+              const int ne = j + (e & 1) * half;
+              a.out[(size_t)n * a.ldo + which * a.d + head * a.dh + ne] = o;
+              if (which == 1) a.Kc[cbase + ne] = __float2bfloat16_rn(o);
+            } else {
+              a.out[(size_t)n * a.ldo + pr] = val;
+              a.Vc[cbase + e] = __float2bfloat16_rn(val);
+            }
+          }
+        }
+        continue;
+      }
+#pragma unroll
+      for (int sx = 0; sx < 2; ++sx) {
+        const int n = 2 * t + sx;
+        if (n >= a.rows) continue;
+        const float v0 = r4[sx], v1 = r4[2 + sx];
+        if (KIND == VK_GATEUP) {
+          const int o = rt * 8 + g;
+          if (o < a.n_out) a.out[(size_t)n * a.ldo + o] = silu(v0) * v1;
+          continue;
+        }
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int pr = rt * 16 + g + 8 * hh;
+          if (pr >= a.n_out) continue;
+          int nat = pr;
+          if (KIND == VK_QKV) {
+            const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
+            nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
+          }
+          a.out[(size_t)n * a.ldo + nat] = hh ? v1 : v0;
+        }
+      }
+    } else {
+      const int kc = s % nks;
+      if (kc == nks - 1 || s == s1 - 1) {
+        // split-K: this CTA's part of the sums of row tile (group, warp) onto the in-place residual
+        const int rt = (s / nks) * SK_RT + warp;
+#pragma unroll
+        for (int sx = 0; sx < 2; ++sx) {
+          const int n = 2 * t + sx;
+          if (n >= a.rows) continue;
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            const int pr = rt * 16 + g + 8 * hh;
+            if (pr < a.n_out) atomicAdd(a.out + (size_t)n * a.ldo + pr, c[2 * hh + sx] + cl[2 * hh + sx]);
+          }
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { c[e] = 0.f; cl[e] = 0.f; }
+      }
+    }
+  }
+  if (tid == 0) RTL(7);
+}
+template <int KIND>
+static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int zero, cudaStream_t st) {
+  const int nks = a.nstage_k;
+  int kx, xs_chunks = 1;   // staged inputs per row
+  if (!a.split) {
+    kx = nks * STAGE_K;
+  } else {
+    const int S = (a.n_rt / SK_RT) * nks, maxL = (S + G - 1) / G + 1;
+    xs_chunks = std::min(nks, (maxL + 7) / 8 * 8);
+    kx = xs_chunks * SK_K;
+  }
+  const int ld2 = kx / 2 + 4;   // (hi, lo) words per staged row; = 4 mod 16: the LDS.64 of a half-warp hit 16 distinct bank pairs
+  const size_t xbytes = (size_t)(a.rows + 1) * ld2 * sizeof(uint2);
+  const size_t fixed = xbytes + (size_t)RR_NB * 4 * 32 * sizeof(float) + 512 + (size_t)8 * (a.dh / 2) * sizeof(float2) + 64;
+  if ((size_t)smem_max < fixed + 1024 + 2 * (size_t)STAGE_BYTES) return M2R2_UNSUPPORTED;
+  // ring depth: what fits, at most 6 and no more than a CTA's stages (a short matrix leaves shared memory to the
+  // attention CTAs that are still resident when this kernel's CTAs arrive)
+  const int max_stages = a.split ? ((a.n_rt / SK_RT) * nks + G - 1) / G : (a.n_rt + G - 1) / G * nks;
+  const int nst = std::max(2, std::min((int)std::min<size_t>(6, ((size_t)smem_max - fixed - 1024) / STAGE_BYTES), max_stages));
+  const size_t sh = (size_t)nst * STAGE_BYTES + fixed;
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(rows_ring_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
+    attr_set = true;
+  }
+  return launch_pdl(rows_ring_kernel<KIND>, dim3(G), dim3(RR_THREADS), sh, st, a, nst, ld2, xs_chunks, zero) == cudaSuccess ? 0 : M2R2_CUDA;
+}
+
 template <int KIND, int NG, bool SW>
 static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
   const size_t sh = (size_t)2 * NG * 8 * ((SW ? 4 : 1) * RM_KC + 8) * sizeof(bf16);
@@ -2210,7 +2549,7 @@ static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) 
 }
 
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
-                    int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora) {
+                    int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora, const RowsFuse* fz) {
   if (!fs->supported || !fs->impl || !fs->impl->bound || rows < 1 || rows > 64 || (c.d_model % 4) || (c.d_ff % 4)) return M2R2_UNSUPPORTED;
   FusedImpl* im = fs->impl;
   PackedDims q = packed_dims(c);
@@ -2233,6 +2572,34 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     a.Bm = (const bf16*)lora->Bm; a.Bm2 = (const bf16*)lora->Bm2; a.bmap = lora->bmap; a.U = lora->U;
     a.ldu = lora->ldu; a.r = lora->r; a.lora_row0 = lora->lora_row0; a.usel_div = lora->usel_div;
   }
+  static const bool no_ring = getenv("M2R2_XNORING") != nullptr;
+  const bool ring = rows <= 8 && !(lora && lora->Bm) && !no_ring && ((kind != VK_OPROJ && kind != VK_DOWN) || (resid == out && !trace));
+  if (fz) {
+    // the caller left the GEMM's neighbours to the ring kernel: only that kernel can honour it
+    if (!ring || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
+    a.gain = (const bf16*)fz->gain; a.eps = fz->eps;
+    a.n_heads = c.n_heads;
+    a.row_seq = fz->row_seq; a.row_pos = fz->row_pos; a.rope_tab = fz->rope_tab; a.Kc = (bf16*)fz->Kc; a.Vc = (bf16*)fz->Vc;
+    a.max_seq = c.max_seq;
+  }
+  if (ring) {
+    // batch-1 verify pass / prefill chunks: the persistent ring kernel (one CTA per SM)
+    static int smem_max = 0;
+    if (!smem_max) {
+      int dev = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    }
+    int rc;
+    switch (kind) {
+      case VK_QKV:    rc = launch_rows_ring<VK_QKV>(a, im->G, smem_max, 0u, st); break;
+      case VK_OPROJ:  rc = launch_rows_ring<VK_OPROJ>(a, im->G, smem_max, 0u, st); break;
+      case VK_GATEUP: rc = launch_rows_ring<VK_GATEUP>(a, im->G, smem_max, 0u, st); break;
+      case VK_DOWN:   rc = launch_rows_ring<VK_DOWN>(a, im->G, smem_max, 0u, st); break;
+      default:        rc = launch_rows_ring<VK_HEAD>(a, im->G, smem_max, 0u, st); break;
+    }
+    if (rc != M2R2_UNSUPPORTED || fz) return rc;
+  }
   {
     // 4 row tiles per CTA; O / down split along K (atomic adds onto the in-place residual) so that every SM streams
     const int ng = (rows + 7) / 8;
@@ -2254,3 +2621,7 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   }
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }
+
+#ifdef M2R2_RING_TL
+extern "C" int m2r2_ring_tl(void* out) { return (int)cudaMemcpyFromSymbol(out, rr_tl, sizeof(rr_tl)); }
+#endif

@@ -700,6 +700,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   // tensor-core GEMM (kernels_fused.cu) reads each weight once for all rows (a11)
   // (dual passes at batch >= 5 have 9..32 rows: the same kernel carries the accelerated rows' adapters)
   const bool mma_rows = ((!dual && ns <= 64) || (dual && 2 * B > 8 && 2 * B <= 64)) && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
+  static const bool no_ring_fuse = getenv("M2R2_XNOFUSE") != nullptr;
   float* tr0 = p.trace ? x->trace : nullptr;
   launch_embed(x->cs, c.dtype, x->embed, x->d_row_tok, ns, d, x->resid, any_accel ? x->resid + (size_t)ns * d : nullptr,
                tr0, (tr0 && dual) ? tr0 + (size_t)B * d : nullptr);
@@ -718,15 +719,29 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     char* Vc = Kc + (size_t)c.n_layers * c.max_batch * nh * c.max_seq * dh * x->esz;
     // a2: RMSNorm + QKV (slow: all heads; accelerated: heads in S + adapters)
     prof_mark(x, M2R2_PROF_QKV);
-    launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g1, c.rms_eps, x->xn, acc_on ? L.Aqkv : nullptr, 3, r, ns, x->U, 64);
+    // <= 8 slow rows (the verify pass and prefill chunks at batch 1): the ring GEMM absorbs the layer's small kernels
+    // (RMSNorm in its staging, RoPE + KV append in the QKV epilogue)
+    const bool ring_fuse = mma_rows && !acc_on && rows <= 8 && !no_ring_fuse;
+    int saved = 0;   // launches the fusion removed
     GemvArgs g;
-    memset(&g, 0, sizeof(g));
-    g.W = L.wqkv; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = 3 * d; g.out = x->qkv; g.ldo = 3 * d;
-    if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
-    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
-    // a3: RoPE + KV append
-    prof_mark(x, M2R2_PROF_ROPE);
-    launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
+    bool qkv_done = false;
+    if (ring_fuse) {
+      RowsFuse fz;
+      fz.gain = L.g1; fz.eps = c.rms_eps; fz.row_seq = x->d_row_seq; fz.row_pos = x->d_row_pos; fz.rope_tab = x->rope_tab;
+      fz.Kc = Kc; fz.Vc = Vc;
+      qkv_done = fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->resid, d, rows, x->qkv, 3 * d, nullptr, nullptr, nullptr, &fz) == 0;
+      if (qkv_done) saved += 2;
+    }
+    if (!qkv_done) {
+      launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g1, c.rms_eps, x->xn, acc_on ? L.Aqkv : nullptr, 3, r, ns, x->U, 64);
+      memset(&g, 0, sizeof(g));
+      g.W = L.wqkv; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = 3 * d; g.out = x->qkv; g.ldo = 3 * d;
+      if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
+      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+      // a3: RoPE + KV append
+      prof_mark(x, M2R2_PROF_ROPE);
+      launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
+    }
     // a4: split-K attention + merge
     prof_mark(x, M2R2_PROF_ATTN);
     AttnArgs a;
@@ -757,7 +772,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
                              c.max_seq, c.accel_topk_tokens, scale);
       count(x);
     }
-    count(x, 5);
+    count(x, 5 - saved);
     // a5: O-proj + residual
     prof_mark(x, M2R2_PROF_OPROJ);
     if (acc_on) { launch_lora_down(x->cs, c.dtype, x->attn_o, d, ns, na, da, x->d_accel_cols, L.Ao, r, x->U, 64); count(x); }
@@ -770,11 +785,19 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     if (!c.n_experts) {
       // a6: RMSNorm + gate/up + SwiGLU;  a7: down + residual (accelerated-residual update)
       prof_mark(x, M2R2_PROF_GATEUP);
-      launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, acc_on ? L.Agu : nullptr, 2, r, ns, x->U, 64);
-      memset(&g, 0, sizeof(g));
-      g.W = L.wgate; g.W2 = L.wup; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = c.d_ff; g.out = x->act; g.ldo = c.d_ff;
-      if (acc_on) { g.Bm = L.Bg; g.Bm2 = L.Bu; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, true);
+      bool gu_done = false;
+      if (ring_fuse) {
+        RowsFuse fz;
+        fz.gain = L.g2; fz.eps = c.rms_eps;
+        gu_done = fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->resid, d, rows, x->act, c.d_ff, nullptr, nullptr, nullptr, &fz) == 0;
+      }
+      if (!gu_done) {
+        launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, acc_on ? L.Agu : nullptr, 2, r, ns, x->U, 64);
+        memset(&g, 0, sizeof(g));
+        g.W = L.wgate; g.W2 = L.wup; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = c.d_ff; g.out = x->act; g.ldo = c.d_ff;
+        if (acc_on) { g.Bm = L.Bg; g.Bm2 = L.Bu; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
+        if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, true);
+      }
       prof_mark(x, M2R2_PROF_DOWN);
       if (acc_on) { launch_lora_down(x->cs, c.dtype, x->act, c.d_ff, ns, na, c.d_ff, nullptr, L.Ad, r, x->U, 64); count(x); }
       memset(&g, 0, sizeof(g));
@@ -782,7 +805,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       g.trace = trl;
       if (acc_on) { g.Bm = L.Bd; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
       if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
-      count(x, 3);
+      count(x, gu_done ? 2 : 3);
     } else {
       int rc = moe_mlp(x, p, i, ns, na);
       if (rc) return rc;
@@ -812,15 +835,24 @@ static int final_head(m2r2_ctx* x, int ns, int* tok_out, int tok_stride) {
   const m2r2_config& c = x->c;
   const int d = c.d_model, V = c.vocab;
   prof_mark(x, M2R2_PROF_HEAD);
-  launch_norm_lora(x->cs, c.dtype, x->resid, ns, d, x->gf, c.rms_eps, x->xn, nullptr, 0, 0, 0, x->U, 64);
-  GemvArgs g;
-  memset(&g, 0, sizeof(g));
-  g.W = x->lm_head; g.X = x->xn; g.ldx = d; g.n_rows = ns; g.K = d; g.n_out = V; g.out = x->logits; g.ldo = V;
   const bool mma_rows = ns <= 64 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
-  if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, 0, 4, x->xn, d, ns, x->logits, V, nullptr, nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+  bool done = false;
+  if (mma_rows && ns <= 8) {
+    RowsFuse fz;   // RMSNorm inside the ring GEMM's staging
+    fz.gain = x->gf; fz.eps = c.rms_eps;
+    done = fused_gemv_rows(c, &x->fs, x->cs, 0, 4, x->resid, d, ns, x->logits, V, nullptr, nullptr, nullptr, &fz) == 0;
+  }
+  if (!done) {
+    launch_norm_lora(x->cs, c.dtype, x->resid, ns, d, x->gf, c.rms_eps, x->xn, nullptr, 0, 0, 0, x->U, 64);
+    GemvArgs g;
+    memset(&g, 0, sizeof(g));
+    g.W = x->lm_head; g.X = x->xn; g.ldx = d; g.n_rows = ns; g.K = d; g.n_out = V; g.out = x->logits; g.ldo = V;
+    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, 0, 4, x->xn, d, ns, x->logits, V, nullptr, nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+    count(x);
+  }
   launch_argmax(x->cs, x->logits, V, ns, V, x->d_row_seq, x->d_row_pos, x->ls_on ? x->d_ls_full : nullptr,
                 x->ls_first, x->ls_n, x->ls_beta, tok_out, tok_stride);
-  count(x, 3);
+  count(x, 2);
   return 0;
 }
 
