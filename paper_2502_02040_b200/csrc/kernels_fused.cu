@@ -2199,41 +2199,63 @@ int fused_check(FusedState* fs, cudaStream_t st, char* msg, size_t n) {
 // The kernel can absorb its neighbours in the layer (RowsFuse): RMSNorm of the rows while they are staged (the sums of
 // squares are collected on the way, 1 / rms multiplies the finished sums: W (g (.) x / rms) = (W (g (.) x)) / rms), and
 // RoPE + the K/V cache append in the QKV epilogue.
-#ifdef M2R2_RING_TL
-__device__ unsigned long long rr_tl[5][160][16];
-__device__ __forceinline__ u64 rr_time() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-#define RTL(i) (rr_tl[KIND][blockIdx.x][i] = rr_time())
-#else
-#define RTL(i) do { } while (0)
-#endif
+// thread-block cluster of two CTAs: the pair stages the activation rows of a row-owned matrix together (each loads half of
+// the columns from L2 and writes the converted words into both CTAs' shared memory)
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t mapa_peer(const void* local, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_u32(local)), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void st_cluster_v4(uint32_t raddr, uint4 v) {
+  asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(raddr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void st_cluster_f32(uint32_t raddr, float v) {
+  asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(raddr), "f"(v) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t raddr) {   // releases the thread's earlier (remote) stores
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(raddr) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait_cluster(u64* b, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+               : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 constexpr int RR_THREADS = NCT + 32;
 constexpr int RR_NB = 8;   // row-tile accumulators; a warp runs at most nst (<= 6) stages ahead of the slowest one
 template <int KIND>
-__global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a, int nst, int ld2, int xs_chunks, unsigned int zero) {
+__global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a, int nst, int ld2, int xs_chunks, int csize, unsigned int zero) {
   extern __shared__ __align__(1024) unsigned char rr_smem[];
   unsigned char* const ring = rr_smem;
   uint2* const xp = (uint2*)(rr_smem + (size_t)nst * STAGE_BYTES);    // [rows + 1][ld2]: inputs 2p, 2p + 1 as (hi, lo); last row zeros
   float* const acc = (float*)(xp + (size_t)(a.rows + 1) * ld2);       // [RR_NB][4][32]
   u64* const full = (u64*)(acc + RR_NB * 4 * 32);
   u64* const empty = full + 8;
-  float* const ssq = (float*)(empty + 8);                             // [8][NCW] sums of squares (fused RMSNorm)
-  unsigned int* const cnt = (unsigned int*)(ssq + 8 * NCW);           // [RR_NB] warps that have added their part
-  float2* const rope_s = (float2*)(cnt + RR_NB);                      // [8][dh / 2] RoPE (cos, sin) of the rows' positions (QKV)
+  float* const ssq = (float*)(empty + 8);                             // [2 ranks][8] sums of squares of the rows (fused RMSNorm)
+  unsigned int* const cnt = (unsigned int*)(ssq + 2 * 8);             // [RR_NB] warps that have added their part
+  u64* const xdone = (u64*)(cnt + RR_NB);                             // the cluster peer's half of the rows has arrived (NCT arrivals)
+  float2* const rope_s = (float2*)(xdone + 1);                        // [8][dh / 2] RoPE (cos, sin) of the rows' positions (QKV)
   int* const seq_s = (int*)(rope_s + 8 * (a.dh >> 1));                // [8] row -> sequence, [8] row -> position
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   const int G = gridDim.x, v = blockIdx.x;
-  const bool split = a.split != 0;
+  constexpr bool split = KIND == VK_OPROJ || KIND == VK_DOWN;   // (= a.split)
   const int nks = a.nstage_k;
   int s0, s1;
   if (!split) { s0 = range_lo(a.n_rt, v, G) * nks; s1 = range_lo(a.n_rt, v + 1, G) * nks; }
   else { const int S = (a.n_rt / SK_RT) * nks; s0 = range_lo(S, v, G); s1 = range_lo(S, v + 1, G); }
   if (tid == 0) {
-    RTL(0);
     for (int i = 0; i < nst; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], NCW); }
+    mbar_init(xdone, NCT);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __syncthreads();
-  if (tid == 0) RTL(1);
+  if (tid < 2 * 8) ssq[tid] = 0.f;
+  const bool pair = csize == 2 && !split;        // the two CTAs of the cluster stage the rows together
+  const uint32_t rank = csize == 2 ? cluster_ctarank() : 0u;
+  if (csize == 2) cluster_sync_all(); else __syncthreads();   // barriers and ssq are initialised in both CTAs
   pdl_launch_dependents();
   if (tid >= NCT) {
     if (tid == NCT) {   // producer: every stage of the CTA's range, independent of the previous kernel
@@ -2246,7 +2268,6 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
         mbar_expect_tx(&full[slot], STAGE_BYTES);
         bulk_g2s(ring + (size_t)slot * STAGE_BYTES, a.W + (size_t)s * (STAGE_BYTES / 16), STAGE_BYTES, &full[slot], pol);
       }
-      RTL(6);
     }
     return;
   }
@@ -2255,7 +2276,6 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
   if (tid < RR_NB) cnt[tid] = 0u;
   for (int i = tid; i < ld2; i += NCT) xp[(size_t)a.rows * ld2 + i] = make_uint2(0u, 0u);   // rows >= a.rows read zeros
   pdl_wait();
-  if (tid == 0) RTL(2);
   if (KIND == VK_QKV && a.rope_tab) {
     const int half = a.dh >> 1;
     for (int i = tid; i < a.rows * half; i += NCT) {
@@ -2264,68 +2284,75 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
     }
     if (tid < a.rows) { seq_s[tid] = a.row_seq[tid]; seq_s[8 + tid] = a.row_pos[tid]; }
   }
+  // (kept compact on purpose: this loop form measured faster than a version with all eight rows unrolled per thread;
+  // after the wait a CTA needs ~1.3 us for the loads to land, ~1.6 us to convert and store, ~0.7 us for the exchange)
   if (!split) {
-    // all inputs of every row: two column groups x eight rows of loads in flight per thread; every CTA starts its sweep
-    // at another column (all CTAs read the same rows: in step they would queue on the same L2 lines)
-    const int nq = nks * (STAGE_K / 4), nit = nq / NCT;   // STAGE_K / 4 == NCT
-    const int rot = (int)((unsigned)v * 37u % (unsigned)nq);
-    float ss[8];
+    // all inputs of every row, in units of eight inputs (one 32-byte sector of fp32): this CTA loads the units u = rank
+    // (mod cluster size), converts them and writes the words into its own and the peer's shared memory (all CTAs read
+    // the same rows at the same moment: a pair halves that L2 traffic)
+    const int nu = nks * (STAGE_K / 8);            // units per row
+    const int step = pair ? 2 : 1, nu_mine = nu / step, items = a.rows * nu_mine;   // nu_mine % 32 == 0: a warp's items share the row
+    const uint32_t peer_xp = pair ? mapa_peer(xp, rank ^ 1u) : 0u;
+#pragma unroll 1
+    for (int i0 = tid; i0 < items; i0 += 4 * NCT) {
+      float4 xa[4], xb[4];
+      uint4 gr[4];
 #pragma unroll
-    for (int row = 0; row < 8; ++row) ss[row] = 0.f;
-    for (int it = 0; it < nit; it += 2) {
-      float4 xr[2][8];
-      int qq[2];
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        int q = (it + u) * NCT + tid + rot;
-        if (q >= nq) q -= nq;
-        qq[u] = (it + u) < nit ? q : -1;
-        const int k = 4 * q;
-#pragma unroll
-        for (int row = 0; row < 8; ++row) {
-          xr[u][row] = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (qq[u] >= 0 && row < a.rows && k < a.K) xr[u][row] = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < 2; ++u) {
-        if (qq[u] < 0) continue;
-        const int q = qq[u], k = 4 * q;
-        float4 g4 = make_float4(1.f, 1.f, 1.f, 1.f);
-        if (a.gain && k < a.K) {
-          const uint2 gr = __ldg((const uint2*)(a.gain + k));
-          const float2 g01 = __bfloat1622float2(*(const __nv_bfloat162*)&gr.x), g23 = __bfloat1622float2(*(const __nv_bfloat162*)&gr.y);
-          g4 = make_float4(g01.x, g01.y, g23.x, g23.y);
-        }
-#pragma unroll
-        for (int row = 0; row < 8; ++row) {
-          if (row < a.rows) {
-            const float4 x4 = xr[u][row];
-            ss[row] += x4.x * x4.x + x4.y * x4.y + x4.z * x4.z + x4.w * x4.w;
-            uint32_t l0, l1;
-            const uint32_t h0 = pack_hi_lo(x4.x * g4.x, x4.y * g4.y, l0), h1 = pack_hi_lo(x4.z * g4.z, x4.w * g4.w, l1);
-            *(uint4*)(xp + (size_t)row * ld2 + 2 * q) = make_uint4(h0, l0, h1, l1);
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + u * NCT;
+        xa[u] = xb[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        gr[u] = make_uint4(0x3f803f80u, 0x3f803f80u, 0x3f803f80u, 0x3f803f80u);   // bf16 ones
+        if (i < items) {
+          const int row = i / nu_mine, k = 8 * ((i - row * nu_mine) * step + (pair ? (int)rank : 0));
+          if (k < a.K) {
+            const float4* src = (const float4*)(a.X + (size_t)row * a.ldx + k);
+            xa[u] = __ldg(src);
+            xb[u] = __ldg(src + 1);
+            if (a.gain) gr[u] = __ldg((const uint4*)(a.gain + k));
           }
         }
       }
-      if (tid == 0 && it == 0) RTL(10);
-    }
-    if (tid == 0) RTL(11);
-    if (a.gain) {
 #pragma unroll
-      for (int row = 0; row < 8; ++row) {
-        const float tot = warp_sum(ss[row]);
-        if (lane == 0) ssq[row * NCW + warp] = tot;
+      for (int u = 0; u < 4; ++u) {
+        const int i = i0 + u * NCT;
+        if (i < items) {
+          const int row = i / nu_mine, k = 8 * ((i - row * nu_mine) * step + (pair ? (int)rank : 0));
+          const float4 x0 = xa[u], x1 = xb[u];
+          const float2 g0 = __bfloat1622float2(*(const __nv_bfloat162*)&gr[u].x), g1 = __bfloat1622float2(*(const __nv_bfloat162*)&gr[u].y);
+          const float2 g2 = __bfloat1622float2(*(const __nv_bfloat162*)&gr[u].z), g3 = __bfloat1622float2(*(const __nv_bfloat162*)&gr[u].w);
+          uint4 w0, w1;
+          w0.x = pack_hi_lo(x0.x * g0.x, x0.y * g0.y, w0.y); w0.z = pack_hi_lo(x0.z * g1.x, x0.w * g1.y, w0.w);
+          w1.x = pack_hi_lo(x1.x * g2.x, x1.y * g2.y, w1.y); w1.z = pack_hi_lo(x1.z * g3.x, x1.w * g3.y, w1.w);
+          const size_t off = (size_t)row * ld2 + (k >> 1);
+          *(uint4*)(xp + off) = w0;
+          *(uint4*)(xp + off + 2) = w1;
+          if (pair) {
+            st_cluster_v4(peer_xp + (uint32_t)(off * sizeof(uint2)), w0);
+            st_cluster_v4(peer_xp + (uint32_t)((off + 2) * sizeof(uint2)), w1);
+          }
+          if (a.gain) {
+            const float sq = warp_sum(x0.x * x0.x + x0.y * x0.y + x0.z * x0.z + x0.w * x0.w + x1.x * x1.x + x1.y * x1.y + x1.z * x1.z + x1.w * x1.w);
+            if (lane == 0) atomicAdd(&ssq[rank * 8 + row], sq);
+          }
+        }
       }
     }
+    if (pair) {
+      if (a.gain) {
+        bar_consumers();   // this CTA's sums of squares are complete
+        if (tid < 8) st_cluster_f32(mapa_peer(ssq, rank ^ 1u) + (uint32_t)((rank * 8 + tid) * sizeof(float)), ssq[rank * 8 + tid]);
+      }
+      mbar_arrive_cluster(mapa_peer(xdone, rank ^ 1u));
+    }
   } else if (s1 > s0) {
-    // the k-chunks of the CTA's range (slots by chunk index modulo xs_chunks), eight loads in flight per thread
+    // the k-chunks of the CTA's range (slots by chunk index modulo xs_chunks), four loads in flight per thread
     const int kc0 = s0 % nks, cnt_c = min(s1 - s0, nks), items = a.rows * cnt_c * (SK_K / 4);   // SK_K / 4 == 32
-    for (int i0 = tid; i0 < items; i0 += 8 * NCT) {
-      float4 xr[8];
-      int xo[8];
+#pragma unroll 1
+    for (int i0 = tid; i0 < items; i0 += 4 * NCT) {
+      float4 xr[4];
+      int xo[4];
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
+      for (int u = 0; u < 4; ++u) {
         const int i = i0 + u * NCT;
         xr[u] = make_float4(0.f, 0.f, 0.f, 0.f);
         xo[u] = -1;
@@ -2339,42 +2366,31 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
         }
       }
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
+      for (int u = 0; u < 4; ++u) {
         if (xo[u] >= 0) {
-          uint32_t l0, l1;
-          const uint32_t h0 = pack_hi_lo(xr[u].x, xr[u].y, l0), h1 = pack_hi_lo(xr[u].z, xr[u].w, l1);
-          *(uint4*)(xp + xo[u]) = make_uint4(h0, l0, h1, l1);
+          uint4 w;
+          w.x = pack_hi_lo(xr[u].x, xr[u].y, w.y); w.z = pack_hi_lo(xr[u].z, xr[u].w, w.w);
+          *(uint4*)(xp + xo[u]) = w;
         }
       }
     }
   }
-  if (tid == 0) RTL(12);
   bar_consumers();
-  if (tid == 0) RTL(3);
-#ifdef M2R2_RING_TL
-  u64 spin = 0;
-#endif
+  if (pair) while (!mbar_try_wait_cluster(xdone, 0u)) { }
+
   const uint2* bp = xp + (size_t)min(g, a.rows) * ld2 + t;
   float c[4] = {0.f, 0.f, 0.f, 0.f}, cl[4] = {0.f, 0.f, 0.f, 0.f};
   float rs[2] = {1.f, 1.f};   // 1 / rms of activation rows 2t, 2t + 1
   if (!split && a.gain) {
 #pragma unroll
     for (int sx = 0; sx < 2; ++sx) {
-      float tot = 0.f;
-#pragma unroll
-      for (int w8 = 0; w8 < NCW; ++w8) tot += ssq[(2 * t + sx) * NCW + w8];
+      const float tot = ssq[2 * t + sx] + ssq[8 + 2 * t + sx];
       rs[sx] = rsqrtf(tot / (float)a.K + a.eps);
     }
   }
   for (int s = s0, i = 0; s < s1; ++s, ++i) {
     const int slot = i % nst, use = i / nst;
-#ifdef M2R2_RING_TL
-    const u64 tw0 = rr_time();
-#endif
     while (!mbar_try_wait(&full[slot], use & 1u)) { }
-#ifdef M2R2_RING_TL
-    if (tid == 0) { spin += rr_time() - tw0; if (i == 0) RTL(4); }
-#endif
     const uint4* A = (const uint4*)(ring + (size_t)slot * STAGE_BYTES) + (warp * TPW) * 32 + lane;
     int p0;   // first input pair of the warp's eight tiles, in staged coordinates
     if (!split) p0 = ((s % nks) * STAGE_K + warp * (TPW * 16)) >> 1;
@@ -2390,9 +2406,6 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
     }
     __syncwarp();
     if (lane == 0) release_stage(&empty[slot], zero, __uint_as_float(dep));
-#ifdef M2R2_RING_TL
-    if (tid == 0 && s == s1 - 1) { RTL(5); rr_tl[KIND][blockIdx.x][8] = spin; rr_tl[KIND][blockIdx.x][9] = (u64)(s1 - s0); }
-#endif
     if (!split) {
       if ((s % nks) != nks - 1) continue;
       // the row tile is finished in this warp's k range: add the partial sums into the tile's accumulator; the warp that
@@ -2412,32 +2425,37 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
       for (int e = 0; e < 4; ++e) { r4[e] = ab[e * 32 + lane] * rs[e & 1]; ab[e * 32 + lane] = 0.f; }
       if (lane == 0) cnt[b] = 0u;
       // r4[0], r4[1] = weight row g x activation rows 2t, 2t + 1; r4[2], r4[3] = weight row g + 8
-      if (KIND == VK_QKV && a.rope_tab) {
-        // RoPE on q and k (packed rows 2i, 2i + 1 = the pair (i, i + dh / 2): the partner sits in lane ^ 4) and the
-        // append of k, v to the cache (a3, rope_append_kernel's arithmetic)
+      if (KIND == VK_QKV) {
+        // the tile's 16 packed rows lie in one head of q, k or v (d % 16 == 0, dh % 16 == 0): packed row 2i / 2i + 1 of a
+        // q or k head = elements i / i + dh / 2 (the RoPE pair, the partner sits in lane ^ 4); v rows are in natural order
+        const int base = rt * 16, which = base / a.d, w_ = base - which * a.d, head = w_ / a.dh, e0 = w_ - head * a.dh;
         const int half = a.dh >> 1;
+        const bool rope = a.rope_tab != nullptr;
 #pragma unroll
         for (int sx = 0; sx < 2; ++sx) {
           const int n = 2 * t + sx;
+          const bool live = n < a.rows;
+          float* orow = a.out + (size_t)n * a.ldo + which * a.d + head * a.dh;
+          size_t cbase = 0;
+          if (rope && live) cbase = (((size_t)seq_s[n] * a.n_heads + head) * a.max_seq + seq_s[8 + n]) * a.dh;
 #pragma unroll
           for (int hh = 0; hh < 2; ++hh) {
             const float val = r4[2 * hh + sx];
             const float pv = __shfl_xor_sync(0xffffffffu, val, 4);
-            const int pr = rt * 16 + g + 8 * hh;
-            if (n >= a.rows || pr >= a.n_out) continue;
-            const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
-            const int pos = seq_s[8 + n], seq = seq_s[n];
-            const size_t cbase = (((size_t)seq * a.n_heads + head) * a.max_seq + pos) * a.dh;
+            const int e = e0 + g + 8 * hh;
+            if (!live || base + g + 8 * hh >= a.n_out) continue;
             if (which < 2) {
-              const int j = e >> 1;
-              const float2 cs = rope_s[n * half + j];
-              const float o = (e & 1) ? val * cs.x + pv * cs.y : val * cs.x - pv * cs.y;
-              const int ne = j + (e & 1) * half;
-              a.out[(size_t)n * a.ldo + which * a.d + head * a.dh + ne] = o;
-              if (which == 1) a.Kc[cbase + ne] = __float2bfloat16_rn(o);
+              const int j = e >> 1, ne = j + (e & 1) * half;
+              float o = val;
+              if (rope) {   // a3, rope_append_kernel's arithmetic
+                const float2 cs = rope_s[n * half + j];
+                o = (e & 1) ? val * cs.x + pv * cs.y : val * cs.x - pv * cs.y;
+                if (which == 1) a.Kc[cbase + ne] = __float2bfloat16_rn(o);
+              }
+              orow[ne] = o;
             } else {
-              a.out[(size_t)n * a.ldo + pr] = val;
-              a.Vc[cbase + e] = __float2bfloat16_rn(val);
+              orow[e] = val;
+              if (rope) a.Vc[cbase + e] = __float2bfloat16_rn(val);
             }
           }
         }
@@ -2456,13 +2474,7 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh) {
           const int pr = rt * 16 + g + 8 * hh;
-          if (pr >= a.n_out) continue;
-          int nat = pr;
-          if (KIND == VK_QKV) {
-            const int which = pr / a.d, w_ = pr % a.d, head = w_ / a.dh, e = w_ % a.dh;
-            nat = which < 2 ? which * a.d + head * a.dh + (e >> 1) + (e & 1) * (a.dh >> 1) : pr;
-          }
-          a.out[(size_t)n * a.ldo + nat] = hh ? v1 : v0;
+          if (pr < a.n_out) a.out[(size_t)n * a.ldo + pr] = hh ? v1 : v0;
         }
       }
     } else {
@@ -2485,7 +2497,6 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
       }
     }
   }
-  if (tid == 0) RTL(7);
 }
 template <int KIND>
 static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int zero, cudaStream_t st) {
@@ -2500,7 +2511,7 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
   }
   const int ld2 = kx / 2 + 4;   // (hi, lo) words per staged row; = 4 mod 16: the LDS.64 of a half-warp hit 16 distinct bank pairs
   const size_t xbytes = (size_t)(a.rows + 1) * ld2 * sizeof(uint2);
-  const size_t fixed = xbytes + (size_t)RR_NB * 4 * 32 * sizeof(float) + 512 + (size_t)8 * (a.dh / 2) * sizeof(float2) + 64;
+  const size_t fixed = xbytes + (size_t)RR_NB * 4 * 32 * sizeof(float) + 768 + (size_t)8 * (a.dh / 2) * sizeof(float2) + 64;
   if ((size_t)smem_max < fixed + 1024 + 2 * (size_t)STAGE_BYTES) return M2R2_UNSUPPORTED;
   // ring depth: what fits, at most 6 and no more than a CTA's stages (a short matrix leaves shared memory to the
   // attention CTAs that are still resident when this kernel's CTAs arrive)
@@ -2512,7 +2523,17 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
     cudaFuncSetAttribute(rows_ring_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
     attr_set = true;
   }
-  return launch_pdl(rows_ring_kernel<KIND>, dim3(G), dim3(RR_THREADS), sh, st, a, nst, ld2, xs_chunks, zero) == cudaSuccess ? 0 : M2R2_CUDA;
+  static const bool no_cluster = getenv("M2R2_XNOCLUSTER") != nullptr;
+  const int csize = (G % 2 == 0 && !no_cluster) ? 2 : 1;
+  cudaLaunchConfig_t cfg = cudaLaunchConfig_t();
+  cfg.gridDim = dim3(G); cfg.blockDim = dim3(RR_THREADS); cfg.dynamicSmemBytes = sh; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  at[1].id = cudaLaunchAttributeClusterDimension;
+  at[1].val.clusterDim.x = csize; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 2;
+  return cudaLaunchKernelEx(&cfg, rows_ring_kernel<KIND>, a, nst, ld2, xs_chunks, csize, zero) == cudaSuccess ? 0 : M2R2_CUDA;
 }
 
 template <int KIND, int NG, bool SW>
@@ -2573,7 +2594,8 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     a.ldu = lora->ldu; a.r = lora->r; a.lora_row0 = lora->lora_row0; a.usel_div = lora->usel_div;
   }
   static const bool no_ring = getenv("M2R2_XNORING") != nullptr;
-  const bool ring = rows <= 8 && !(lora && lora->Bm) && !no_ring && ((kind != VK_OPROJ && kind != VK_DOWN) || (resid == out && !trace));
+  const bool ring = rows <= 8 && !(lora && lora->Bm) && !no_ring && ((kind != VK_OPROJ && kind != VK_DOWN) || (resid == out && !trace)) &&
+                    (kind != VK_QKV || (c.d_model % 16 == 0 && c.head_dim % 16 == 0));
   if (fz) {
     // the caller left the GEMM's neighbours to the ring kernel: only that kernel can honour it
     if (!ring || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
@@ -2621,7 +2643,3 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   }
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
 }
-
-#ifdef M2R2_RING_TL
-extern "C" int m2r2_ring_tl(void* out) { return (int)cudaMemcpyFromSymbol(out, rr_tl, sizeof(rr_tl)); }
-#endif
