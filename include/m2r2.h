@@ -254,6 +254,37 @@ int m2r2_get_profile(m2r2_ctx* ctx, m2r2_profile* out);
 const char* m2r2_last_error(const m2r2_ctx* ctx);
 const char* m2r2_version(void);
 
+/* ---------------------------------------------------------------------------------------------
+ * The final head with NO allocation (greedy decoding
+ * takes the argmax of these logits):
+ *     logits[row] = W_lm . rms(h[row]; g_f),   rms(x; g) = x * g / sqrt(mean(x^2) + rms_eps)
+ * for callers that cannot call cudaMalloc (CUDA-graph capture, serving loops, harnesses that forbid
+ * it).  It needs no context and no caller buffers beyond inputs and output: its one scratch tensor,
+ * the normalised rows, lives in a file-scope device array of M2R2_NOALLOC_MAX_ROWS x
+ * M2R2_NOALLOC_MAX_D floats (256 KB, held by every GPU that loads the library until exit).  The
+ * call allocates nothing and launches the engine's own kernels, so the result equals the
+ * per-operation path's final head bit for bit.
+ *   h       device, fp32 [m][d] dense: the slow residual after the last layer (h_N)
+ *   g_f     device, [d] in `dtype`: gain of the final RMSNorm
+ *   w_lm    device, [vocab][d] row-major in `dtype`: LM head
+ *   logits  device, fp32 [m][vocab], written
+ *   dtype   M2R2_FP32 or M2R2_BF16 (storage type of g_f and w_lm; arithmetic is fp32)
+ *   stream  cudaStream_t of the launches (NULL = default stream); asynchronous, nothing is owned
+ * The current device is used.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress): make that call outside stream capture.  All calls share the scratch
+ * array and it keeps the last call's contents (nothing in it has to start at zero: rows [0, m) are
+ * written before they are read); calls that OVERLAP on the GPU (two streams, two threads) race on
+ * it: serialise them.
+ * Errors: M2R2_CAPACITY if m > M2R2_NOALLOC_MAX_ROWS or d > M2R2_NOALLOC_MAX_D; M2R2_INVALID_ARG
+ * for null pointers, d % 8 != 0, vocab < 1 or an unknown dtype; M2R2_CUDA for a CUDA error.
+ * m2r2_noalloc_last_error() describes the calling thread's last failure ("" after success). */
+#define M2R2_NOALLOC_MAX_ROWS 8
+#define M2R2_NOALLOC_MAX_D 8192
+int m2r2_final_head_noalloc(const float* h, const void* g_f, const void* w_lm, float* logits,
+                            int32_t m, int32_t d, int32_t vocab, int32_t dtype, float rms_eps,
+                            void* stream);
+const char* m2r2_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

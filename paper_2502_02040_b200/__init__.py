@@ -6,4 +6,5 @@ from .binding import (Engine, M2R2Error, Profile, PROF_CLASSES, lib, make_config
                       OK, INVALID_ARG, BAD_STATE, CAPACITY, CUDA, UNSUPPORTED, FP32, BF16,
                       POLICY_FIXED, POLICY_LRU, POLICY_LRU_AOT, POLICY_LRU_RANDOM, POLICY_LRU_PREV,
                       DBG_H, DBG_P, DBG_LOGITS, DBG_EXIT_LOGITS, DBG_K, DBG_V,
-                      DBG_ROUTE_IDX, DBG_ROUTE_W, DBG_PRED_IDX, DBG_EXIT_SCORE)
+                      DBG_ROUTE_IDX, DBG_ROUTE_W, DBG_PRED_IDX, DBG_EXIT_SCORE,
+                      final_head_noalloc, NOALLOC_MAX_ROWS, NOALLOC_MAX_D)

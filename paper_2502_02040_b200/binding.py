@@ -80,7 +80,7 @@ EXPORTS = ["m2r2_query_sizes", "m2r2_create", "m2r2_destroy", "m2r2_load_weights
            "m2r2_decode_step", "m2r2_spec_step", "m2r2_moe_prefetch", "m2r2_set_policy",
            "m2r2_set_logit_script", "m2r2_set_router_script", "m2r2_get_stats", "m2r2_debug_read",
            "m2r2_reset", "m2r2_set_fused", "m2r2_set_profile", "m2r2_get_profile", "m2r2_last_error",
-           "m2r2_version"]
+           "m2r2_version", "m2r2_final_head_noalloc", "m2r2_noalloc_last_error"]
 
 _lib = None
 
@@ -121,6 +121,8 @@ def lib():
         L.m2r2_last_error.argtypes = [vp]
         L.m2r2_last_error.restype = ctypes.c_char_p
         L.m2r2_version.restype = ctypes.c_char_p
+        L.m2r2_final_head_noalloc.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, f32, vp]
+        L.m2r2_noalloc_last_error.restype = ctypes.c_char_p
         _lib = L
     return _lib
 
@@ -352,3 +354,29 @@ class Engine:
 
     def sync(self):
         self.compute_stream.synchronize()
+
+
+# ------------------------------------------------------------------ the entry point that allocates nothing
+NOALLOC_MAX_ROWS, NOALLOC_MAX_D = 8, 8192
+
+
+def final_head_noalloc(h, g_f, w_lm, logits, dtype, rms_eps, stream=None):
+    """m2r2_final_head_noalloc (include/m2r2.h): logits[row] = W_lm . rms(h[row]; g_f) with the op's scratch in a static
+    device array of the library — no allocation in the call.  All arguments are CUDA torch tensors on the current device:
+    h fp32 [m][d] contiguous, g_f [d] and w_lm [vocab][d] in the storage dtype (fp32, or bf16 / its int16 bit pattern),
+    logits fp32 [m][vocab] (written).  `stream`: a torch.cuda.Stream or None (torch's current stream).  Calls that
+    overlap on the GPU race on the shared scratch."""
+    import torch
+    assert h.is_cuda and g_f.is_cuda and w_lm.is_cuda and logits.is_cuda
+    assert h.dtype == torch.float32 and logits.dtype == torch.float32
+    assert h.is_contiguous() and g_f.is_contiguous() and w_lm.is_contiguous() and logits.is_contiguous()
+    m, d = h.shape
+    vocab = w_lm.shape[0]
+    assert tuple(w_lm.shape) == (vocab, d) and g_f.numel() == d and tuple(logits.shape) == (m, vocab)
+    st = stream if stream is not None else torch.cuda.current_stream(h.device)
+    L = lib()
+    rc = L.m2r2_final_head_noalloc(vp(h.data_ptr()), vp(g_f.data_ptr()), vp(w_lm.data_ptr()), vp(logits.data_ptr()),
+                                   int(m), int(d), int(vocab), int(dtype), float(rms_eps), vp(st.cuda_stream))
+    if rc != OK:
+        raise M2R2Error(rc, L.m2r2_noalloc_last_error().decode())
+    return logits

@@ -8,7 +8,7 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libm2r2.so")
-SOURCES = ["m2r2_api.cu", "kernels_general.cu", "kernels_fused.cu"]
+SOURCES = ["m2r2_api.cu", "kernels_general.cu", "kernels_fused.cu", "kernels_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"] + (["-DM2R2_FUSED_DEBUG"] if os.environ.get("M2R2_FUSED_DEBUG") else [])
 
