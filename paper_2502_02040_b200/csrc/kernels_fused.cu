@@ -1696,6 +1696,8 @@ struct VArgs {
   const bf16* gain;      // row-owned: X is the raw residual; RMSNorm(x; gain, eps) applied inside
   float eps;
   int n_heads;
+  const float *part_o, *part_ml;   // O: X = the merge of the attention partials [rows][n_heads][n_splits] (<= 8 splits)
+  int n_splits;
   const int *row_seq, *row_pos;    // QKV: RoPE on q, k and the K/V cache append in the epilogue
   const float2* rope_tab;
   bf16 *Kc, *Vc;
@@ -2226,20 +2228,21 @@ __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 constexpr int RR_THREADS = NCT + 32;
-constexpr int RR_NB = 8;   // row-tile accumulators; a warp runs at most nst (<= 6) stages ahead of the slowest one
+constexpr int RR_NB = 8;   // row-tile accumulators: a warp runs at most nst (<= 6) stages = 6 / nks row tiles ahead of the slowest one;
+                           // matrices with nks >= 2 stages per row tile use 4 of them
 template <int KIND>
-__global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a, int nst, int ld2, int xs_chunks, int csize, unsigned int zero) {
+__global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a, int nst, int ld2, int xs_chunks, int csize, int nb, unsigned int zero) {
   extern __shared__ __align__(1024) unsigned char rr_smem[];
   unsigned char* const ring = rr_smem;
-  uint2* const xp = (uint2*)(rr_smem + (size_t)nst * STAGE_BYTES);    // [rows + 1][ld2]: inputs 2p, 2p + 1 as (hi, lo); last row zeros
-  float* const acc = (float*)(xp + (size_t)(a.rows + 1) * ld2);       // [RR_NB][4][32]
-  u64* const full = (u64*)(acc + RR_NB * 4 * 32);
+  uint2* const xp = (uint2*)(rr_smem + (size_t)nst * STAGE_BYTES);    // [rows][ld2]: inputs 2p, 2p + 1 as (hi, lo)
+  float* const acc = (float*)(xp + (size_t)a.rows * ld2);             // [nb][4][32]
+  u64* const full = (u64*)(acc + nb * 4 * 32);
   u64* const empty = full + 8;
   float* const ssq = (float*)(empty + 8);                             // [2 ranks][8] sums of squares of the rows (fused RMSNorm)
   unsigned int* const cnt = (unsigned int*)(ssq + 2 * 8);             // [RR_NB] warps that have added their part
   u64* const xdone = (u64*)(cnt + RR_NB);                             // the cluster peer's half of the rows has arrived (NCT arrivals)
-  float2* const rope_s = (float2*)(xdone + 1);                        // [8][dh / 2] RoPE (cos, sin) of the rows' positions (QKV)
-  int* const seq_s = (int*)(rope_s + 8 * (a.dh >> 1));                // [8] row -> sequence, [8] row -> position
+  float2* const rope_s = (float2*)(xdone + 1);                        // [rows][dh / 2] RoPE (cos, sin) of the rows' positions (QKV)
+  int* const seq_s = (int*)(rope_s + a.rows * (a.dh >> 1));           // [8] row -> sequence, [8] row -> position (QKV)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
   const int G = gridDim.x, v = blockIdx.x;
   constexpr bool split = KIND == VK_OPROJ || KIND == VK_DOWN;   // (= a.split)
@@ -2272,9 +2275,8 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
     return;
   }
   // ---- consumers
-  for (int i = tid; i < RR_NB * 4 * 32; i += NCT) acc[i] = 0.f;
+  for (int i = tid; i < nb * 4 * 32; i += NCT) acc[i] = 0.f;
   if (tid < RR_NB) cnt[tid] = 0u;
-  for (int i = tid; i < ld2; i += NCT) xp[(size_t)a.rows * ld2 + i] = make_uint2(0u, 0u);   // rows >= a.rows read zeros
   pdl_wait();
   if (KIND == VK_QKV && a.rope_tab) {
     const int half = a.dh >> 1;
@@ -2344,6 +2346,50 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
       }
       mbar_arrive_cluster(mapa_peer(xdone, rank ^ 1u));
     }
+  } else if (KIND == VK_OPROJ && a.part_o != nullptr && s1 > s0) {
+    // O with the split merge absorbed (a4): the inputs of the CTA's k-chunks are merged from the attention partials of
+    // their heads, merge_kernel's arithmetic (slow rows); the loads of all splits of an item are in flight together
+    const int kc0 = s0 % nks, cnt_c = min(s1 - s0, nks), items = a.rows * cnt_c * (SK_K / 4);
+    const int ns = a.n_splits;
+#pragma unroll 1
+    for (int i = tid; i < items; i += NCT) {
+      const int q = i & 31, j = i >> 5, row = j / cnt_c, ci = j - row * cnt_c;
+      int kc = kc0 + ci;
+      if (kc >= nks) kc -= nks;
+      const int k = kc * SK_K + 4 * q;
+      float4 x4 = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (k < a.K) {
+        const int head = k / a.dh, e = k - head * a.dh;   // dh % 4 == 0: the four inputs share the head
+        const size_t pbase = ((size_t)row * a.n_heads + head) * ns;
+        float2 ml[8];
+        float4 o[8];
+#pragma unroll
+        for (int sp = 0; sp < 8; ++sp) {
+          ml[sp] = make_float2(0.f, 0.f);
+          o[sp] = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (sp < ns) {
+            ml[sp] = __ldcg((const float2*)a.part_ml + pbase + sp);
+            o[sp] = __ldcg((const float4*)(a.part_o + (pbase + sp) * a.dh + e));
+          }
+        }
+        float M = -INFINITY, L = 0.f;
+#pragma unroll
+        for (int sp = 0; sp < 8; ++sp)
+          if (ml[sp].y > 0.f) M = fmaxf(M, ml[sp].x);
+#pragma unroll
+        for (int sp = 0; sp < 8; ++sp) {
+          if (ml[sp].y > 0.f) {
+            const float w = __expf(ml[sp].x - M);
+            L += ml[sp].y * w;
+            x4.x += o[sp].x * w; x4.y += o[sp].y * w; x4.z += o[sp].z * w; x4.w += o[sp].w * w;
+          }
+        }
+        x4.x /= L; x4.y /= L; x4.z /= L; x4.w /= L;
+      }
+      uint4 w;
+      w.x = pack_hi_lo(x4.x, x4.y, w.y); w.z = pack_hi_lo(x4.z, x4.w, w.w);
+      *(uint4*)(xp + (size_t)row * ld2 + (((kc % xs_chunks) * SK_K + 4 * q) >> 1)) = w;
+    }
   } else if (s1 > s0) {
     // the k-chunks of the CTA's range (slots by chunk index modulo xs_chunks), four loads in flight per thread
     const int kc0 = s0 % nks, cnt_c = min(s1 - s0, nks), items = a.rows * cnt_c * (SK_K / 4);   // SK_K / 4 == 32
@@ -2378,7 +2424,8 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
   bar_consumers();
   if (pair) while (!mbar_try_wait_cluster(xdone, 0u)) { }
 
-  const uint2* bp = xp + (size_t)min(g, a.rows) * ld2 + t;
+  // (lanes of the MMA's columns >= a.rows read row a.rows - 1: those columns of the result are never stored)
+  const uint2* bp = xp + (size_t)min(g, a.rows - 1) * ld2 + t;
   float c[4] = {0.f, 0.f, 0.f, 0.f}, cl[4] = {0.f, 0.f, 0.f, 0.f};
   float rs[2] = {1.f, 1.f};   // 1 / rms of activation rows 2t, 2t + 1
   if (!split && a.gain) {
@@ -2410,7 +2457,7 @@ __global__ void __launch_bounds__(RR_THREADS, 1) rows_ring_kernel(const VArgs a,
       if ((s % nks) != nks - 1) continue;
       // the row tile is finished in this warp's k range: add the partial sums into the tile's accumulator; the warp that
       // arrives last holds the complete sums and finishes the tile
-      const int rt = s / nks, b = (i / nks) % RR_NB;
+      const int rt = s / nks, b = (i / nks) % nb;
       float* ab = acc + b * 4 * 32;
 #pragma unroll
       for (int e = 0; e < 4; ++e) { atomicAdd(ab + e * 32 + lane, c[e] + cl[e]); c[e] = 0.f; cl[e] = 0.f; }
@@ -2510,13 +2557,17 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
     kx = xs_chunks * SK_K;
   }
   const int ld2 = kx / 2 + 4;   // (hi, lo) words per staged row; = 4 mod 16: the LDS.64 of a half-warp hit 16 distinct bank pairs
-  const size_t xbytes = (size_t)(a.rows + 1) * ld2 * sizeof(uint2);
-  const size_t fixed = xbytes + (size_t)RR_NB * 4 * 32 * sizeof(float) + 768 + (size_t)8 * (a.dh / 2) * sizeof(float2) + 64;
-  if ((size_t)smem_max < fixed + 1024 + 2 * (size_t)STAGE_BYTES) return M2R2_UNSUPPORTED;
-  // ring depth: what fits, at most 6 and no more than a CTA's stages (a short matrix leaves shared memory to the
-  // attention CTAs that are still resident when this kernel's CTAs arrive)
+  const int nb = (!a.split && nks < 2) ? RR_NB : 4;
+  const size_t xbytes = (size_t)a.rows * ld2 * sizeof(uint2);
+  const size_t fixed = xbytes + (size_t)nb * 4 * 32 * sizeof(float) + 512 + (KIND == VK_QKV ? (size_t)a.rows * (a.dh / 2) * sizeof(float2) + 64 : 0);
+  if ((size_t)smem_max < fixed + 2 * (size_t)STAGE_BYTES) return M2R2_UNSUPPORTED;
+  // ring depth: what fits, no more than a CTA's stages, at most 6 (split-K) / 4 (row-owned: a fifth stage fits at d = 3072
+  // with 5 rows and measured 0.6 % slower per C3 spec_step — more copies in flight while the rows are staged slow the
+  // rows' loads down, as the L2 prefetch did)
   const int max_stages = a.split ? ((a.n_rt / SK_RT) * nks + G - 1) / G : (a.n_rt + G - 1) / G * nks;
-  const int nst = std::max(2, std::min((int)std::min<size_t>(6, ((size_t)smem_max - fixed - 1024) / STAGE_BYTES), max_stages));
+  static const int xcap_r = getenv("M2R2_XCAPR") ? atoi(getenv("M2R2_XCAPR")) : 4, xcap_s = getenv("M2R2_XCAPS") ? atoi(getenv("M2R2_XCAPS")) : 6;
+  const size_t cap = a.split ? xcap_s : xcap_r;
+  const int nst = std::max(2, std::min((int)std::min<size_t>(cap, ((size_t)smem_max - fixed) / STAGE_BYTES), max_stages));
   const size_t sh = (size_t)nst * STAGE_BYTES + fixed;
   static bool attr_set = false;
   if (!attr_set) {
@@ -2533,7 +2584,7 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
   at[1].id = cudaLaunchAttributeClusterDimension;
   at[1].val.clusterDim.x = csize; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
   cfg.attrs = at; cfg.numAttrs = 2;
-  return cudaLaunchKernelEx(&cfg, rows_ring_kernel<KIND>, a, nst, ld2, xs_chunks, csize, zero) == cudaSuccess ? 0 : M2R2_CUDA;
+  return cudaLaunchKernelEx(&cfg, rows_ring_kernel<KIND>, a, nst, ld2, xs_chunks, csize, nb, zero) == cudaSuccess ? 0 : M2R2_CUDA;
 }
 
 template <int KIND, int NG, bool SW>
@@ -2601,6 +2652,8 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     if (!ring || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
     a.gain = (const bf16*)fz->gain; a.eps = fz->eps;
     a.n_heads = c.n_heads;
+    a.part_o = fz->part_o; a.part_ml = fz->part_ml; a.n_splits = fz->n_splits;
+    if (a.part_o && (kind != VK_OPROJ || a.n_splits < 1 || a.n_splits > 8)) return M2R2_UNSUPPORTED;
     a.row_seq = fz->row_seq; a.row_pos = fz->row_pos; a.rope_tab = fz->rope_tab; a.Kc = (bf16*)fz->Kc; a.Vc = (bf16*)fz->Vc;
     a.max_seq = c.max_seq;
   }

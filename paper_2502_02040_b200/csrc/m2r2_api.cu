@@ -700,7 +700,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   // tensor-core GEMM (kernels_fused.cu) reads each weight once for all rows (a11)
   // (dual passes at batch >= 5 have 9..32 rows: the same kernel carries the accelerated rows' adapters)
   const bool mma_rows = ((!dual && ns <= 64) || (dual && 2 * B > 8 && 2 * B <= 64)) && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
-  static const bool no_ring_fuse = getenv("M2R2_XNOFUSE") != nullptr;
+  static const bool no_ring_fuse = getenv("M2R2_XNOFUSE") != nullptr, no_merge_fuse = getenv("M2R2_XNOMERGEFUSE") != nullptr;
   float* tr0 = p.trace ? x->trace : nullptr;
   launch_embed(x->cs, c.dtype, x->embed, x->d_row_tok, ns, d, x->resid, any_accel ? x->resid + (size_t)ns * d : nullptr,
                tr0, (tr0 && dual) ? tr0 + (size_t)B * d : nullptr);
@@ -766,7 +766,15 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     memcpy(mg.accel_head_mask, x->accel_mask, sizeof(mg.accel_head_mask));
     if (topk_accel) memset(mg.accel_head_mask, 0, sizeof(mg.accel_head_mask));   // accelerated rows: zero here, S heads written below
     mg.scale = scale;
-    launch_merge(x->cs, mg, rows);
+    // (verify / prefill rows at batch 1: the O ring GEMM merges the splits while it stages its inputs)
+    bool o_done = false;
+    if (ring_fuse && !no_merge_fuse) {
+      RowsFuse fz;
+      fz.part_o = x->part_o; fz.part_ml = x->part_ml; fz.n_splits = splits;
+      o_done = fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr, nullptr, &fz) == 0;
+      if (o_done) saved += 1;
+    }
+    if (!o_done) launch_merge(x->cs, mg, rows);
     if (topk_accel) {
       launch_accel_topk_attn(x->cs, c.dtype, x->qkv, Kc, Vc, x->d_row_limit, x->d_accel_heads, c.n_accel_heads, x->attn_o, B, nh, dh, d,
                              c.max_seq, c.accel_topk_tokens, scale);
@@ -776,10 +784,12 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     // a5: O-proj + residual
     prof_mark(x, M2R2_PROF_OPROJ);
     if (acc_on) { launch_lora_down(x->cs, c.dtype, x->attn_o, d, ns, na, da, x->d_accel_cols, L.Ao, r, x->U, 64); count(x); }
-    memset(&g, 0, sizeof(g));
-    g.W = L.wo; g.X = x->attn_o; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
-    if (acc_on) { g.Bm = L.Bo; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-    if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+    if (!o_done) {
+      memset(&g, 0, sizeof(g));
+      g.W = L.wo; g.X = x->attn_o; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
+      if (acc_on) { g.Bm = L.Bo; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
+      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+    }
     count(x);
     float* trl = p.trace ? x->trace + (size_t)(i + 1) * 2 * B * d : nullptr;
     if (!c.n_experts) {

@@ -56,6 +56,9 @@ bool fused_abort_pending(const FusedState* fs);
 struct RowsFuse {
   const void* gain = nullptr;      // QKV, gate/up, LM head: X is the raw residual; RMSNorm(x; gain, eps) inside (a2, a6, a9)
   float eps = 0.f;
+  const float* part_o = nullptr;   // O: X is ignored; the rows are merged from the attention partials of <= 8 splits (a4)
+  const float* part_ml = nullptr;
+  int n_splits = 0;
   const int* row_seq = nullptr;    // QKV: RoPE on q, k and the K/V cache append in the epilogue (a3)
   const int* row_pos = nullptr;
   const float2* rope_tab = nullptr;
