@@ -1692,6 +1692,9 @@ struct VArgs {
   const int* bmap;       // nullable -> identity; -1 = no adapter row for this output
   const float* U;
   int ldu, r, lora_row0, usel_div;
+  const uint2* Xp;       // rows > 8: the rows as (bf16 hi pair, bf16 lo pair) words [NG * 8][Kp / 2], zero padded (pack_rows_kernel)
+  int Kp;
+  float* part;           // QKV / gate-up with ksplit > 1: partial sums [n_rt][NG][4][32], zero between launches
   // neighbours absorbed by rows_ring_kernel (RowsFuse)
   const bf16* gain;      // row-owned: X is the raw residual; RMSNorm(x; gain, eps) applied inside
   float eps;
@@ -1710,96 +1713,29 @@ __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   lo = bf2_u32(l);
   return bf2_u32(h);
 }
-// A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows of a 256-input chunk are staged
-// ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row tiles, so every weight is read from HBM
-// once for all rows and the replicated activation traffic from L2 stays near the weight traffic; each warp keeps the
-// chunk's 16 weight tiles (8 KB) in flight while the rows are staged.  NG groups of 8 rows = NG n8 MMA tiles (x2: hi, lo)
-// per weight tile.  Epilogues: QKV undoes the RoPE row permutation of the packed matrix, gate/up applies SwiGLU on the
-// lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
-// writes logits; accelerated rows add their parallel adapter term B u (PAPER.md L74).
-constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
-// SW (NG == 1): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
-// takes its w-th quarter) and their sums meet in shared memory: four times the CTAs for matrices with few row tiles.
-template <int KIND, int NG, bool SW>
-__global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
-  constexpr int NQ = SW ? 4 : 1;                   // 256-input chunks staged per iteration
-  constexpr int LD = NQ * RM_KC + 8;               // bf16 elements per staged row (+8: bank spread)
-  extern __shared__ __align__(16) unsigned char rm_smem[];
-  bf16* xh = (bf16*)rm_smem;                       // [NG * 8][LD] hi parts
-  bf16* xl = xh + (size_t)NG * 8 * LD;             // lo parts
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  const int rt = SW ? blockIdx.x : blockIdx.x * 4 + warp;
-  const bool mine = rt < a.n_rt;
-  float c[NG][4];
-#pragma unroll
-  for (int i = 0; i < NG; ++i)
-#pragma unroll
-    for (int e = 0; e < 4; ++e) c[i][e] = 0.f;
-  const int nch = (a.nkt + 16 * NQ - 1) / (16 * NQ);   // (super-)chunks of the whole K
-  const int ch_lo = (int)(((long long)nch * blockIdx.y) / a.ksplit), ch_hi = (int)(((long long)nch * (blockIdx.y + 1)) / a.ksplit);
-  const int wq = SW ? warp : 0;                    // the warp's quarter of the staged inputs
-  pdl_launch_dependents();                         // the next kernel of the chain may begin to launch
-  for (int ch = ch_lo; ch < ch_hi; ++ch) {
-    const int kbase = ch * NQ * RM_KC;
-    // the warp's 16 weight tiles of this iteration: 16 LDG.128 per lane in flight while the activations are staged
-    // (requesting the next iteration's tiles before the MMAs as well costs 60 registers and an SM's third CTA: slower)
-    uint4 w[16];
-#pragma unroll
-    for (int u = 0; u < 16; ++u) {
-      const int kt = (ch * NQ + wq) * 16 + u;
-      w[u] = make_uint4(0u, 0u, 0u, 0u);
-      if (mine && kt < a.nkt) {
-        const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
-                                    : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
-        w[u] = ldg_stream(a.W + tile * 32 + lane);
-      }
-    }
-    // weights never depend on the previous kernel: under programmatic dependent launch the first iteration's tiles are
-    // already in flight while the producer of the activation rows finishes
-    if (ch == ch_lo) pdl_wait();
-    __syncthreads();   // the previous iteration's staged rows are consumed
-    for (int i = tid; i < NG * 8 * (NQ * RM_KC / 4); i += 128) {
-      const int row = i / (NQ * RM_KC / 4), q = i - row * (NQ * RM_KC / 4), k = kbase + 4 * q;
-      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (row < a.rows && k < a.K) v = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));   // K % 4 == 0
-      uint32_t l0, l1;
-      const uint32_t h0 = pack_hi_lo(v.x, v.y, l0), h1 = pack_hi_lo(v.z, v.w, l1);
-      *(uint2*)(xh + (size_t)row * LD + 4 * q) = make_uint2(h0, h1);
-      *(uint2*)(xl + (size_t)row * LD + 4 * q) = make_uint2(l0, l1);
-    }
-    __syncthreads();
-#pragma unroll
-    for (int u = 0; u < 16; ++u) {
-#pragma unroll
-      for (int gi = 0; gi < NG; ++gi) {
-        const bf16* ph = xh + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
-        const bf16* pl = xl + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
-        mma_bf16(c[gi], w[u], *(const uint32_t*)ph, *(const uint32_t*)(ph + 8));
-        mma_bf16(c[gi], w[u], *(const uint32_t*)pl, *(const uint32_t*)(pl + 8));
-      }
-    }
+// rows > 8: every CTA of the GEMM needs all rows of its k-chunks, and converting them to bf16 hi + lo in each CTA costs
+// more instructions than the MMAs: convert ONCE, the GEMM's staging is then a plain 16-byte copy
+__global__ void __launch_bounds__(256) pack_rows_kernel(const float* __restrict__ X, int ldx, int rows, int K, int rows_pad,
+                                                        int Kp, uint2* __restrict__ Xp) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int nq = Kp >> 2;
+  for (int i = blockIdx.x * 256 + threadIdx.x; i < rows_pad * nq; i += gridDim.x * 256) {
+    const int row = i / nq, q = i - row * nq, k = 4 * q;
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (row < rows && k < K) v = __ldcg((const float4*)(X + (size_t)row * ldx + k));
+    uint4 w;
+    w.x = pack_hi_lo(v.x, v.y, w.y);
+    w.z = pack_hi_lo(v.z, v.w, w.w);
+    *(uint4*)(Xp + (size_t)row * (Kp >> 1) + 2 * q) = w;
   }
-  if (ch_lo >= ch_hi) pdl_wait();                  // (a CTA without chunks still orders its epilogue behind the predecessor)
-  if (SW) {
-    // the four warps' partial sums of the row tile -> warp 0
-    __syncthreads();
-    float* red = (float*)rm_smem;                  // [3][NG * 4][32]
-    if (warp > 0) {
-#pragma unroll
-      for (int gi = 0; gi < NG; ++gi)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) red[((warp - 1) * NG * 4 + gi * 4 + e) * 32 + lane] = c[gi][e];
-    }
-    __syncthreads();
-    if (warp > 0) return;
-#pragma unroll
-    for (int ww = 0; ww < 3; ++ww)
-#pragma unroll
-      for (int gi = 0; gi < NG; ++gi)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) c[gi][e] += red[(ww * NG * 4 + gi * 4 + e) * 32 + lane];
-  }
-  if (!mine) return;
+}
+// the epilogue of one 16-row weight tile, given the complete (or, for O / down under split-K, the CTA's partial) sums in
+// the accumulator layout of mma.sync: c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2],
+// c[gi][3] = weight row g + 8.  first_k: this CTA adds the once-only terms (the accelerated rows' adapters).
+template <int KIND, int NG>
+__device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)[NG][4], int lane, bool first_k) {
+  const int g = lane >> 2, t = lane & 3;
   // c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2], c[gi][3] = weight row g + 8
 #pragma unroll
   for (int gi = 0; gi < NG; ++gi) {
@@ -1808,7 +1744,7 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
       const int n = gi * 8 + 2 * t + s;
       if (n >= a.rows) continue;
       float v0 = c[gi][s], v1 = c[gi][2 + s];
-      const bool lora = a.Bm != nullptr && n >= a.lora_row0 && blockIdx.y == 0;   // + B (A x^) on accelerated rows
+      const bool lora = a.Bm != nullptr && n >= a.lora_row0 && first_k;   // + B (A x^) on accelerated rows
       const float* urow = a.U + (size_t)n * a.ldu;
       if (KIND == VK_GATEUP) {
         const int o = rt * 8 + g;
@@ -1853,6 +1789,149 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
     }
   }
 }
+// second stage of a row-owned matrix that was split along K: one warp per row tile reads the summed partials (and leaves
+// zeros behind for the next launch) and runs the epilogue
+template <int KIND, int NG>
+__global__ void __launch_bounds__(128) rows_epilogue_kernel(const VArgs a) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int lane = threadIdx.x & 31, rt = blockIdx.x * 4 + (threadIdx.x >> 5);
+  if (rt >= a.n_rt) return;
+  float c[NG][4];
+  float* src = a.part + (size_t)rt * NG * 4 * 32 + lane;
+#pragma unroll
+  for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      c[gi][e] = __ldcg(src + (gi * 4 + e) * 32);
+      src[(gi * 4 + e) * 32] = 0.f;
+    }
+  rows_epilogue<KIND, NG>(a, rt, c, lane, true);
+}
+// A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows of a 256-input chunk are staged
+// ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row tiles, so every weight is read from HBM
+// once for all rows and the replicated activation traffic from L2 stays near the weight traffic; each warp keeps the
+// chunk's 16 weight tiles (8 KB) in flight while the rows are staged.  NG groups of 8 rows = NG n8 MMA tiles (x2: hi, lo)
+// per weight tile.  Epilogues: QKV undoes the RoPE row permutation of the packed matrix, gate/up applies SwiGLU on the
+// lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
+// writes logits; accelerated rows add their parallel adapter term B u (PAPER.md L74).
+constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
+// SW (NG == 1): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
+// takes its w-th quarter) and their sums meet in shared memory: four times the CTAs for matrices with few row tiles.
+template <int KIND, int NG, bool SW>
+__global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
+  constexpr int NQ = SW ? 4 : 1;                   // 256-input chunks staged per iteration
+  constexpr int LD = NQ * RM_KC + 8;               // bf16 elements per staged row (+8: bank spread)
+  extern __shared__ __align__(16) unsigned char rm_smem[];
+  bf16* xh = (bf16*)rm_smem;                       // [NG * 8][LD] hi parts
+  bf16* xl = xh + (size_t)NG * 8 * LD;             // lo parts
+  constexpr bool PK = !SW;                         // the rows arrive converted (a.Xp): staged by copy as (hi, lo) words
+  constexpr int LD2 = RM_KC / 2 + 4;               // words per staged row; = 4 mod 16: a half-warp's LDS.64 hit 16 bank pairs
+  uint2* xs = (uint2*)rm_smem;                     // [NG * 8][LD2]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
+  const int rt = SW ? blockIdx.x : blockIdx.x * 4 + warp;
+  const bool mine = rt < a.n_rt;
+  float c[NG][4];
+#pragma unroll
+  for (int i = 0; i < NG; ++i)
+#pragma unroll
+    for (int e = 0; e < 4; ++e) c[i][e] = 0.f;
+  const int nch = (a.nkt + 16 * NQ - 1) / (16 * NQ);   // (super-)chunks of the whole K
+  const int ch_lo = (int)(((long long)nch * blockIdx.y) / a.ksplit), ch_hi = (int)(((long long)nch * (blockIdx.y + 1)) / a.ksplit);
+  const int wq = SW ? warp : 0;                    // the warp's quarter of the staged inputs
+  pdl_launch_dependents();                         // the next kernel of the chain may begin to launch
+  for (int ch = ch_lo; ch < ch_hi; ++ch) {
+    const int kbase = ch * NQ * RM_KC;
+    // the warp's 16 weight tiles of this iteration: 16 LDG.128 per lane in flight while the activations are staged
+    // (requesting the next iteration's tiles before the MMAs as well costs 60 registers and an SM's third CTA: slower)
+    uint4 w[16];
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+      const int kt = (ch * NQ + wq) * 16 + u;
+      w[u] = make_uint4(0u, 0u, 0u, 0u);
+      if (mine && kt < a.nkt) {
+        const size_t tile = a.split ? ((size_t)((rt >> 3) * a.nstage_k + (kt >> 3)) * 64 + (rt & 7) * 8 + (kt & 7))
+                                    : ((size_t)(rt * a.nstage_k + (kt >> 6)) * 64 + (kt & 63));
+        w[u] = ldg_stream(a.W + tile * 32 + lane);
+      }
+    }
+    // weights never depend on the previous kernel: under programmatic dependent launch the first iteration's tiles are
+    // already in flight while the producer of the activation rows finishes
+    if (ch == ch_lo) pdl_wait();
+    __syncthreads();   // the previous iteration's staged rows are consumed
+    if (PK) {
+      for (int i = tid; i < NG * 8 * (RM_KC / 4); i += 128) {
+        const int row = i >> 6, q = i & 63;   // RM_KC / 4 == 64 copies of 16 bytes per row
+        cp_async16(xs + (size_t)row * LD2 + 2 * q, a.Xp + (size_t)row * (a.Kp >> 1) + (kbase >> 1) + 2 * q);
+      }
+      cp_async_wait_all();
+    } else
+    for (int i = tid; i < NG * 8 * (NQ * RM_KC / 4); i += 128) {
+      const int row = i / (NQ * RM_KC / 4), q = i - row * (NQ * RM_KC / 4), k = kbase + 4 * q;
+      float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (row < a.rows && k < a.K) v = __ldg((const float4*)(a.X + (size_t)row * a.ldx + k));   // K % 4 == 0
+      uint32_t l0, l1;
+      const uint32_t h0 = pack_hi_lo(v.x, v.y, l0), h1 = pack_hi_lo(v.z, v.w, l1);
+      *(uint2*)(xh + (size_t)row * LD + 4 * q) = make_uint2(h0, h1);
+      *(uint2*)(xl + (size_t)row * LD + 4 * q) = make_uint2(l0, l1);
+    }
+    __syncthreads();
+    if (PK) {
+#pragma unroll
+      for (int u = 0; u < 16; ++u) {
+#pragma unroll
+        for (int gi = 0; gi < NG; ++gi) {
+          const uint2* bp = xs + (size_t)(gi * 8 + g) * LD2 + u * 8 + t;   // inputs 16u + 2t (+1) and + 8: (hi, lo)
+          const uint2 b0 = bp[0], b1 = bp[4];
+          mma_bf16(c[gi], w[u], b0.x, b1.x);
+          mma_bf16(c[gi], w[u], b0.y, b1.y);
+        }
+      }
+    } else
+#pragma unroll
+    for (int u = 0; u < 16; ++u) {
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi) {
+        const bf16* ph = xh + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
+        const bf16* pl = xl + (size_t)(gi * 8 + g) * LD + wq * RM_KC + u * 16 + 2 * t;
+        mma_bf16(c[gi], w[u], *(const uint32_t*)ph, *(const uint32_t*)(ph + 8));
+        mma_bf16(c[gi], w[u], *(const uint32_t*)pl, *(const uint32_t*)(pl + 8));
+      }
+    }
+  }
+  if (ch_lo >= ch_hi) pdl_wait();                  // (a CTA without chunks still orders its epilogue behind the predecessor)
+  if (SW) {
+    // the four warps' partial sums of the row tile -> warp 0
+    __syncthreads();
+    float* red = (float*)rm_smem;                  // [3][NG * 4][32]
+    if (warp > 0) {
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) red[((warp - 1) * NG * 4 + gi * 4 + e) * 32 + lane] = c[gi][e];
+    }
+    __syncthreads();
+    if (warp > 0) return;
+#pragma unroll
+    for (int ww = 0; ww < 3; ++ww)
+#pragma unroll
+      for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) c[gi][e] += red[(ww * NG * 4 + gi * 4 + e) * 32 + lane];
+  }
+  if (!mine) return;
+  if ((KIND == VK_QKV || KIND == VK_GATEUP) && a.ksplit > 1) {
+    // row-owned matrix split along K (many rows): the partial sums meet in a[part] in the accumulator layout;
+    // rows_epilogue_kernel finishes the tile
+    float* dst = a.part + (size_t)rt * NG * 4 * 32 + lane;
+#pragma unroll
+    for (int gi = 0; gi < NG; ++gi)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) atomicAdd(dst + (gi * 4 + e) * 32, c[gi][e]);
+    return;
+  }
+  rows_epilogue<KIND, NG>(a, rt, c, lane, blockIdx.y == 0);
+}
 
 }  // namespace
 
@@ -1877,6 +1956,10 @@ struct FusedImpl {
   float *R, *act, *qbuf, *khat, *vhat, *apart, *apu, *udpart;
   u64* upart;
   int* accel_cols;
+  uint2* xpack;               // rows_mma_kernel with > 8 rows: the rows as (hi, lo) words (pack_rows_kernel)
+  size_t xpack_n = 0;
+  float* rows_part;           // rows_mma_kernel: partial sums of a row-owned matrix split along K (zero between launches)
+  size_t rows_part_n = 0;
 };
 
 static int pad_to(int v, int m) { return (v + m - 1) / m * m; }
@@ -1940,6 +2023,14 @@ void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs) {
   FTAKE(upart, u64, (size_t)UPART_N * UPART_STRIDE)
   FTAKE(apu, float, (size_t)c.n_heads * M2R2_MAX_SPLITS * RV_STRIDE)
   FTAKE(udpart, float, (size_t)1024 * RV_STRIDE)
+  {
+    const size_t n = (size_t)std::max(q.rt_qkv, q.rt_gu) * 8 * 4 * 32;   // [row tiles][NG <= 8][4][32]
+    FTAKE(rows_part, float, n)
+    if (im) im->rows_part_n = n;
+    const size_t np = (size_t)64 * ((size_t)std::max(q.d_pad, q.F_pad) + 256) / 2;   // 64 rows x K (padded to 256) / 2 words
+    FTAKE(xpack, uint2, np)
+    if (im) im->xpack_n = np;
+  }
 #undef FTAKE
 }
 
@@ -2075,6 +2166,7 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   cudaMemsetAsync(im->act, 0, sizeof(float) * 2 * q.F_pad, st);
   cudaMemsetAsync(im->R, 0, sizeof(float) * 2 * d, st);
   cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * RV_STRIDE, st);
+  cudaMemsetAsync(im->rows_part, 0, sizeof(float) * im->rows_part_n, st);
   cudaMemsetAsync(im->upart, 0, sizeof(u64) * UPART_N * UPART_STRIDE, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;   // hl / sidx / cols are stack-owned
   im->bar_base = 0;
@@ -2606,6 +2698,22 @@ static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
   cfg.attrs = at; cfg.numAttrs = 1;
   cudaLaunchKernelEx(&cfg, rows_mma_kernel<KIND, NG, SW>, a);
 }
+template <int KIND, int NG>
+static void launch_rows_epilogue_t(const VArgs& a, cudaStream_t st) {
+  launch_pdl(rows_epilogue_kernel<KIND, NG>, dim3((a.n_rt + 3) / 4), dim3(128), 0, st, a);
+}
+template <int KIND>
+static void launch_rows_epilogue(const VArgs& a, int ng, cudaStream_t st) {
+  switch (ng) {
+    case 2: launch_rows_epilogue_t<KIND, 2>(a, st); break;
+    case 3: launch_rows_epilogue_t<KIND, 3>(a, st); break;
+    case 4: launch_rows_epilogue_t<KIND, 4>(a, st); break;
+    case 5: launch_rows_epilogue_t<KIND, 5>(a, st); break;
+    case 6: launch_rows_epilogue_t<KIND, 6>(a, st); break;
+    case 7: launch_rows_epilogue_t<KIND, 7>(a, st); break;
+    default: launch_rows_epilogue_t<KIND, 8>(a, st); break;
+  }
+}
 template <int KIND>
 static void launch_rows_mma(const VArgs& a, dim3 grid, int ng, cudaStream_t st) {
   switch (ng) {
@@ -2681,11 +2789,36 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     const bool sw = ng <= 1;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW); with more
                                                    // rows the replicated activation reads would exceed the weight stream
     const int gx = sw ? n_rt : (n_rt + 3) / 4, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
+    static const int slots_per_sm = getenv("M2R2_XSLOTS") ? atoi(getenv("M2R2_XSLOTS")) : 4;   // rows_mma_kernel: <= 128 registers x 128 threads
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
-      const int want = (4 * im->G + gx - 1) / gx;
+      const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
       a.ksplit = std::max(1, std::min(want, nch));
     }
+    if (!sw) {
+      // > 8 rows: convert the rows once (pack_rows_kernel); the GEMM stages them by copy
+      const int rows_pad = ng * 8, Kp = nch * RM_KC;
+      if ((size_t)rows_pad * (Kp / 2) > im->xpack_n) return M2R2_UNSUPPORTED;
+      const int items = rows_pad * (Kp / 4);
+      launch_pdl(pack_rows_kernel, dim3(std::min((items + 255) / 256, 8 * im->G)), dim3(256), 0, st, a.X, a.ldx, a.rows, a.K, rows_pad, Kp, im->xpack);
+      a.Xp = im->xpack; a.Kp = Kp;
+      if (fs->launch_counter) ++*fs->launch_counter;
+    }
+    // QKV / gate-up with 9..64 rows: a CTA of 4 row tiles walks all of K with 8 KB per warp in flight, and there are only
+    // n_rt / 4 = 144..256 CTAs: latency-bound at a fraction of the HBM rate.  Split along K as well; the partial sums meet
+    // in rows_part (fp32 atomics, accumulator layout) and rows_epilogue_kernel finishes the tiles.
+    static const bool no_two_stage = getenv("M2R2_XNOTWOSTAGE") != nullptr;
+    if ((kind == VK_QKV || kind == VK_GATEUP) && ng >= 2 && !no_two_stage && (size_t)n_rt * ng * 128 <= im->rows_part_n) {
+      const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
+      a.ksplit = std::max(1, std::min(want, nch));
+      if (a.ksplit > 1) a.part = im->rows_part;
+    }
     const dim3 grid(gx, a.ksplit);
+    if (a.part) {
+      if (kind == VK_QKV) { launch_rows_mma<VK_QKV>(a, grid, ng, st); launch_rows_epilogue<VK_QKV>(a, ng, st); }
+      else { launch_rows_mma<VK_GATEUP>(a, grid, ng, st); launch_rows_epilogue<VK_GATEUP>(a, ng, st); }
+      if (fs->launch_counter) ++*fs->launch_counter;
+      return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
+    }
     switch (kind) {
       case VK_QKV:    launch_rows_mma<VK_QKV>(a, grid, ng, st); break;
       case VK_OPROJ:  launch_rows_mma<VK_OPROJ>(a, grid, ng, st); break;

@@ -101,6 +101,8 @@ __global__ void __launch_bounds__(256) lora_down_kernel(const float* __restrict_
                                                         const int* __restrict__ xmap,
                                                         const WT* __restrict__ A, int r,
                                                         float* __restrict__ U, int ldu) {
+  pdl_launch_dependents();
+  pdl_wait();
   int row = row0 + blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const float* x = X + (size_t)row * ldx;
   for (int j = warp; j < r; j += 8) {
@@ -121,9 +123,9 @@ void launch_lora_down(cudaStream_t st, int dtype, const float* X, int ldx, int r
                       const int* xmap, const void* A, int r, float* U, int ldu) {
   if (rows <= 0) return;
   if (dtype == M2R2_FP32)
-    lora_down_kernel<float><<<rows, 256, 0, st>>>(X, ldx, row0, K, xmap, (const float*)A, r, U, ldu);
+    launch_pdl(lora_down_kernel<float>, dim3(rows), dim3(256), 0, st, X, ldx, row0, K, xmap, (const float*)A, r, U, ldu);
   else
-    lora_down_kernel<__nv_bfloat16><<<rows, 256, 0, st>>>(X, ldx, row0, K, xmap, (const __nv_bfloat16*)A, r, U, ldu);
+    launch_pdl(lora_down_kernel<__nv_bfloat16>, dim3(rows), dim3(256), 0, st, X, ldx, row0, K, xmap, (const __nv_bfloat16*)A, r, U, ldu);
 }
 
 // =====================================================================================

@@ -366,6 +366,7 @@ extern "C" int m2r2_create(const m2r2_config* cfg, const m2r2_buffers* bufs, voi
   walk_weights(c, w, x);
   rc = fused_create(c, &x->fs);   // before the carve: the fused scratch pointers land in fs.impl
   if (rc) { delete x; return rc; }
+  x->fs.launch_counter = &x->st.kernel_launches;
   Carver cv(bufs->scratch);
   carve_scratch(c, cv, x);
   memset(x->accel_mask, 0, sizeof(x->accel_mask));
@@ -675,7 +676,10 @@ static int exit_head(m2r2_ctx* x, int B, int ns, float* logits_out, int* tok_out
   g.W = x->lm_head; g.X = x->xn + (size_t)ns * d; g.ldx = d; g.n_rows = B; g.K = d; g.n_out = V;
   g.out = logits_out; g.ldo = V;
   if (ad) { g.Bm = x->lm_B; g.U = x->U + (size_t)ns * 64; g.ldu = 64; g.r = r; g.lora_row0 = 0; }
-  launch_gemv(x->cs, c.dtype, g, false);
+  // bf16 dense models with the fragment-major copy bound: the skinny tensor-core GEMM, adapter in its epilogue
+  const bool mma_rows = B <= 64 && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
+  if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, 0, 4, g.X, d, B, logits_out, V, nullptr, nullptr, ad ? &g : nullptr))
+    launch_gemv(x->cs, c.dtype, g, false);
   launch_argmax(x->cs, logits_out, V, B, V, x->d_row_seq + ns, x->d_row_pos + ns,
                 x->ls_on ? x->d_ls_draft : nullptr, x->ls_first, x->ls_n, x->ls_beta, tok_out, tok_stride);
   count(x, 3);

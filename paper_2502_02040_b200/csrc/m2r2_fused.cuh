@@ -12,6 +12,7 @@ struct FusedImpl;
 struct FusedState {
   bool supported = false;
   FusedImpl* impl = nullptr;
+  int64_t* launch_counter = nullptr;   // fused_gemv_rows adds the launches beyond the one its caller counts
 };
 
 // what one launch runs
