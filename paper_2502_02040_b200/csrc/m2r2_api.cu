@@ -641,9 +641,16 @@ static int prefetch_pairs(m2r2_ctx* x, const int* pairs, int n) {
 }
 
 // ------------------------------------------------------------------ forward pass (per-operation kernels)
-static int n_splits_for(const m2r2_ctx* x, int groups, int max_len) {
-  int want = (4 * x->sm_count + x->c.n_heads * groups - 1) / (x->c.n_heads * groups);
+// mma: the tensor-core kernel of the k-token / dual-row attention (attn_mma_kernel: 2 CTAs of 4 warps per SM) takes the pass
+static int n_splits_for(const m2r2_ctx* x, int groups, int max_len, bool mma = false) {
+  const int items = x->c.n_heads * groups;
+  int want = (4 * x->sm_count + items - 1) / items;
+  // attn_mma_kernel: one wave of CTAs, rounded to the nearest count: at C4 (256 items, 296 slots) 1 / 2 / 3 / 4 / 8 splits
+  // run a spec_step in 14.39 / 14.88 / 15.05 / 15.31 / 16.17 ms (every split pays its prologue, its partials and the merge)
+  if (mma) want = std::max(1, (2 * x->sm_count + items / 2) / items);
   int cap = std::max(1, (max_len + 127) / 128);   // >= 128 positions per split: shorter items are all prologue and merge
+  static const int force = getenv("M2R2_XSPLITS") ? atoi(getenv("M2R2_XSPLITS")) : 0;
+  if (force > 0) return std::min(force, (int)M2R2_MAX_SPLITS);
   return std::max(1, std::min(std::min(want, cap), M2R2_MAX_SPLITS));
 }
 
@@ -712,7 +719,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   int max_len = 0;
   for (int b = 0; b < B; ++b) max_len = std::max(max_len, x->kv_h[b]);
   max_len += (dual ? p.joff + 1 : (p.mode == MODE_VERIFY ? p.m : p.c0 + p.m));
-  const int splits = n_splits_for(x, B, max_len);
+  const int splits = n_splits_for(x, B, max_len, c.dtype == M2R2_BF16 && (dual ? 2 : p.m) >= 2 && (dh == 64 || dh == 96 || dh == 128));
   const float scale = 1.0f / sqrtf((float)dh);
 
   for (int i = 0; i < p.n_layers; ++i) {
@@ -1191,7 +1198,7 @@ extern "C" int m2r2_spec_step(m2r2_ctx* x, int32_t k, int32_t* accepted, int32_t
   {
     int max_len = 0;
     for (int b = 0; b < B; ++b) max_len = std::max(max_len, x->kv_h[b]);
-    const int splits = n_splits_for(x, B, max_len + k + 1);
+    const int splits = n_splits_for(x, B, max_len + k + 1, c.dtype == M2R2_BF16 && (c.head_dim == 64 || c.head_dim == 96 || c.head_dim == 128));   // as run_pass will
     const unsigned long long key = ((unsigned long long)x->ls_version << 32) | ((unsigned long long)(x->ls_on ? 1 : 0) << 31) |
                                    ((unsigned long long)(x->fused ? 1 : 0) << 30) | ((unsigned long long)splits << 12) |
                                    ((unsigned long long)B << 4) | (unsigned long long)k;
