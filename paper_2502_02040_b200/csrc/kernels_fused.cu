@@ -1705,6 +1705,8 @@ struct VArgs {
   const float2* rope_tab;
   bf16 *Kc, *Vc;
   int max_seq;
+  int slow_rows;         // rows_mma_kernel with rope_tab: rows < slow_rows append k, v to the cache
+  int tile_in_head;      // d % 16 == 0 && dh % 16 == 0 (QKV epilogue: index arithmetic once per tile)
 };
 __device__ __forceinline__ uint32_t pack_hi_lo(float a, float b, uint32_t& lo) {
   const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -1736,6 +1738,55 @@ __global__ void __launch_bounds__(256) pack_rows_kernel(const float* __restrict_
 template <int KIND, int NG>
 __device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)[NG][4], int lane, bool first_k) {
   const int g = lane >> 2, t = lane & 3;
+  if (KIND == VK_QKV && a.tile_in_head) {
+    // d % 16 == 0 and dh % 16 == 0: the tile's 16 packed rows lie in one head of q, k or v.  Packed rows 2i, 2i + 1 of a
+    // q / k head are the elements i, i + dh / 2: the RoPE pair, the partner in lane ^ 4.  With rope_tab the epilogue also
+    // rotates q, k (after the adapter term) and appends the slow rows' k, v to the cache (a3,
+    // rope_append_kernel's arithmetic); accelerated rows keep k^, v^ in `out` only.
+    const int base = rt * 16, which = base / a.d, w_ = base - which * a.d, head = w_ / a.dh, e0 = w_ - head * a.dh;
+    const int half = a.dh >> 1;
+#pragma unroll
+    for (int gi = 0; gi < NG; ++gi) {
+#pragma unroll
+      for (int s = 0; s < 2; ++s) {
+        const int n = gi * 8 + 2 * t + s;
+        const bool live = n < a.rows;
+        const bool lora = a.Bm != nullptr && live && n >= a.lora_row0 && first_k;
+        int pos = 0;
+        size_t cbase = 0;
+        if (a.rope_tab && live) {
+          pos = a.row_pos[n];
+          cbase = (((size_t)a.row_seq[n] * a.n_heads + head) * a.max_seq + pos) * a.dh;
+        }
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+          const int e = e0 + g + 8 * hh, ne = which < 2 ? (e >> 1) + (e & 1) * half : e;
+          const int nat = which * a.d + head * a.dh + ne;
+          const bool inb = base + g + 8 * hh < a.n_out;
+          float v = c[gi][2 * hh + s];
+          if (lora && inb) {
+            const int bn = a.bmap ? a.bmap[nat] : nat;
+            if (bn >= 0) {
+              const float* u = a.U + (size_t)n * a.ldu + (a.usel_div ? which : 0) * a.r;   // usel_div == d for QKV
+              for (int q = 0; q < a.r; ++q) v += bf(a.Bm + (size_t)bn * a.r + q) * u[q];
+            }
+          }
+          const float pv = __shfl_xor_sync(0xffffffffu, v, 4);
+          if (!live || !inb) continue;
+          if (a.rope_tab && which < 2) {
+            const float2 cs = a.rope_tab[(size_t)pos * half + (e >> 1)];
+            v = (e & 1) ? v * cs.x + pv * cs.y : v * cs.x - pv * cs.y;
+          }
+          a.out[(size_t)n * a.ldo + nat] = v;
+          if (a.rope_tab && n < a.slow_rows) {
+            if (which == 1) a.Kc[cbase + ne] = __float2bfloat16_rn(v);
+            if (which == 2) a.Vc[cbase + e] = __float2bfloat16_rn(v);
+          }
+        }
+      }
+    }
+    return;
+  }
   // c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2], c[gi][3] = weight row g + 8
 #pragma unroll
   for (int gi = 0; gi < NG; ++gi) {
@@ -2755,9 +2806,14 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   static const bool no_ring = getenv("M2R2_XNORING") != nullptr;
   const bool ring = rows <= 8 && !(lora && lora->Bm) && !no_ring && ((kind != VK_OPROJ && kind != VK_DOWN) || (resid == out && !trace)) &&
                     (kind != VK_QKV || (c.d_model % 16 == 0 && c.head_dim % 16 == 0));
+  a.tile_in_head = (c.d_model % 16 == 0 && c.head_dim % 16 == 0) ? 1 : 0;
+  a.slow_rows = rows;
   if (fz) {
-    // the caller left the GEMM's neighbours to the ring kernel: only that kernel can honour it
-    if (!ring || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
+    // the caller left the GEMM's neighbours to the kernel: the ring kernel honours all of them, rows_mma_kernel (> 8 rows)
+    // RoPE + KV append in the QKV epilogue
+    const bool rope_only = !fz->gain && !fz->part_o && fz->rope_tab && kind == VK_QKV && a.tile_in_head && c.dtype == M2R2_BF16;
+    if ((!ring && !rope_only) || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
+    if (fz->rope_tab) a.slow_rows = fz->slow_rows > 0 ? fz->slow_rows : rows;
     a.gain = (const bf16*)fz->gain; a.eps = fz->eps;
     a.n_heads = c.n_heads;
     a.part_o = fz->part_o; a.part_ml = fz->part_ml; a.n_splits = fz->n_splits;

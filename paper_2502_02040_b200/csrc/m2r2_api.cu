@@ -748,10 +748,20 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       memset(&g, 0, sizeof(g));
       g.W = L.wqkv; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = 3 * d; g.out = x->qkv; g.ldo = 3 * d;
       if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
-      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
-      // a3: RoPE + KV append
-      prof_mark(x, M2R2_PROF_ROPE);
-      launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
+      bool roped = false;
+      if (mma_rows && rows > 8 && !no_ring_fuse) {
+        // batched passes: RoPE + KV append in the tensor-core GEMM's epilogue
+        RowsFuse fz;
+        fz.row_seq = x->d_row_seq; fz.row_pos = x->d_row_pos; fz.rope_tab = x->rope_tab; fz.Kc = Kc; fz.Vc = Vc; fz.slow_rows = ns;
+        roped = fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr, &fz) == 0;
+        if (roped) saved += 1;
+      }
+      if (!roped) {
+        if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+        // a3: RoPE + KV append
+        prof_mark(x, M2R2_PROF_ROPE);
+        launch_rope_append(x->cs, c.dtype, x->qkv, rows, ns, x->d_row_seq, x->d_row_pos, x->rope_tab, Kc, Vc, nh, dh, c.max_seq);
+      }
     }
     // a4: split-K attention + merge
     prof_mark(x, M2R2_PROF_ATTN);

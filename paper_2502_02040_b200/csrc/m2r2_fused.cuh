@@ -52,7 +52,7 @@ bool fused_abort_pending(const FusedState* fs);
 // rows 9..64 (rows_mma_kernel) may carry the accelerated rows' parallel adapters: `lora` supplies Bm / Bm2 / bmap / U /
 // ldu / r / lora_row0 / usel_div with the meaning they have in GemvArgs (nullptr: none).
 // rows <= 8 without adapters (rows_ring_kernel, one CTA per SM streaming the matrix through a shared-memory ring) can also
-// absorb the GEMM's neighbours in the layer, given in `fz`; M2R2_UNSUPPORTED then means nothing was launched and the
+// absorb the GEMM's neighbours in the layer, given in `fz`; with more rows (rows_mma_kernel) only RoPE + KV append; M2R2_UNSUPPORTED then means nothing was launched and the
 // caller runs the separate kernels.
 struct RowsFuse {
   const void* gain = nullptr;      // QKV, gate/up, LM head: X is the raw residual; RMSNorm(x; gain, eps) inside (a2, a6, a9)
@@ -65,6 +65,7 @@ struct RowsFuse {
   const float2* rope_tab = nullptr;
   void* Kc = nullptr;
   void* Vc = nullptr;
+  int slow_rows = 0;               // rows >= slow_rows (accelerated rows, > 8-row passes) are rotated but not cached; 0: all rows
 };
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
                     int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora = nullptr,
