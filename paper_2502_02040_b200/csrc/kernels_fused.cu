@@ -1736,7 +1736,7 @@ __global__ void __launch_bounds__(256) pack_rows_kernel(const float* __restrict_
 // the accumulator layout of mma.sync: c[gi][0], c[gi][1] = weight row g x activation rows 8 gi + 2t, + 1; c[gi][2],
 // c[gi][3] = weight row g + 8.  first_k: this CTA adds the once-only terms (the accelerated rows' adapters).
 template <int KIND, int NG>
-__device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)[NG][4], int lane, bool first_k) {
+__device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)[NG][4], int lane, bool first_k, int n0 = 0) {
   const int g = lane >> 2, t = lane & 3;
   if (KIND == VK_QKV && a.tile_in_head) {
     // d % 16 == 0 and dh % 16 == 0: the tile's 16 packed rows lie in one head of q, k or v.  Packed rows 2i, 2i + 1 of a
@@ -1749,7 +1749,7 @@ __device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)
     for (int gi = 0; gi < NG; ++gi) {
 #pragma unroll
       for (int s = 0; s < 2; ++s) {
-        const int n = gi * 8 + 2 * t + s;
+        const int n = n0 + gi * 8 + 2 * t + s;
         const bool live = n < a.rows;
         const bool lora = a.Bm != nullptr && live && n >= a.lora_row0 && first_k;
         int pos = 0;
@@ -1792,7 +1792,7 @@ __device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)
   for (int gi = 0; gi < NG; ++gi) {
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
-      const int n = gi * 8 + 2 * t + s;
+      const int n = n0 + gi * 8 + 2 * t + s;
       if (n >= a.rows) continue;
       float v0 = c[gi][s], v1 = c[gi][2 + s];
       const bool lora = a.Bm != nullptr && n >= a.lora_row0 && first_k;   // + B (A x^) on accelerated rows
@@ -1840,24 +1840,23 @@ __device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)
     }
   }
 }
-// second stage of a row-owned matrix that was split along K: one warp per row tile reads the summed partials (and leaves
-// zeros behind for the next launch) and runs the epilogue
+// second stage of a row-owned matrix that was split along K: one warp per (row tile, group of 8 activation rows) reads the
+// summed partials (and leaves zeros behind for the next launch) and runs the epilogue.  (One warp per tile for all groups
+// left 4 warps per SM with a chain of dependent loads each: 13 us for the 40-row QKV.)
 template <int KIND, int NG>
 __global__ void __launch_bounds__(128) rows_epilogue_kernel(const VArgs a) {
   pdl_launch_dependents();
   pdl_wait();
-  const int lane = threadIdx.x & 31, rt = blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31, rt = blockIdx.x * 4 + (threadIdx.x >> 5), gi = blockIdx.y;
   if (rt >= a.n_rt) return;
-  float c[NG][4];
-  float* src = a.part + (size_t)rt * NG * 4 * 32 + lane;
+  float c[1][4];
+  float* src = a.part + ((size_t)rt * NG + gi) * 4 * 32 + lane;
 #pragma unroll
-  for (int gi = 0; gi < NG; ++gi)
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      c[gi][e] = __ldcg(src + (gi * 4 + e) * 32);
-      src[(gi * 4 + e) * 32] = 0.f;
-    }
-  rows_epilogue<KIND, NG>(a, rt, c, lane, true);
+  for (int e = 0; e < 4; ++e) {
+    c[0][e] = __ldcg(src + e * 32);
+    src[e * 32] = 0.f;
+  }
+  rows_epilogue<KIND, 1>(a, rt, c, lane, true, gi * 8);
 }
 // A CTA = 4 warps = 4 consecutive 16-row tiles over a K range; the activation rows of a 256-input chunk are staged
 // ONCE per CTA in shared memory as bf16 hi + lo parts and shared by the four row tiles, so every weight is read from HBM
@@ -2751,7 +2750,7 @@ static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
 }
 template <int KIND, int NG>
 static void launch_rows_epilogue_t(const VArgs& a, cudaStream_t st) {
-  launch_pdl(rows_epilogue_kernel<KIND, NG>, dim3((a.n_rt + 3) / 4), dim3(128), 0, st, a);
+  launch_pdl(rows_epilogue_kernel<KIND, NG>, dim3((a.n_rt + 3) / 4, NG), dim3(128), 0, st, a);
 }
 template <int KIND>
 static void launch_rows_epilogue(const VArgs& a, int ng, cudaStream_t st) {
