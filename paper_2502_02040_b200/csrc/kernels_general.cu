@@ -50,6 +50,10 @@ __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict_
   pdl_launch_dependents();   // the GEMM that consumes xn may begin to launch and prefetch its weights
   pdl_wait();
   int row = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  // blockIdx.y: part 0 writes xn; part p computes the adapter rows [8 p, 8 p + 8) of an accelerated row (every part
+  // recomputes the norm: d elements, cheaper than a warp walking three adapter rows in turn)
+  const int part = blockIdx.y;
+  if (part > 0 && (A == nullptr || row < lora_row0)) return;
   const float* x = X + (size_t)row * d;
   float ss = 0.f;
   for (int j = tid; j < d; j += 256) {
@@ -67,11 +71,11 @@ __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict_
   for (int j = tid; j < d; j += 256) {
     float v = sx[j] * inv * to_f32(g[j]);
     sx[j] = v;
-    xn[(size_t)row * d + j] = v;
+    if (part == 0) xn[(size_t)row * d + j] = v;
   }
   if (A == nullptr || row < lora_row0) return;
   __syncthreads();
-  for (int t = warp; t < nA * r; t += 8) {
+  for (int t = part * 8 + warp; t < nA * r; t += 8 * gridDim.y) {
     const WT* a = A + (size_t)t * d;
     float acc = 0.f;
     for (int k = lane * 8; k < d; k += 256) {
@@ -89,10 +93,11 @@ void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int 
                       float eps, float* xn, const void* A, int nA, int r, int lora_row0, float* U,
                       int ldu) {
   size_t sh = (size_t)d * sizeof(float);
+  const dim3 grid(rows, A ? std::max(1, (nA * r + 7) / 8) : 1);
   if (dtype == M2R2_FP32)
-    launch_pdl(norm_lora_kernel<float>, dim3(rows), dim3(256), sh, st, X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<float>, grid, dim3(256), sh, st, X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
   else
-    launch_pdl(norm_lora_kernel<__nv_bfloat16>, dim3(rows), dim3(256), sh, st, X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<__nv_bfloat16>, grid, dim3(256), sh, st, X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
 }
 
 // u[row][j] = A[j, :] . x[row][xmap(:)]   (no norm; A_o on the compact o^, A_d on the activations)
