@@ -1866,10 +1866,14 @@ __global__ void __launch_bounds__(128) rows_epilogue_kernel(const VArgs a) {
 // lane's (gate, up) pair, O / down add the residual (split along K: atomic adds onto the in-place residual), LM head
 // writes logits; accelerated rows add their parallel adapter term B u.
 constexpr int RM_KC = 256;               // inputs per staged chunk (16 k16 tiles)
+#ifndef M2R2_RM_NW
+#define M2R2_RM_NW 8
+#endif
+constexpr int RM_NW = M2R2_RM_NW;        // warps = row tiles of a CTA with > 8 rows: they share one staged chunk of the rows
 // SW (NG == 1): the CTA's four warps split the inputs of ONE row tile (a super-chunk of 4 x 256 inputs is staged, warp w
 // takes its w-th quarter) and their sums meet in shared memory: four times the CTAs for matrices with few row tiles.
 template <int KIND, int NG, bool SW>
-__global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
+__global__ void __launch_bounds__(SW ? 128 : RM_NW * 32) rows_mma_kernel(const VArgs a) {
   constexpr int NQ = SW ? 4 : 1;                   // 256-input chunks staged per iteration
   constexpr int LD = NQ * RM_KC + 8;               // bf16 elements per staged row (+8: bank spread)
   extern __shared__ __align__(16) unsigned char rm_smem[];
@@ -1879,7 +1883,7 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
   constexpr int LD2 = RM_KC / 2 + 4;               // words per staged row; = 4 mod 16: a half-warp's LDS.64 hit 16 bank pairs
   uint2* xs = (uint2*)rm_smem;                     // [NG * 8][LD2]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, g = lane >> 2, t = lane & 3;
-  const int rt = SW ? blockIdx.x : blockIdx.x * 4 + warp;
+  const int rt = SW ? blockIdx.x : blockIdx.x * RM_NW + warp;
   const bool mine = rt < a.n_rt;
   float c[NG][4];
 #pragma unroll
@@ -1910,7 +1914,7 @@ __global__ void __launch_bounds__(128) rows_mma_kernel(const VArgs a) {
     if (ch == ch_lo) pdl_wait();
     __syncthreads();   // the previous iteration's staged rows are consumed
     if (PK) {
-      for (int i = tid; i < NG * 8 * (RM_KC / 4); i += 128) {
+      for (int i = tid; i < NG * 8 * (RM_KC / 4); i += RM_NW * 32) {
         const int row = i >> 6, q = i & 63;   // RM_KC / 4 == 64 copies of 16 bytes per row
         cp_async16(xs + (size_t)row * LD2 + 2 * q, a.Xp + (size_t)row * (a.Kp >> 1) + (kbase >> 1) + 2 * q);
       }
@@ -2741,7 +2745,7 @@ static void launch_rows_mma_t(const VArgs& a, dim3 grid, cudaStream_t st) {
   // weight tiles; it reads activations only behind pdl_wait()
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
-  cfg.gridDim = grid; cfg.blockDim = dim3(128); cfg.dynamicSmemBytes = sh; cfg.stream = st;
+  cfg.gridDim = grid; cfg.blockDim = dim3(SW ? 128 : RM_NW * 32); cfg.dynamicSmemBytes = sh; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -2843,8 +2847,8 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     const int ng = (rows + 7) / 8;
     const bool sw = ng <= 1;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW); with more
                                                    // rows the replicated activation reads would exceed the weight stream
-    const int gx = sw ? n_rt : (n_rt + 3) / 4, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
-    static const int slots_per_sm = getenv("M2R2_XSLOTS") ? atoi(getenv("M2R2_XSLOTS")) : 4;   // rows_mma_kernel: <= 128 registers x 128 threads
+    const int gx = sw ? n_rt : (n_rt + RM_NW - 1) / RM_NW, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
+    static const int slots_per_sm = getenv("M2R2_XSLOTS") ? atoi(getenv("M2R2_XSLOTS")) : 512 / (RM_NW * 32);   // rows_mma_kernel: <= 128 registers per thread, 512 threads per SM
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
       const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
       a.ksplit = std::max(1, std::min(want, nch));
