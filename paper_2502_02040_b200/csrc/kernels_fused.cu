@@ -2711,7 +2711,7 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
   // with 5 rows and measured 0.6 % slower per C3 spec_step — more copies in flight while the rows are staged slow the
   // rows' loads down, as the L2 prefetch did)
   const int max_stages = a.split ? ((a.n_rt / SK_RT) * nks + G - 1) / G : (a.n_rt + G - 1) / G * nks;
-  static const int xcap_r = getenv("M2R2_XCAPR") ? atoi(getenv("M2R2_XCAPR")) : 4, xcap_s = getenv("M2R2_XCAPS") ? atoi(getenv("M2R2_XCAPS")) : 6;
+  static const int xcap_r = xknob("M2R2_XCAPR", 4), xcap_s = xknob("M2R2_XCAPS", 6);
   const size_t cap = a.split ? xcap_s : xcap_r;
   const int nst = std::max(2, std::min((int)std::min<size_t>(cap, ((size_t)smem_max - fixed) / STAGE_BYTES), max_stages));
   const size_t sh = (size_t)nst * STAGE_BYTES + fixed;
@@ -2720,7 +2720,7 @@ static int launch_rows_ring(const VArgs& a, int G, int smem_max, unsigned int ze
     cudaFuncSetAttribute(rows_ring_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_max);
     attr_set = true;
   }
-  static const bool no_cluster = getenv("M2R2_XNOCLUSTER") != nullptr;
+  static const bool no_cluster = xknob("M2R2_XNOCLUSTER", 0) != 0;
   const int csize = (G % 2 == 0 && !no_cluster) ? 2 : 1;
   cudaLaunchConfig_t cfg = cudaLaunchConfig_t();
   cfg.gridDim = dim3(G); cfg.blockDim = dim3(RR_THREADS); cfg.dynamicSmemBytes = sh; cfg.stream = st;
@@ -2806,7 +2806,7 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     a.Bm = (const bf16*)lora->Bm; a.Bm2 = (const bf16*)lora->Bm2; a.bmap = lora->bmap; a.U = lora->U;
     a.ldu = lora->ldu; a.r = lora->r; a.lora_row0 = lora->lora_row0; a.usel_div = lora->usel_div;
   }
-  static const bool no_ring = getenv("M2R2_XNORING") != nullptr;
+  static const bool no_ring = xknob("M2R2_XNORING", 0) != 0;
   const bool ring = rows <= 8 && !(lora && lora->Bm) && !no_ring && ((kind != VK_OPROJ && kind != VK_DOWN) || (resid == out && !trace)) &&
                     (kind != VK_QKV || (c.d_model % 16 == 0 && c.head_dim % 16 == 0));
   a.tile_in_head = (c.d_model % 16 == 0 && c.head_dim % 16 == 0) ? 1 : 0;
@@ -2848,7 +2848,7 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     const bool sw = ng <= 1;                       // one row tile per CTA, the warps split K (rows_mma_kernel SW); with more
                                                    // rows the replicated activation reads would exceed the weight stream
     const int gx = sw ? n_rt : (n_rt + RM_NW - 1) / RM_NW, nch = sw ? (a.nkt + 63) / 64 : (a.nkt + 15) / 16;
-    static const int slots_per_sm = getenv("M2R2_XSLOTS") ? atoi(getenv("M2R2_XSLOTS")) : 512 / (RM_NW * 32);   // rows_mma_kernel: <= 128 registers per thread, 512 threads per SM
+    static const int slots_per_sm = xknob("M2R2_XSLOTS", 512 / (RM_NW * 32));   // rows_mma_kernel: <= 128 registers per thread, 512 threads per SM
     if ((kind == VK_OPROJ || kind == VK_DOWN) && resid == out && !trace) {
       const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
       a.ksplit = std::max(1, std::min(want, nch));
@@ -2865,7 +2865,7 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     // QKV / gate-up with 9..64 rows: a CTA of 4 row tiles walks all of K with 8 KB per warp in flight, and there are only
     // n_rt / 4 = 144..256 CTAs: latency-bound at a fraction of the HBM rate.  Split along K as well; the partial sums meet
     // in rows_part (fp32 atomics, accumulator layout) and rows_epilogue_kernel finishes the tiles.
-    static const bool no_two_stage = getenv("M2R2_XNOTWOSTAGE") != nullptr;
+    static const bool no_two_stage = xknob("M2R2_XNOTWOSTAGE", 0) != 0;
     if ((kind == VK_QKV || kind == VK_GATEUP) && ng >= 2 && !no_two_stage && (size_t)n_rt * ng * 128 <= im->rows_part_n) {
       const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
       a.ksplit = std::max(1, std::min(want, nch));

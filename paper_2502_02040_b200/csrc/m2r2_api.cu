@@ -649,7 +649,7 @@ static int n_splits_for(const m2r2_ctx* x, int groups, int max_len, bool mma = f
   // run a spec_step in 14.39 / 14.88 / 15.05 / 15.31 / 16.17 ms (every split pays its prologue, its partials and the merge)
   if (mma) want = std::max(1, (2 * x->sm_count + items / 2) / items);
   int cap = std::max(1, (max_len + 127) / 128);   // >= 128 positions per split: shorter items are all prologue and merge
-  static const int force = getenv("M2R2_XSPLITS") ? atoi(getenv("M2R2_XSPLITS")) : 0;
+  static const int force = xknob("M2R2_XSPLITS", 0);
   if (force > 0) return std::min(force, (int)M2R2_MAX_SPLITS);
   return std::max(1, std::min(std::min(want, cap), M2R2_MAX_SPLITS));
 }
@@ -711,7 +711,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
   // tensor-core GEMM (kernels_fused.cu) reads each weight once for all rows (a11)
   // (dual passes at batch >= 5 have 9..32 rows: the same kernel carries the accelerated rows' adapters)
   const bool mma_rows = ((!dual && ns <= 64) || (dual && 2 * B > 8 && 2 * B <= 64)) && c.dtype == M2R2_BF16 && !c.n_experts && x->fused && fused_supported(c, &x->fs);
-  static const bool no_ring_fuse = getenv("M2R2_XNOFUSE") != nullptr, no_merge_fuse = getenv("M2R2_XNOMERGEFUSE") != nullptr;
+  static const bool no_ring_fuse = xknob("M2R2_XNOFUSE", 0) != 0, no_merge_fuse = xknob("M2R2_XNOMERGEFUSE", 0) != 0;
   float* tr0 = p.trace ? x->trace : nullptr;
   launch_embed(x->cs, c.dtype, x->embed, x->d_row_tok, ns, d, x->resid, any_accel ? x->resid + (size_t)ns * d : nullptr,
                tr0, (tr0 && dual) ? tr0 + (size_t)B * d : nullptr);

@@ -1,6 +1,7 @@
 // m2r2_internal.cuh — shared declarations of the CUDA path (host orchestration + kernels).
 // Product code: nothing here is shared with oracle/.
 #pragma once
+#include <cstdlib>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -68,6 +69,18 @@ static inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 b
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+// A/B switches of the experiments recorded under profiles/ (M2R2_X...): read from the environment in M2R2_FUSED_DEBUG
+// builds only (M2R2_FUSED_DEBUG=1 python -m paper_2502_02040_b200.build --force); the product build always takes `dflt`.
+static inline int xknob(const char* name, int dflt) {
+#ifdef M2R2_FUSED_DEBUG
+  const char* v = getenv(name);
+  return v ? atoi(v) : dflt;
+#else
+  (void)name;
+  return dflt;
+#endif
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
