@@ -534,7 +534,6 @@ def test_c3_full_size_long_context_properties():
         if int(a_tok[0]) != int(b_tok[0]):
             break   # a near-tie desynchronised the free-running engines: the logits check above already passed
         assert float(np.max(np.abs(la - lb))) <= 5e-2 and rel_l2(la, lb) <= 5e-3
-    b.close()
     # (ii) + (iii) on the fused engine
     f, g = S.gen_logit_script(cfg, 200, alpha)
     a.set_logit_script(f, g, P)
@@ -554,7 +553,26 @@ def test_c3_full_size_long_context_properties():
     for _ in range(3):
         assert int(a.decode_step()[0]) == f[pos + 1 - P]
         pos += 1
+    # (iv) the verify pass at full width and this context: the ring GEMMs with RMSNorm, RoPE + KV append and the split merge
+    # absorbed (engine a) against the per-operation kernels (engine b: row-major fp32-FMA GEMV, separate norm / RoPE /
+    # merge kernels) on the same scripted steps: logits of every verify row, and the K/V the pass left in the cache
+    b.set_logit_script(f, g, P)
+    assert int(a.prefill(prompt)[0]) == f[0] and int(b.prefill(prompt)[0]) == f[0]
+    for _ in range(2):
+        acc_a, n_a = a.spec_step(gamma)
+        acc_b, n_b = b.spec_step(gamma)
+        assert int(n_a[0]) == int(n_b[0]) and acc_a[0][:int(n_a[0])].tolist() == acc_b[0][:int(n_b[0])].tolist()
+        for j in range(gamma + 1):
+            la, lb = a.debug_read(M.DBG_LOGITS, j), b.debug_read(M.DBG_LOGITS, j)
+            assert float(np.max(np.abs(la - lb))) <= 5e-2 and rel_l2(la, lb) <= 5e-3, (j, float(np.max(np.abs(la - lb))), rel_l2(la, lb))
+    T = a.get_stats()["kv_len"][0]
+    assert T == b.get_stats()["kv_len"][0] and T > P
+    for layer in (0, cfg.n_layers // 2, cfg.n_layers - 1):
+        for v in (False, True):
+            ka, kb = a.kcache(layer, T, v=v), b.kcache(layer, T, v=v)
+            assert rel_l2(ka[P:], kb[P:]) <= 1e-2, (layer, v, rel_l2(ka[P:], kb[P:]))   # the rows the verify passes appended
     a.close()
+    b.close()
 
 
 def _first_steps_stress(cycles):
