@@ -176,6 +176,45 @@ def test_c5_full_size_three_policies_match_oracle():
     orc.close()
 
 
+def test_c4_full_width_batch8_passes_match_per_operation_kernels():
+    """BASELINE configs[3] at FULL width (d 3072, 32 layers, F 8192, vocabulary 32064) and batch 8, context 1024 to bound
+    the time: the batched passes as bench.py times them — 16 dual rows per draft pass and 40 verify rows on
+    rows_mma_kernel (rows packed once, K split of all four matrices with second-stage epilogues, adapters, RoPE + KV append
+    in the QKV epilogue), tensor-core attention, the draft head on the tensor-core GEMM — against the per-operation
+    kernels of the same library (row-major fp32-FMA GEMV, separate RoPE kernel) on the same scripted spec_step: accepted
+    tokens, logits of every verify row of sequences 0, 3 and 7, the K/V rows the step appended.  Both engines prefill
+    on the fast path; the second switches to the per-operation kernels for the step."""
+    B, P, gamma, alpha = 8, 1024, 4, 0.7
+    cfg = replace(S.config_c4(), max_seq=P + 64)
+    W = S.gen_weights(cfg)
+    a, b = M.Engine(cfg, W), M.Engine(cfg, W)
+    prompts = np.stack([S.gen_prompt(cfg, P, seq=q) for q in range(B)])
+    scripts = [S.gen_logit_script(cfg, 64, alpha, seq=q) for q in range(B)]
+    for e in (a, b):
+        e.set_logit_script(np.stack([s[0] for s in scripts]), np.stack([s[1] for s in scripts]), P)
+        first = e.prefill(prompts)
+        assert [int(t) for t in first] == [int(s[0][0]) for s in scripts]
+    b.set_fused(False)
+    acc_a, n_a = a.spec_step(gamma)
+    acc_b, n_b = b.spec_step(gamma)
+    assert n_a.tolist() == n_b.tolist()
+    for q in range(B):
+        assert acc_a[q][:int(n_a[q])].tolist() == acc_b[q][:int(n_b[q])].tolist()
+    for q in (0, 3, 7):
+        for j in range(gamma + 1):
+            la, lb = a.debug_read(M.DBG_LOGITS, j, q), b.debug_read(M.DBG_LOGITS, j, q)
+            err, rel = float(np.max(np.abs(la - lb))), rel_l2(la, lb)
+            assert err <= 5e-2 and rel <= 5e-3, (q, j, err, rel)
+        T = a.get_stats()["kv_len"][q]
+        assert T == b.get_stats()["kv_len"][q] and T > P
+        for layer in (0, cfg.n_layers - 1):
+            for v in (False, True):
+                ka, kb = a.kcache(layer, T, b=q, v=v), b.kcache(layer, T, b=q, v=v)
+                assert rel_l2(ka[P:], kb[P:]) <= 1e-2, (q, layer, v, rel_l2(ka[P:], kb[P:]))
+    a.close()
+    b.close()
+
+
 def test_c4_reduced_width_full_length_batch8():
     """BASELINE configs[3] at FULL length and batch (B = 8 sequences x 4096-token KV, spec_step(4), per-sequence
     scripts so that kv_len diverges) on a reduced-width model (8 heads x 96, 2 layers): the batched per-operation
