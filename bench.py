@@ -18,7 +18,8 @@ ABI with host buffers (the forced input token goes host->device, the produced to
 every step, inside the timed region).  `roofline` is for the dominant kernel class measured live by
 the library's event profile; `selfspec` is the metric's other half, the same model under self-speculative
 decoding (BASELINE.json configs[2], "C3": gamma 4, acceptance 0.9 and 0.5, 256 tokens, device-timed over the whole
-generation); `cpu_baseline` is the oracle timed on this box's host cores.
+generation), `selfspec_batch8` the batched case (configs[3], "C4": 8 sequences x 4096-token KV, gamma 4, acceptance 0.9, 48
+spec_steps); `cpu_baseline` is the oracle timed on this box's host cores.
 `--impl reference` times the oracle (CPU) on the same config and metric.
 
 Secondary workloads (one JSON line each): c3 = self-spec sweep (gamma x alpha), c4 = batch 8 x 4096-token KV self-spec,
@@ -345,6 +346,8 @@ def run_ours(args, rk):
     if rk.rank == 0 and rk.world == 1 and not args.no_selfspec:
         line["selfspec"] = selfspec_record(peak)
         torch.cuda.empty_cache()
+        line["selfspec_batch8"] = selfspec_batch8_record(peak)
+        torch.cuda.empty_cache()
     if rk.rank == 0 and rk.world == 1 and not args.no_cpu_baseline:
         tps, n, dt, desc = time_oracle(cfg, W, 12, 1, budget_s=25.0)
         line["cpu_baseline"] = {"value": tps, "unit": "tokens/s", "cores": host_cores(), "kind": "oracle", "sample": desc}
@@ -411,6 +414,47 @@ def selfspec_record(peak, gamma=4, alphas=(0.9, 0.5), n_tokens=256):
     e1.record(stream)
     e1.synchronize()
     rec["plain_decode_control_tokens_per_s"] = 128 / (e0.elapsed_time(e1) * 1e-3)
+    eng.close()
+    return rec
+
+
+def selfspec_batch8_record(peak, gamma=4, alpha=0.9, n_steps=48):
+    """C4 (BASELINE.json configs[3]): the same model, 8 sequences x 4096-token KV, spec_step(4) with per-sequence seeded logit
+    scripts at acceptance alpha; the batched passes run on the tensor-core GEMM / attention kernels.  Device-timed over
+    n_steps spec_steps (every step returns its accepted tokens to the host)."""
+    import torch
+    import m2r2_synth as S
+    import paper_2502_02040_b200 as M
+    cfg = S.config_c4()
+    B, P = 8, 4096
+    eng = M.Engine(cfg, S.gen_weights(cfg), device="cuda:0")
+    stream = eng.compute_stream
+    prompts = np.stack([S.gen_prompt(cfg, P, seq=b) for b in range(B)])
+    scripts = [S.gen_logit_script(cfg, 8 * (n_steps + 8), alpha, seq=b) for b in range(B)]
+    eng.set_logit_script(np.stack([x[0] for x in scripts]), np.stack([x[1] for x in scripts]), P)
+    eng.prefill(prompts)
+    for _ in range(3):
+        eng.spec_step(gamma)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    emitted, by = 0, 0
+    l0 = eng.get_stats()["kernel_launches"]
+    e0.record(stream)
+    for _ in range(n_steps):
+        _, n = eng.spec_step(gamma)
+        emitted += int(n.sum())
+        by += eng.get_stats()["algorithmic_bytes_last"]
+    e1.record(stream)
+    e1.synchronize()
+    ms = e0.elapsed_time(e1)
+    gbs = by / (ms * 1e-3) / 1e9
+    rec = {"workload": "C4 (BASELINE.json configs[3]): the C3 model, batch 8, 4096-token KV per sequence, draft length gamma = %d, "
+                       "acceptance %.1f forced by per-sequence seeded logit biasing, %d spec_steps" % (gamma, alpha, n_steps),
+           "gamma": gamma, "alpha": alpha, "batch": B, "kv_len_start": P, "spec_steps": n_steps,
+           "aggregate_tokens_per_s": emitted / (ms * 1e-3), "ms_per_spec_step": ms / n_steps,
+           "tokens_per_spec_step": emitted / n_steps, "algorithmic_bytes_per_spec_step": by / n_steps, "GB/s": gbs,
+           "frac_of_measured_peak": gbs / peak, "frac_of_nominal_8TBs": gbs / HBM_NOMINAL_GBS,
+           "gpu_launches_per_spec_step": (eng.get_stats()["kernel_launches"] - l0) / n_steps}
     eng.close()
     return rec
 
