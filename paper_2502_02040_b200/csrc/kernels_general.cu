@@ -680,6 +680,10 @@ __global__ void __launch_bounds__(128) attn_mma_kernel(AttnArgs a) {
         O += src[j] * wgt;
       }
     }
+    if (a.direct_out) {   // one split, slow rows only: this IS the merged output (merge_kernel's O / L)
+      a.direct_out[(size_t)r * a.d + head * DH + j] = O / L;
+      continue;
+    }
     const size_t pidx = ((size_t)r * a.n_heads + head) * a.n_splits + split;
     a.part_o[pidx * DH + j] = O;
     if (j == 0) { a.part_ml[pidx * 2] = M; a.part_ml[pidx * 2 + 1] = L; }
@@ -714,12 +718,16 @@ static void launch_attn_nq(cudaStream_t st, const AttnArgs& a, dim3 grid, int nq
 }
 
 // rows_per_group: live query rows of a group (<= M2R2_MAXQ), packed from slot 0 of grp_rows
-void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group) {
+bool launch_attn(cudaStream_t st, int dtype, const AttnArgs& a_in, int n_groups, int rows_per_group) {
+  AttnArgs a = a_in;
   dim3 grid(a.n_heads, n_groups, a.n_splits);
+  const bool direct = a.direct_out != nullptr && a.n_splits == 1 && dtype != M2R2_FP32 && rows_per_group >= 2 &&
+                      (a.dh == 64 || a.dh == 96 || a.dh == 128);
+  if (!direct) a.direct_out = nullptr;
   if (dtype != M2R2_FP32 && rows_per_group >= 2) {   // k-token verification attention: tensor pipe (bf16 cache)
-    if (a.dh == 64) { launch_attn_mma<64>(st, a, grid); return; }
-    if (a.dh == 96) { launch_attn_mma<96>(st, a, grid); return; }
-    if (a.dh == 128) { launch_attn_mma<128>(st, a, grid); return; }
+    if (a.dh == 64) { launch_attn_mma<64>(st, a, grid); return direct; }
+    if (a.dh == 96) { launch_attn_mma<96>(st, a, grid); return direct; }
+    if (a.dh == 128) { launch_attn_mma<128>(st, a, grid); return direct; }
   }
   int epl = dtype == M2R2_FP32 ? 4 : 8;
   int lpp = a.dh / epl;
@@ -735,6 +743,7 @@ void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, in
     else if (seg == 16) launch_attn_nq<__nv_bfloat16, 16>(st, a, grid, rows_per_group);
     else launch_attn_nq<__nv_bfloat16, 32>(st, a, grid, rows_per_group);
   }
+  return false;
 }
 
 // ------------------------------------------------------------------ accelerated attention over the slow stream's top-k positions

@@ -779,7 +779,10 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       a.slow_rows = ns;
       memset(a.accel_head_mask, 0, sizeof(a.accel_head_mask));
     }
-    launch_attn(x->cs, c.dtype, a, B, dual ? 2 : p.m);
+    // slow rows only (verify, prefill) and one split: the tensor-core kernel writes the merged output itself
+    if (!dual && splits == 1) a.direct_out = x->attn_o;
+    const bool merged = launch_attn(x->cs, c.dtype, a, B, dual ? 2 : p.m);
+    if (merged) saved += 1;
     MergeArgs mg;
     memset(&mg, 0, sizeof(mg));
     mg.qkv = x->qkv; mg.part_o = x->part_o; mg.part_ml = x->part_ml; mg.row_limit = x->d_row_limit; mg.out = x->attn_o;
@@ -789,13 +792,13 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     mg.scale = scale;
     // (verify / prefill rows at batch 1: the O ring GEMM merges the splits while it stages its inputs)
     bool o_done = false;
-    if (ring_fuse && !no_merge_fuse) {
+    if (ring_fuse && !no_merge_fuse && !merged) {
       RowsFuse fz;
       fz.part_o = x->part_o; fz.part_ml = x->part_ml; fz.n_splits = splits;
       o_done = fused_gemv_rows(c, &x->fs, x->cs, i, 1, x->attn_o, d, rows, x->resid, d, x->resid, nullptr, nullptr, &fz) == 0;
       if (o_done) saved += 1;
     }
-    if (!o_done) launch_merge(x->cs, mg, rows);
+    if (!o_done && !merged) launch_merge(x->cs, mg, rows);
     if (topk_accel) {
       launch_accel_topk_attn(x->cs, c.dtype, x->qkv, Kc, Vc, x->d_row_limit, x->d_accel_heads, c.n_accel_heads, x->attn_o, B, nh, dh, d,
                              c.max_seq, c.accel_topk_tokens, scale);

@@ -142,6 +142,8 @@ struct AttnArgs {
   int n_heads, dh, d, max_seq, n_splits, slow_rows;  // rows >= slow_rows are accelerated rows
   uint32_t accel_head_mask[4];
   float scale;
+  float* direct_out;    // nullable: with ONE split and slow rows only the tensor-core kernel writes the merged output
+                        // [rows][d] itself (launch_attn returns true: no merge_kernel needed)
 };
 
 struct MergeArgs {
@@ -167,7 +169,7 @@ void launch_gemv(cudaStream_t st, int dtype, const GemvArgs& a, bool swiglu);
 void launch_rope_append(cudaStream_t st, int dtype, float* qkv, int rows, int slow_rows, const int* row_seq,
                         const int* row_pos, const float2* rope_tab, void* Kc, void* Vc, int n_heads,
                         int dh, int max_seq);
-void launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group);
+bool launch_attn(cudaStream_t st, int dtype, const AttnArgs& a, int n_groups, int rows_per_group);   // true: merged output written
 void launch_merge(cudaStream_t st, const MergeArgs& a, int rows);
 void launch_accel_topk_attn(cudaStream_t st, int dtype, const float* qkv, const void* Kc, const void* Vc, const int* row_limit,
                             const int* accel_heads, int n_accel, float* out, int B, int n_heads, int dh, int d, int max_seq,
