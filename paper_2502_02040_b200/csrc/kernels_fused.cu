@@ -1694,6 +1694,8 @@ struct VArgs {
   int ldu, r, lora_row0, usel_div;
   const uint2* Xp;       // rows > 8: the rows as (bf16 hi pair, bf16 lo pair) words [NG * 8][Kp / 2], zero padded (pack_rows_kernel)
   int Kp;
+  uint2* out_pk;         // gate/up, nullable: the activations also as (hi, lo) words [row][out_pk_ld] (down's packed input)
+  int out_pk_ld;
   float* part;           // QKV / gate-up with ksplit > 1: partial sums [n_rt][NG][4][32], zero between launches
   // neighbours absorbed by rows_ring_kernel (RowsFuse)
   const bf16* gain;      // row-owned: X is the raw residual; RMSNorm(x; gain, eps) applied inside
@@ -1793,23 +1795,34 @@ __device__ __forceinline__ void rows_epilogue(const VArgs& a, int rt, float (&c)
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
       const int n = n0 + gi * 8 + 2 * t + s;
+      if (KIND == VK_GATEUP) {
+        const int o = rt * 8 + g;
+        const bool live = n < a.rows && o < a.n_out;
+        float v0 = c[gi][s], v1 = c[gi][2 + s];
+        if (live && a.Bm != nullptr && n >= a.lora_row0 && first_k) {   // + B (A x^) on accelerated rows
+          const float* urow = a.U + (size_t)n * a.ldu;
+          for (int q = 0; q < a.r; ++q) {
+            v0 += bf(a.Bm + (size_t)o * a.r + q) * urow[q];
+            v1 += bf(a.Bm2 + (size_t)o * a.r + q) * urow[a.r + q];
+          }
+        }
+        const float act = live ? silu(v0) * v1 : 0.f;
+        if (live) a.out[(size_t)n * a.ldo + o] = act;
+        if (a.out_pk) {   // outputs o, o + 1 sit in lanes g, g + 1 (lane ^ 4): the even one writes the pair
+          const float nb = __shfl_xor_sync(0xffffffffu, act, 4);
+          if (!(g & 1) && n < a.rows && o < a.n_out) {
+            const __nv_bfloat162 h = __floats2bfloat162_rn(act, nb);
+            const float2 f = __bfloat1622float2(h);
+            const __nv_bfloat162 l = __floats2bfloat162_rn(act - f.x, nb - f.y);
+            a.out_pk[(size_t)n * a.out_pk_ld + (o >> 1)] = make_uint2(bf2_u32(h), bf2_u32(l));
+          }
+        }
+        continue;
+      }
       if (n >= a.rows) continue;
       float v0 = c[gi][s], v1 = c[gi][2 + s];
       const bool lora = a.Bm != nullptr && n >= a.lora_row0 && first_k;   // + B (A x^) on accelerated rows
       const float* urow = a.U + (size_t)n * a.ldu;
-      if (KIND == VK_GATEUP) {
-        const int o = rt * 8 + g;
-        if (o < a.n_out) {
-          if (lora) {
-            for (int q = 0; q < a.r; ++q) {
-              v0 += bf(a.Bm + (size_t)o * a.r + q) * urow[q];
-              v1 += bf(a.Bm2 + (size_t)o * a.r + q) * urow[a.r + q];
-            }
-          }
-          a.out[(size_t)n * a.ldo + o] = silu(v0) * v1;
-        }
-        continue;
-      }
 #pragma unroll
       for (int hh = 0; hh < 2; ++hh) {
         const int pr = rt * 16 + g + 8 * hh;
@@ -2010,6 +2023,8 @@ struct FusedImpl {
   float *R, *act, *qbuf, *khat, *vhat, *apart, *apu, *udpart;
   u64* upart;
   int* accel_cols;
+  uint2 *xn_pack, *act_pack;  // the same, written by their producers: norm_lora_kernel (QKV / gate-up input), the gate/up epilogue (down input)
+  int xn_pack_ld = 0, act_pack_ld = 0;   // words per row; the columns beyond d / d_ff stay zero from fused_bind
   uint2* xpack;               // rows_mma_kernel with > 8 rows: the rows as (hi, lo) words (pack_rows_kernel)
   size_t xpack_n = 0;
   float* rows_part;           // rows_mma_kernel: partial sums of a row-owned matrix split along K (zero between launches)
@@ -2018,6 +2033,7 @@ struct FusedImpl {
 
 static int pad_to(int v, int m) { return (v + m - 1) / m * m; }
 
+constexpr int RM_KC_HOST = 256;   // = RM_KC (rows_mma_kernel's staged chunk)
 struct PackedDims {
   int d_pad, F_pad, rt_qkv, rt_gu, rt_v, ng_d, nkc_o, nkc_d;
   size_t st_qkv, st_o, st_gu, st_d, st_v;   // stages
@@ -2084,6 +2100,10 @@ void fused_carve(const m2r2_config& c, Carver& cv, FusedState* fs) {
     const size_t np = (size_t)64 * ((size_t)std::max(q.d_pad, q.F_pad) + 256) / 2;   // 64 rows x K (padded to 256) / 2 words
     FTAKE(xpack, uint2, np)
     if (im) im->xpack_n = np;
+    const int ldx_ = q.d_pad / 2, lda_ = (pad_to(q.F_pad, RM_KC_HOST)) / 2;
+    FTAKE(xn_pack, uint2, (size_t)64 * ldx_)
+    FTAKE(act_pack, uint2, (size_t)64 * lda_)
+    if (im) { im->xn_pack_ld = ldx_; im->act_pack_ld = lda_; }
   }
 #undef FTAKE
 }
@@ -2221,6 +2241,8 @@ int fused_bind(const m2r2_config& c, FusedState* fs, cudaStream_t st, void* pack
   cudaMemsetAsync(im->R, 0, sizeof(float) * 2 * d, st);
   cudaMemsetAsync(im->udpart, 0, sizeof(float) * 1024 * RV_STRIDE, st);
   cudaMemsetAsync(im->rows_part, 0, sizeof(float) * im->rows_part_n, st);
+  cudaMemsetAsync(im->xn_pack, 0, sizeof(uint2) * 64 * im->xn_pack_ld, st);
+  cudaMemsetAsync(im->act_pack, 0, sizeof(uint2) * 64 * im->act_pack_ld, st);
   cudaMemsetAsync(im->upart, 0, sizeof(u64) * UPART_N * UPART_STRIDE, st);
   if (cudaStreamSynchronize(st) != cudaSuccess) return M2R2_CUDA;   // hl / sidx / cols are stack-owned
   im->bar_base = 0;
@@ -2814,8 +2836,10 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
   if (fz) {
     // the caller left the GEMM's neighbours to the kernel: the ring kernel honours all of them, rows_mma_kernel (> 8 rows)
     // RoPE + KV append in the QKV epilogue
-    const bool rope_only = !fz->gain && !fz->part_o && fz->rope_tab && kind == VK_QKV && a.tile_in_head && c.dtype == M2R2_BF16;
-    if ((!ring && !rope_only) || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
+    // (x_packed / pack_out concern rows_mma_kernel only and never make a call unsupported)
+    const bool rope_ok = !fz->rope_tab || (kind == VK_QKV && a.tile_in_head && c.dtype == M2R2_BF16);
+    const bool mma_ok = !fz->gain && !fz->part_o && rope_ok && rows > 8;
+    if ((!ring && !mma_ok) || (c.head_dim % 4)) return M2R2_UNSUPPORTED;
     if (fz->rope_tab) a.slow_rows = fz->slow_rows > 0 ? fz->slow_rows : rows;
     a.gain = (const bf16*)fz->gain; a.eps = fz->eps;
     a.n_heads = c.n_heads;
@@ -2853,7 +2877,17 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
       const int want = sw ? (4 * im->G + gx - 1) / gx : std::max(1, (slots_per_sm * im->G) / gx);   // one wave of CTAs
       a.ksplit = std::max(1, std::min(want, nch));
     }
-    if (!sw) {
+    if (!sw && fz && fz->pack_out && kind == VK_GATEUP) { a.out_pk = im->act_pack; a.out_pk_ld = im->act_pack_ld; }
+    const uint2* given = nullptr;   // the rows already as (hi, lo) words, left by their producer
+    int given_ld = 0;
+    if (!sw && fz && fz->x_packed) {
+      if (kind == VK_QKV || kind == VK_GATEUP) { given = im->xn_pack; given_ld = im->xn_pack_ld; }
+      else if (kind == VK_DOWN) { given = im->act_pack; given_ld = im->act_pack_ld; }
+      if (given && 2 * given_ld < nch * RM_KC) given = nullptr;
+    }
+    if (given) {
+      a.Xp = given; a.Kp = 2 * given_ld;
+    } else if (!sw) {
       // > 8 rows: convert the rows once (pack_rows_kernel); the GEMM stages them by copy
       const int rows_pad = ng * 8, Kp = nch * RM_KC;
       if ((size_t)rows_pad * (Kp / 2) > im->xpack_n) return M2R2_UNSUPPORTED;
@@ -2887,4 +2921,11 @@ int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int l
     }
   }
   return cudaGetLastError() == cudaSuccess ? 0 : M2R2_CUDA;
+}
+
+// the (hi, lo) word buffers that producers outside this file fill for rows_mma_kernel (nullptr if the fused copy is not bound)
+uint2* fused_xn_pack(const FusedState* fs, int* ld) {
+  if (!fs || !fs->supported || !fs->impl || !fs->impl->bound) return nullptr;
+  *ld = fs->impl->xn_pack_ld;
+  return fs->impl->xn_pack;
 }

@@ -39,12 +39,22 @@ void launch_embed(cudaStream_t st, int dtype, const void* emb, const int* tok, i
 //   rms(x; g) = x * g / sqrt(mean(x^2) + eps)                       (Q1)
 //   u[row][a*r + j] = A_a[j, :] . x^       a < nA packed adapters   (Q3)
 // =====================================================================================
+// (a, b) -> bf16 pair of the values and bf16 pair of what the first rounding lost: the two B operands of the GEMMs
+__device__ __forceinline__ uint2 hi_lo_words(float a, float b) {
+  const __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  const float2 f = __bfloat1622float2(h);
+  const __nv_bfloat162 l = __floats2bfloat162_rn(a - f.x, b - f.y);
+  return make_uint2(*(const uint32_t*)&h, *(const uint32_t*)&l);
+}
+// xn_pk (nullable): the normalised row also as (hi, lo) words [row][pk_ld], what rows_mma_kernel stages by copy for
+// passes with more than 8 rows (the columns beyond d stay as the caller zeroed them)
 template <typename WT>
 __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict__ X, int d,
                                                         const WT* __restrict__ g, float eps,
                                                         float* __restrict__ xn, const WT* __restrict__ A,
                                                         int nA, int r, int lora_row0,
-                                                        float* __restrict__ U, int ldu) {
+                                                        float* __restrict__ U, int ldu,
+                                                        uint2* __restrict__ xn_pk, int pk_ld) {
   extern __shared__ float sx[];
   __shared__ float red[8];
   pdl_launch_dependents();   // the GEMM that consumes xn may begin to launch and prefetch its weights
@@ -68,10 +78,15 @@ __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict_
 #pragma unroll
   for (int w = 0; w < 8; ++w) tot += red[w];
   float inv = rsqrtf(tot / (float)d + eps);
-  for (int j = tid; j < d; j += 256) {
-    float v = sx[j] * inv * to_f32(g[j]);
-    sx[j] = v;
-    if (part == 0) xn[(size_t)row * d + j] = v;
+  for (int p = tid; p < (d >> 1); p += 256) {   // d is even: pairs of elements
+    const int j = 2 * p;
+    const float v0 = sx[j] * inv * to_f32(g[j]), v1 = sx[j + 1] * inv * to_f32(g[j + 1]);
+    sx[j] = v0;
+    sx[j + 1] = v1;
+    if (part == 0) {
+      *(float2*)(xn + (size_t)row * d + j) = make_float2(v0, v1);
+      if (xn_pk) xn_pk[(size_t)row * pk_ld + p] = hi_lo_words(v0, v1);
+    }
   }
   if (A == nullptr || row < lora_row0) return;
   __syncthreads();
@@ -91,13 +106,13 @@ __global__ void __launch_bounds__(256) norm_lora_kernel(const float* __restrict_
 
 void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int d, const void* g,
                       float eps, float* xn, const void* A, int nA, int r, int lora_row0, float* U,
-                      int ldu) {
+                      int ldu, uint2* xn_pk, int pk_ld) {
   size_t sh = (size_t)d * sizeof(float);
   const dim3 grid(rows, A ? std::max(1, (nA * r + 7) / 8) : 1);
   if (dtype == M2R2_FP32)
-    launch_pdl(norm_lora_kernel<float>, grid, dim3(256), sh, st, X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<float>, grid, dim3(256), sh, st, X, d, (const float*)g, eps, xn, (const float*)A, nA, r, lora_row0, U, ldu, xn_pk, pk_ld);
   else
-    launch_pdl(norm_lora_kernel<__nv_bfloat16>, grid, dim3(256), sh, st, X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu);
+    launch_pdl(norm_lora_kernel<__nv_bfloat16>, grid, dim3(256), sh, st, X, d, (const __nv_bfloat16*)g, eps, xn, (const __nv_bfloat16*)A, nA, r, lora_row0, U, ldu, xn_pk, pk_ld);
 }
 
 // u[row][j] = A[j, :] . x[row][xmap(:)]   (no norm; A_o on the compact o^, A_d on the activations)

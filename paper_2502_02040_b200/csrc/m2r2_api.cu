@@ -744,7 +744,10 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       if (qkv_done) saved += 2;
     }
     if (!qkv_done) {
-      launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g1, c.rms_eps, x->xn, acc_on ? L.Aqkv : nullptr, 3, r, ns, x->U, 64);
+      // passes with more than 8 rows: the norm also leaves the rows as (hi, lo) words for the tensor-core GEMM
+      int pk_ld = 0;
+      uint2* pk = (mma_rows && rows > 8 && !no_ring_fuse) ? fused_xn_pack(&x->fs, &pk_ld) : nullptr;
+      launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g1, c.rms_eps, x->xn, acc_on ? L.Aqkv : nullptr, 3, r, ns, x->U, 64, pk, pk_ld);
       memset(&g, 0, sizeof(g));
       g.W = L.wqkv; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = 3 * d; g.out = x->qkv; g.ldo = 3 * d;
       if (acc_on) { g.Bm = L.Bqkv; g.bmap = x->d_qkv_bmap; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; g.usel_div = d; }
@@ -753,6 +756,7 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
         // batched passes: RoPE + KV append in the tensor-core GEMM's epilogue
         RowsFuse fz;
         fz.row_seq = x->d_row_seq; fz.row_pos = x->d_row_pos; fz.rope_tab = x->rope_tab; fz.Kc = Kc; fz.Vc = Vc; fz.slow_rows = ns;
+        fz.x_packed = pk != nullptr;
         roped = fused_gemv_rows(c, &x->fs, x->cs, i, 0, x->xn, d, rows, x->qkv, 3 * d, nullptr, nullptr, acc_on ? &g : nullptr, &fz) == 0;
         if (roped) saved += 1;
       }
@@ -819,18 +823,26 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
     if (!c.n_experts) {
       // a6: RMSNorm + gate/up + SwiGLU;  a7: down + residual (accelerated-residual update)
       prof_mark(x, M2R2_PROF_GATEUP);
-      bool gu_done = false;
+      bool gu_done = false, act_packed = false;
       if (ring_fuse) {
         RowsFuse fz;
         fz.gain = L.g2; fz.eps = c.rms_eps;
         gu_done = fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->resid, d, rows, x->act, c.d_ff, nullptr, nullptr, nullptr, &fz) == 0;
       }
       if (!gu_done) {
-        launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, acc_on ? L.Agu : nullptr, 2, r, ns, x->U, 64);
+        int pk_ld = 0;
+        uint2* pk = (mma_rows && rows > 8 && !no_ring_fuse) ? fused_xn_pack(&x->fs, &pk_ld) : nullptr;
+        launch_norm_lora(x->cs, c.dtype, x->resid, rows, d, L.g2, c.rms_eps, x->xn, acc_on ? L.Agu : nullptr, 2, r, ns, x->U, 64, pk, pk_ld);
         memset(&g, 0, sizeof(g));
         g.W = L.wgate; g.W2 = L.wup; g.X = x->xn; g.ldx = d; g.n_rows = rows; g.K = d; g.n_out = c.d_ff; g.out = x->act; g.ldo = c.d_ff;
         if (acc_on) { g.Bm = L.Bg; g.Bm2 = L.Bu; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-        if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, true);
+        if (pk) {
+          // rows already packed by the norm; the epilogue leaves the activations packed for the down projection
+          RowsFuse fz;
+          fz.x_packed = true; fz.pack_out = true;
+          act_packed = fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr, &fz) == 0;
+        }
+        if (!act_packed && (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 2, x->xn, d, rows, x->act, c.d_ff, nullptr, nullptr, acc_on ? &g : nullptr))) launch_gemv(x->cs, c.dtype, g, true);
       }
       prof_mark(x, M2R2_PROF_DOWN);
       if (acc_on) { launch_lora_down(x->cs, c.dtype, x->act, c.d_ff, ns, na, c.d_ff, nullptr, L.Ad, r, x->U, 64); count(x); }
@@ -838,7 +850,13 @@ static int run_pass(m2r2_ctx* x, const Pass& p) {
       g.W = L.wdown; g.X = x->act; g.ldx = c.d_ff; g.n_rows = rows; g.K = c.d_ff; g.n_out = d; g.out = x->resid; g.ldo = d; g.resid = x->resid;
       g.trace = trl;
       if (acc_on) { g.Bm = L.Bd; g.U = x->U; g.ldu = 64; g.r = r; g.lora_row0 = ns; }
-      if (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl, acc_on ? &g : nullptr)) launch_gemv(x->cs, c.dtype, g, false);
+      bool down_done = false;
+      if (act_packed) {
+        RowsFuse fz;
+        fz.x_packed = true;
+        down_done = fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl, acc_on ? &g : nullptr, &fz) == 0;
+      }
+      if (!down_done && (!mma_rows || fused_gemv_rows(c, &x->fs, x->cs, i, 3, x->act, c.d_ff, rows, x->resid, d, x->resid, trl, acc_on ? &g : nullptr))) launch_gemv(x->cs, c.dtype, g, false);
       count(x, gu_done ? 2 : 3);
     } else {
       int rc = moe_mlp(x, p, i, ns, na);

@@ -65,8 +65,12 @@ struct RowsFuse {
   const float2* rope_tab = nullptr;
   void* Kc = nullptr;
   void* Vc = nullptr;
+  bool x_packed = false;           // > 8 rows: the rows are already in the fused state's (hi, lo) word buffer (QKV, gate/up: by
+                                   // norm_lora_kernel through fused_xn_pack; down: by a gate/up call with pack_out): no pack_rows_kernel
+  bool pack_out = false;           // gate/up, > 8 rows: also leave the activations as (hi, lo) words for the down call
   int slow_rows = 0;               // rows >= slow_rows (accelerated rows, > 8-row passes) are rotated but not cached; 0: all rows
 };
 int fused_gemv_rows(const m2r2_config& c, FusedState* fs, cudaStream_t st, int layer, int kind, const float* X, int ldx,
                     int rows, float* out, int ldo, const float* resid, float* trace, const GemvArgs* lora = nullptr,
                     const RowsFuse* fz = nullptr);
+uint2* fused_xn_pack(const FusedState* fs, int* ld);

@@ -162,7 +162,7 @@ void launch_embed(cudaStream_t st, int dtype, const void* emb, const int* tok, i
                   float* out, float* out2, float* trace, float* trace2);
 void launch_norm_lora(cudaStream_t st, int dtype, const float* X, int rows, int d, const void* g,
                       float eps, float* xn, const void* A, int nA, int r, int lora_row0, float* U,
-                      int ldu);
+                      int ldu, uint2* xn_pk = nullptr, int pk_ld = 0);
 void launch_lora_down(cudaStream_t st, int dtype, const float* X, int ldx, int row0, int rows, int K,
                       const int* xmap, const void* A, int r, float* U, int ldu);
 void launch_gemv(cudaStream_t st, int dtype, const GemvArgs& a, bool swiglu);
